@@ -1,0 +1,211 @@
+"""ctypes binding of the CPU oracle (oracle/em_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It imports nothing from the CUDA package and shares no code with it.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "em_oracle.c")
+_LIB = os.path.join(_HERE, "libemo.so")
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp -shared; rebuilt when the source is newer than the library."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.check_call(cmd)
+    return _LIB
+
+
+class _Grid(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("dx", C.POINTER(C.c_double)), ("dy", C.POINTER(C.c_double)), ("dz", C.POINTER(C.c_double)),
+                ("loss_mode", C.c_int32), ("bc", C.c_int32 * 6)]
+
+
+class _Material(C.Structure):
+    _fields_ = [("eps", C.c_double), ("mu", C.c_double), ("sigma", C.c_double), ("flags", C.c_int32)]
+
+
+class _Port(C.Structure):
+    _fields_ = [("edge_begin", C.c_int64), ("edge_end", C.c_int64), ("amplitude", C.c_double),
+                ("wave_offset", C.c_int64), ("wave_len", C.c_int64)]
+
+
+class _Edge(C.Structure):
+    _fields_ = [("comp", C.c_int32), ("i", C.c_int32), ("j", C.c_int32), ("k", C.c_int32),
+                ("weight", C.c_double)]
+
+
+class _ProbePt(C.Structure):
+    _fields_ = [("comp", C.c_int32), ("i", C.c_int32), ("j", C.c_int32), ("k", C.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.emo_step_index.restype = C.c_int64
+    return _lib
+
+
+def _dp(a: np.ndarray):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _shapes(nx, ny, nz):
+    return [(nz + 1, ny + 1, nx), (nz + 1, ny, nx + 1), (nz, ny + 1, nx + 1),
+            (nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)]
+
+
+def _mk_grid(nx, ny, nz, dx, dy, dz, loss_mode):
+    g = _Grid()
+    g.nx, g.ny, g.nz = nx, ny, nz
+    g.dx, g.dy, g.dz = _dp(dx), _dp(dy), _dp(dz)
+    g.loss_mode = loss_mode
+    for b in range(6):
+        g.bc[b] = 0
+    return g
+
+
+def _mk_table(table, flags):
+    n = table.shape[0]
+    arr = (_Material * n)()
+    for m in range(n):
+        arr[m].eps, arr[m].mu, arr[m].sigma = float(table[m, 0]), float(table[m, 1]), float(table[m, 2])
+        arr[m].flags = int(flags[m]) if flags is not None else 0
+    return arr
+
+
+def cfl_dt(nx, ny, nz, dx, dy, dz, mat_id, table, flags=None) -> float:
+    dx = np.ascontiguousarray(dx, np.float64); dy = np.ascontiguousarray(dy, np.float64)
+    dz = np.ascontiguousarray(dz, np.float64)
+    mat_id = np.ascontiguousarray(mat_id, np.uint8)
+    g = _mk_grid(nx, ny, nz, dx, dy, dz, 0)
+    tab = _mk_table(table, flags)
+    out = C.c_double()
+    rc = lib().emo_cfl_dt(C.byref(g), mat_id.ctypes.data_as(C.c_void_p), tab, table.shape[0], C.byref(out))
+    if rc:
+        raise RuntimeError("emo_cfl_dt rc=%d" % rc)
+    return out.value
+
+
+def set_threads(n: int) -> int:
+    return int(lib().emo_set_threads(int(n)))
+
+
+class Oracle:
+    """fp64 CPU oracle instance built from a workloads.Problem-like object."""
+
+    def __init__(self, p, load_sources: bool = True, load_init: bool = True):
+        self.nx, self.ny, self.nz = int(p.nx), int(p.ny), int(p.nz)
+        self.shapes = _shapes(self.nx, self.ny, self.nz)
+        self._dx = np.ascontiguousarray(p.dx, np.float64)
+        self._dy = np.ascontiguousarray(p.dy, np.float64)
+        self._dz = np.ascontiguousarray(p.dz, np.float64)
+        mat = np.ascontiguousarray(p.mat_id, np.uint8)
+        assert mat.shape == (self.nz, self.ny, self.nx)
+        g = _mk_grid(self.nx, self.ny, self.nz, self._dx, self._dy, self._dz, int(p.loss_mode))
+        tab = _mk_table(p.table, p.flags)
+        self._h = C.c_void_p()
+        rc = lib().emo_create(C.byref(g), mat.ctypes.data_as(C.c_void_p), tab, p.table.shape[0],
+                              C.c_double(p.dt), C.byref(self._h))
+        if rc:
+            raise RuntimeError("emo_create rc=%d" % rc)
+        if load_sources and p.n_ports > 0:
+            self.set_source(p)
+        if load_init and p.init:
+            for comp, arr in p.init.items():
+                self.set_field(comp, arr)
+
+    def close(self):
+        if self._h:
+            lib().emo_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_source(self, p):
+        np_ = p.n_ports
+        ports = (_Port * max(np_, 1))()
+        for q in range(np_):
+            ports[q].edge_begin = int(p.port_edge_begin[q]); ports[q].edge_end = int(p.port_edge_end[q])
+            ports[q].amplitude = float(p.port_amplitude[q])
+            ports[q].wave_offset = int(p.port_wave_offset[q]); ports[q].wave_len = int(p.port_wave_len[q])
+        ne = int(p.edge_comp.shape[0])
+        edges = (_Edge * max(ne, 1))()
+        for e in range(ne):
+            edges[e].comp = int(p.edge_comp[e])
+            edges[e].i, edges[e].j, edges[e].k = (int(v) for v in p.edge_ijk[e])
+            edges[e].weight = float(p.edge_weight[e])
+        wave = np.ascontiguousarray(p.wave, np.float64)
+        rc = lib().emo_set_source(self._h, np_, ports, edges, C.c_int64(ne), _dp(wave), C.c_int64(wave.shape[0]))
+        if rc:
+            raise RuntimeError("emo_set_source rc=%d" % rc)
+
+    def set_field(self, comp: int, arr):
+        a = np.ascontiguousarray(arr, np.float64)
+        assert a.shape == self.shapes[comp], (a.shape, self.shapes[comp])
+        rc = lib().emo_set_field(self._h, comp, _dp(a))
+        if rc:
+            raise RuntimeError("emo_set_field rc=%d" % rc)
+
+    def get_field(self, comp: int) -> np.ndarray:
+        out = np.empty(self.shapes[comp], np.float64)
+        rc = lib().emo_get_field(self._h, comp, _dp(out))
+        if rc:
+            raise RuntimeError("emo_get_field rc=%d" % rc)
+        return out
+
+    def fields(self):
+        return [self.get_field(c) for c in range(6)]
+
+    def step(self, n: int = 1):
+        rc = lib().emo_step(self._h, C.c_int64(n))
+        if rc:
+            raise RuntimeError("emo_step rc=%d" % rc)
+
+    def joule(self, power: bool = True, energy: bool = True, total: bool = True, reset: bool = False):
+        ncell = (self.nz, self.ny, self.nx)
+        p = np.empty(ncell, np.float64) if power else None
+        q = np.empty(ncell, np.float64) if energy else None
+        t = C.c_double()
+        rc = lib().emo_joule(self._h, _dp(p) if power else None, _dp(q) if energy else None,
+                             C.byref(t) if total else None, int(reset))
+        if rc:
+            raise RuntimeError("emo_joule rc=%d" % rc)
+        return p, q, (t.value if total else None)
+
+    def probe(self, pts) -> np.ndarray:
+        pts = np.asarray(pts, np.int32).reshape(-1, 4)
+        arr = (_ProbePt * max(len(pts), 1))()
+        for n, (c, i, j, k) in enumerate(pts):
+            arr[n].comp, arr[n].i, arr[n].j, arr[n].k = int(c), int(i), int(j), int(k)
+        out = np.empty(len(pts), np.float64)
+        rc = lib().emo_probe(self._h, len(pts), arr, _dp(out))
+        if rc:
+            raise RuntimeError("emo_probe rc=%d" % rc)
+        return out
+
+    def reset(self):
+        lib().emo_reset(self._h)
+
+    @property
+    def step_index(self) -> int:
+        return int(lib().emo_step_index(self._h))
