@@ -1,0 +1,160 @@
+/*
+ * em.h -- C ABI of the B200 (sm_100a) explicit EM time-marching + Joule-heat library (libem.so).
+ *
+ * The operation is the paper's explicit central-difference update of the edge-based vector wave
+ * equation on a structured non-uniform grid,
+ *     D_eps e'' + (D_sigma e)' + S e = -J'                       (eq. 1)
+ *     M e^{n+1} = N e^n - K e^{n-1} - dt^2 (dJ/dt)^n             (eq. 2)
+ *     M,K = D_eps +- dt/2 D_sigma,  N = 2 D_eps - dt^2 S,  S = curl mu^-1 curl   (L65, L73-L76, eq. 3)
+ * marched as the algebraically identical material-weighted E/H leapfrog,
+ * with external current-source injection (L63-L69, L144) and the per-cell Joule heat
+ * P = D_sigma e^2 (L86) that drives the paper's thermal stage (L90).
+ *
+ * Conventions
+ *  - Every call returns an int32 status (EM_OK = 0); it never throws, aborts or prints.
+ *    em_last_error() returns a human-readable string for the last failure on this thread.
+ *  - The library NEVER allocates device memory: the caller passes one device workspace
+ *    (em_workspace_bytes) and every output buffer.  The context borrows the workspace and the
+ *    CUDA stream until em_destroy.  All device work is enqueued on that stream; calls are
+ *    asynchronous unless a host scalar / host array is returned (documented per call).
+ *  - "host" / "device" is stated for every pointer.  Setup inputs are host pointers and are copied
+ *    during the call.  SI units; material table entries are absolute eps [F/m], mu [H/m],
+ *    sigma [S/m] as double whatever the working precision.
+ *  - User-visible field arrays are dense, C order [k][j][i] (x fastest), in the WORKING precision
+ *    (float for precision 32, double for 64):
+ *        Ex (nz+1, ny+1, nx)   Ey (nz+1, ny, nx+1)   Ez (nz, ny+1, nx+1)     edge tangentials
+ *        Hx (nz, ny, nx+1)     Hy (nz, ny+1, nx)     Hz (nz+1, ny, nx)       face normals
+ *        mat_id, Joule maps (nz, ny, nx)
+ *    Ex(i,j,k) is the edge from node (i,j,k) to (i+1,j,k); Hx(i,j,k) the x-normal face at node
+ *    plane i over cell (j,k); cyclic for y, z.  (Placement pinned by the DOF count of PAPER.md L160.)
+ *  - State after n steps: E at t = n dt, H at t = (n - 1/2) dt, Joule energy over [0, n dt].
+ *  - One context = one host thread at a time.  Several contexts may coexist.
+ */
+#ifndef EM_H_
+#define EM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EM_OK 0
+#define EM_ERR_INVALID_ARG 1
+#define EM_ERR_WORKSPACE_TOO_SMALL 2
+#define EM_ERR_CUDA 3
+#define EM_ERR_STATE 4
+#define EM_ERR_UNSUPPORTED 5
+
+#define EM_LOSS_CD 0  /* paper eq. (3): trapezoidal conduction term, M,K = D_eps +- dt/2 D_sigma */
+#define EM_LOSS_EXP 1 /* exponential-loss update: ca = exp(-s dt/eps), cb = -expm1(-s dt/eps)/s  */
+
+#define EM_BC_PEC 0 /* tangential E = 0 on the wall (the only supported truncation)             */
+#define EM_BC_PMC 1 /* paper's truncation: not implemented -> EM_ERR_UNSUPPORTED */
+
+#define EM_MAT_PEC 1 /* em_material.flags bit0: every edge touching such a cell is held at 0      */
+
+/* em_grid.kernel: kernel strategy.  AUTO picks the fused sweep; SPLIT runs the separate
+ * H / E / Joule kernels (kept for cross-checking; both are CUDA paths of this library). */
+#define EM_KERNEL_AUTO 0
+#define EM_KERNEL_SPLIT 1
+#define EM_KERNEL_FUSED 2
+
+typedef struct em_ctx em_ctx; /* opaque, host-side */
+
+typedef struct em_grid {
+    int32_t nx, ny, nz;          /* cells per axis, each >= 1                                       */
+    const double *dx, *dy, *dz;  /* HOST: cell sizes [m], lengths nx, ny, nz, all > 0                */
+    int32_t precision;           /* 32 or 64: working precision of fields, maps and arithmetic      */
+    int32_t loss_mode;           /* EM_LOSS_CD or EM_LOSS_EXP                                        */
+    int32_t bc[6];               /* -x,+x,-y,+y,-z,+z: EM_BC_PEC                                     */
+    int32_t kernel;              /* EM_KERNEL_*                                                      */
+    int32_t max_ports;           /* capacity reserved in the workspace for em_set_source            */
+    int64_t max_source_edges;
+    int64_t max_wave_samples;
+} em_grid;
+
+typedef struct em_material { double eps, mu, sigma; int32_t flags; int32_t pad_; } em_material;
+
+/* Port p drives edges[edge_begin .. edge_end) with
+ *   J_e(t_{n+1/2}) = amplitude * edges[e].weight * wave[wave_offset + n]   for n < wave_len, else 0,
+ * n = absolute step index since em_create / em_reset; wave[n] samples J [A/m^2] at t = (n+1/2) dt
+ * so that (dJ/dt)^n of eq. (2) is the centred difference of two consecutive samples. */
+typedef struct em_port { int64_t edge_begin, edge_end; double amplitude; int64_t wave_offset, wave_len; } em_port;
+typedef struct em_edge { int32_t comp /*0=x,1=y,2=z*/, i, j, k; double weight; } em_edge;
+typedef struct em_probe_pt { int32_t comp /*0..5 = Ex,Ey,Ez,Hx,Hy,Hz*/, i, j, k; } em_probe_pt;
+
+/* Thread-local description of the last error returned by any call on this thread. */
+const char *em_last_error(void);
+
+/* Bytes of device workspace needed for this grid (fields with padding and their ping-pong copies,
+ * material ids, Joule accumulator, coefficient tables, source lists up to the max_* capacities).
+ * Host-only.  Errors: EM_ERR_INVALID_ARG (null, dims < 1, precision not 32/64). */
+int32_t em_workspace_bytes(const em_grid *g, size_t *out_bytes);
+
+/* Build a context.  mat_id: HOST uint8 [nz][ny][nx], every id < n_mat <= 255.  table: HOST,
+ * n_mat entries, eps > 0, mu > 0, sigma >= 0.  dt > 0 (CFL is the caller's business: em_cfl_dt).
+ * workspace: DEVICE, 256-byte aligned, >= em_workspace_bytes.  stream: cudaStream_t (may be 0).
+ * Zeroes fields, Joule accumulator and the step counter.  Synchronises the stream before returning
+ * (the host inputs may be freed on return).
+ * Errors: INVALID_ARG, WORKSPACE_TOO_SMALL, UNSUPPORTED (a bc != EM_BC_PEC), CUDA. */
+int32_t em_create(const em_grid *g, const uint8_t *mat_id, const em_material *table, int32_t n_mat,
+                  double dt, void *workspace, size_t workspace_bytes, void *stream, em_ctx **out);
+
+/* Frees the host-side context only; the workspace stays with the caller. */
+int32_t em_destroy(em_ctx *ctx);
+
+/* Host-only helper ("constrained by the CFL condition"):
+ * *dt_max = min over cells of sqrt(eps mu) / sqrt(dx_i^-2 + dy_j^-2 + dz_k^-2).  The caller applies
+ * its own safety factor (0.9 in the five configurations). */
+int32_t em_cfl_dt(const em_grid *g, const uint8_t *mat_id, const em_material *table, int32_t n_mat,
+                  double *dt_max);
+
+/* Replace the source set.  All pointers HOST; copied.  Edges must be inside the grid and must not be
+ * PEC-fixed (INVALID_ARG).  Ports that share an edge add.  n_ports = 0 removes all sources.
+ * Errors: INVALID_ARG, WORKSPACE_TOO_SMALL (capacities of em_grid exceeded), CUDA. */
+int32_t em_set_source(em_ctx *ctx, int32_t n_ports, const em_port *ports, const em_edge *edges,
+                      int64_t n_edges, const double *wave, int64_t n_samples);
+
+/* Copy one field component (0..5 = Ex,Ey,Ez,Hx,Hy,Hz) from/to a dense array in the working
+ * precision.  src/dst may be a HOST (is_device = 0) or DEVICE (is_device != 0) pointer.  Tangential E
+ * on PEC-fixed edges is forced to 0 on set.  Host transfers synchronise the stream. */
+int32_t em_set_field(em_ctx *ctx, int32_t comp, const void *src, int32_t src_is_device);
+int32_t em_get_field(em_ctx *ctx, int32_t comp, void *dst, int32_t dst_is_device);
+
+/* Advance n >= 0 steps (n = 0 is a no-op).  Per step: H^{n+1/2} = H^{n-1/2} - dt nu (C_e E^n);
+ * E^{n+1} = ca E^n + cb (C_h H^{n+1/2} - J^{n+1/2}) on non-fixed edges; Joule energy density
+ * q_c += dt sigma_c 1/4 sum over the 12 edges of c of ((E^{n+1} + E^n)/2)^2.  Asynchronous. */
+int32_t em_step(em_ctx *ctx, int64_t n);
+
+/* Joule outputs.  power_density (DEVICE, nullable): p_c = sigma_c 1/4 sum_12 (E_e^n)^2 [W/m^3] from
+ * the current field (literal).  energy_density (DEVICE, nullable): q_c [J/m^3].  Both
+ * dense [nz][ny][nx] in the working precision.  total_energy (HOST, nullable): sum_c q_c V_c [J],
+ * reduced in fp64 in a fixed order; requesting it synchronises the stream.  reset != 0 zeroes q
+ * after the outputs are produced. */
+int32_t em_joule(em_ctx *ctx, void *power_density, void *energy_density, double *total_energy,
+                 int32_t reset);
+
+/* Raw staggered samples (E at t_n, H at t_{n-1/2}) as double.  pts, out: HOST.  Synchronises. */
+int32_t em_probe(em_ctx *ctx, int32_t n_pts, const em_probe_pt *pts, double *out);
+
+/* Zero the six fields, q and the step counter; keep grid, materials and sources. */
+int32_t em_reset(em_ctx *ctx);
+
+/* Absolute step index n (host bookkeeping). */
+int32_t em_step_index(em_ctx *ctx, int64_t *n);
+
+/* Number of kernel launches enqueued by this context so far (for bench accounting). */
+int32_t em_launch_count(em_ctx *ctx, int64_t *n);
+
+/* Name, launch count and accumulated device time of the dominant kernel of em_step since the last
+ * em_timing_reset, measured with CUDA events on the context's stream when timing is enabled
+ * (enable != 0 adds one event pair per launch of that kernel).  ms may be read after a sync. */
+int32_t em_timing_enable(em_ctx *ctx, int32_t enable);
+int32_t em_timing_read(em_ctx *ctx, const char **kernel_name, int64_t *launches, double *ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EM_H_ */

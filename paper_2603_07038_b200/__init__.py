@@ -1,0 +1,12 @@
+"""B200-native explicit EM time-marching + Joule-heat hot path of arxiv/paper_2603_07038.
+
+The product is the C-ABI library ``libem.so`` (include/em.h, csrc/*.cu, hand-written sm_100a CUDA
+kernels).  This package is the thin Python binding with the same call names; PyTorch is used only
+for device memory and streams.  There is no CPU fallback: importing the binding without the built
+library raises.
+"""
+from .binding import (  # noqa: F401
+    EM, EMError, lib_path, load,
+    EM_LOSS_CD, EM_LOSS_EXP, EM_KERNEL_AUTO, EM_KERNEL_SPLIT, EM_KERNEL_FUSED,
+    em_workspace_bytes, em_cfl_dt,
+)

@@ -1,0 +1,136 @@
+// em_aux.cuh -- setup / output kernels around the hot path: PEC masking after em_set_field,
+// source coefficients and injection (a3), power-density map, fp64 Joule total, probe gather.
+#pragma once
+#include "em_common.cuh"
+#include "em_split.cuh"
+
+namespace em {
+
+// Source lists on the device.  "Unique edge" u owns contributions [cbeg[u], cbeg[u+1]) so that
+// overlapping ports add in a fixed order.
+template <typename R>
+struct DevSources {
+    int n_unique;
+    const long long *off;     // padded offset of the edge
+    const int *comp;          // 0,1,2
+    R *r;                     // loss coefficient r_e of the edge (filled by k_source_coef)
+    const int *cbeg;          // n_unique + 1
+    const int *con_port;      // per contribution
+    const R *con_scale;       // amplitude * weight
+    const long long *port_woff, *port_wlen;
+    const R *wave;
+};
+
+// Zero E[comp] wherever the edge is PEC-fixed (mask product of its 4 cells is 0).
+template <typename R>
+__global__ void __launch_bounds__(256) k_mask_fixed(DevParams<R> p, int comp) {
+    __shared__ MatEntry<R> s_tab[kMaxTable];
+    load_table(s_tab, p);
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i > p.nx || j > p.ny) return;
+    const long long PX = p.PX, PXY = p.PXY;
+    const long long o = ((long long)k * p.PY + j) * PX + i;
+    const uint8_t *mat = p.mat;
+    R m;
+    if (comp == 0)      m = s_tab[mat[o]].m * s_tab[mat[o - PX]].m * s_tab[mat[o - PXY]].m * s_tab[mat[o - PXY - PX]].m;
+    else if (comp == 1) m = s_tab[mat[o]].m * s_tab[mat[o - 1]].m * s_tab[mat[o - PXY]].m * s_tab[mat[o - PXY - 1]].m;
+    else                m = s_tab[mat[o]].m * s_tab[mat[o - 1]].m * s_tab[mat[o - PX]].m * s_tab[mat[o - PX - 1]].m;
+    if (m == R(0)) p.E[comp][o] = R(0);
+}
+
+// r_e for every unique source edge; flags[u] = 1 if the edge is PEC-fixed (argument error).
+template <typename R, int LOSS>
+__global__ void k_source_coef(DevParams<R> p, DevSources<R> s, int *fixed_flags) {
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= s.n_unique) return;
+    const long long o = s.off[u];
+    const long long PX = p.PX, PXY = p.PXY;
+    const long long kk = o / PXY, rem = o - kk * PXY;   // o >= 0 for in-range edges
+    const int j = (int)(rem / PX), i = (int)(rem - (long long)j * PX), k = (int)kk;
+    R r[3], sg[3];
+    edge_coeffs<R, LOSS>(p.table, p.mat, o, PX, PXY, p.fx[i], p.fy[j], p.fz[k], r, sg);
+    const R re = r[s.comp[u]];
+    s.r[u] = re;
+    fixed_flags[u] = (re == R(0)) ? 1 : 0;
+}
+
+// a3 -- E^{n+1} -= r_e * J_e^{n+1/2}   ("-dt^2 (dJ/dt)^n")
+template <typename R>
+__global__ void k_apply_source(R *e0, R *e1, R *e2, DevSources<R> s, long long step) {
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= s.n_unique) return;
+    R J = 0;
+    for (int c = s.cbeg[u]; c < s.cbeg[u + 1]; ++c) {
+        const int pt = s.con_port[c];
+        if (step < s.port_wlen[pt]) J = mad(s.con_scale[c], s.wave[s.port_woff[pt] + step], J);
+    }
+    R *e = s.comp[u] == 0 ? e0 : (s.comp[u] == 1 ? e1 : e2);
+    e[s.off[u]] = mad(-s.r[u], J, e[s.off[u]]);
+}
+
+// p_c = sigma_c * 1/4 sum_12 (E_e)^2 into a dense [nz][ny][nx] map
+template <typename R>
+__global__ void __launch_bounds__(256) k_power(DevParams<R> p, R *out) {
+    __shared__ MatEntry<R> s_tab[kMaxTable];
+    load_table(s_tab, p);
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= p.nx || j >= p.ny) return;
+    const long long PX = p.PX, PXY = p.PXY;
+    const long long o = ((long long)k * p.PY + j) * PX + i;
+    R s = 0;
+#define EM_SQ(c, off) { const R t_ = p.E[c][o + (off)]; s = mad(t_, t_, s); }
+    EM_SQ(0, 0) EM_SQ(0, PX) EM_SQ(0, PXY) EM_SQ(0, PXY + PX)
+    EM_SQ(1, 0) EM_SQ(1, 1)  EM_SQ(1, PXY) EM_SQ(1, PXY + 1)
+    EM_SQ(2, 0) EM_SQ(2, 1)  EM_SQ(2, PX)  EM_SQ(2, PX + 1)
+#undef EM_SQ
+    out[((long long)k * p.ny + j) * p.nx + i] = s_tab[p.mat[o]].b * R(0.25) * s;
+}
+
+// Q = sum_c q_c V_c in fp64, fixed order: per-block partials then one block.
+template <typename R>
+__global__ void __launch_bounds__(256) k_energy_partial(DevParams<R> p, const double *vx, const double *vy,
+                                                        const double *vz, double *partial) {
+    __shared__ double sh[256];
+    const long long ncell = (long long)p.nx * p.ny * p.nz;
+    double acc = 0.0;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(c % p.nx); const long long t = c / p.nx;
+        const int j = (int)(t % p.ny); const int k = (int)(t / p.ny);
+        acc += (double)p.q[((long long)k * p.PY + j) * p.PX + i] * (vx[i] * vy[j] * vz[k]);
+    }
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+
+__global__ void __launch_bounds__(256) k_energy_final(const double *partial, int n, double *out) {
+    __shared__ double sh[256];
+    double acc = 0.0;
+    for (int c = threadIdx.x; c < n; c += 256) acc += partial[c];
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sh[0];
+}
+
+template <typename R>
+struct ProbeArrays { const R *f[6]; };
+
+template <typename R>
+__global__ void k_probe(ProbeArrays<R> a, const long long *off, const int *comp, int n, double *out) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n) out[t] = (double)a.f[comp[t]][off[t]];
+}
+
+}  // namespace em

@@ -1,0 +1,69 @@
+// em_common.cuh -- device-side data layout and small helpers shared by every kernel of libem.so.
+//
+// Data layout in HBM: structure of arrays.  Every per-node/per-cell array
+// (six field components and their ping-pong copies, the uint8 material ids, the Joule
+// accumulator) uses ONE padded index geometry
+//     off(i,j,k) = (k*PY + j)*PX + i,   i in [-1, PX-2], j in [-1, ny+1], k in [-1, nz+1]
+// with PX = roundup(nx+2, 32), PY = ny+3, PZ = nz+3 and the array pointer already shifted to the
+// logical origin, so that one offset serves all arrays and +-1 neighbours are +-1, +-PX, +-PX*PY.
+// Entries outside a component's logical range are kept at 0 ("halo-free padded pitches": the pad
+// plays the role of the halo, no special-casing at the walls); material ids outside the grid hold
+// the extra table entry n_mat = "outside/PEC" whose mask is 0.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace em {
+
+constexpr int kMaxTable = 256;   // n_mat <= 255 plus the "outside" entry
+
+template <typename R> struct Vec4;
+template <> struct Vec4<float>  { using type = float4;  };
+template <> struct Vec4<double> { using type = double4; };
+
+// Per-material coefficient entry, built in fp64 on the host and rounded once:
+//   a = eps/dt,  b = sigma,  m = 1 (ordinary) or 0 (PEC-flagged / outside),  n = dt/mu
+template <typename R> struct alignas(4 * sizeof(R)) MatEntry { R a, b, m, n; };
+
+template <typename R>
+struct DevParams {
+    int nx, ny, nz;
+    int PX, PY;              // pitches (elements)
+    long long PXY;           // plane stride
+    R *E[3], *En[3];         // E^n and E^{n+1} (ping-pong)
+    R *H[3], *Hn[3];         // H^{n-1/2} and H^{n+1/2} (ping-pong, fused sweep only; split: Hn == H)
+    R *q;                    // Joule energy density accumulator
+    const uint8_t *mat;      // material ids, same geometry
+    const MatEntry<R> *table;// n_table entries in global memory
+    int n_table;
+    // per-axis arrays indexed [-1 .. n+1] (pointer shifted to index 0):
+    //   rd = 1/d (0 outside), rt = 1/d~, f = d[i]/(d[i-1]+d[i]) with d[-1] = d[n] = 0
+    const R *rdx, *rtx, *fx, *rdy, *rty, *fy, *rdz, *rtz, *fz;
+    R dt;
+};
+
+__device__ __forceinline__ float  mad(float a, float b, float c)    { return ::fmaf(a, b, c); }
+__device__ __forceinline__ double mad(double a, double b, double c) { return ::fma(a, b, c); }
+template <typename R> __device__ __forceinline__ R lerp(R lo, R hi, R f) { return mad(f, hi - lo, lo); }
+
+template <typename R> __device__ __forceinline__ R rcp(R x);
+template <> __device__ __forceinline__ float  rcp<float>(float x)   { return __frcp_rn(x); }
+template <> __device__ __forceinline__ double rcp<double>(double x) { return 1.0 / x; }
+
+// Loss coefficient r of the incremental form  E' = E + r (curlH - J - sigma E):
+//   CD  (paper eq. 3): r = 1/(eps/dt + sigma/2)          == cb,  ca = 1 - sigma r
+//   EXP               : r = -expm1(-sigma dt/eps)/sigma  == cb,  ca = 1 - sigma r = exp(-sigma dt/eps)
+template <typename R, int LOSS>
+__device__ __forceinline__ R loss_r(R A /*eps/dt*/, R B /*sigma*/) {
+    if (LOSS == 0) {
+        return rcp<R>(mad(R(0.5), B, A));
+    } else {
+        if (B > R(0)) {
+            R u = B / A;
+            return -::expm1(-u) / B;
+        }
+        return rcp<R>(A);
+    }
+}
+
+}  // namespace em

@@ -1,0 +1,673 @@
+// em_lib.cu -- host side of libem.so: the C ABI declared in include/em.h.
+// No torch types, no device allocation: the caller's workspace is carved here.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/em.h"
+#include "em_aux.cuh"
+#include "em_common.cuh"
+#include "em_fused.cuh"
+#include "em_split.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+int32_t fail(int32_t code, const std::string &msg) { g_err = msg; return code; }
+
+#define CU(call)                                                                               \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail(EM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));      \
+    } while (0)
+
+constexpr size_t kAlign = 256;
+size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a; }
+
+struct Geometry {
+    int nx, ny, nz, PX, PY, PZ;
+    long long PXY, vol, origin;   // origin: elements from the allocation start to logical (0,0,0)
+    long long alloc_elems;        // vol + guards
+};
+
+Geometry make_geometry(int nx, int ny, int nz) {
+    Geometry g;
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.PX = (nx + 2 + 31) / 32 * 32;
+    g.PY = ny + 3; g.PZ = nz + 3;
+    g.PXY = (long long)g.PX * g.PY;
+    g.vol = g.PXY * g.PZ;
+    // one guard row in front (i = -1 of row j = -1, plane k = -1) and 2 behind (vector tails)
+    g.origin = g.PX + g.PXY + g.PX;   // guard + plane k=-1 + row j=-1
+    g.alloc_elems = g.vol + 3LL * g.PX;
+    return g;
+}
+
+constexpr int kProbeChunk = 4096;
+constexpr int kReduceBlocks = 1024;
+constexpr int kTimingRing = 4096;
+
+// Workspace carving: identical code computes sizes (base == nullptr) and pointers.
+struct Carver {
+    char *base; size_t off = 0;
+    explicit Carver(void *b) : base(static_cast<char *>(b)) {}
+    template <typename T> T *take(size_t n) {
+        off = align_up(off);
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
+};
+
+template <typename R>
+struct Carved {
+    R *field[12];            // E[3], En[3], H[3], Hn[3] allocation starts
+    R *q;
+    uint8_t *mat;
+    em::MatEntry<R> *table;
+    R *axis[9];              // rdx, rtx, fx, rdy, rty, fy, rdz, rtz, fz (allocation starts; index -1 first)
+    double *vx, *vy, *vz;    // cell sizes in fp64 for the Joule total
+    double *partial, *scalar;
+    long long *probe_off; int *probe_comp; double *probe_out;
+    // sources
+    long long *src_off; int *src_comp; R *src_r; int *src_cbeg; int *src_flags;
+    int *con_port; R *con_scale; long long *port_woff, *port_wlen; R *wave;
+    // fused-sweep tile source index
+    int *tile_sbeg;
+};
+
+template <typename R>
+size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int n_tiles) {
+    Carver w(base);
+    Carved<R> tmp;
+    Carved<R> &o = c ? *c : tmp;
+    for (int a = 0; a < 12; ++a) o.field[a] = w.take<R>(g.alloc_elems);
+    o.q = w.take<R>(g.alloc_elems);
+    o.mat = w.take<uint8_t>(g.alloc_elems);
+    o.table = w.take<em::MatEntry<R>>(em::kMaxTable);
+    const int len[3] = {g.PX + 2, g.PY + 2, g.PZ + 2};
+    for (int a = 0; a < 9; ++a) o.axis[a] = w.take<R>(len[a / 3]);
+    o.vx = w.take<double>(g.nx); o.vy = w.take<double>(g.ny); o.vz = w.take<double>(g.nz);
+    o.partial = w.take<double>(kReduceBlocks); o.scalar = w.take<double>(1);
+    o.probe_off = w.take<long long>(kProbeChunk); o.probe_comp = w.take<int>(kProbeChunk);
+    o.probe_out = w.take<double>(kProbeChunk);
+    const size_t me = (size_t)std::max<int64_t>(gr.max_source_edges, 1), mp = (size_t)std::max(gr.max_ports, 1);
+    o.src_off = w.take<long long>(me); o.src_comp = w.take<int>(me); o.src_r = w.take<R>(me);
+    o.src_cbeg = w.take<int>(me + 1); o.src_flags = w.take<int>(me);
+    o.con_port = w.take<int>(me); o.con_scale = w.take<R>(me);
+    o.port_woff = w.take<long long>(mp); o.port_wlen = w.take<long long>(mp);
+    o.wave = w.take<R>((size_t)std::max<int64_t>(gr.max_wave_samples, 1));
+    o.tile_sbeg = w.take<int>((size_t)n_tiles + 1);
+    return align_up(w.off);
+}
+
+struct Timing {
+    bool enabled = false;
+    std::vector<cudaEvent_t> beg, end;
+    int head = 0, pending = 0;
+    long long launches = 0; double ms = 0.0;
+};
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+struct em_ctx {
+    virtual ~em_ctx() {}
+    virtual int32_t set_source(int32_t, const em_port *, const em_edge *, int64_t, const double *, int64_t) = 0;
+    virtual int32_t set_field(int32_t, const void *, int32_t) = 0;
+    virtual int32_t get_field(int32_t, void *, int32_t) = 0;
+    virtual int32_t step(int64_t) = 0;
+    virtual int32_t joule(void *, void *, double *, int32_t) = 0;
+    virtual int32_t probe(int32_t, const em_probe_pt *, double *) = 0;
+    virtual int32_t reset() = 0;
+    int64_t step_index = 0, launches = 0;
+    Timing timing;
+    const char *main_kernel = "";
+    cudaStream_t stream = nullptr;
+    int32_t timing_flush();
+};
+
+int32_t em_ctx::timing_flush() {
+    Timing &t = timing;
+    while (t.pending > 0) {
+        const int idx = (t.head - t.pending + kTimingRing) % kTimingRing;
+        CU(cudaEventSynchronize(t.end[idx]));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, t.beg[idx], t.end[idx]));
+        t.ms += ms; t.launches += 1; t.pending -= 1;
+    }
+    return EM_OK;
+}
+
+namespace {
+
+template <typename R>
+struct Ctx final : em_ctx {
+    Geometry g;
+    em_grid grid;
+    int loss = 0, kernel = EM_KERNEL_SPLIT;
+    double dt = 0;
+    Carved<R> c;
+    em::DevParams<R> p;
+    std::vector<em_material> table;
+    std::vector<uint8_t> fixed_cell;   // host copy of "mask == 0" per material (incl. outside)
+    std::vector<uint8_t> host_mat;     // host copy of the ids (for argument checks of sources)
+    int n_unique = 0, n_ports = 0;
+    em::DevSources<R> src;
+    em::FusedPlan plan;
+    bool uniform_mu = true;
+
+    R *org(int a) const { return c.field[a] + g.origin; }
+
+    void bind() {
+        for (int a = 0; a < 3; ++a) {
+            p.E[a] = org(e_cur * 3 + a); p.En[a] = org((1 - e_cur) * 3 + a);
+            p.H[a] = org(6 + h_cur * 3 + a); p.Hn[a] = org(6 + (1 - h_cur) * 3 + a);
+        }
+    }
+    int e_cur = 0, h_cur = 0;
+
+    int32_t init(const em_grid *gr, const uint8_t *mat_id, const em_material *tab, int32_t n_mat, double dt_,
+                 void *workspace, size_t ws_bytes, void *stream_);
+    int32_t zero_state();
+    int32_t set_source(int32_t, const em_port *, const em_edge *, int64_t, const double *, int64_t) override;
+    int32_t set_field(int32_t, const void *, int32_t) override;
+    int32_t get_field(int32_t, void *, int32_t) override;
+    int32_t step(int64_t) override;
+    int32_t joule(void *, void *, double *, int32_t) override;
+    int32_t probe(int32_t, const em_probe_pt *, double *) override;
+    int32_t reset() override { return zero_state(); }
+    int32_t step_split();
+    int32_t step_fused();
+    void comp_dims(int comp, int *sx, int *sy, int *sz) const {
+        const int nx = g.nx, ny = g.ny, nz = g.nz;
+        switch (comp) {
+        case 0: *sx = nx;     *sy = ny + 1; *sz = nz + 1; break;
+        case 1: *sx = nx + 1; *sy = ny;     *sz = nz + 1; break;
+        case 2: *sx = nx + 1; *sy = ny + 1; *sz = nz;     break;
+        case 3: *sx = nx + 1; *sy = ny;     *sz = nz;     break;
+        case 4: *sx = nx;     *sy = ny + 1; *sz = nz;     break;
+        default:*sx = nx;     *sy = ny;     *sz = nz + 1; break;
+        }
+    }
+    R *comp_ptr(int comp) const { return comp < 3 ? p.E[comp] : p.H[comp - 3]; }
+    dim3 node_grid(dim3 b, int ex) const { return dim3((g.nx + ex + b.x - 1) / b.x, (g.ny + ex + b.y - 1) / b.y, g.nz + ex); }
+    int32_t record_begin();
+    int32_t record_end();
+};
+
+int32_t validate_grid(const em_grid *g) {
+    if (!g) return fail(EM_ERR_INVALID_ARG, "grid is null");
+    if (g->nx < 1 || g->ny < 1 || g->nz < 1) return fail(EM_ERR_INVALID_ARG, "grid dims must be >= 1");
+    if ((long long)g->nx + 34 > 2147483647LL / 4) return fail(EM_ERR_INVALID_ARG, "nx too large");
+    if (g->precision != 32 && g->precision != 64) return fail(EM_ERR_INVALID_ARG, "precision must be 32 or 64");
+    if (g->loss_mode != EM_LOSS_CD && g->loss_mode != EM_LOSS_EXP) return fail(EM_ERR_INVALID_ARG, "bad loss_mode");
+    if (g->kernel < EM_KERNEL_AUTO || g->kernel > EM_KERNEL_FUSED) return fail(EM_ERR_INVALID_ARG, "bad kernel strategy");
+    if (g->max_ports < 0 || g->max_source_edges < 0 || g->max_wave_samples < 0)
+        return fail(EM_ERR_INVALID_ARG, "negative source capacity");
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::zero_state() {
+    for (int a = 0; a < 12; ++a) CU(cudaMemsetAsync(c.field[a], 0, sizeof(R) * g.alloc_elems, stream));
+    CU(cudaMemsetAsync(c.q, 0, sizeof(R) * g.alloc_elems, stream));
+    e_cur = h_cur = 0; bind();
+    step_index = 0;
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material *tab, int32_t n_mat, double dt_,
+                     void *workspace, size_t ws_bytes, void *stream_) {
+    grid = *gr; grid.dx = grid.dy = grid.dz = nullptr;
+    g = make_geometry(gr->nx, gr->ny, gr->nz);
+    loss = gr->loss_mode; dt = dt_;
+    stream = static_cast<cudaStream_t>(stream_);
+    plan = em::make_fused_plan(g.nx, g.ny, g.nz, (int)sizeof(R));
+    kernel = gr->kernel == EM_KERNEL_AUTO ? EM_KERNEL_SPLIT : gr->kernel;
+    const size_t need = carve<R>(g, *gr, nullptr, nullptr, plan.n_tiles);
+    if (ws_bytes < need) return fail(EM_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
+    carve<R>(g, *gr, workspace, &c, plan.n_tiles);
+    main_kernel = kernel == EM_KERNEL_FUSED ? "k_fused_sweep" : "k_split_e";
+
+    // ---- material table -> (eps/dt, sigma, mask, dt/mu), built in fp64, rounded once ----------
+    table.assign(tab, tab + n_mat);
+    std::vector<em::MatEntry<R>> ht(n_mat + 1);
+    fixed_cell.assign(n_mat + 1, 0);
+    for (int m = 0; m < n_mat; ++m) {
+        const bool pec = (tab[m].flags & EM_MAT_PEC) != 0;
+        ht[m].a = (R)(tab[m].eps / dt); ht[m].b = (R)tab[m].sigma;
+        ht[m].m = pec ? R(0) : R(1); ht[m].n = (R)(dt / tab[m].mu);
+        fixed_cell[m] = pec;
+    }
+    ht[n_mat].a = R(1); ht[n_mat].b = R(0); ht[n_mat].m = R(0); ht[n_mat].n = R(0);
+    fixed_cell[n_mat] = 1;
+    CU(cudaMemcpyAsync(c.table, ht.data(), sizeof(em::MatEntry<R>) * (n_mat + 1), cudaMemcpyHostToDevice, stream));
+
+    // ---- per-axis arrays, index -1 .. n+1 (+ slack), fp64 then rounded once -------------------
+    const double *d[3] = {gr->dx, gr->dy, gr->dz};
+    const int n[3] = {g.nx, g.ny, g.nz};
+    const int len[3] = {g.PX + 2, g.PY + 2, g.PZ + 2};
+    std::vector<std::vector<R>> hax(9);
+    for (int a = 0; a < 3; ++a) {
+        auto dd = [&](int i) { return (i >= 0 && i < n[a]) ? d[a][i] : 0.0; };
+        std::vector<R> rd(len[a], R(0)), rt(len[a], R(0)), f(len[a], R(0));
+        for (int s = 0; s < len[a]; ++s) {
+            const int i = s - 1;
+            if (i >= 0 && i < n[a]) rd[s] = (R)(1.0 / d[a][i]);
+            const double lo = dd(i - 1), hi = dd(i);
+            if (lo + hi > 0.0) { rt[s] = (R)(2.0 / (lo + hi)); f[s] = (R)(hi / (lo + hi)); }
+        }
+        hax[a * 3 + 0] = rd; hax[a * 3 + 1] = rt; hax[a * 3 + 2] = f;
+    }
+    for (int a = 0; a < 9; ++a)
+        CU(cudaMemcpyAsync(c.axis[a], hax[a].data(), sizeof(R) * hax[a].size(), cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(c.vx, gr->dx, sizeof(double) * g.nx, cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(c.vy, gr->dy, sizeof(double) * g.ny, cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(c.vz, gr->dz, sizeof(double) * g.nz, cudaMemcpyHostToDevice, stream));
+
+    // ---- material ids: halo = "outside" id n_mat, interior copied with a pitched 3-D copy ------
+    CU(cudaMemsetAsync(c.mat, n_mat, g.alloc_elems, stream));
+    {
+        cudaMemcpy3DParms m = {};
+        m.srcPtr = make_cudaPitchedPtr(const_cast<uint8_t *>(mat_id), g.nx, g.nx, g.ny);
+        m.dstPtr = make_cudaPitchedPtr(c.mat + g.origin, g.PX, g.PX, g.PY);
+        m.extent = make_cudaExtent(g.nx, g.ny, g.nz);
+        m.kind = cudaMemcpyHostToDevice;
+        CU(cudaMemcpy3DAsync(&m, stream));
+    }
+    host_mat.assign(mat_id, mat_id + (size_t)g.nx * g.ny * g.nz);
+    uniform_mu = true;
+    {
+        std::vector<char> used(n_mat, 0);
+        for (uint8_t v : host_mat) used[v] = 1;
+        double mu0 = -1;
+        for (int m = 0; m < n_mat; ++m) if (used[m]) { if (mu0 < 0) mu0 = tab[m].mu; else if (tab[m].mu != mu0) uniform_mu = false; }
+    }
+
+    // ---- device parameter block -----------------------------------------------------------------
+    p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.PX = g.PX; p.PY = g.PY; p.PXY = g.PXY;
+    p.q = c.q + g.origin; p.mat = c.mat + g.origin; p.table = c.table; p.n_table = n_mat + 1;
+    p.rdx = c.axis[0] + 1; p.rtx = c.axis[1] + 1; p.fx = c.axis[2] + 1;
+    p.rdy = c.axis[3] + 1; p.rty = c.axis[4] + 1; p.fy = c.axis[5] + 1;
+    p.rdz = c.axis[6] + 1; p.rtz = c.axis[7] + 1; p.fz = c.axis[8] + 1;
+    p.dt = (R)dt;
+    src = em::DevSources<R>{};
+    src.n_unique = 0;
+    CU(cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (plan.n_tiles + 1), stream));
+    int32_t rc = zero_state();
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(stream));
+    return EM_OK;
+}
+
+// ---- sources ------------------------------------------------------------------------------------
+template <typename R>
+int32_t Ctx<R>::set_source(int32_t np, const em_port *ports, const em_edge *edges, int64_t ne,
+                           const double *wave, int64_t ns) {
+    if (np < 0 || ne < 0 || ns < 0) return fail(EM_ERR_INVALID_ARG, "negative count");
+    if ((np && !ports) || (ne && !edges) || (ns && !wave)) return fail(EM_ERR_INVALID_ARG, "null source array");
+    if (np > grid.max_ports || ne > grid.max_source_edges || ns > grid.max_wave_samples)
+        return fail(EM_ERR_WORKSPACE_TOO_SMALL, "source set exceeds the capacities given to em_create");
+    for (int64_t e = 0; e < ne; ++e) {
+        if (edges[e].comp < 0 || edges[e].comp > 2) return fail(EM_ERR_INVALID_ARG, "edge comp must be 0..2");
+        int sx, sy, sz; comp_dims(edges[e].comp, &sx, &sy, &sz);
+        if (edges[e].i < 0 || edges[e].i >= sx || edges[e].j < 0 || edges[e].j >= sy || edges[e].k < 0 || edges[e].k >= sz)
+            return fail(EM_ERR_INVALID_ARG, "source edge outside the grid");
+    }
+    for (int q = 0; q < np; ++q) {
+        if (ports[q].edge_begin < 0 || ports[q].edge_end < ports[q].edge_begin || ports[q].edge_end > ne)
+            return fail(EM_ERR_INVALID_ARG, "port edge range");
+        if (ports[q].wave_offset < 0 || ports[q].wave_len < 0 || ports[q].wave_offset + ports[q].wave_len > ns)
+            return fail(EM_ERR_INVALID_ARG, "port waveform range");
+    }
+    // contributions (edge, port) sorted by tile of the fused sweep, then by offset: unique edges own
+    // their contributions in input order, so overlapping ports add deterministically
+    struct Con { long long off; int comp, port, tile; R scale; int64_t seq; };
+    std::vector<Con> cons;
+    for (int q = 0; q < np; ++q)
+        for (int64_t e = ports[q].edge_begin; e < ports[q].edge_end; ++e) {
+            Con cn;
+            cn.off = ((long long)edges[e].k * g.PY + edges[e].j) * g.PX + edges[e].i;
+            cn.comp = edges[e].comp; cn.port = q; cn.scale = (R)(ports[q].amplitude * edges[e].weight);
+            cn.tile = em::tile_of(plan, edges[e].i, edges[e].j, edges[e].k);
+            cn.seq = (int64_t)cons.size();
+            cons.push_back(cn);
+        }
+    if ((int64_t)cons.size() > grid.max_source_edges)
+        return fail(EM_ERR_WORKSPACE_TOO_SMALL, "more (edge, port) pairs than max_source_edges");
+    std::sort(cons.begin(), cons.end(), [](const Con &a, const Con &b) {
+        if (a.tile != b.tile) return a.tile < b.tile;
+        if (a.off != b.off) return a.off < b.off;
+        if (a.comp != b.comp) return a.comp < b.comp;
+        return a.seq < b.seq;
+    });
+    std::vector<long long> u_off; std::vector<int> u_comp, u_cbeg, c_port, u_tile; std::vector<R> c_scale;
+    for (size_t s = 0; s < cons.size(); ++s) {
+        if (s == 0 || cons[s].off != cons[s - 1].off || cons[s].comp != cons[s - 1].comp) {
+            u_off.push_back(cons[s].off); u_comp.push_back(cons[s].comp); u_cbeg.push_back((int)s); u_tile.push_back(cons[s].tile);
+        }
+        c_port.push_back(cons[s].port); c_scale.push_back(cons[s].scale);
+    }
+    u_cbeg.push_back((int)cons.size());
+    const int nu = (int)u_off.size();
+    std::vector<int> tile_beg(plan.n_tiles + 1, 0);
+    for (int u = 0; u < nu; ++u) tile_beg[u_tile[u] + 1] += 1;
+    for (int t = 0; t < plan.n_tiles; ++t) tile_beg[t + 1] += tile_beg[t];
+    std::vector<long long> woff(std::max(np, 1)), wlen(std::max(np, 1));
+    for (int q = 0; q < np; ++q) { woff[q] = ports[q].wave_offset; wlen[q] = ports[q].wave_len; }
+    std::vector<R> hw((size_t)std::max<int64_t>(ns, 1));
+    for (int64_t s = 0; s < ns; ++s) hw[s] = (R)wave[s];
+
+    CU(cudaStreamSynchronize(stream));
+    if (nu) {
+        CU(cudaMemcpyAsync(c.src_off, u_off.data(), sizeof(long long) * nu, cudaMemcpyHostToDevice, stream));
+        CU(cudaMemcpyAsync(c.src_comp, u_comp.data(), sizeof(int) * nu, cudaMemcpyHostToDevice, stream));
+        CU(cudaMemcpyAsync(c.con_port, c_port.data(), sizeof(int) * c_port.size(), cudaMemcpyHostToDevice, stream));
+        CU(cudaMemcpyAsync(c.con_scale, c_scale.data(), sizeof(R) * c_scale.size(), cudaMemcpyHostToDevice, stream));
+    }
+    CU(cudaMemcpyAsync(c.src_cbeg, u_cbeg.data(), sizeof(int) * (nu + 1), cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(c.tile_sbeg, tile_beg.data(), sizeof(int) * (plan.n_tiles + 1), cudaMemcpyHostToDevice, stream));
+    if (np) {
+        CU(cudaMemcpyAsync(c.port_woff, woff.data(), sizeof(long long) * np, cudaMemcpyHostToDevice, stream));
+        CU(cudaMemcpyAsync(c.port_wlen, wlen.data(), sizeof(long long) * np, cudaMemcpyHostToDevice, stream));
+    }
+    if (ns) CU(cudaMemcpyAsync(c.wave, hw.data(), sizeof(R) * ns, cudaMemcpyHostToDevice, stream));
+    src.n_unique = nu; src.off = c.src_off; src.comp = c.src_comp; src.r = c.src_r; src.cbeg = c.src_cbeg;
+    src.con_port = c.con_port; src.con_scale = c.con_scale; src.port_woff = c.port_woff; src.port_wlen = c.port_wlen;
+    src.wave = c.wave;
+    n_unique = nu; n_ports = np;
+    if (nu) {
+        const int bs = 128, gs = (nu + bs - 1) / bs;
+        if (loss == EM_LOSS_CD) em::k_source_coef<R, 0><<<gs, bs, 0, stream>>>(p, src, c.src_flags);
+        else                    em::k_source_coef<R, 1><<<gs, bs, 0, stream>>>(p, src, c.src_flags);
+        CU(cudaGetLastError());
+        std::vector<int> flags(nu);
+        CU(cudaMemcpyAsync(flags.data(), c.src_flags, sizeof(int) * nu, cudaMemcpyDeviceToHost, stream));
+        CU(cudaStreamSynchronize(stream));
+        for (int u = 0; u < nu; ++u)
+            if (flags[u]) {
+                src.n_unique = 0; n_unique = 0;
+                cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (plan.n_tiles + 1), stream);
+                return fail(EM_ERR_INVALID_ARG, "a source edge is PEC-fixed");
+            }
+    }
+    CU(cudaStreamSynchronize(stream));
+    return EM_OK;
+}
+
+// ---- dense <-> padded copies ----------------------------------------------------------------------
+template <typename R>
+int32_t Ctx<R>::set_field(int32_t comp, const void *srcp, int32_t is_dev) {
+    if (comp < 0 || comp > 5 || !srcp) return fail(EM_ERR_INVALID_ARG, "set_field arguments");
+    int sx, sy, sz; comp_dims(comp, &sx, &sy, &sz);
+    cudaMemcpy3DParms m = {};
+    m.srcPtr = make_cudaPitchedPtr(const_cast<void *>(srcp), sizeof(R) * sx, sx, sy);
+    m.dstPtr = make_cudaPitchedPtr(comp_ptr(comp), sizeof(R) * g.PX, g.PX, g.PY);
+    m.extent = make_cudaExtent(sizeof(R) * sx, sy, sz);
+    m.kind = is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CU(cudaMemcpy3DAsync(&m, stream));
+    if (comp < 3) {
+        dim3 b(32, 8);
+        em::k_mask_fixed<R><<<node_grid(b, 1), b, 0, stream>>>(p, comp);
+        CU(cudaGetLastError());
+    }
+    if (!is_dev) CU(cudaStreamSynchronize(stream));
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::get_field(int32_t comp, void *dst, int32_t is_dev) {
+    if (comp < 0 || comp > 5 || !dst) return fail(EM_ERR_INVALID_ARG, "get_field arguments");
+    int sx, sy, sz; comp_dims(comp, &sx, &sy, &sz);
+    cudaMemcpy3DParms m = {};
+    m.srcPtr = make_cudaPitchedPtr(comp_ptr(comp), sizeof(R) * g.PX, g.PX, g.PY);
+    m.dstPtr = make_cudaPitchedPtr(dst, sizeof(R) * sx, sx, sy);
+    m.extent = make_cudaExtent(sizeof(R) * sx, sy, sz);
+    m.kind = is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    CU(cudaMemcpy3DAsync(&m, stream));
+    if (!is_dev) CU(cudaStreamSynchronize(stream));
+    return EM_OK;
+}
+
+// ---- time stepping ----------------------------------------------------------------------------------
+template <typename R>
+int32_t Ctx<R>::record_begin() {
+    if (!timing.enabled) return EM_OK;
+    if (timing.pending == kTimingRing) { int32_t rc = timing_flush(); if (rc) return rc; }
+    CU(cudaEventRecord(timing.beg[timing.head], stream));
+    return EM_OK;
+}
+template <typename R>
+int32_t Ctx<R>::record_end() {
+    if (!timing.enabled) return EM_OK;
+    CU(cudaEventRecord(timing.end[timing.head], stream));
+    timing.head = (timing.head + 1) % kTimingRing; timing.pending += 1;
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::step_split() {
+    dim3 b(32, 8);
+    em::k_split_h<R><<<node_grid(b, 1), b, 0, stream>>>(p);
+    int32_t rc = record_begin(); if (rc) return rc;
+    if (loss == EM_LOSS_CD) em::k_split_e<R, 0><<<node_grid(b, 1), b, 0, stream>>>(p);
+    else                    em::k_split_e<R, 1><<<node_grid(b, 1), b, 0, stream>>>(p);
+    rc = record_end(); if (rc) return rc;
+    launches += 2;
+    if (n_unique) {
+        em::k_apply_source<R><<<(n_unique + 127) / 128, 128, 0, stream>>>(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
+        launches += 1;
+    }
+    em::k_split_joule<R><<<node_grid(b, 0), b, 0, stream>>>(p);
+    launches += 1;
+    CU(cudaGetLastError());
+    e_cur ^= 1; bind();
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::step_fused() {
+    int32_t rc = record_begin(); if (rc) return rc;
+    cudaError_t e = em::launch_fused<R>(plan, p, src, c.tile_sbeg, loss, uniform_mu, (long long)step_index, stream);
+    if (e != cudaSuccess) return fail(EM_ERR_CUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
+    rc = record_end(); if (rc) return rc;
+    launches += 1;
+    e_cur ^= 1; h_cur ^= 1; bind();
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::step(int64_t n) {
+    if (n < 0) return fail(EM_ERR_INVALID_ARG, "n < 0");
+    for (int64_t s = 0; s < n; ++s) {
+        int32_t rc = (kernel == EM_KERNEL_FUSED) ? step_fused() : step_split();
+        if (rc) return rc;
+        step_index += 1;
+    }
+    return EM_OK;
+}
+
+// ---- outputs ----------------------------------------------------------------------------------------
+template <typename R>
+int32_t Ctx<R>::joule(void *power, void *energy, double *total, int32_t do_reset) {
+    dim3 b(32, 8);
+    if (power) {
+        em::k_power<R><<<node_grid(b, 0), b, 0, stream>>>(p, static_cast<R *>(power));
+        CU(cudaGetLastError()); launches += 1;
+    }
+    if (energy) {
+        cudaMemcpy3DParms m = {};
+        m.srcPtr = make_cudaPitchedPtr(p.q, sizeof(R) * g.PX, g.PX, g.PY);
+        m.dstPtr = make_cudaPitchedPtr(energy, sizeof(R) * g.nx, g.nx, g.ny);
+        m.extent = make_cudaExtent(sizeof(R) * g.nx, g.ny, g.nz);
+        m.kind = cudaMemcpyDeviceToDevice;
+        CU(cudaMemcpy3DAsync(&m, stream));
+    }
+    if (total) {
+        em::k_energy_partial<R><<<kReduceBlocks, 256, 0, stream>>>(p, c.vx, c.vy, c.vz, c.partial);
+        em::k_energy_final<<<1, 256, 0, stream>>>(c.partial, kReduceBlocks, c.scalar);
+        CU(cudaGetLastError()); launches += 2;
+        CU(cudaMemcpyAsync(total, c.scalar, sizeof(double), cudaMemcpyDeviceToHost, stream));
+        CU(cudaStreamSynchronize(stream));
+    }
+    if (do_reset) CU(cudaMemsetAsync(c.q, 0, sizeof(R) * g.alloc_elems, stream));
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::probe(int32_t n, const em_probe_pt *pts, double *out) {
+    if (n < 0 || (n && (!pts || !out))) return fail(EM_ERR_INVALID_ARG, "probe arguments");
+    for (int q = 0; q < n; ++q) {
+        if (pts[q].comp < 0 || pts[q].comp > 5) return fail(EM_ERR_INVALID_ARG, "probe comp must be 0..5");
+        int sx, sy, sz; comp_dims(pts[q].comp, &sx, &sy, &sz);
+        if (pts[q].i < 0 || pts[q].i >= sx || pts[q].j < 0 || pts[q].j >= sy || pts[q].k < 0 || pts[q].k >= sz)
+            return fail(EM_ERR_INVALID_ARG, "probe point outside the grid");
+    }
+    em::ProbeArrays<R> pa;
+    for (int a = 0; a < 3; ++a) { pa.f[a] = p.E[a]; pa.f[3 + a] = p.H[a]; }
+    std::vector<long long> off(kProbeChunk); std::vector<int> comp(kProbeChunk);
+    for (int base = 0; base < n; base += kProbeChunk) {
+        const int m = std::min(kProbeChunk, n - base);
+        for (int q = 0; q < m; ++q) {
+            const em_probe_pt &pt = pts[base + q];
+            off[q] = ((long long)pt.k * g.PY + pt.j) * g.PX + pt.i; comp[q] = pt.comp;
+        }
+        CU(cudaMemcpyAsync(c.probe_off, off.data(), sizeof(long long) * m, cudaMemcpyHostToDevice, stream));
+        CU(cudaMemcpyAsync(c.probe_comp, comp.data(), sizeof(int) * m, cudaMemcpyHostToDevice, stream));
+        em::k_probe<R><<<(m + 127) / 128, 128, 0, stream>>>(pa, c.probe_off, c.probe_comp, m, c.probe_out);
+        CU(cudaGetLastError()); launches += 1;
+        CU(cudaMemcpyAsync(out + base, c.probe_out, sizeof(double) * m, cudaMemcpyDeviceToHost, stream));
+        CU(cudaStreamSynchronize(stream));
+    }
+    return EM_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+const char *em_last_error(void) { return g_err.c_str(); }
+
+int32_t em_workspace_bytes(const em_grid *gr, size_t *out) {
+    if (!out) return fail(EM_ERR_INVALID_ARG, "out is null");
+    int32_t rc = validate_grid(gr); if (rc) return rc;
+    const Geometry g = make_geometry(gr->nx, gr->ny, gr->nz);
+    const em::FusedPlan plan = em::make_fused_plan(g.nx, g.ny, g.nz, gr->precision / 8);
+    *out = gr->precision == 32 ? carve<float>(g, *gr, nullptr, nullptr, plan.n_tiles)
+                               : carve<double>(g, *gr, nullptr, nullptr, plan.n_tiles);
+    return EM_OK;
+}
+
+int32_t em_cfl_dt(const em_grid *gr, const uint8_t *mat_id, const em_material *tab, int32_t n_mat, double *dt_max) {
+    if (!gr || !mat_id || !tab || !dt_max || !gr->dx || !gr->dy || !gr->dz) return fail(EM_ERR_INVALID_ARG, "null argument");
+    if (gr->nx < 1 || gr->ny < 1 || gr->nz < 1 || n_mat < 1 || n_mat > 255) return fail(EM_ERR_INVALID_ARG, "bad sizes");
+    std::vector<double> slow(n_mat);
+    for (int m = 0; m < n_mat; ++m) slow[m] = std::sqrt(tab[m].eps * tab[m].mu);
+    double best = INFINITY;
+    for (int k = 0; k < gr->nz; ++k) {
+        const double gz = 1.0 / (gr->dz[k] * gr->dz[k]);
+        for (int j = 0; j < gr->ny; ++j) {
+            const double gyz = gz + 1.0 / (gr->dy[j] * gr->dy[j]);
+            const uint8_t *row = mat_id + ((size_t)k * gr->ny + j) * gr->nx;
+            for (int i = 0; i < gr->nx; ++i) {
+                if (row[i] >= n_mat) return fail(EM_ERR_INVALID_ARG, "material id >= n_mat");
+                const double v = slow[row[i]] / std::sqrt(gyz + 1.0 / (gr->dx[i] * gr->dx[i]));
+                if (v < best) best = v;
+            }
+        }
+    }
+    *dt_max = best;
+    return EM_OK;
+}
+
+int32_t em_create(const em_grid *gr, const uint8_t *mat_id, const em_material *tab, int32_t n_mat, double dt,
+                  void *workspace, size_t ws_bytes, void *stream, em_ctx **out) {
+    if (!out) return fail(EM_ERR_INVALID_ARG, "out is null");
+    *out = nullptr;
+    int32_t rc = validate_grid(gr); if (rc) return rc;
+    if (!mat_id || !tab || !gr->dx || !gr->dy || !gr->dz) return fail(EM_ERR_INVALID_ARG, "null input array");
+    if (n_mat < 1 || n_mat > 255) return fail(EM_ERR_INVALID_ARG, "n_mat must be 1..255");
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(EM_ERR_INVALID_ARG, "dt must be > 0");
+    for (int b = 0; b < 6; ++b) {
+        if (gr->bc[b] == EM_BC_PMC) return fail(EM_ERR_UNSUPPORTED, "PMC walls are not implemented");
+        if (gr->bc[b] != EM_BC_PEC) return fail(EM_ERR_INVALID_ARG, "unknown boundary condition");
+    }
+    for (int m = 0; m < n_mat; ++m)
+        if (!(tab[m].eps > 0.0) || !(tab[m].mu > 0.0) || !(tab[m].sigma >= 0.0) || !std::isfinite(tab[m].eps + tab[m].mu + tab[m].sigma))
+            return fail(EM_ERR_INVALID_ARG, "material table: need eps > 0, mu > 0, sigma >= 0");
+    const double *d[3] = {gr->dx, gr->dy, gr->dz}; const int n[3] = {gr->nx, gr->ny, gr->nz};
+    for (int a = 0; a < 3; ++a) for (int i = 0; i < n[a]; ++i)
+        if (!(d[a][i] > 0.0) || !std::isfinite(d[a][i])) return fail(EM_ERR_INVALID_ARG, "cell sizes must be > 0");
+    const size_t ncell = (size_t)gr->nx * gr->ny * gr->nz;
+    for (size_t q = 0; q < ncell; ++q) if (mat_id[q] >= n_mat) return fail(EM_ERR_INVALID_ARG, "material id >= n_mat");
+    if (!workspace) return fail(EM_ERR_INVALID_ARG, "workspace is null");
+    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return fail(EM_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return fail(EM_ERR_CUDA, "no CUDA device");
+    em_ctx *ctx = nullptr;
+    if (gr->precision == 32) {
+        auto *c = new Ctx<float>(); ctx = c;
+        rc = c->init(gr, mat_id, tab, n_mat, dt, workspace, ws_bytes, stream);
+    } else {
+        auto *c = new Ctx<double>(); ctx = c;
+        rc = c->init(gr, mat_id, tab, n_mat, dt, workspace, ws_bytes, stream);
+    }
+    if (rc) { delete ctx; return rc; }
+    *out = ctx;
+    return EM_OK;
+}
+
+int32_t em_destroy(em_ctx *ctx) {
+    if (!ctx) return EM_OK;
+    for (auto e : ctx->timing.beg) cudaEventDestroy(e);
+    for (auto e : ctx->timing.end) cudaEventDestroy(e);
+    delete ctx;
+    return EM_OK;
+}
+
+#define EM_CHECK_CTX if (!ctx) return fail(EM_ERR_INVALID_ARG, "ctx is null")
+
+int32_t em_set_source(em_ctx *ctx, int32_t n_ports, const em_port *ports, const em_edge *edges, int64_t n_edges,
+                      const double *wave, int64_t n_samples) {
+    EM_CHECK_CTX; return ctx->set_source(n_ports, ports, edges, n_edges, wave, n_samples);
+}
+int32_t em_set_field(em_ctx *ctx, int32_t comp, const void *src, int32_t is_dev) { EM_CHECK_CTX; return ctx->set_field(comp, src, is_dev); }
+int32_t em_get_field(em_ctx *ctx, int32_t comp, void *dst, int32_t is_dev) { EM_CHECK_CTX; return ctx->get_field(comp, dst, is_dev); }
+int32_t em_step(em_ctx *ctx, int64_t n) { EM_CHECK_CTX; return ctx->step(n); }
+int32_t em_joule(em_ctx *ctx, void *p, void *q, double *t, int32_t reset) { EM_CHECK_CTX; return ctx->joule(p, q, t, reset); }
+int32_t em_probe(em_ctx *ctx, int32_t n, const em_probe_pt *pts, double *out) { EM_CHECK_CTX; return ctx->probe(n, pts, out); }
+int32_t em_reset(em_ctx *ctx) { EM_CHECK_CTX; return ctx->reset(); }
+int32_t em_step_index(em_ctx *ctx, int64_t *n) { EM_CHECK_CTX; if (!n) return fail(EM_ERR_INVALID_ARG, "null"); *n = ctx->step_index; return EM_OK; }
+int32_t em_launch_count(em_ctx *ctx, int64_t *n) { EM_CHECK_CTX; if (!n) return fail(EM_ERR_INVALID_ARG, "null"); *n = ctx->launches; return EM_OK; }
+
+int32_t em_timing_enable(em_ctx *ctx, int32_t enable) {
+    EM_CHECK_CTX;
+    Timing &t = ctx->timing;
+    if (enable && t.beg.empty()) {
+        t.beg.resize(kTimingRing); t.end.resize(kTimingRing);
+        for (int i = 0; i < kTimingRing; ++i) { CU(cudaEventCreate(&t.beg[i])); CU(cudaEventCreate(&t.end[i])); }
+    }
+    int32_t rc = ctx->timing_flush(); if (rc) return rc;
+    t.enabled = enable != 0; t.launches = 0; t.ms = 0.0;
+    return EM_OK;
+}
+
+int32_t em_timing_read(em_ctx *ctx, const char **name, int64_t *launches, double *ms) {
+    EM_CHECK_CTX;
+    int32_t rc = ctx->timing_flush(); if (rc) return rc;
+    if (name) *name = ctx->main_kernel;
+    if (launches) *launches = ctx->timing.launches;
+    if (ms) *ms = ctx->timing.ms;
+    return EM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,264 @@
+"""GPU-vs-oracle parity (all through the C ABI).  Tolerances are BASELINE.json north_star's:
+relative L2 <= 1e-12 (fp64) and <= 2e-5 (fp32) for E, H, the Joule map and the Joule total."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import workloads as W
+from workloads.problem import LOSS_CD, LOSS_EXP, C0
+import paper_2603_07038_b200 as P
+from oracle import emo
+from parity import TOL, compare_state, rel_l2, subbox_problem
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [pytest.param(P.EM_KERNEL_SPLIT, id="split"), pytest.param(P.EM_KERNEL_FUSED, id="fused")]
+KNAME = {P.EM_KERNEL_SPLIT: "split", P.EM_KERNEL_FUSED: "fused"}
+
+
+def run_pair(p, steps, precision, kernel, checkpoints=()):
+    g = P.EM(p, precision=precision, kernel=kernel)
+    o = emo.Oracle(p)
+    tol = TOL[precision]
+    done = 0
+    res = None
+    for cp in list(checkpoints) + [steps]:
+        g.em_step(cp - done); o.step(cp - done); done = cp
+        res = compare_state(g, o, tol)
+    assert g.step_index == steps
+    g.close(); o.close()
+    return res
+
+
+# ------------------------------------------------------------------------------ worked examples
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("precision", [64, 32])
+def test_impulse_example(kernel, precision):
+    p = W.impulse_problem()
+    run_pair(p, 3, precision, kernel, checkpoints=(1, 2))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config1_cavity_te101(kernel):
+    """config 1: 16^3 PEC cavity, fp64, 1000 steps; also checks the GPU against the closed form."""
+    p = W.config1_cavity()
+    g = P.EM(p, precision=64, kernel=kernel)
+    o = emo.Oracle(p)
+    n, h, dt = 16, 1.0e-3, p.dt
+    s = math.sin(math.pi / (2 * n))
+    w_num = (2.0 / dt) * math.asin(C0 * dt * math.sqrt(2 * s * s / (h * h)))
+    tr = [g.em_probe(p.probes)[0]]
+    for _ in range(10):
+        g.em_step(100); o.step(100)
+        tr.append(g.em_probe(p.probes)[0])
+    want = np.cos(w_num * dt * 100 * np.arange(11))
+    assert np.max(np.abs(np.asarray(tr) - want)) < 2e-12
+    res = compare_state(g, o, 1e-12)
+    assert res["Q"] == 0.0
+    g.close()
+
+
+# ------------------------------------------------------------- randomised heterogeneous grids
+SMALL = [(37, 29, 23), (1, 5, 7), (130, 3, 2), (5, 1, 9), (6, 7, 1), (1, 1, 1), (2, 2, 2), (33, 65, 4), (64, 17, 40)]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("dims", SMALL)
+def test_random_grids_cd(dims, precision, kernel):
+    p = W.random_problem(*dims, seed=1000 + sum(dims), loss_mode=LOSS_CD, steps=40, n_ports=3)
+    run_pair(p, 40, precision, kernel, checkpoints=(1, 10))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("dims", [(37, 29, 23), (9, 4, 70)])
+def test_random_grids_exp(dims, precision, kernel):
+    p = W.random_problem(*dims, seed=2000 + sum(dims), loss_mode=LOSS_EXP, steps=40, n_ports=3)
+    run_pair(p, 40, precision, kernel, checkpoints=(1,))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_random_grid_percell_ids_and_pec_material(kernel):
+    p = W.random_problem(21, 19, 17, seed=3001, blocky=False, steps=30, n_ports=2)
+    run_pair(p, 30, 64, kernel)
+    p = W.random_problem(21, 19, 17, seed=3002, pec_material=True, steps=30, n_ports=0)
+    run_pair(p, 30, 64, kernel)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_overlapping_ports_add(kernel):
+    p = W.random_problem(9, 8, 7, seed=3003, steps=12, n_ports=2)
+    # make port 1 drive the same edges as port 0 (contributions add, C14)
+    e0 = slice(int(p.port_edge_begin[0]), int(p.port_edge_end[0]))
+    n0 = e0.stop - e0.start
+    p.edge_comp = np.concatenate([p.edge_comp[e0], p.edge_comp[e0]])
+    p.edge_ijk = np.concatenate([p.edge_ijk[e0], p.edge_ijk[e0]])
+    p.edge_weight = np.concatenate([p.edge_weight[e0], -0.5 * p.edge_weight[e0]])
+    p.port_edge_begin = np.asarray([0, n0], np.int64); p.port_edge_end = np.asarray([n0, 2 * n0], np.int64)
+    run_pair(p, 12, 64, kernel)
+
+
+# --------------------------------------------------------------------- the five configurations
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config2_slab_scaled_full_steps(kernel):
+    """config 2 at 32x32x64 (oracle in seconds), all 5000 steps, fp64, EXP loss."""
+    p = W.make_config(2, scale=4)
+    res = run_pair(p, p.steps, 64, kernel, checkpoints=(1, 10))
+    assert res["Q"] <= 1e-12
+
+
+def test_config2_slab_full_size():
+    """config 2 at its full 128x128x64 size, 250 steps (bounded for the oracle)."""
+    p = W.make_config(2, steps=250)
+    run_pair(p, 250, 64, P.EM_KERNEL_AUTO)
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("kappa", [1.0, 100.0])
+def test_config3_interposer_scaled(precision, kappa):
+    p = W.make_config(3, scale=4, steps=400, kappa=kappa, precision=precision)
+    run_pair(p, 400, precision, P.EM_KERNEL_AUTO, checkpoints=(10,))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_config4_package_scaled(kernel):
+    p = W.make_config(4, scale=8, zscale=2, steps=300)
+    g = P.EM(p, precision=32, kernel=kernel)
+    o = emo.Oracle(p)
+    for _ in range(3):                    # Joule map output every 100 steps, as in the config
+        g.em_step(100); o.step(100)
+        compare_state(g, o, TOL[32])
+    g.close()
+
+
+def test_config5_graded_scaled():
+    p = W.make_config(5, scale=8, zscale=4, steps=300)
+    assert p.dx.max() / p.dx.min() > 20
+    run_pair(p, 300, 32, P.EM_KERNEL_AUTO, checkpoints=(10,))
+    run_pair(p, 100, 64, P.EM_KERNEL_AUTO)
+
+
+# ------------------------------------------------- full BASELINE sizes: sampled light-cone parity
+def _fullsize_sampled(cfg, precision, n_steps=3, n_boxes=4, half=7, **kw):
+    """At the full configuration size in the launch configuration bench.py times: random device
+    initial state, n_steps on the GPU, then every output inside a few sample boxes is recomputed by
+    the oracle on the box enlarged by the domain of dependence (n_steps + 2 cells)."""
+    import torch
+    p = W.make_config(cfg, **kw)
+    g = P.EM(p, precision=precision, kernel=P.EM_KERNEL_AUTO)
+    gen = torch.Generator(device="cuda"); gen.manual_seed(1234 + cfg)
+    shapes = g.shapes
+    init = []
+    for c in range(6):
+        t = torch.randn(shapes[c], generator=gen, device="cuda", dtype=g.dtype)
+        if c >= 3:
+            t /= 376.73
+        g.em_set_field(c, t)
+        init.append(g.em_get_field(c, device=True).clone())     # after PEC masking
+        del t
+    g.em_step(n_steps)
+    out = [g.em_get_field(c, device=True) for c in range(6)]
+    qmap = torch.empty((p.nz, p.ny, p.nx), dtype=g.dtype, device="cuda")
+    g.em_joule(None, qmap, total=False)
+    rng = np.random.default_rng(77 + cfg)
+    m = n_steps + 2
+    centres = []
+    if p.n_ports:                                                 # boxes at port edges first
+        for q in rng.choice(p.n_ports, size=min(2, p.n_ports), replace=False):
+            centres.append(tuple(int(v) for v in p.edge_ijk[int(p.port_edge_begin[q])]))
+    while len(centres) < n_boxes:
+        centres.append((int(rng.integers(0, p.nx)), int(rng.integers(0, p.ny)), int(rng.integers(0, p.nz))))
+    centres.append((0, 0, 0)); centres.append((p.nx - 1, p.ny - 1, p.nz - 1))
+    worst = 0.0
+    for (ci, cj, ck) in centres:
+        core_lo = [max(0, ci - half), max(0, cj - half), max(0, ck - half)]
+        core_hi = [min(p.nx, ci + half), min(p.ny, cj + half), min(p.nz, ck + half)]
+        lo = [max(0, v - m) for v in core_lo]
+        hi = [min(n, v + m) for v, n in zip(core_hi, (p.nx, p.ny, p.nz))]
+        (i0, j0, k0), (i1, j1, k1) = lo, hi
+        ext = [(0, 1, 1), (1, 0, 1), (1, 1, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1)]     # +1 per axis (x, y, z)
+        sub = lambda arr, c: arr[k0:k1 + ext[c][2], j0:j1 + ext[c][1], i0:i1 + ext[c][0]].cpu().numpy()
+        bp = subbox_problem(p, lo, hi, [sub(init[c], c) for c in range(6)])
+        o = emo.Oracle(bp)
+        o.step(n_steps)
+        Fo = o.fields()
+        _, qo, _ = o.joule()
+        # compare only the core (unaffected by the artificial PEC walls of the box)
+        a = [core_lo[d] - lo[d] for d in range(3)]; b = [core_hi[d] - lo[d] for d in range(3)]
+        sl = lambda f: f[a[2]:b[2], a[1]:b[1], a[0]:b[0]]
+        got = [sl(sub(out[c], c)) for c in range(6)]
+        want = [sl(Fo[c]) for c in range(6)]
+        eE = rel_l2(got[:3], want[:3]); eH = rel_l2(got[3:], want[3:])
+        qg = qmap[k0:k1, j0:j1, i0:i1].cpu().numpy()
+        eq = rel_l2([sl(qg)], [sl(qo)])
+        worst = max(worst, eE, eH, eq)
+        assert eE <= TOL[precision] and eH <= TOL[precision] and eq <= TOL[precision], ((ci, cj, ck), eE, eH, eq)
+    g.close()
+    return worst
+
+
+def test_fullsize_sampled_config3_fp32():
+    _fullsize_sampled(3, 32)
+
+
+def test_fullsize_sampled_config3_fp64():
+    _fullsize_sampled(3, 64)
+
+
+def test_fullsize_sampled_config4_fp32():
+    _fullsize_sampled(4, 32)
+
+
+def test_fullsize_sampled_config5_fp32():
+    _fullsize_sampled(5, 32)
+
+
+# ------------------------------------------------------------------------------ C-ABI contract
+def test_api_contract():
+    p = W.random_problem(12, 11, 10, seed=4001, steps=10, n_ports=2)
+    g = P.EM(p, precision=64)
+    F0 = g.fields()
+    g.em_step(0)
+    assert g.step_index == 0 and all(np.array_equal(a, b) for a, b in zip(F0, g.fields()))
+    # PEC-fixed tangential E is forced to 0 on set
+    assert np.all(F0[0][:, 0, :] == 0) and np.all(F0[0][0, :, :] == 0) and np.all(F0[2][:, :, 0] == 0)
+    # bad arguments
+    with pytest.raises(P.EMError):
+        g.em_probe([(0, p.nx, 0, 0)])
+    with pytest.raises(P.EMError):
+        g.em_step(-1)
+    bad = W.impulse_problem(); bad.edge_ijk = np.asarray([[2, 0, 1]], np.int32)
+    with pytest.raises(P.EMError):
+        P.EM(bad)
+    # capacities
+    with pytest.raises(P.EMError) as e:
+        P.EM(p, max_source_edges=1)
+    assert e.value.code == 2
+    # reset semantics of em_joule and em_reset
+    g.em_step(5)
+    _, q1, Q1 = g.joule_maps(reset=True)
+    _, q2, Q2 = g.joule_maps()
+    assert Q1 > 0 and Q2 == 0.0 and not q2.any()
+    g.em_reset()
+    assert g.step_index == 0 and not any(f.any() for f in g.fields())
+    # two contexts coexist; repeated create/destroy
+    for _ in range(3):
+        a, b = P.EM(p, precision=64), P.EM(p, precision=32)
+        a.em_step(2); b.em_step(2)
+        assert rel_l2(b.fields()[:3], a.fields()[:3]) < 1e-5
+        a.close(); b.close()
+    g.close()
+
+
+def test_probe_matches_fields():
+    p = W.random_problem(10, 9, 8, seed=4002, steps=5, n_ports=1)
+    g = P.EM(p, precision=64)
+    g.em_step(5)
+    F = g.fields()
+    vals = g.em_probe(p.probes)
+    for v, (c, i, j, k) in zip(vals, p.probes):
+        assert v == F[c][k, j, i]
+    g.close()

@@ -1,0 +1,81 @@
+"""CPU-side checks of the C-ABI library: it builds, loads and exports every symbol that include/em.h
+declares; host-only entry points work; device entry points fail loudly without a GPU."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import workloads as W
+import paper_2603_07038_b200 as P
+from paper_2603_07038_b200 import binding as B
+from oracle import emo
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "em.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = sorted(set(re.findall(r"\b(em_[a-z_]+)\s*\(", hdr)))
+    assert {"em_create", "em_set_source", "em_step", "em_joule", "em_probe"} <= set(names)
+    L = P.load()
+    for n in names:
+        assert hasattr(L, n), n
+
+
+def test_workspace_bytes_and_argument_errors():
+    n = P.em_workspace_bytes(1024, 1024, 192, 32, 256, 8192, 256000)
+    cells = 1024 * 1024 * 192
+    assert 13 * 4 * cells < n < 1.2 * (13 * 4 + 1) * cells + (64 << 20)
+    with pytest.raises(P.EMError) as e:
+        P.em_workspace_bytes(16, 16, 16, precision=16)
+    assert e.value.code == 1
+    with pytest.raises(P.EMError):
+        P.em_workspace_bytes(0, 16, 16)
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_cfl_dt_matches_oracle_and_generator(seed):
+    p = W.random_problem(9, 8, 7, seed=seed, n_ports=0)
+    a = P.em_cfl_dt(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, p.mat_id, p.table)
+    b = emo.cfl_dt(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, p.mat_id, p.table)
+    assert abs(a - b) <= 1e-15 * b
+    assert abs(0.9 * a - p.dt) <= 1e-14 * p.dt
+    p5 = W.make_config(5, scale=8, zscale=4)
+    a5 = P.em_cfl_dt(p5.nx, p5.ny, p5.nz, p5.dx, p5.dy, p5.dz, p5.mat_id, p5.table)
+    assert abs(0.9 * a5 - p5.dt) <= 1e-14 * p5.dt
+
+
+def test_create_validates_before_touching_the_device():
+    L = P.load()
+    p = W.random_problem(4, 4, 4, seed=3, n_ports=0)
+    g = B._mk_grid(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, 64)
+    tab = B._mk_table(p.table, p.flags)
+    h = C.c_void_p()
+    mat = np.ascontiguousarray(p.mat_id)
+    ws = C.c_void_p(256)
+
+    def create(grid=g, n_mat=16, dt=p.dt, m=mat, w=ws):
+        return L.em_create(C.byref(grid), m.ctypes.data_as(C.c_void_p), tab, n_mat, C.c_double(dt), w, 1 << 40, None, C.byref(h))
+    assert create(dt=0.0) == 1
+    assert create(n_mat=300) == 1
+    bad = mat.copy(); bad[0, 0, 0] = 99
+    assert create(m=bad) == 1
+    assert create(w=C.c_void_p(8)) == 1                      # misaligned workspace
+    assert create(w=None) == 1
+    gp = B._mk_grid(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, 64, bc=(1, 0, 0, 0, 0, 0))
+    assert create(grid=gp) == 5                              # PMC: EM_ERR_UNSUPPORTED
+    assert b"PMC" in L.em_last_error()
+    for fn in (L.em_step, L.em_reset):
+        assert fn(None, 1) == 1 if fn is L.em_step else fn(None) == 1
+
+
+def test_no_cpu_fallback_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    p = W.random_problem(4, 4, 4, seed=3, n_ports=0)
+    with pytest.raises(RuntimeError):
+        P.EM(p)
