@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py -- EM cell-updates/s of the hot path (H update + E update + source injection + Joule
+accumulation + PEC masks, one em_step) on the full-package config of BASELINE.json (config 4:
+1024 x 1024 x 192 cells, fp32, 16-entry material table, 256 bursty sources, Joule map output every
+100 steps), plus the roofline of the dominant kernel and the CPU-oracle baseline.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--scale 1] [--impl reference]
+
+N > 1 (torchrun): every rank runs an independent replica of the same problem ("replicas only":
+the path has no data-parallel split inside one problem that would not need a halo exchange; see
+DESIGN.md "Multi-GPU"); value = cells * steps * N / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+B_MIN = {32: 57, 64: 113}     # algorithmic bytes per cell-update (DESIGN.md / SURVEY.md 8(d))
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--scale", type=int, default=1)
+    ap.add_argument("--precision", type=int, default=0, help="0 = the config's own")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "split", "fused"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index = index; self.samples = []; self.stop_flag = False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [x.strip() for x in out.strip().split(",")]
+                if len(parts) >= 7:
+                    self.samples.append(parts)
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        sm = sorted(float(s[0]) for s in self.samples if s[0].replace(".", "").isdigit())
+        mx = [float(s[1]) for s in self.samples if s[1].replace(".", "").isdigit()]
+        reasons = set()
+        for s in self.samples:
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), s[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(self.samples)}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(kernel_name: str, cells: int):
+    """dram bytes per launch of the dominant kernel from the committed ncu summary, if any."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as f:
+            t = json.load(f)
+        ent = t.get(kernel_name)
+        if ent and ent.get("cells") == cells:
+            return float(ent["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
+def make_problem(args):
+    import workloads as W
+    kw = {}
+    if args.config in (4, 5):
+        kw["steps"] = max(args.steps + args.warmup, 1000) if args.scale == 1 else args.steps + args.warmup
+    elif args.config in (2, 3):
+        kw["steps"] = args.steps + args.warmup
+    if args.config == 1:
+        return W.make_config(1)
+    return W.make_config(args.config, scale=args.scale, **kw)
+
+
+# ------------------------------------------------------------------------------------------------
+def cpu_oracle_rate(args, seconds: float):
+    """The oracle as it stands, timed on the host cores on a bounded sample of the same workload."""
+    import workloads as W
+    from oracle import emo
+    threads = emo.set_threads(os.cpu_count() or 1)
+    scale = max(args.scale, 4) if args.config in (3, 4, 5) else 1
+    kw = {"steps": 64} if args.config != 1 else {}
+    p = W.make_config(args.config, scale=scale, **kw) if args.config != 1 else W.make_config(1)
+    o = emo.Oracle(p)
+    o.step(1)                                        # warm the pages
+    t0 = time.perf_counter(); n = 0
+    while True:
+        o.step(1); n += 1
+        el = time.perf_counter() - t0
+        if el >= seconds or n >= 60:
+            break
+    rate = p.n_cells * n / el
+    sample = "%s at %dx%dx%d cells (scale 1/%d in x,y), %d steps, fp64" % (p.name, p.nx, p.ny, p.nz, scale, n)
+    o.close()
+    return rate, threads, sample, el / n * 1e3, p
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    # bounded: K timed "steps", each = one oracle time step on the sample grid
+    import workloads as W
+    from oracle import emo
+    threads = emo.set_threads(os.cpu_count() or 1)
+    scale = max(args.scale, 4) if args.config in (3, 4, 5) else 1
+    K, Wm = args.steps, args.warmup
+    # keep the whole run within a few minutes: shrink further if K is large
+    while args.config in (3, 4, 5) and K * (1024 // scale) ** 2 * 192 / 1.5e8 > 150 and scale < 32:
+        scale *= 2
+    p = W.make_config(args.config, scale=scale, steps=K + Wm) if args.config != 1 else W.make_config(1)
+    o = emo.Oracle(p)
+    o.step(Wm)
+    t0 = time.perf_counter()
+    o.step(K)
+    el = time.perf_counter() - t0
+    val = p.n_cells * K / el
+    sample = "%s at %dx%dx%d cells (scale 1/%d in x,y), fp64 oracle" % (p.name, p.nx, p.ny, p.nz, scale)
+    line = {
+        "impl": "reference", "metric": "EM cell-updates/sec", "value": val, "unit": "cell-updates/s",
+        "n_gpus": args.gpus, "steps": K, "warmup": Wm, "ms_per_step": el / K * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config %d (%s), bounded sample: %s" % (args.config, p.name, sample)},
+        "cpu_baseline": {"value": val, "unit": "cell-updates/s", "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+def run_b200(args):
+    import numpy as np
+    import torch
+    import paper_2603_07038_b200 as P
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist = dist_
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+
+    p = make_problem(args)
+    precision = args.precision or p.precision
+    kernel = {"auto": P.EM_KERNEL_AUTO, "split": P.EM_KERNEL_SPLIT, "fused": P.EM_KERNEL_FUSED}[args.kernel]
+    K, Wm = args.steps, args.warmup
+    em = P.EM(p, precision=precision, kernel=kernel, device=dev)
+    cells = p.n_cells
+    je = p.joule_every if p.joule_every else 0
+    pw_map = torch.empty((p.nz, p.ny, p.nx), dtype=em.dtype, device=dev) if je else None
+    q_map = torch.empty((p.nz, p.ny, p.nx), dtype=em.dtype, device=dev) if je else None
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def run_steps(n, start):
+        """n steps with the config's Joule-map outputs (to device buffers) inside."""
+        done = 0
+        while done < n:
+            nxt = n - done
+            if je:
+                to_out = je - ((start + done) % je)
+                nxt = min(nxt, to_out)
+            em.em_step(nxt); done += nxt
+            if je and (start + done) % je == 0:
+                em.em_joule(pw_map, q_map, total=False)
+
+    # ---- device-resident timing ------------------------------------------------------------------
+    run_steps(Wm, 0)
+    em.em_timing_enable(True)
+    sampler = ClockSampler(local); sampler.start()
+    l0 = em.launch_count
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    run_steps(K, Wm)
+    ev1.record()
+    barrier()
+    sampler.stop_flag = True
+    ms = ev0.elapsed_time(ev1)
+    launches = em.launch_count - l0
+    kname, klaunch, kms = em.em_timing_read()
+    em.em_timing_enable(False)
+    if dist is not None:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = cells * K * world / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers -------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        shapes = em.shapes
+        host_in = [torch.zeros(s, dtype=em.dtype).pin_memory() for s in shapes]
+        rng = np.random.default_rng(7)
+        for c, h in enumerate(host_in):                      # small seeded seed field, not all zeros
+            h.view(-1)[:: max(1, h.numel() // 4096)] = float(rng.standard_normal()) * (1.0 if c < 3 else 1 / 376.73)
+        host_out = [torch.empty(s, dtype=em.dtype).pin_memory() for s in shapes]
+        host_q = torch.empty((p.nz, p.ny, p.nx), dtype=em.dtype).pin_memory()
+        probes = p.probes if len(p.probes) else np.asarray([[0, 0, 1, 1]], np.int32)
+        em.em_reset()
+        barrier()
+        t0 = time.perf_counter()
+        h2d = d2h = 0
+        for c in range(6):
+            em.em_set_field(c, host_in[c].numpy()); h2d += host_in[c].numel() * host_in[c].element_size()
+        done = 0
+        while done < K:
+            nxt = min(K - done, (je - (done % je)) if je else 64)
+            em.em_step(nxt); done += nxt
+            vals = em.em_probe(probes); d2h += vals.nbytes     # per-chunk read of the run's observable
+            if je and done % je == 0:
+                em.em_joule(pw_map, q_map, total=False)
+                host_q.copy_(q_map, non_blocking=False); d2h += host_q.numel() * host_q.element_size()
+        for c in range(6):
+            em.em_get_field(c, host_out[c].numpy()); d2h += host_out[c].numel() * host_out[c].element_size()
+        tot = em.em_joule(None, None, total=True); d2h += 8
+        torch.cuda.synchronize(dev)
+        el = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([el], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            el = float(t.item())
+        e2e = {"value": cells * K * world / el, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d / K,
+               "d2h_bytes_per_step": d2h / K,
+               "what": "em_set_field x6 from pinned host, %d x em_step with em_probe reads%s, em_get_field x6 + Joule total to host"
+                       % (K, " and Joule maps to host every %d steps" % je if je else "")}
+        del host_in, host_out, host_q
+
+    if rank != 0:
+        em.close()
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = measured_peak()
+    bmin = B_MIN[precision]
+    avg_ms = kms / max(klaunch, 1)
+    achieved = bmin * cells / (avg_ms * 1e-3) / 1e9 if klaunch else None
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak if achieved else None, "traffic": ncu_traffic(kname, cells),
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": bmin * cells,
+                "avg_launch_ms": avg_ms, "launches_timed": klaunch,
+                "step_effective_GBps": bmin * value / world / 1e9, "step_frac_of_peak": bmin * value / world / 1e9 / peak,
+                "frac_of_8TBps_nominal": (achieved / 8000.0) if achieved else None}
+    cpu = None
+    if not args.no_cpu_baseline:
+        rate, threads, sample, ms_cpu, _ = cpu_oracle_rate(args, args.cpu_seconds)
+        cpu = {"value": rate, "unit": "cell-updates/s", "cores": threads, "kind": "oracle", "sample": sample,
+               "ms_per_step_on_sample": ms_cpu}
+    line = {
+        "metric": "EM cell-updates/sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
+        "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32" if precision == 32 else "f64", "data": "synthetic",
+        "config": {"workload": "config %d: %s %dx%dx%d cells (%d), %d ports, %s loss, Joule map every %s steps"
+                               % (args.config, p.name, p.nx, p.ny, p.nz, cells, p.n_ports,
+                                  "EXP" if p.loss_mode else "CD", je or "-"),
+                   "kernel_strategy": args.kernel, "l2": "state %.1f GB >> 126 MB L2 (no flush needed)" % (em.workspace_bytes / 1e9)
+                   if em.workspace_bytes > 1e9 else "state fits L2: %.0f MB" % (em.workspace_bytes / 1e6),
+                   "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
+        "clocks": sampler.summary(),
+    }
+    print(json.dumps(line))
+    em.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()
