@@ -45,7 +45,7 @@ Geometry make_geometry(int nx, int ny, int nz) {
     g.vol = g.PXY * g.PZ;
     // one guard row in front (i = -1 of row j = -1, plane k = -1) and 2 behind (vector tails)
     g.origin = g.PX + g.PXY + g.PX;   // guard + plane k=-1 + row j=-1
-    g.alloc_elems = g.vol + 3LL * g.PX;
+    g.alloc_elems = g.vol + g.PX + std::max(2LL * g.PX, (long long)g.PX + 256);
     return g;
 }
 
@@ -79,7 +79,7 @@ struct Carved {
     long long *src_off; int *src_comp; R *src_r; int *src_cbeg; int *src_flags;
     int *con_port; R *con_scale; long long *port_woff, *port_wlen; R *wave;
     // fused-sweep tile source index
-    int *tile_sbeg;
+    int *tile_sbeg; int4 *tile_ent;
 };
 
 template <typename R>
@@ -104,6 +104,7 @@ size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int
     o.port_woff = w.take<long long>(mp); o.port_wlen = w.take<long long>(mp);
     o.wave = w.take<R>((size_t)std::max<int64_t>(gr.max_wave_samples, 1));
     o.tile_sbeg = w.take<int>((size_t)n_tiles + 1);
+    o.tile_ent = w.take<int4>(4 * me);
     return align_up(w.off);
 }
 
@@ -231,7 +232,7 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     loss = gr->loss_mode; dt = dt_;
     stream = static_cast<cudaStream_t>(stream_);
     plan = em::make_fused_plan(g.nx, g.ny, g.nz, (int)sizeof(R));
-    kernel = gr->kernel == EM_KERNEL_AUTO ? EM_KERNEL_SPLIT : gr->kernel;
+    kernel = gr->kernel == EM_KERNEL_AUTO ? EM_KERNEL_FUSED : gr->kernel;
     const size_t need = carve<R>(g, *gr, nullptr, nullptr, plan.n_tiles);
     if (ws_bytes < need) return fail(EM_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
     carve<R>(g, *gr, workspace, &c, plan.n_tiles);
@@ -330,36 +331,48 @@ int32_t Ctx<R>::set_source(int32_t np, const em_port *ports, const em_edge *edge
     }
     // contributions (edge, port) sorted by tile of the fused sweep, then by offset: unique edges own
     // their contributions in input order, so overlapping ports add deterministically
-    struct Con { long long off; int comp, port, tile; R scale; int64_t seq; };
+    struct Con { long long off; int comp, port, i, j, k; R scale; int64_t seq; };
     std::vector<Con> cons;
     for (int q = 0; q < np; ++q)
         for (int64_t e = ports[q].edge_begin; e < ports[q].edge_end; ++e) {
             Con cn;
             cn.off = ((long long)edges[e].k * g.PY + edges[e].j) * g.PX + edges[e].i;
             cn.comp = edges[e].comp; cn.port = q; cn.scale = (R)(ports[q].amplitude * edges[e].weight);
-            cn.tile = em::tile_of(plan, edges[e].i, edges[e].j, edges[e].k);
+            cn.i = edges[e].i; cn.j = edges[e].j; cn.k = edges[e].k;
             cn.seq = (int64_t)cons.size();
             cons.push_back(cn);
         }
     if ((int64_t)cons.size() > grid.max_source_edges)
         return fail(EM_ERR_WORKSPACE_TOO_SMALL, "more (edge, port) pairs than max_source_edges");
     std::sort(cons.begin(), cons.end(), [](const Con &a, const Con &b) {
-        if (a.tile != b.tile) return a.tile < b.tile;
         if (a.off != b.off) return a.off < b.off;
         if (a.comp != b.comp) return a.comp < b.comp;
         return a.seq < b.seq;
     });
-    std::vector<long long> u_off; std::vector<int> u_comp, u_cbeg, c_port, u_tile; std::vector<R> c_scale;
+    std::vector<long long> u_off; std::vector<int> u_comp, u_cbeg, c_port; std::vector<R> c_scale;
+    struct TE { int tile; int4 e; };
+    std::vector<TE> tes;
     for (size_t s = 0; s < cons.size(); ++s) {
         if (s == 0 || cons[s].off != cons[s - 1].off || cons[s].comp != cons[s - 1].comp) {
-            u_off.push_back(cons[s].off); u_comp.push_back(cons[s].comp); u_cbeg.push_back((int)s); u_tile.push_back(cons[s].tile);
+            const int u = (int)u_off.size();
+            u_off.push_back(cons[s].off); u_comp.push_back(cons[s].comp); u_cbeg.push_back((int)s);
+            int tl[4];
+            const int nt = em::tiles_of_node(plan, cons[s].i, cons[s].j, tl);
+            for (int t = 0; t < nt; ++t) tes.push_back(TE{tl[t], make_int4(cons[s].i, cons[s].j, cons[s].k, u * 4 + cons[s].comp)});
         }
         c_port.push_back(cons[s].port); c_scale.push_back(cons[s].scale);
     }
     u_cbeg.push_back((int)cons.size());
     const int nu = (int)u_off.size();
+    std::stable_sort(tes.begin(), tes.end(), [](const TE &a, const TE &b) {
+        if (a.tile != b.tile) return a.tile < b.tile;
+        if (a.e.z != b.e.z) return a.e.z < b.e.z;
+        if (a.e.y != b.e.y) return a.e.y < b.e.y;
+        return a.e.x < b.e.x;
+    });
     std::vector<int> tile_beg(plan.n_tiles + 1, 0);
-    for (int u = 0; u < nu; ++u) tile_beg[u_tile[u] + 1] += 1;
+    std::vector<int4> tile_ent(tes.size());
+    for (size_t s = 0; s < tes.size(); ++s) { tile_beg[tes[s].tile + 1] += 1; tile_ent[s] = tes[s].e; }
     for (int t = 0; t < plan.n_tiles; ++t) tile_beg[t + 1] += tile_beg[t];
     std::vector<long long> woff(std::max(np, 1)), wlen(std::max(np, 1));
     for (int q = 0; q < np; ++q) { woff[q] = ports[q].wave_offset; wlen[q] = ports[q].wave_len; }
@@ -375,6 +388,8 @@ int32_t Ctx<R>::set_source(int32_t np, const em_port *ports, const em_edge *edge
     }
     CU(cudaMemcpyAsync(c.src_cbeg, u_cbeg.data(), sizeof(int) * (nu + 1), cudaMemcpyHostToDevice, stream));
     CU(cudaMemcpyAsync(c.tile_sbeg, tile_beg.data(), sizeof(int) * (plan.n_tiles + 1), cudaMemcpyHostToDevice, stream));
+    if (!tile_ent.empty())
+        CU(cudaMemcpyAsync(c.tile_ent, tile_ent.data(), sizeof(int4) * tile_ent.size(), cudaMemcpyHostToDevice, stream));
     if (np) {
         CU(cudaMemcpyAsync(c.port_woff, woff.data(), sizeof(long long) * np, cudaMemcpyHostToDevice, stream));
         CU(cudaMemcpyAsync(c.port_wlen, wlen.data(), sizeof(long long) * np, cudaMemcpyHostToDevice, stream));
@@ -476,7 +491,8 @@ int32_t Ctx<R>::step_split() {
 template <typename R>
 int32_t Ctx<R>::step_fused() {
     int32_t rc = record_begin(); if (rc) return rc;
-    cudaError_t e = em::launch_fused<R>(plan, p, src, c.tile_sbeg, loss, uniform_mu, (long long)step_index, stream);
+    em::FusedSources fsrc{c.tile_sbeg, c.tile_ent};
+    cudaError_t e = em::launch_fused<R>(plan, p, src, fsrc, loss, uniform_mu, (long long)step_index, stream);
     if (e != cudaSuccess) return fail(EM_ERR_CUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
     rc = record_end(); if (rc) return rc;
     launches += 1;
