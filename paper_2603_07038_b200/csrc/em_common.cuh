@@ -47,7 +47,12 @@ __device__ __forceinline__ double mad(double a, double b, double c) { return ::f
 template <typename R> __device__ __forceinline__ R lerp(R lo, R hi, R f) { return mad(f, hi - lo, lo); }
 
 template <typename R> __device__ __forceinline__ R rcp(R x);
-template <> __device__ __forceinline__ float  rcp<float>(float x)   { return __frcp_rn(x); }
+template <> __device__ __forceinline__ float  rcp<float>(float x) {
+    // MUFU.RCP (<= 1 ulp) + one Newton step: no slow-path branch; x is a positive normal number here
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return fmaf(r, fmaf(-x, r, 1.0f), r);
+}
 template <> __device__ __forceinline__ double rcp<double>(double x) { return 1.0 / x; }
 
 // Loss coefficient r of the incremental form  E' = E + r (curlH - J - sigma E):

@@ -91,7 +91,7 @@ size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int
     o.q = w.take<R>(g.alloc_elems);
     o.mat = w.take<uint8_t>(g.alloc_elems);
     o.table = w.take<em::MatEntry<R>>(em::kMaxTable);
-    const int len[3] = {g.PX + 2, g.PY + 2, g.PZ + 2};
+    const int len[3] = {g.PX + 8, g.PY + 8, g.PZ + 8};   // 4 leading + 4 trailing pads (aligned vector loads)
     for (int a = 0; a < 9; ++a) o.axis[a] = w.take<R>(len[a / 3]);
     o.vx = w.take<double>(g.nx); o.vy = w.take<double>(g.ny); o.vz = w.take<double>(g.nz);
     o.partial = w.take<double>(kReduceBlocks); o.scalar = w.take<double>(1);
@@ -255,13 +255,13 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     // ---- per-axis arrays, index -1 .. n+1 (+ slack), fp64 then rounded once -------------------
     const double *d[3] = {gr->dx, gr->dy, gr->dz};
     const int n[3] = {g.nx, g.ny, g.nz};
-    const int len[3] = {g.PX + 2, g.PY + 2, g.PZ + 2};
+    const int len[3] = {g.PX + 8, g.PY + 8, g.PZ + 8};
     std::vector<std::vector<R>> hax(9);
     for (int a = 0; a < 3; ++a) {
         auto dd = [&](int i) { return (i >= 0 && i < n[a]) ? d[a][i] : 0.0; };
         std::vector<R> rd(len[a], R(0)), rt(len[a], R(0)), f(len[a], R(0));
         for (int s = 0; s < len[a]; ++s) {
-            const int i = s - 1;
+            const int i = s - 4;
             if (i >= 0 && i < n[a]) rd[s] = (R)(1.0 / d[a][i]);
             const double lo = dd(i - 1), hi = dd(i);
             if (lo + hi > 0.0) { rt[s] = (R)(2.0 / (lo + hi)); f[s] = (R)(hi / (lo + hi)); }
@@ -296,9 +296,9 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     // ---- device parameter block -----------------------------------------------------------------
     p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.PX = g.PX; p.PY = g.PY; p.PXY = g.PXY;
     p.q = c.q + g.origin; p.mat = c.mat + g.origin; p.table = c.table; p.n_table = n_mat + 1;
-    p.rdx = c.axis[0] + 1; p.rtx = c.axis[1] + 1; p.fx = c.axis[2] + 1;
-    p.rdy = c.axis[3] + 1; p.rty = c.axis[4] + 1; p.fy = c.axis[5] + 1;
-    p.rdz = c.axis[6] + 1; p.rtz = c.axis[7] + 1; p.fz = c.axis[8] + 1;
+    p.rdx = c.axis[0] + 4; p.rtx = c.axis[1] + 4; p.fx = c.axis[2] + 4;
+    p.rdy = c.axis[3] + 4; p.rty = c.axis[4] + 4; p.fy = c.axis[5] + 4;
+    p.rdz = c.axis[6] + 4; p.rtz = c.axis[7] + 4; p.fz = c.axis[8] + 4;
     p.dt = (R)dt;
     src = em::DevSources<R>{};
     src.n_unique = 0;
