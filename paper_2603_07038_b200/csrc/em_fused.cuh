@@ -45,7 +45,7 @@ inline FusedPlan make_fused_plan(int nx, int ny, int nz, int sizeof_real) {
     const size_t table = (size_t)kMaxTable * 4 * sizeof_real;
     const size_t rows = (size_t)4 * kFusedRows * 32 * 16;                 // H'x, H'z, Bx, Bz exchange rows
     const size_t slots = (size_t)kFusedSlots * kFusedThreads * 16;        // private slots
-    const size_t extra = (size_t)2 * 32 * 16 + (size_t)2 * kFusedRows * 32 * 4;   // top row + ids (2 parities)
+    const size_t extra = (size_t)(4 + 3) * 32 * 16 + (size_t)2 * kFusedRows * 32 * 4;   // top row (2 parities), x geometry, ids (2 parities)
     f.smem_bytes = table + rows + slots + extra;
     return f;
 }
@@ -113,8 +113,9 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
     VecR(*smBx)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 2 * kFusedRows * 32);
     VecR(*smBz)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 3 * kFusedRows * 32);
     VecR *S = s_rows + 4 * kFusedRows * 32;                   // private slots [kNumSlots][NT]
-    VecR *s_top = S + kNumSlots * NT;                         // [2][32]: Ex(k), Ez(k) of row TY+1
-    unsigned(*smId)[32] = reinterpret_cast<unsigned(*)[32]>(s_top + 64);   // [2 parity][kFusedRows][32]
+    VecR *s_top = S + kNumSlots * NT;                         // [2 parity][2][32]: Ex(k), Ez(k) of row TY+1
+    VecR *s_geo = s_top + 128;                                // [3][32]: 1/dx, 1/dx~, fx of the lanes' columns
+    unsigned(*smId)[32] = reinterpret_cast<unsigned(*)[32]>(s_geo + 96);   // [2 parity][kFusedRows][32]
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int tile = blockIdx.x, tx = tile % ntx, ty = tile / ntx;
@@ -140,7 +141,8 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
         for (int t = tid; t < 4 * kFusedRows * 32; t += NT) s_rows[t] = z;
         for (int t = 0; t < kNumSlots; ++t) S[t * NT + tid] = z;
         S[(kSlotL + 0) * NT + tid] = one; S[(kSlotL + 3) * NT + tid] = one;
-        if (tid < 64) s_top[tid] = z;
+        if (tid < 128) s_top[tid] = z;
+        if (tid < 96) s_geo[tid] = z;
         for (int t = tid; t < 2 * kFusedRows * 32; t += NT) (&smId[0][0])[t] = out_pack;
     }
     __syncthreads();
@@ -154,66 +156,85 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
         return (unsigned)*reinterpret_cast<const unsigned short *>(p.mat + off) | (out_pack & 0xffff0000u);
     };
     VecR *mine = S + tid;
+    // x geometry of the 32 lanes of this tile column (same for every row of the CTA)
+    if (w == 0 && (i0 + V <= p.PX)) {
+        s_geo[0 * 32 + lane] = ldv(p.rdx, i0); s_geo[1 * 32 + lane] = ldv(p.rtx, i0); s_geo[2 * 32 + lane] = ldv(p.fx, i0);
+    }
 
-    // inputs of iteration k: Ex(k+1), Ey(k+1) into ring slot (k+1)%3, Ez(k) into (k&1), H(k)
-    auto issue_stage = [&](int k, int ring_k1) {
-        if (active) {
-            const long long o = off0 + (long long)k * PXY;
-            cp_async16(mine + (kSlotEx + ring_k1) * NT, p.E[0] + o + PXY);
-            cp_async16(mine + (kSlotEy + ring_k1) * NT, p.E[1] + o + PXY);
-            cp_async16(mine + (kSlotEz + (k & 1)) * NT, p.E[2] + o);
-            cp_async16(mine + (kSlotH + 0) * NT, p.H[0] + o);
-            cp_async16(mine + (kSlotH + 1) * NT, p.H[1] + o);
-            cp_async16(mine + (kSlotH + 2) * NT, p.H[2] + o);
+    // cp.async groups (every thread commits the same sequence):
+    //   G_E(k): inputs of iteration k that the neighbours also read: Ex(k+1), Ey(k+1) -> ring slot
+    //           (k+1)%3, Ez(k) -> parity slot, row TY+1 for the top warp; issued in phase C(k-2)
+    //   G_H(k): H(k), own use only; issued at the end of phase A(k-1)
+    //   G_q(k): q(k) for phase C(k+1); issued in phase C(k)
+    // issue order per iteration k: G_H(k+1) | G_q(k), G_E(k+2)
+    auto issue_E = [&](int kk, int ring, int par) {
+        if (active && kk <= nz) {
+            const long long o = off0 + (long long)kk * PXY;
+            cp_async16(mine + (kSlotEx + ring) * NT, p.E[0] + o + PXY);
+            cp_async16(mine + (kSlotEy + ring) * NT, p.E[1] + o + PXY);
+            cp_async16(mine + (kSlotEz + par) * NT, p.E[2] + o);
             if (top_row_ok) {
-                cp_async16(s_top + lane, p.E[0] + o + PX);
-                cp_async16(s_top + 32 + lane, p.E[2] + o + PX);
+                cp_async16(s_top + par * 64 + lane, p.E[0] + o + PX);
+                cp_async16(s_top + par * 64 + 32 + lane, p.E[2] + o + PX);
             }
         }
         cp_async_commit();
     };
-    unsigned idw_next = out_pack, idw_prev = out_pack;
+    auto issue_H = [&](int kk) {
+        if (active && kk <= nz) {
+            const long long o = off0 + (long long)kk * PXY;
+            cp_async16(mine + (kSlotH + 0) * NT, p.H[0] + o);
+            cp_async16(mine + (kSlotH + 1) * NT, p.H[1] + o);
+            cp_async16(mine + (kSlotH + 2) * NT, p.H[2] + o);
+        }
+        cp_async_commit();
+    };
+    unsigned idw = out_pack, idw_next = out_pack, idw_prev = out_pack;
     if (active) {
         cp_async16(mine + (kSlotEx + 0) * NT, p.E[0] + off0);     // plane 0 into ring slot 0
         cp_async16(mine + (kSlotEy + 0) * NT, p.E[1] + off0);
-        idw_next = ld_ids(off0);
+        idw = ld_ids(off0);
+        if (nz > 1) idw_next = ld_ids(off0 + PXY);
     }
-    issue_stage(0, 1);
-    cp_async_commit();                            // empty "q" group: uniform group arithmetic
+    issue_E(0, 1, 0);                             // G_E(0)
+    issue_H(0);                                   // G_H(0)
+    cp_async_commit();                            // G_q(-1), empty
+    issue_E(1, 2, 1);                             // G_E(1)
+    smId[0 * kFusedRows + r][lane] = idw;
+    cp_async_wait<3>();                           // G_E(0) has landed
+    __syncthreads();
 
     int s_cur = fs.tile_sbeg[tile];               // source cursor of this tile
     const int s_end = fs.tile_sbeg[tile + 1];
+    int s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
     int rk = 0;                                   // k % 3
+    R fz = p.fz[0], rdz = p.rdz[0], rtz = p.rtz[0];
 
     for (int k = 0; k <= nz; ++k) {
-        const int rk1 = (rk == 2) ? 0 : rk + 1, rk2 = (rk1 == 2) ? 0 : rk1 + 1;
-        const R fz = p.fz[k], rdz = p.rdz[k], rtz = p.rtz[k];
+        const int rk1 = (rk == 2) ? 0 : rk + 1;
+        const int par = k & 1;
         const long long o = off0 + (long long)k * PXY;
-        // ---- ids of layer k to the exchange rows; stage(k) has landed -------------------------------
-        cp_async_wait<1>();                       // all but the newest group (q) are complete
-        const unsigned idw = idw_next;
-        smId[(k & 1) * kFusedRows + r][lane] = idw;
-        idw_next = (active && k < nz) ? ld_ids(o + PXY) : out_pack;
-        __syncthreads();                          // B1
+        const R fz_n = p.fz[k + 1], rdz_n = p.rdz[k + 1], rtz_n = p.rtz[k + 1];   // used next iteration
 
         // ---- phase A: H' = H - nbar * curl E  (inner factor of S = curl mu^-1 curl) ----
-        const unsigned idj = smId[(k & 1) * kFusedRows + r - 1][lane];
+        cp_async_wait<2>();                       // G_H(k) has landed
+        const unsigned idj = smId[par * kFusedRows + r - 1][lane];
         VecR hxn, hyn, hzn;
-        const VecR ex0 = mine[(kSlotEx + rk) * NT], ey0 = mine[(kSlotEy + rk) * NT], ez = mine[(kSlotEz + (k & 1)) * NT];
+        const VecR ex0 = mine[(kSlotEx + rk) * NT], ey0 = mine[(kSlotEy + rk) * NT], ez = mine[(kSlotEz + par) * NT];
         {
             const VecR ex1 = mine[(kSlotEx + rk1) * NT], ey1 = mine[(kSlotEy + rk1) * NT];
             const VecR hx = mine[(kSlotH + 0) * NT], hy = mine[(kSlotH + 1) * NT], hz = mine[(kSlotH + 2) * NT];
-            const VecR exn = is_top ? s_top[lane] : mine[(kSlotEx + rk) * NT + 32];
-            const VecR ezn = is_top ? s_top[32 + lane] : mine[(kSlotEz + (k & 1)) * NT + 32];
+            const VecR exn = is_top ? s_top[par * 64 + lane] : mine[(kSlotEx + rk) * NT + 32];
+            const VecR ezn = is_top ? s_top[par * 64 + 32 + lane] : mine[(kSlotEz + par) * NT + 32];
             const R ey0_r = shfl_down1(ey0.v[0]), ez_r = shfl_down1(ez.v[0]);
-            VecR rdxv = active ? ldv(p.rdx, i0) : ex0;
+            const VecR rdxv = s_geo[0 * 32 + lane];
             VecR nbx, nby, nbz;
             if (UMU) {
                 const R n0 = s_tab[0].n;
 #pragma unroll
                 for (int c = 0; c < V; ++c) nbx.v[c] = nby.v[c] = nbz.v[c] = n0;
             } else {
-                const VecR fxv = active ? ldv(p.fx, i0) : ex0;
+                const VecR fxv = s_geo[2 * 32 + lane];
                 R ncur[V];
 #pragma unroll
                 for (int c = 0; c < V; ++c) ncur[c] = s_tab[(idw >> (8 * c)) & 0xff].n;
@@ -246,16 +267,16 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
             *reinterpret_cast<VecR *>(p.Hn[2] + o) = hzn;
         }
         smHx[r][lane] = hxn; smHz[r][lane] = hzn;
-        if (k < nz) issue_stage(k + 1, rk2); else cp_async_commit();   // H slots and ring slot rk2 are free
-        __syncthreads();                          // B2
+        issue_H(k + 1);                           // G_H(k+1): the H slots are free again
+        __syncthreads();                          // B2: H' rows visible
 
         // ---- phase B: E' = E + r (curl H' - J - sigma E), Joule squares (eq. 2-3) -------
         VecR bx, by, bz;         // (2 Ebar)^2
-        const bool any_src = (s_cur < s_end) && (fs.tile_ent[s_cur].z <= k);
-        if (any_src) {
+        if (s_next_k <= k) {
 #define EM_HAS_J 1
 #include "em_fused_phaseb.inc"
 #undef EM_HAS_J
+            s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
         } else {
 #define EM_HAS_J 0
 #include "em_fused_phaseb.inc"
@@ -267,10 +288,11 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
         }
         smBx[r][lane] = bx; smBz[r][lane] = bz;
         mine[(kSlotHp + 0) * NT] = hxn; mine[(kSlotHp + 1) * NT] = hyn;
-        __syncthreads();                          // B3
+        smId[(par ^ 1) * kFusedRows + r][lane] = idw_next;     // ids of layer k+1 for the next iteration
+        cp_async_wait<1>();                       // G_E(k+1) (and G_q(k-1)) have landed
+        __syncthreads();                          // B3: B rows, next inputs and ids visible
 
         // ---- phase C: q(k-1) += dt sigma/16 (pend + Sxy(k)); pend = Sxy(k) + Sz(k) ---------------------
-        cp_async_wait<1>();                       // q(k-1) has landed (stage(k+1) may still fly)
         {
             const VecR bxn = smBx[r + 1][lane], bzn = smBz[r + 1][lane];
             const R by_r = shfl_down1(by.v[0]), bz_r = shfl_down1(bz.v[0]), bzn_r = shfl_down1(bzn.v[0]);
@@ -289,10 +311,13 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
             }
             mine[kSlotPend * NT] = pend;
             if (own_q && k >= 1) *reinterpret_cast<VecR *>(p.q + o - PXY) = qv;
-            if (own_q && k < nz) cp_async16(mine + kSlotQ * NT, p.q + o);   // q(k) for the next iteration
+            if (own_q && k < nz) cp_async16(mine + kSlotQ * NT, p.q + o);   // G_q(k)
             cp_async_commit();
         }
-        idw_prev = idw;
+        issue_E(k + 2, rk, par);                  // G_E(k+2): ring slot k%3 and parity k&1 are dead now
+        idw_prev = idw; idw = idw_next;
+        idw_next = (active && k + 2 < nz) ? ld_ids(o + 2 * PXY) : out_pack;
+        fz = fz_n; rdz = rdz_n; rtz = rtz_n;
         rk = rk1;
     }
     cp_async_wait<0>();
