@@ -45,7 +45,7 @@ inline FusedPlan make_fused_plan(int nx, int ny, int nz, int sizeof_real) {
     const size_t table = (size_t)kMaxTable * 4 * sizeof_real;
     const size_t rows = (size_t)4 * kFusedRows * 32 * 16;                 // H'x, H'z, Bx, Bz exchange rows
     const size_t slots = (size_t)kFusedSlots * kFusedThreads * 16;        // private slots
-    const size_t extra = (size_t)(4 + 3) * 32 * 16 + (size_t)2 * kFusedRows * 32 * 4;   // top row (2 parities), x geometry, ids (2 parities)
+    const size_t extra = (size_t)(4 + 3) * 32 * 16 + 64 + (size_t)2 * kFusedRows * 32 * 4;   // top row (2 parities), x geometry, ids (2 parities)
     f.smem_bytes = table + rows + slots + extra;
     return f;
 }
@@ -70,6 +70,14 @@ template <typename R> struct alignas(16) Vec { R v[16 / sizeof(R)]; };
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void *smem_dst, const void *gsrc) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(s), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
@@ -115,7 +123,8 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
     VecR *S = s_rows + 4 * kFusedRows * 32;                   // private slots [kNumSlots][NT]
     VecR *s_top = S + kNumSlots * NT;                         // [2 parity][2][32]: Ex(k), Ez(k) of row TY+1
     VecR *s_geo = s_top + 128;                                // [3][32]: 1/dx, 1/dx~, fx of the lanes' columns
-    unsigned(*smId)[32] = reinterpret_cast<unsigned(*)[32]>(s_geo + 96);   // [2 parity][kFusedRows][32]
+    R *s_z = reinterpret_cast<R *>(s_geo + 96);               // [2 parity][4]: fz, 1/dz, 1/dz~ of plane k
+    unsigned(*smId)[32] = reinterpret_cast<unsigned(*)[32]>(s_geo + 96 + 4);   // [2 parity][kFusedRows][32]
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int tile = blockIdx.x, tx = tile % ntx, ty = tile / ntx;
@@ -151,16 +160,18 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
     const R gq = p.dt * R(0.0625);
     const long long off0 = (long long)j * PX + i0;    // this thread's vector at plane 0
     auto ldv = [&](const R *a, long long off) -> VecR { return *reinterpret_cast<const VecR *>(a + off); };
-    auto ld_ids = [&](long long off) -> unsigned {
-        if (V == 4) return *reinterpret_cast<const unsigned *>(p.mat + off);
-        return (unsigned)*reinterpret_cast<const unsigned short *>(p.mat + off) | (out_pack & 0xffff0000u);
-    };
+    // ids travel as one aligned 32-bit word per lane (V = 4: exactly the lane's ids; V = 2: the
+    // lane's two ids are the low or high half, selected by id_shift)
+    const int id_shift = (V == 4) ? 0 : (int)((off0 & 2) * 8);
+    auto id_src = [&](long long off) -> const uint8_t * { return p.mat + ((off) & ~3LL); };
+    auto id_unpack = [&](unsigned wv) -> unsigned { return (V == 4) ? wv : ((wv >> id_shift) & 0xffffu) | (out_pack & 0xffff0000u); };
     VecR *mine = S + tid;
     // x geometry of the 32 lanes of this tile column (same for every row of the CTA)
     if (w == 0 && (i0 + V <= p.PX)) {
         s_geo[0 * 32 + lane] = ldv(p.rdx, i0); s_geo[1 * 32 + lane] = ldv(p.rtx, i0); s_geo[2 * 32 + lane] = ldv(p.fx, i0);
     }
 
+    const R *zarr = (tid == 0) ? p.fz : (tid == 1 ? p.rdz : p.rtz);   // threads 0..2 feed s_z
     // cp.async groups (every thread commits the same sequence):
     //   G_E(k): inputs of iteration k that the neighbours also read: Ex(k+1), Ey(k+1) -> ring slot
     //           (k+1)%3, Ez(k) -> parity slot, row TY+1 for the top warp; issued in phase C(k-2)
@@ -173,10 +184,14 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
             cp_async16(mine + (kSlotEx + ring) * NT, p.E[0] + o + PXY);
             cp_async16(mine + (kSlotEy + ring) * NT, p.E[1] + o + PXY);
             cp_async16(mine + (kSlotEz + par) * NT, p.E[2] + o);
+            cp_async4(&smId[par * kFusedRows + r][lane], id_src(o));
             if (top_row_ok) {
                 cp_async16(s_top + par * 64 + lane, p.E[0] + o + PX);
                 cp_async16(s_top + par * 64 + 32 + lane, p.E[2] + o + PX);
             }
+        }
+        if (tid < 3 && kk <= nz) {                // z geometry of plane kk
+            if (sizeof(R) == 4) cp_async4(&s_z[par * 4 + tid], zarr + kk); else cp_async8(&s_z[par * 4 + tid], zarr + kk);
         }
         cp_async_commit();
     };
@@ -189,18 +204,15 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
         }
         cp_async_commit();
     };
-    unsigned idw = out_pack, idw_next = out_pack, idw_prev = out_pack;
+    unsigned idw_prev = out_pack;
     if (active) {
         cp_async16(mine + (kSlotEx + 0) * NT, p.E[0] + off0);     // plane 0 into ring slot 0
         cp_async16(mine + (kSlotEy + 0) * NT, p.E[1] + off0);
-        idw = ld_ids(off0);
-        if (nz > 1) idw_next = ld_ids(off0 + PXY);
     }
     issue_E(0, 1, 0);                             // G_E(0)
     issue_H(0);                                   // G_H(0)
     cp_async_commit();                            // G_q(-1), empty
     issue_E(1, 2, 1);                             // G_E(1)
-    smId[0 * kFusedRows + r][lane] = idw;
     cp_async_wait<3>();                           // G_E(0) has landed
     __syncthreads();
 
@@ -208,17 +220,17 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
     const int s_end = fs.tile_sbeg[tile + 1];
     int s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
     int rk = 0;                                   // k % 3
-    R fz = p.fz[0], rdz = p.rdz[0], rtz = p.rtz[0];
 
     for (int k = 0; k <= nz; ++k) {
         const int rk1 = (rk == 2) ? 0 : rk + 1;
         const int par = k & 1;
         const long long o = off0 + (long long)k * PXY;
-        const R fz_n = p.fz[k + 1], rdz_n = p.rdz[k + 1], rtz_n = p.rtz[k + 1];   // used next iteration
+        const R fz = s_z[par * 4 + 0], rdz = s_z[par * 4 + 1], rtz = s_z[par * 4 + 2];
 
         // ---- phase A: H' = H - nbar * curl E  (inner factor of S = curl mu^-1 curl) ----
         cp_async_wait<2>();                       // G_H(k) has landed
-        const unsigned idj = smId[par * kFusedRows + r - 1][lane];
+        const unsigned idw = id_unpack(smId[par * kFusedRows + r][lane]);
+        const unsigned idj = id_unpack(smId[par * kFusedRows + r - 1][lane]);
         VecR hxn, hyn, hzn;
         const VecR ex0 = mine[(kSlotEx + rk) * NT], ey0 = mine[(kSlotEy + rk) * NT], ez = mine[(kSlotEz + par) * NT];
         {
@@ -288,7 +300,6 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
         }
         smBx[r][lane] = bx; smBz[r][lane] = bz;
         mine[(kSlotHp + 0) * NT] = hxn; mine[(kSlotHp + 1) * NT] = hyn;
-        smId[(par ^ 1) * kFusedRows + r][lane] = idw_next;     // ids of layer k+1 for the next iteration
         cp_async_wait<1>();                       // G_E(k+1) (and G_q(k-1)) have landed
         __syncthreads();                          // B3: B rows, next inputs and ids visible
 
@@ -315,9 +326,7 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
             cp_async_commit();
         }
         issue_E(k + 2, rk, par);                  // G_E(k+2): ring slot k%3 and parity k&1 are dead now
-        idw_prev = idw; idw = idw_next;
-        idw_next = (active && k + 2 < nz) ? ld_ids(o + 2 * PXY) : out_pack;
-        fz = fz_n; rdz = rdz_n; rtz = rtz_n;
+        idw_prev = idw;
         rk = rk1;
     }
     cp_async_wait<0>();
