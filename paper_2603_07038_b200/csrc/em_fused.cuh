@@ -19,6 +19,7 @@
 #pragma once
 #include "em_aux.cuh"
 #include "em_common.cuh"
+#include <algorithm>
 #include <type_traits>
 
 namespace em {
@@ -29,19 +30,42 @@ constexpr int kFusedThreads = kFusedWarps * 32;    // 576
 constexpr int kFusedRows = kFusedTY + 4;           // exchange rows, r = cy + 2 (row 0 and last: dummies)
 constexpr int kFusedSlots = 21;                    // private 16-B slots per thread (see enum below)
 
+constexpr int kFusedMaxZSplit = 8;                // z chunks per tile column (work items = tiles x chunks)
+
 struct FusedPlan {
     int V, TXo, ntx, nty, n_tiles;
+    int nzs;                         // z chunks; chunk c owns the planes kb[c] <= k < kb[c+1], kb[nzs] = nz+1
+    int kb[kFusedMaxZSplit + 1];
     size_t smem_bytes;
+    int chunk_of(int k) const { int c = 0; while (c + 1 < nzs && k >= kb[c + 1]) ++c; return c; }
 };
 
-inline FusedPlan make_fused_plan(int nx, int ny, int nz, int sizeof_real) {
-    (void)nz;
+// Number of z chunks: a chunk re-runs up to two planes of its lower neighbour (warm-up plane kb-1 and
+// the closing plane kb[c+1]), so the cost model is waves x (planes per chunk + 2); n_sm = 0 (no
+// device known yet: workspace sizing) returns the maximum.
+inline int choose_zsplit(int n_tiles, int nz, int n_sm, int forced) {
+    const int cap = std::max(1, std::min(kFusedMaxZSplit, (nz + 1) / 4));
+    if (forced > 0) return std::min(forced, cap);
+    if (n_sm <= 0) return kFusedMaxZSplit;
+    int best = 1; double best_cost = 1e300;
+    for (int s = 1; s <= cap; ++s) {
+        const long long waves = ((long long)n_tiles * s + n_sm - 1) / n_sm;
+        const double cost = (double)waves * ((double)(nz + 1) / s + (s > 1 ? 2.0 : 0.0));
+        if (cost < best_cost * 0.999) { best_cost = cost; best = s; }
+    }
+    return best;
+}
+
+inline FusedPlan make_fused_plan(int nx, int ny, int nz, int sizeof_real, int n_sm = 0, int forced_zsplit = 0) {
     FusedPlan f;
     f.V = 16 / sizeof_real;
     f.TXo = 30 * f.V;
     f.ntx = (nx + 1 + f.TXo - 1) / f.TXo;
     f.nty = (ny + 1 + kFusedTY - 1) / kFusedTY;
     f.n_tiles = f.ntx * f.nty;
+    f.nzs = choose_zsplit(f.n_tiles, nz, n_sm, forced_zsplit);
+    for (int c = 0; c <= kFusedMaxZSplit; ++c) f.kb[c] = nz + 1;
+    for (int c = 0; c < f.nzs; ++c) f.kb[c] = (int)(((long long)(nz + 1) * c) / f.nzs);
     const size_t table = (size_t)kMaxTable * 4 * sizeof_real;
     const size_t rows = (size_t)4 * kFusedRows * 32 * 16;                 // H'x, H'z, Bx, Bz exchange rows
     const size_t slots = (size_t)kFusedSlots * kFusedThreads * 16;        // private slots
@@ -88,8 +112,14 @@ template <typename R> __device__ __forceinline__ R shfl_down1(R v) { return __sh
 // Fused-sweep source index (built by em_set_source): entries of tile t are
 // tile_ent[tile_sbeg[t] .. tile_sbeg[t+1]) sorted by (k, j, i); ent = {i, j, k, u*4 + comp}.
 struct FusedSources {
-    const int *tile_sbeg;
+    const int *tile_sbeg;     // indexed by work item = tile * nzs + chunk (entries of a tile are sorted by k)
     const int4 *tile_ent;
+};
+
+// z chunks of the sweep (FusedPlan::kb), passed by value
+struct FusedChunks {
+    int nzs;
+    int kb[kFusedMaxZSplit + 1];
 };
 
 // Private shared-memory slots of a thread (16 B each, [slot][tid], so slot rows of the neighbouring
@@ -108,7 +138,7 @@ enum : int {
 
 template <typename R, int LOSS, bool UMU>
 __global__ void __launch_bounds__(kFusedThreads, 1)
-k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long long step) {
+k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc, int ntx, long long step) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TXo = 30 * V;
     constexpr int NT = kFusedThreads;
@@ -127,7 +157,13 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
     unsigned(*smId)[32] = reinterpret_cast<unsigned(*)[32]>(s_geo + 96 + 4);   // [2 parity][kFusedRows][32]
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int tile = blockIdx.x, tx = tile % ntx, ty = tile / ntx;
+    // work item = (tile, z chunk); chunk c stores the planes kz0 <= k < kz1 and the q layers of the same
+    // range; it starts one plane lower (warm-up: H'(kz0-1), the coefficient means and the ids of plane
+    // kz0-1, nothing stored) and ends on plane ke = kz1 (E'(kz1) closes the Joule sum of layer kz1-1).
+    const int item = blockIdx.x, tile = item / zc.nzs, chunk = item - tile * zc.nzs;
+    const int tx = tile % ntx, ty = tile / ntx;
+    const int kz0 = zc.kb[chunk], kz1 = zc.kb[chunk + 1];
+    const int ks = kz0 > 0 ? kz0 - 1 : 0, ke = kz1 <= p.nz ? kz1 : p.nz;
     const int cy = w - 1, r = cy + 2;
     const int j = ty * kFusedTY + cy;
     const int i0 = tx * TXo - V + V * lane;
@@ -179,7 +215,7 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
     //   G_q(k): q(k) for phase C(k+1); issued in phase C(k)
     // issue order per iteration k: G_H(k+1) | G_q(k), G_E(k+2)
     auto issue_E = [&](int kk, int ring, int par) {
-        if (active && kk <= nz) {
+        if (active && kk <= ke) {
             const long long o = off0 + (long long)kk * PXY;
             cp_async16(mine + (kSlotEx + ring) * NT, p.E[0] + o + PXY);
             cp_async16(mine + (kSlotEy + ring) * NT, p.E[1] + o + PXY);
@@ -190,13 +226,13 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
                 cp_async16(s_top + par * 64 + 32 + lane, p.E[2] + o + PX);
             }
         }
-        if (tid < 3 && kk <= nz) {                // z geometry of plane kk
+        if (tid < 3 && kk <= ke) {                // z geometry of plane kk
             if (sizeof(R) == 4) cp_async4(&s_z[par * 4 + tid], zarr + kk); else cp_async8(&s_z[par * 4 + tid], zarr + kk);
         }
         cp_async_commit();
     };
     auto issue_H = [&](int kk) {
-        if (active && kk <= nz) {
+        if (active && kk <= ke) {
             const long long o = off0 + (long long)kk * PXY;
             cp_async16(mine + (kSlotH + 0) * NT, p.H[0] + o);
             cp_async16(mine + (kSlotH + 1) * NT, p.H[1] + o);
@@ -205,26 +241,29 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
         cp_async_commit();
     };
     unsigned idw_prev = out_pack;
+    int rk = ks % 3;                              // k % 3
     if (active) {
-        cp_async16(mine + (kSlotEx + 0) * NT, p.E[0] + off0);     // plane 0 into ring slot 0
-        cp_async16(mine + (kSlotEy + 0) * NT, p.E[1] + off0);
+        cp_async16(mine + (kSlotEx + rk) * NT, p.E[0] + off0 + (long long)ks * PXY);   // plane ks into ring slot ks%3
+        cp_async16(mine + (kSlotEy + rk) * NT, p.E[1] + off0 + (long long)ks * PXY);
     }
-    issue_E(0, 1, 0);                             // G_E(0)
-    issue_H(0);                                   // G_H(0)
-    cp_async_commit();                            // G_q(-1), empty
-    issue_E(1, 2, 1);                             // G_E(1)
+    issue_E(ks, (rk + 1) % 3, ks & 1);            // G_E(ks)
+    issue_H(ks);                                  // G_H(ks)
+    cp_async_commit();                            // G_q(ks-1), empty
+    issue_E(ks + 1, (rk + 2) % 3, (ks + 1) & 1);  // G_E(ks+1)
     cp_async_wait<3>();                           // G_E(0) has landed
     __syncthreads();
 
-    int s_cur = fs.tile_sbeg[tile];               // source cursor of this tile
-    const int s_end = fs.tile_sbeg[tile + 1];
+    // source cursor: starts at the tile's first entry with k >= kz0 and may run into the next chunk's
+    // entries on the closing plane k = kz1 (E'(kz1) enters the Joule sum of layer kz1-1)
+    int s_cur = fs.tile_sbeg[item];
+    const int s_end = fs.tile_sbeg[(tile + 1) * zc.nzs];
     int s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
-    int rk = 0;                                   // k % 3
 
-    for (int k = 0; k <= nz; ++k) {
+    for (int k = ks; k <= ke; ++k) {
         const int rk1 = (rk == 2) ? 0 : rk + 1;
         const int par = k & 1;
         const long long o = off0 + (long long)k * PXY;
+        const bool st = own && k >= kz0 && k < kz1;          // this chunk stores H'(k), E'(k)
         const R fz = s_z[par * 4 + 0], rdz = s_z[par * 4 + 1], rtz = s_z[par * 4 + 2];
 
         // ---- phase A: H' = H - nbar * curl E  (inner factor of S = curl mu^-1 curl) ----
@@ -273,7 +312,7 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
 #pragma unroll
             for (int c = 0; c < V; ++c) hxn.v[c] = hyn.v[c] = hzn.v[c] = R(0);
         }
-        if (own) {
+        if (st) {
             *reinterpret_cast<VecR *>(p.Hn[0] + o) = hxn;
             *reinterpret_cast<VecR *>(p.Hn[1] + o) = hyn;
             *reinterpret_cast<VecR *>(p.Hn[2] + o) = hzn;
@@ -321,8 +360,8 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
                 pend.v[c] = sxy + sz;
             }
             mine[kSlotPend * NT] = pend;
-            if (own_q && k >= 1) *reinterpret_cast<VecR *>(p.q + o - PXY) = qv;
-            if (own_q && k < nz) cp_async16(mine + kSlotQ * NT, p.q + o);   // G_q(k)
+            if (own_q && k > kz0) *reinterpret_cast<VecR *>(p.q + o - PXY) = qv;             // layer k-1 in [kz0, kz1)
+            if (own_q && k >= kz0 && k < ke) cp_async16(mine + kSlotQ * NT, p.q + o);        // G_q(k)
             cp_async_commit();
         }
         issue_E(k + 2, rk, par);                  // G_E(k+2): ring slot k%3 and parity k&1 are dead now
@@ -335,7 +374,10 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, int ntx, long 
 template <typename R>
 cudaError_t launch_fused(const FusedPlan &plan, const DevParams<R> &p, const DevSources<R> &src,
                          const FusedSources &fs, int loss, bool uniform_mu, long long step, cudaStream_t stream) {
-    using K = void (*)(DevParams<R>, DevSources<R>, FusedSources, int, long long);
+    using K = void (*)(DevParams<R>, DevSources<R>, FusedSources, FusedChunks, int, long long);
+    FusedChunks zc;
+    zc.nzs = plan.nzs;
+    for (int c = 0; c <= kFusedMaxZSplit; ++c) zc.kb[c] = plan.kb[c];
     K kern;
     if (loss == 0) kern = uniform_mu ? (K)k_fused_sweep<R, 0, true> : (K)k_fused_sweep<R, 0, false>;
     else           kern = uniform_mu ? (K)k_fused_sweep<R, 1, true> : (K)k_fused_sweep<R, 1, false>;
@@ -347,7 +389,7 @@ cudaError_t launch_fused(const FusedPlan &plan, const DevParams<R> &p, const Dev
         if (e != cudaSuccess) return e;
         for (auto &c : configured) if (!c) { c = (const void *)kern; break; }
     }
-    kern<<<plan.n_tiles, kFusedThreads, plan.smem_bytes, stream>>>(p, src, fs, plan.ntx, step);
+    kern<<<plan.n_tiles * plan.nzs, kFusedThreads, plan.smem_bytes, stream>>>(p, src, fs, zc, plan.ntx, step);
     return cudaGetLastError();
 }
 

@@ -3,6 +3,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -83,7 +84,7 @@ struct Carved {
 };
 
 template <typename R>
-size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int n_tiles) {
+size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int n_items) {
     Carver w(base);
     Carved<R> tmp;
     Carved<R> &o = c ? *c : tmp;
@@ -103,7 +104,7 @@ size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int
     o.con_port = w.take<int>(me); o.con_scale = w.take<R>(me);
     o.port_woff = w.take<long long>(mp); o.port_wlen = w.take<long long>(mp);
     o.wave = w.take<R>((size_t)std::max<int64_t>(gr.max_wave_samples, 1));
-    o.tile_sbeg = w.take<int>((size_t)n_tiles + 1);
+    o.tile_sbeg = w.take<int>((size_t)n_items + 1);
     o.tile_ent = w.take<int4>(4 * me);
     return align_up(w.off);
 }
@@ -231,11 +232,18 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     g = make_geometry(gr->nx, gr->ny, gr->nz);
     loss = gr->loss_mode; dt = dt_;
     stream = static_cast<cudaStream_t>(stream_);
-    plan = em::make_fused_plan(g.nx, g.ny, g.nz, (int)sizeof(R));
+    {
+        int dev = 0, n_sm = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+        const char *forced = std::getenv("EM_FUSED_ZSPLIT");      // tuning/test knob: force the z chunk count
+        plan = em::make_fused_plan(g.nx, g.ny, g.nz, (int)sizeof(R), n_sm, forced ? std::atoi(forced) : 0);
+    }
     kernel = gr->kernel == EM_KERNEL_AUTO ? EM_KERNEL_FUSED : gr->kernel;
-    const size_t need = carve<R>(g, *gr, nullptr, nullptr, plan.n_tiles);
+    const int max_items = plan.n_tiles * em::kFusedMaxZSplit;
+    const size_t need = carve<R>(g, *gr, nullptr, nullptr, max_items);
     if (ws_bytes < need) return fail(EM_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
-    carve<R>(g, *gr, workspace, &c, plan.n_tiles);
+    carve<R>(g, *gr, workspace, &c, max_items);
     main_kernel = kernel == EM_KERNEL_FUSED ? "k_fused_sweep" : "k_split_e";
 
     // ---- material table -> (eps/dt, sigma, mask, dt/mu), built in fp64, rounded once ----------
@@ -291,6 +299,7 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
         for (uint8_t v : host_mat) used[v] = 1;
         double mu0 = -1;
         for (int m = 0; m < n_mat; ++m) if (used[m]) { if (mu0 < 0) mu0 = tab[m].mu; else if (tab[m].mu != mu0) uniform_mu = false; }
+        if (tab[0].mu != mu0) uniform_mu = false;     // the uniform-mu kernels read dt/mu from table entry 0
     }
 
     // ---- device parameter block -----------------------------------------------------------------
@@ -302,7 +311,7 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     p.dt = (R)dt;
     src = em::DevSources<R>{};
     src.n_unique = 0;
-    CU(cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (plan.n_tiles + 1), stream));
+    CU(cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (plan.n_tiles * plan.nzs + 1), stream));
     int32_t rc = zero_state();
     if (rc) return rc;
     CU(cudaStreamSynchronize(stream));
@@ -370,10 +379,16 @@ int32_t Ctx<R>::set_source(int32_t np, const em_port *ports, const em_edge *edge
         if (a.e.y != b.e.y) return a.e.y < b.e.y;
         return a.e.x < b.e.x;
     });
-    std::vector<int> tile_beg(plan.n_tiles + 1, 0);
+    // cursor per work item (tile, z chunk): the entries of a tile are sorted by k, so the items of a tile
+    // are consecutive ranges
+    const int n_items = plan.n_tiles * plan.nzs;
+    std::vector<int> tile_beg(n_items + 1, 0);
     std::vector<int4> tile_ent(tes.size());
-    for (size_t s = 0; s < tes.size(); ++s) { tile_beg[tes[s].tile + 1] += 1; tile_ent[s] = tes[s].e; }
-    for (int t = 0; t < plan.n_tiles; ++t) tile_beg[t + 1] += tile_beg[t];
+    for (size_t s = 0; s < tes.size(); ++s) {
+        tile_beg[tes[s].tile * plan.nzs + plan.chunk_of(tes[s].e.z) + 1] += 1;
+        tile_ent[s] = tes[s].e;
+    }
+    for (int t = 0; t < n_items; ++t) tile_beg[t + 1] += tile_beg[t];
     std::vector<long long> woff(std::max(np, 1)), wlen(std::max(np, 1));
     for (int q = 0; q < np; ++q) { woff[q] = ports[q].wave_offset; wlen[q] = ports[q].wave_len; }
     std::vector<R> hw((size_t)std::max<int64_t>(ns, 1));
@@ -387,7 +402,7 @@ int32_t Ctx<R>::set_source(int32_t np, const em_port *ports, const em_edge *edge
         CU(cudaMemcpyAsync(c.con_scale, c_scale.data(), sizeof(R) * c_scale.size(), cudaMemcpyHostToDevice, stream));
     }
     CU(cudaMemcpyAsync(c.src_cbeg, u_cbeg.data(), sizeof(int) * (nu + 1), cudaMemcpyHostToDevice, stream));
-    CU(cudaMemcpyAsync(c.tile_sbeg, tile_beg.data(), sizeof(int) * (plan.n_tiles + 1), cudaMemcpyHostToDevice, stream));
+    CU(cudaMemcpyAsync(c.tile_sbeg, tile_beg.data(), sizeof(int) * (n_items + 1), cudaMemcpyHostToDevice, stream));
     if (!tile_ent.empty())
         CU(cudaMemcpyAsync(c.tile_ent, tile_ent.data(), sizeof(int4) * tile_ent.size(), cudaMemcpyHostToDevice, stream));
     if (np) {
@@ -410,7 +425,7 @@ int32_t Ctx<R>::set_source(int32_t np, const em_port *ports, const em_edge *edge
         for (int u = 0; u < nu; ++u)
             if (flags[u]) {
                 src.n_unique = 0; n_unique = 0;
-                cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (plan.n_tiles + 1), stream);
+                cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (n_items + 1), stream);
                 return fail(EM_ERR_INVALID_ARG, "a source edge is PEC-fixed");
             }
     }
@@ -578,8 +593,9 @@ int32_t em_workspace_bytes(const em_grid *gr, size_t *out) {
     int32_t rc = validate_grid(gr); if (rc) return rc;
     const Geometry g = make_geometry(gr->nx, gr->ny, gr->nz);
     const em::FusedPlan plan = em::make_fused_plan(g.nx, g.ny, g.nz, gr->precision / 8);
-    *out = gr->precision == 32 ? carve<float>(g, *gr, nullptr, nullptr, plan.n_tiles)
-                               : carve<double>(g, *gr, nullptr, nullptr, plan.n_tiles);
+    const int max_items = plan.n_tiles * em::kFusedMaxZSplit;
+    *out = gr->precision == 32 ? carve<float>(g, *gr, nullptr, nullptr, max_items)
+                               : carve<double>(g, *gr, nullptr, nullptr, max_items);
     return EM_OK;
 }
 
