@@ -39,6 +39,7 @@ struct DevParams {
     // per-axis arrays indexed [-1 .. n+1] (pointer shifted to index 0):
     //   rd = 1/d (0 outside), rt = 1/d~, f = d[i]/(d[i-1]+d[i]) with d[-1] = d[n] = 0
     const R *rdx, *rtx, *fx, *rdy, *rty, *fy, *rdz, *rtz, *fz;
+    const R *zgeo;           // interleaved {fz, 1/dz, 1/dz~, 0} per plane (one 4-vector fetch per plane in the fused sweep)
     R dt;
 };
 

@@ -24,7 +24,14 @@
 
 namespace em {
 
-constexpr int kFusedTY = 14;                       // owned rows per tile (16 warps x 128 regs)
+#ifndef EM_FUSED_TY
+#define EM_FUSED_TY 14
+#endif
+#ifndef EM_FUSED_OCC
+#define EM_FUSED_OCC 1
+#endif
+constexpr int kFusedTY = EM_FUSED_TY;               // owned rows per tile (16 warps x 128 regs)
+constexpr int kFusedOcc = EM_FUSED_OCC;             // resident CTAs per SM
 constexpr int kFusedWarps = kFusedTY + 2;          // rows -1 .. TY
 constexpr int kFusedThreads = kFusedWarps * 32;    // 576
 constexpr int kFusedRows = kFusedTY + 4;           // exchange rows, r = cy + 2 (row 0 and last: dummies)
@@ -63,7 +70,7 @@ inline FusedPlan make_fused_plan(int nx, int ny, int nz, int sizeof_real, int n_
     f.ntx = (nx + 1 + f.TXo - 1) / f.TXo;
     f.nty = (ny + 1 + kFusedTY - 1) / kFusedTY;
     f.n_tiles = f.ntx * f.nty;
-    f.nzs = choose_zsplit(f.n_tiles, nz, n_sm, forced_zsplit);
+    f.nzs = choose_zsplit(f.n_tiles, nz, n_sm * kFusedOcc, forced_zsplit);
     for (int c = 0; c <= kFusedMaxZSplit; ++c) f.kb[c] = nz + 1;
     for (int c = 0; c < f.nzs; ++c) f.kb[c] = (int)(((long long)(nz + 1) * c) / f.nzs);
     const size_t table = (size_t)kMaxTable * 4 * sizeof_real;
@@ -137,7 +144,7 @@ enum : int {
 };
 
 template <typename R, int LOSS, bool UMU>
-__global__ void __launch_bounds__(kFusedThreads, 1)
+__global__ void __launch_bounds__(kFusedThreads, kFusedOcc)
 k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc, int ntx, long long step) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TXo = 30 * V;
@@ -201,13 +208,14 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
     const int id_shift = (V == 4) ? 0 : (int)((off0 & 2) * 8);
     auto id_src = [&](long long off) -> const uint8_t * { return p.mat + ((off) & ~3LL); };
     auto id_unpack = [&](unsigned wv) -> unsigned { return (V == 4) ? wv : ((wv >> id_shift) & 0xffffu) | (out_pack & 0xffff0000u); };
+    // all V cells of an unpacked id word hold the same material
+    auto id_uniform = [&](unsigned wv) -> bool { return (V == 4) ? (wv == (wv & 0xffu) * 0x01010101u) : (((wv >> 8) & 0xffu) == (wv & 0xffu)); };
     VecR *mine = S + tid;
     // x geometry of the 32 lanes of this tile column (same for every row of the CTA)
     if (w == 0 && (i0 + V <= p.PX)) {
         s_geo[0 * 32 + lane] = ldv(p.rdx, i0); s_geo[1 * 32 + lane] = ldv(p.rtx, i0); s_geo[2 * 32 + lane] = ldv(p.fx, i0);
     }
 
-    const R *zarr = (tid == 0) ? p.fz : (tid == 1 ? p.rdz : p.rtz);   // threads 0..2 feed s_z
     // cp.async groups (every thread commits the same sequence):
     //   G_E(k): inputs of iteration k that the neighbours also read: Ex(k+1), Ey(k+1) -> ring slot
     //           (k+1)%3, Ez(k) -> parity slot, row TY+1 for the top warp; issued in phase C(k-2)
@@ -226,9 +234,9 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
                 cp_async16(s_top + par * 64 + 32 + lane, p.E[2] + o + PX);
             }
         }
-        if (tid < 3 && kk <= ke) {                // z geometry of plane kk
-            if (sizeof(R) == 4) cp_async4(&s_z[par * 4 + tid], zarr + kk); else cp_async8(&s_z[par * 4 + tid], zarr + kk);
-        }
+        if (tid < (int)sizeof(R) / 4 && kk <= ke)   // z geometry of plane kk: {fz, 1/dz, 1/dz~, 0}
+            cp_async16(reinterpret_cast<unsigned char *>(&s_z[par * 4]) + 16 * tid,
+                       reinterpret_cast<const unsigned char *>(p.zgeo + 4 * (long long)kk) + 16 * tid);
         cp_async_commit();
     };
     auto issue_H = [&](int kk) {
@@ -241,6 +249,9 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
         cp_async_commit();
     };
     unsigned idw_prev = out_pack;
+    bool rowu_prev = false;      // plane k-1: rows j-1 and j of this lane held one material
+    bool l_stale = false;        // warp-uniform: the L slots were skipped by the one-material path
+    bool q_live = false;         // q of layer k-1 was fetched (some sigma != 0 among the lane's cells)
     int rk = ks % 3;                              // k % 3
     if (active) {
         cp_async16(mine + (kSlotEx + rk) * NT, p.E[0] + off0 + (long long)ks * PXY);   // plane ks into ring slot ks%3
@@ -270,6 +281,14 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
         cp_async_wait<2>();                       // G_H(k) has landed
         const unsigned idw = id_unpack(smId[par * kFusedRows + r][lane]);
         const unsigned idj = id_unpack(smId[par * kFusedRows + r - 1][lane]);
+        // one material over the warp's whole coefficient neighbourhood (rows j-1..j, planes k-1..k)?
+        const bool rowu = (idw == idj) && id_uniform(idw);
+        const unsigned idw_lane0 = __shfl_sync(0xffffffffu, idw, 0);     // (not inside the && chain: every lane must execute it)
+#ifdef EM_EXP_NOHOM
+        const bool hom = false;
+#else
+        const bool hom = __all_sync(0xffffffffu, rowu && rowu_prev && idw == idw_prev && idw == idw_lane0);
+#endif
         VecR hxn, hyn, hzn;
         const VecR ex0 = mine[(kSlotEx + rk) * NT], ey0 = mine[(kSlotEy + rk) * NT], ez = mine[(kSlotEz + par) * NT];
         {
@@ -322,28 +341,45 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
         __syncthreads();                          // B2: H' rows visible
 
         // ---- phase B: E' = E + r (curl H' - J - sigma E), Joule squares (eq. 2-3) -------
+        // (warp 0 = halo row -1 only supplies H' to row 0: no E', no Joule)
         VecR bx, by, bz;         // (2 Ebar)^2
-        if (s_next_k <= k) {
+        if (w != 0) {
+            if (hom && s_next_k > k) {
+#include "em_fused_phaseb_hom.inc"
+                l_stale = true;
+            } else {
+                if (l_stale) {   // plane k-1 took the one-material path: its coefficient means are the entry itself
+                    const MatEntry<R> Ap = s_tab[idw_prev & 0xff];
+                    VecR va, vb, vm;
+#pragma unroll
+                    for (int c = 0; c < V; ++c) { va.v[c] = Ap.a; vb.v[c] = Ap.b; vm.v[c] = Ap.m * Ap.m; }
+                    mine[(kSlotL + 0) * NT] = va; mine[(kSlotL + 1) * NT] = vb; mine[(kSlotL + 2) * NT] = vm;
+                    mine[(kSlotL + 3) * NT] = va; mine[(kSlotL + 4) * NT] = vb; mine[(kSlotL + 5) * NT] = vm;
+                    l_stale = false;
+                }
+                if (s_next_k <= k) {
 #define EM_HAS_J 1
 #include "em_fused_phaseb.inc"
 #undef EM_HAS_J
-            s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
-        } else {
+                    s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
+                } else {
 #define EM_HAS_J 0
 #include "em_fused_phaseb.inc"
 #undef EM_HAS_J
-        }
-        if (!active) {
+                }
+            }
+            if (!active) {
 #pragma unroll
-            for (int c = 0; c < V; ++c) bx.v[c] = by.v[c] = bz.v[c] = R(0);
+                for (int c = 0; c < V; ++c) bx.v[c] = by.v[c] = bz.v[c] = R(0);
+            }
+            smBx[r][lane] = bx; smBz[r][lane] = bz;
+            mine[(kSlotHp + 0) * NT] = hxn; mine[(kSlotHp + 1) * NT] = hyn;
         }
-        smBx[r][lane] = bx; smBz[r][lane] = bz;
-        mine[(kSlotHp + 0) * NT] = hxn; mine[(kSlotHp + 1) * NT] = hyn;
         cp_async_wait<1>();                       // G_E(k+1) (and G_q(k-1)) have landed
         __syncthreads();                          // B3: B rows, next inputs and ids visible
 
         // ---- phase C: q(k-1) += dt sigma/16 (pend + Sxy(k)); pend = Sxy(k) + Sz(k) ---------------------
-        {
+        if (w != 0 && !is_top) {
             const VecR bxn = smBx[r + 1][lane], bzn = smBz[r + 1][lane];
             const R by_r = shfl_down1(by.v[0]), bz_r = shfl_down1(bz.v[0]), bzn_r = shfl_down1(bzn.v[0]);
             VecR qv = mine[kSlotQ * NT];
@@ -355,17 +391,24 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
                 const R bznip = (c < V - 1) ? bzn.v[c < V - 1 ? c + 1 : c] : bzn_r;
                 const R sxy = (bx.v[c] + bxn.v[c]) + (by.v[c] + byip);
                 const R sz = (bz.v[c] + bzip) + (bzn.v[c] + bznip);
-                const R sg = s_tab[(idw_prev >> (8 * c)) & 0xff].b;     // sigma of the cell of layer k-1
+                const R sg = s_tab[(idw_prev >> (8 * (hom ? 0 : c))) & 0xff].b;     // sigma of the cell of layer k-1
                 qv.v[c] = mad(gq * sg, pend.v[c] + sxy, qv.v[c]);
                 pend.v[c] = sxy + sz;
             }
             mine[kSlotPend * NT] = pend;
-            if (own_q && k > kz0) *reinterpret_cast<VecR *>(p.q + o - PXY) = qv;             // layer k-1 in [kz0, kz1)
-            if (own_q && k >= kz0 && k < ke) cp_async16(mine + kSlotQ * NT, p.q + o);        // G_q(k)
-            cp_async_commit();
+            // q of a lane whose V cells are one lossless material never changes: neither fetched nor stored
+            if (own_q && k > kz0 && q_live) *reinterpret_cast<VecR *>(p.q + o - PXY) = qv;   // layer k-1 in [kz0, kz1)
+#ifdef EM_EXP_NOQSKIP
+            q_live = true;
+#else
+            q_live = !(id_uniform(idw) && s_tab[idw & 0xff].b == R(0));
+#endif
+            if (own_q && k >= kz0 && k < ke && q_live) cp_async16(mine + kSlotQ * NT, p.q + o);   // G_q(k)
         }
+        cp_async_commit();
         issue_E(k + 2, rk, par);                  // G_E(k+2): ring slot k%3 and parity k&1 are dead now
         idw_prev = idw;
+        rowu_prev = rowu;
         rk = rk1;
     }
     cp_async_wait<0>();

@@ -72,6 +72,7 @@ struct Carved {
     R *q;
     uint8_t *mat;
     em::MatEntry<R> *table;
+    R *zgeo;                 // {fz, rdz, rtz, 0} x (PZ + 8)
     R *axis[9];              // rdx, rtx, fx, rdy, rty, fy, rdz, rtz, fz (allocation starts; index -1 first)
     double *vx, *vy, *vz;    // cell sizes in fp64 for the Joule total
     double *partial, *scalar;
@@ -94,6 +95,7 @@ size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int
     o.table = w.take<em::MatEntry<R>>(em::kMaxTable);
     const int len[3] = {g.PX + 8, g.PY + 8, g.PZ + 8};   // 4 leading + 4 trailing pads (aligned vector loads)
     for (int a = 0; a < 9; ++a) o.axis[a] = w.take<R>(len[a / 3]);
+    o.zgeo = w.take<R>((size_t)4 * len[2]);
     o.vx = w.take<double>(g.nx); o.vy = w.take<double>(g.ny); o.vz = w.take<double>(g.nz);
     o.partial = w.take<double>(kReduceBlocks); o.scalar = w.take<double>(1);
     o.probe_off = w.take<long long>(kProbeChunk); o.probe_comp = w.take<int>(kProbeChunk);
@@ -278,6 +280,12 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     }
     for (int a = 0; a < 9; ++a)
         CU(cudaMemcpyAsync(c.axis[a], hax[a].data(), sizeof(R) * hax[a].size(), cudaMemcpyHostToDevice, stream));
+    {
+        std::vector<R> zg((size_t)4 * len[2], R(0));
+        for (int s = 0; s < len[2]; ++s) { zg[4 * s + 0] = hax[8][s]; zg[4 * s + 1] = hax[6][s]; zg[4 * s + 2] = hax[7][s]; }
+        CU(cudaMemcpyAsync(c.zgeo, zg.data(), sizeof(R) * zg.size(), cudaMemcpyHostToDevice, stream));
+        CU(cudaStreamSynchronize(stream));      // zg is a local
+    }
     CU(cudaMemcpyAsync(c.vx, gr->dx, sizeof(double) * g.nx, cudaMemcpyHostToDevice, stream));
     CU(cudaMemcpyAsync(c.vy, gr->dy, sizeof(double) * g.ny, cudaMemcpyHostToDevice, stream));
     CU(cudaMemcpyAsync(c.vz, gr->dz, sizeof(double) * g.nz, cudaMemcpyHostToDevice, stream));
@@ -308,6 +316,7 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     p.rdx = c.axis[0] + 4; p.rtx = c.axis[1] + 4; p.fx = c.axis[2] + 4;
     p.rdy = c.axis[3] + 4; p.rty = c.axis[4] + 4; p.fy = c.axis[5] + 4;
     p.rdz = c.axis[6] + 4; p.rtz = c.axis[7] + 4; p.fz = c.axis[8] + 4;
+    p.zgeo = c.zgeo + 16;
     p.dt = (R)dt;
     src = em::DevSources<R>{};
     src.n_unique = 0;

@@ -72,6 +72,15 @@ def test_random_grids_cd(dims, precision, kernel):
     run_pair(p, 40, precision, kernel, checkpoints=(1, 10))
 
 
+@pytest.mark.parametrize("zsplit", [1, 2, 3, 5, 8])
+def test_fused_z_chunks(zsplit, monkeypatch):
+    """The fused sweep splits every tile column into z chunks (work items); many ports so that source
+    edges sit on chunk boundary planes (their E' closes the Joule sum of the chunk below)."""
+    monkeypatch.setenv("EM_FUSED_ZSPLIT", str(zsplit))
+    p = W.random_problem(21, 18, 33, seed=77, loss_mode=LOSS_CD, steps=30, n_ports=60)
+    run_pair(p, 30, 64, P.EM_KERNEL_FUSED, checkpoints=(1, 7))
+
+
 @pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("precision", [64, 32])
 @pytest.mark.parametrize("dims", [(37, 29, 23), (9, 4, 70)])
