@@ -35,7 +35,7 @@ def parse():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--scale", type=int, default=1)
     ap.add_argument("--precision", type=int, default=0, help="0 = the config's own")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "split", "fused"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "split", "fused", "tma"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -189,7 +189,7 @@ def run_b200(args):
 
     p = make_problem(args)
     precision = args.precision or p.precision
-    kernel = {"auto": P.EM_KERNEL_AUTO, "split": P.EM_KERNEL_SPLIT, "fused": P.EM_KERNEL_FUSED}[args.kernel]
+    kernel = {"auto": P.EM_KERNEL_AUTO, "split": P.EM_KERNEL_SPLIT, "fused": P.EM_KERNEL_FUSED, "tma": P.EM_KERNEL_TMA}[args.kernel]
     K, Wm = args.steps, args.warmup
     em = P.EM(p, precision=precision, kernel=kernel, device=dev)
     cells = p.n_cells

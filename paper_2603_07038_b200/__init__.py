@@ -7,6 +7,6 @@ library raises.
 """
 from .binding import (  # noqa: F401
     EM, EMError, lib_path, load,
-    EM_LOSS_CD, EM_LOSS_EXP, EM_KERNEL_AUTO, EM_KERNEL_SPLIT, EM_KERNEL_FUSED,
+    EM_LOSS_CD, EM_LOSS_EXP, EM_KERNEL_AUTO, EM_KERNEL_SPLIT, EM_KERNEL_FUSED, EM_KERNEL_TMA,
     em_workspace_bytes, em_cfl_dt,
 )

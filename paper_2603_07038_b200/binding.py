@@ -14,7 +14,7 @@ import numpy as np
 
 EM_OK = 0
 EM_LOSS_CD, EM_LOSS_EXP = 0, 1
-EM_KERNEL_AUTO, EM_KERNEL_SPLIT, EM_KERNEL_FUSED = 0, 1, 2
+EM_KERNEL_AUTO, EM_KERNEL_SPLIT, EM_KERNEL_FUSED, EM_KERNEL_TMA = 0, 1, 2, 3
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 

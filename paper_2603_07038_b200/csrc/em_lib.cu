@@ -15,6 +15,7 @@
 #include "em_common.cuh"
 #include "em_fused.cuh"
 #include "em_split.cuh"
+#include "em_sweep.cuh"
 
 namespace {
 
@@ -40,7 +41,9 @@ struct Geometry {
 Geometry make_geometry(int nx, int ny, int nz) {
     Geometry g;
     g.nx = nx; g.ny = ny; g.nz = nz;
-    g.PX = (nx + 2 + 31) / 32 * 32;
+    // nx + 2 for the i = -1 / nx + 1 pads; + 16 so that the id box of the TMA sweep (based 16 B before the
+    // row) still holds the "outside" id of cell i = nx inside the row
+    g.PX = (nx + 18 + 31) / 32 * 32;
     g.PY = ny + 3; g.PZ = nz + 3;
     g.PXY = (long long)g.PX * g.PY;
     g.vol = g.PXY * g.PZ;
@@ -189,6 +192,10 @@ struct Ctx final : em_ctx {
     int32_t reset() override { return zero_state(); }
     int32_t step_split();
     int32_t step_fused();
+    int32_t step_tma();
+    int32_t make_maps();
+    CUtensorMap map_field[12], map_q, map_mat;   // TMA descriptors of the padded arrays (sweep boxes)
+    size_t sweep_smem = 0;
     void comp_dims(int comp, int *sx, int *sy, int *sz) const {
         const int nx = g.nx, ny = g.ny, nz = g.nz;
         switch (comp) {
@@ -212,7 +219,7 @@ int32_t validate_grid(const em_grid *g) {
     if ((long long)g->nx + 34 > 2147483647LL / 4) return fail(EM_ERR_INVALID_ARG, "nx too large");
     if (g->precision != 32 && g->precision != 64) return fail(EM_ERR_INVALID_ARG, "precision must be 32 or 64");
     if (g->loss_mode != EM_LOSS_CD && g->loss_mode != EM_LOSS_EXP) return fail(EM_ERR_INVALID_ARG, "bad loss_mode");
-    if (g->kernel < EM_KERNEL_AUTO || g->kernel > EM_KERNEL_FUSED) return fail(EM_ERR_INVALID_ARG, "bad kernel strategy");
+    if (g->kernel < EM_KERNEL_AUTO || g->kernel > EM_KERNEL_TMA) return fail(EM_ERR_INVALID_ARG, "bad kernel strategy");
     if (g->max_ports < 0 || g->max_source_edges < 0 || g->max_wave_samples < 0)
         return fail(EM_ERR_INVALID_ARG, "negative source capacity");
     return EM_OK;
@@ -241,12 +248,19 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
         const char *forced = std::getenv("EM_FUSED_ZSPLIT");      // tuning/test knob: force the z chunk count
         plan = em::make_fused_plan(g.nx, g.ny, g.nz, (int)sizeof(R), n_sm, forced ? std::atoi(forced) : 0);
     }
-    kernel = gr->kernel == EM_KERNEL_AUTO ? EM_KERNEL_FUSED : gr->kernel;
+    kernel = gr->kernel;
     const int max_items = plan.n_tiles * em::kFusedMaxZSplit;
     const size_t need = carve<R>(g, *gr, nullptr, nullptr, max_items);
     if (ws_bytes < need) return fail(EM_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
     carve<R>(g, *gr, workspace, &c, max_items);
-    main_kernel = kernel == EM_KERNEL_FUSED ? "k_fused_sweep" : "k_split_e";
+    sweep_smem = em::sweep_smem_bytes((int)sizeof(R), n_mat + 1);
+    if (kernel == EM_KERNEL_AUTO) {
+        int dev = 0, optin = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        kernel = sweep_smem <= (size_t)optin ? EM_KERNEL_TMA : EM_KERNEL_FUSED;   // very large tables: cp.async sweep
+    }
+    main_kernel = kernel == EM_KERNEL_TMA ? "k_sweep_tma" : kernel == EM_KERNEL_FUSED ? "k_fused_sweep" : "k_split_e";
 
     // ---- material table -> (eps/dt, sigma, mask, dt/mu), built in fp64, rounded once ----------
     table.assign(tab, tab + n_mat);
@@ -323,8 +337,48 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     CU(cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (plan.n_tiles * plan.nzs + 1), stream));
     int32_t rc = zero_state();
     if (rc) return rc;
+    if (kernel == EM_KERNEL_TMA) { rc = make_maps(); if (rc) return rc; }
     CU(cudaStreamSynchronize(stream));
     return EM_OK;
+}
+
+// ---- TMA descriptors of the sweep boxes (em_sweep.cuh) -----------------------------------------------
+// Field-like arrays: 3-D map over the padded allocation based at logical (-V, -1, -1) (16-B aligned:
+// V elements = 16 B), dims (PX, PY, PZ); box = 32 lanes x 16 (Ey, H) or 17 (Ex, Ez) rows x 1 plane;
+// q: box 30 lanes x 14 rows; ids (uint8): based 16 B before the row, box 32 V bytes x 18 rows.
+// Out-of-range box parts are zero-filled, which equals the pad content of the field arrays.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+template <typename R>
+int32_t Ctx<R>::make_maps() {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CU(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) return fail(EM_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+    EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(fn);
+    const int V = 16 / (int)sizeof(R);
+    const cuuint32_t ones[3] = {1, 1, 1};
+    auto encode = [&](CUtensorMap *m, CUtensorMapDataType dt, size_t esz, void *base, int bx, int by) -> int32_t {
+        const cuuint64_t dims[3] = {(cuuint64_t)g.PX, (cuuint64_t)g.PY, (cuuint64_t)g.PZ};
+        const cuuint64_t strides[2] = {(cuuint64_t)g.PX * esz, (cuuint64_t)g.PXY * esz};
+        const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
+        CUresult r = enc(m, dt, 3, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(EM_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+        return EM_OK;
+    };
+    const CUtensorMapDataType fdt = sizeof(R) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+    for (int a = 0; a < 12; ++a) {
+        const int comp = a % 3, is_e = a < 6;
+        const int rows = (is_e && comp != 1) ? 17 : 16;         // Ex, Ez carry row TY+1
+        int32_t rc = encode(&map_field[a], fdt, sizeof(R), c.field[a] + g.PX - V, 32 * V, rows);
+        if (rc) return rc;
+    }
+    int32_t rc = encode(&map_q, fdt, sizeof(R), c.q + g.PX - V, 30 * V, em::kSwTY);
+    if (rc) return rc;
+    return encode(&map_mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, c.mat + g.PX - em::kSwIdShift, 32 * V + 16, 18);
 }
 
 // ---- sources ------------------------------------------------------------------------------------
@@ -525,10 +579,25 @@ int32_t Ctx<R>::step_fused() {
 }
 
 template <typename R>
+int32_t Ctx<R>::step_tma() {
+    int32_t rc = record_begin(); if (rc) return rc;
+    em::FusedSources fsrc{c.tile_sbeg, c.tile_ent};
+    em::SweepMaps maps;
+    for (int a = 0; a < 3; ++a) { maps.E[a] = map_field[e_cur * 3 + a]; maps.H[a] = map_field[6 + h_cur * 3 + a]; }
+    maps.q = map_q; maps.mat = map_mat;
+    cudaError_t e = em::launch_sweep_tma<R>(plan, sweep_smem, maps, p, src, fsrc, loss, uniform_mu, (long long)step_index, stream);
+    if (e != cudaSuccess) return fail(EM_ERR_CUDA, std::string("TMA sweep launch: ") + cudaGetErrorString(e));
+    rc = record_end(); if (rc) return rc;
+    launches += 1;
+    e_cur ^= 1; h_cur ^= 1; bind();
+    return EM_OK;
+}
+
+template <typename R>
 int32_t Ctx<R>::step(int64_t n) {
     if (n < 0) return fail(EM_ERR_INVALID_ARG, "n < 0");
     for (int64_t s = 0; s < n; ++s) {
-        int32_t rc = (kernel == EM_KERNEL_FUSED) ? step_fused() : step_split();
+        int32_t rc = kernel == EM_KERNEL_TMA ? step_tma() : kernel == EM_KERNEL_FUSED ? step_fused() : step_split();
         if (rc) return rc;
         step_index += 1;
     }

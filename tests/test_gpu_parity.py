@@ -14,8 +14,9 @@ from parity import TOL, compare_state, rel_l2, subbox_problem
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [pytest.param(P.EM_KERNEL_SPLIT, id="split"), pytest.param(P.EM_KERNEL_FUSED, id="fused")]
-KNAME = {P.EM_KERNEL_SPLIT: "split", P.EM_KERNEL_FUSED: "fused"}
+KERNELS = [pytest.param(P.EM_KERNEL_SPLIT, id="split"), pytest.param(P.EM_KERNEL_FUSED, id="fused"),
+           pytest.param(P.EM_KERNEL_TMA, id="tma")]
+KNAME = {P.EM_KERNEL_SPLIT: "split", P.EM_KERNEL_FUSED: "fused", P.EM_KERNEL_TMA: "tma"}
 
 
 def run_pair(p, steps, precision, kernel, checkpoints=()):
