@@ -55,9 +55,9 @@ extern "C" {
 
 #define EM_MAT_PEC 1 /* em_material.flags bit0: every edge touching such a cell is held at 0      */
 
-/* em_grid.kernel: kernel strategy.  AUTO picks the TMA sweep (one launch per step, planes staged by
- * TMA, mbarrier-synchronised rows); FUSED is the same sweep with cp.async staging and CTA barriers;
- * SPLIT runs the separate H / E / Joule kernels.  All three are CUDA paths of this library and are
+/* em_grid.kernel: kernel strategy.  AUTO picks the FUSED sweep (one launch per step, planes staged by
+ * cp.async, CTA barriers; the fastest measured); TMA is the same sweep with cp.async.bulk.tensor
+ * staging and mbarrier-synchronised rows; SPLIT runs the separate H / E / Joule kernels.  All three are CUDA paths of this library and are
  * cross-checked against each other and the oracle in the tests. */
 #define EM_KERNEL_AUTO 0
 #define EM_KERNEL_SPLIT 1
