@@ -55,10 +55,11 @@ extern "C" {
 
 #define EM_MAT_PEC 1 /* em_material.flags bit0: every edge touching such a cell is held at 0      */
 
-/* em_grid.kernel: kernel strategy.  AUTO picks the FUSED sweep (one launch per step, planes staged by
- * cp.async, CTA barriers; the fastest measured); TMA is the same sweep with cp.async.bulk.tensor
- * staging and mbarrier-synchronised rows; SPLIT runs the separate H / E / Joule kernels.  All three are CUDA paths of this library and are
- * cross-checked against each other and the oracle in the tests. */
+/* em_grid.kernel: kernel strategy.  AUTO picks the TMA sweep (one launch per step; E, H and id planes
+ * staged by cp.async.bulk.tensor boxes counted on mbarriers; the fastest measured) and falls back to
+ * FUSED when the material table is too large for its shared-memory layout; FUSED is the same sweep
+ * with per-thread cp.async staging; SPLIT runs the separate H / E / Joule kernels.  All three are CUDA
+ * paths of this library and are cross-checked against each other and the oracle in the tests. */
 #define EM_KERNEL_AUTO 0
 #define EM_KERNEL_SPLIT 1
 #define EM_KERNEL_FUSED 2

@@ -254,7 +254,7 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     if (ws_bytes < need) return fail(EM_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
     carve<R>(g, *gr, workspace, &c, max_items);
     sweep_smem = em::sweep_smem_bytes((int)sizeof(R), n_mat + 1);
-    if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_FUSED;   // measured on config 4: fused 2.71 ms/step, TMA sweep 5.9 ms/step
+    if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_TMA;     // measured on config 4: TMA sweep 2.44 ms/step, cp.async sweep 2.71 ms/step
     if (kernel == EM_KERNEL_TMA) {
         int dev = 0, optin = 0;
         CU(cudaGetDevice(&dev));

@@ -3,23 +3,17 @@
 // (eq. (2)-(3) L69-L76 in leapfrog form, L86 for the Joule heat) and moves each
 // field value through HBM once per step: 57 B (fp32) / 113 B (fp64) per cell-update.
 //
-// Same decomposition and arithmetic as em_fused.cuh (tile = 30V x 14 columns marched in z, warp = one
-// row, lane = V consecutive x, halo lanes/rows recompute), but the data movement and the
-// synchronisation are Blackwell-native:
-//  * every input plane (E, H, q, material ids) is staged into shared memory by TMA
-//    (cp.async.bulk.tensor.3d, one box per array per plane, issued by one thread, completion counted
-//    on an mbarrier): no per-thread address arithmetic, no LSU traffic for the loads, two planes in
-//    flight per SM;
-//  * there is NO CTA-wide barrier in the plane loop.  A warp waits only for what it consumes:
-//      full[s]    : the TMA boxes of plane k have landed            (producer -> all warps)
-//      flagH[w]   : warp w has published H'(k) of its row          (row w -> row w+1, E update)
-//      flagB[w]   : warp w has published (2 Ebar)^2 of its row     (row w -> row w-1, Joule sum)
-//      emptyA[s]  : every warp has finished reading stage s         (all warps -> producer)
-//    so the warps of a CTA drift by up to a phase and the shared-memory-heavy and the FMA-heavy parts of
-//    different rows overlap instead of running in lock step;
-//  * the coefficient partial means of the previous plane are recomputed from the id ring instead of
-//    being carried (frees 48 KB of shared memory for the second stage and the double-buffered rows).
-// Warp 0 (halo row -1: only H') is also the TMA producer.
+// Same decomposition, arithmetic and barrier structure as em_fused.cuh (tile = 30V x 14 columns marched in
+// z, warp = one row, lane = V consecutive x, halo lanes/rows recompute, two CTA barriers per plane, phase B
+// shared through em_fused_phaseb*.inc), but the input planes are staged by TMA instead of per-thread
+// cp.async:
+//  * every E, H and material-id plane of the tile is ONE cp.async.bulk.tensor.3d box per array, issued by
+//    one thread and counted on an mbarrier: no per-thread address arithmetic, no LDGSTS instructions and
+//    no LSU shared-memory write wavefronts for the loads (they were ~11 % of the instructions of the
+//    cp.async sweep);
+//  * a box lands row-major, 512 B per row, i.e. exactly in the [row = warp][lane] x 16 B slot format the
+//    threads read; the boxes of Ex and Ez carry a 17th row (the top warp's +1 neighbour);
+//  * q (conditionally fetched: lossless lanes skip it) and the per-plane z geometry stay on cp.async.
 #pragma once
 #include <cuda.h>
 
@@ -32,6 +26,7 @@ constexpr int kSwWarps = kSwTY + 2;                // rows -1 .. TY
 constexpr int kSwThreads = kSwWarps * 32;          // 512
 constexpr int kSwRow = 512;                        // bytes of one staged row (32 lanes x 16 B)
 constexpr int kSwIdShift = 16;                     // the id map starts 16 B before the row (16-B aligned base)
+constexpr int kSwPriv = 10;                        // private 16-B slots per thread: q, L x 6, H' x 2, pend
 
 struct alignas(64) SweepMaps { CUtensorMap E[3], H[3], q, mat; };
 
@@ -43,25 +38,22 @@ template <int SZ> struct SweepLayout {
     static constexpr int ex_slot = 17 * kSwRow;
     static constexpr int ey = ex + 3 * ex_slot;                   // Ey ring of 3 planes, rows -1 .. TY
     static constexpr int ey_slot = 16 * kSwRow;
-    static constexpr int ez = ey + 3 * ey_slot;                   // Ez, 2 stages, rows -1 .. TY+1
+    static constexpr int ez = ey + 3 * ey_slot;                   // Ez, 2 parities, rows -1 .. TY+1
     static constexpr int ez_slot = 17 * kSwRow;
-    static constexpr int h = ez + 2 * ez_slot;                    // [stage][Hx, Hy, Hz], rows -1 .. TY
+    static constexpr int h = ez + 2 * ez_slot;                    // Hx, Hy, Hz of plane k, rows -1 .. TY
     static constexpr int h_slot = 16 * kSwRow;
-    static constexpr int q = h + 6 * h_slot;                      // q ring of 3 layers: TY rows x 30 lanes
-    static constexpr int q_row = 30 * 16;
-    static constexpr int q_slot = (kSwTY * q_row + 127) / 128 * 128;
-    static constexpr int ids = q + 3 * q_slot;                    // id ring of 4 planes, rows -2 .. TY+1
+    static constexpr int ids = h + 3 * h_slot;                    // ids, 2 parities, rows -2 .. TY+1
     static constexpr int id_row = 32 * V + 16;                    // box starts on a 16-B boundary: up to 15 B of lead-in
     static constexpr int id_slot = (18 * id_row + 127) / 128 * 128;
-    static constexpr int rows = ids + 4 * id_slot;                // [H'x, H'z, Bx, Bz][parity][16 rows]
-    static constexpr int rows_slot = 16 * kSwRow;
-    static constexpr int carry = rows + 8 * rows_slot;            // H'y of plane k-1
-    static constexpr int geo = carry + 16 * kSwRow;               // 1/dx, 1/dx~, fx of the 32 lanes
-    static constexpr int bar = geo + 3 * kSwRow;                  // full[2], emptyA[2], flagH[16], flagB[16]
-    static constexpr int tab = bar + 8 * (4 + 2 * kSwWarps) + 64; // material table (n_table entries)
-    static constexpr int stage_bytes = ex_slot + ey_slot + ez_slot + 3 * h_slot + 18 * id_row;
-    static constexpr int q_bytes = kSwTY * q_row;
-    static constexpr int first_extra_bytes = ex_slot + ey_slot + 18 * id_row;
+    static constexpr int priv = ids + 2 * id_slot;                // private slots [kSwPriv][512 threads]
+    static constexpr int rows = priv + kSwPriv * 16 * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kFusedRows][32]
+    static constexpr int geo = rows + 4 * kFusedRows * kSwRow;    // 1/dx, 1/dx~, fx of the 32 lanes
+    static constexpr int zg = geo + 3 * kSwRow;                   // [2 parity]{fz, 1/dz, 1/dz~, 0}
+    static constexpr int bar = zg + 64;                           // fullE[2], fullH
+    static constexpr int tab = bar + 64;                          // material table (n_table entries)
+    static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + 18 * id_row;
+    static constexpr int first_extra_bytes = ex_slot + ey_slot;
+    static constexpr int h_bytes = 3 * h_slot;
 };
 
 inline size_t sweep_smem_bytes(int sizeof_real, int n_table) {
@@ -102,9 +94,12 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             FusedChunks zc, int ntx, long long step) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TXo = 30 * V;
+    constexpr int NT = kSwThreads;
     using L = SweepLayout<(int)sizeof(R)>;
     using VecR = Vec<R>;
     using IdT = typename std::conditional<V == 4, unsigned, unsigned short>::type;
+    // private slot numbering of this kernel (shadows the cp.async sweep's enum inside em_fused_phaseb*.inc)
+    constexpr int kSlotQ = 0, kSlotL = 1, kSlotHp = 7, kSlotPend = 9;
     extern __shared__ __align__(1024) unsigned char sm[];
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -114,7 +109,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     const int tx = tile % ntx, ty = tile / ntx;
     const int kz0 = zc.kb[chunk], kz1 = zc.kb[chunk + 1];
     const int ks = kz0 > 0 ? kz0 - 1 : 0, ke = kz1 <= p.nz ? kz1 : p.nz;
-    const int cy = w - 1;
+    const int cy = w - 1, r = cy + 2;
     const int j = ty * kSwTY + cy;
     const int i0 = tx * TXo - V + V * lane;
     const int ny = p.ny, nz = p.nz;
@@ -126,37 +121,39 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     const unsigned out_pack = (unsigned)(p.n_table - 1) * 0x01010101u;
 
     // shared-memory views
-    const int my = w * kSwRow + lane * 16;                    // this thread's vector inside a staged slot
     MatEntry<R> *s_tab = reinterpret_cast<MatEntry<R> *>(sm + L::tab);
-    const VecR *s_geo = reinterpret_cast<const VecR *>(sm + L::geo);
-    auto ldsv = [&](int byte_off) -> VecR { return *reinterpret_cast<const VecR *>(sm + byte_off); };
-    auto stsv = [&](int byte_off, const VecR &v) { *reinterpret_cast<VecR *>(sm + byte_off) = v; };
-    auto rows_off = [&](int arr, int par, int row) -> int { return L::rows + ((arr * 2 + par) * 16 + row) * kSwRow + lane * 16; };
-    const int carry_hy = L::carry + my;
+    VecR *s_rows = reinterpret_cast<VecR *>(sm + L::rows);
+    VecR(*smHx)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 0 * kFusedRows * 32);
+    VecR(*smHz)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 1 * kFusedRows * 32);
+    VecR(*smBx)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 2 * kFusedRows * 32);
+    VecR(*smBz)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 3 * kFusedRows * 32);
+    VecR *mine = reinterpret_cast<VecR *>(sm + L::priv) + tid;    // private slots [kSwPriv][NT]
+    VecR *s_geo = reinterpret_cast<VecR *>(sm + L::geo);
+    R *s_z = reinterpret_cast<R *>(sm + L::zg);
+    const VecR *stg = reinterpret_cast<const VecR *>(sm) + tid;   // this thread's vector inside a staged box
+    auto staged = [&](int byte_off) -> VecR { return *reinterpret_cast<const VecR *>(reinterpret_cast<const unsigned char *>(stg) + byte_off); };
     const unsigned bar0 = smem_u32(sm + L::bar);
-    auto bar_full = [&](int s) -> unsigned { return bar0 + 8 * s; };
-    auto bar_empty = [&](int s) -> unsigned { return bar0 + 8 * (2 + s); };
-    auto bar_H = [&](int ww) -> unsigned { return bar0 + 8 * (4 + ww); };
-    auto bar_B = [&](int ww) -> unsigned { return bar0 + 8 * (4 + kSwWarps + ww); };
+    auto bar_fullE = [&](int s) -> unsigned { return bar0 + 8 * s; };
+    const unsigned bar_fullH = bar0 + 16;
 
-    // ---- prologue: barriers, table, x geometry, zeroed exchange rows and carries ----------------------------
+    // ---- prologue: barriers, table, x geometry, zeroed exchange rows and private slots -------------------
     if (tid == 0) {
-        for (int s = 0; s < 2; ++s) { mbar_init(bar_full(s), 1); mbar_init(bar_empty(s), kSwWarps); }
-        for (int ww = 0; ww < kSwWarps; ++ww) { mbar_init(bar_H(ww), 1); mbar_init(bar_B(ww), 1); }
+        mbar_init(bar_fullE(0), 1); mbar_init(bar_fullE(1), 1); mbar_init(bar_fullH, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int t = tid; t < p.n_table; t += kSwThreads) s_tab[t] = p.table[t];
+    for (int t = tid; t < p.n_table; t += NT) s_tab[t] = p.table[t];
     {
-        VecR z;
+        VecR z, one;
 #pragma unroll
-        for (int c = 0; c < V; ++c) z.v[c] = R(0);
-        for (int t = tid; t < 8 * 16 * 32; t += kSwThreads) reinterpret_cast<VecR *>(sm + L::rows)[t] = z;
-        stsv(carry_hy, z);
+        for (int c = 0; c < V; ++c) { z.v[c] = R(0); one.v[c] = R(1); }
+        for (int t = tid; t < 4 * kFusedRows * 32; t += NT) s_rows[t] = z;
+        for (int t = 0; t < kSwPriv; ++t) mine[t * NT] = z;
+        mine[(kSlotL + 0) * NT] = one; mine[(kSlotL + 3) * NT] = one;
         if (w == 0) {
             const bool in = (i0 + V <= p.PX);
-            reinterpret_cast<VecR *>(sm + L::geo)[0 * 32 + lane] = in ? *reinterpret_cast<const VecR *>(p.rdx + i0) : z;
-            reinterpret_cast<VecR *>(sm + L::geo)[1 * 32 + lane] = in ? *reinterpret_cast<const VecR *>(p.rtx + i0) : z;
-            reinterpret_cast<VecR *>(sm + L::geo)[2 * 32 + lane] = in ? *reinterpret_cast<const VecR *>(p.fx + i0) : z;
+            s_geo[0 * 32 + lane] = in ? *reinterpret_cast<const VecR *>(p.rdx + i0) : z;
+            s_geo[1 * 32 + lane] = in ? *reinterpret_cast<const VecR *>(p.rtx + i0) : z;
+            s_geo[2 * 32 + lane] = in ? *reinterpret_cast<const VecR *>(p.fx + i0) : z;
         }
     }
     __syncthreads();
@@ -165,60 +162,60 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     const int cx = tx * TXo, cyy = ty * kSwTY;
     // a box must start on a 16-B boundary: the id box starts at the boundary at or below the tile's first id
     const int id_x = (cx - V + kSwIdShift) & ~15, id_lead = (cx - V + kSwIdShift) & 15;
-    // stage s = plane s: Ex(s+1), Ey(s+1), Ez(s), H(s), ids(s) and q(s-1) (consumed by phase C of plane s)
-    auto issue_stage = [&](int s, bool first) {
-        const bool with_q = (s - 1 >= kz0) && (s <= ke);
-        const unsigned bar = bar_full(s & 1);
+    // E group of plane kk: Ex(kk+1), Ey(kk+1) -> ring slot (kk+1)%3, Ez(kk) and ids(kk) -> parity kk&1
+    auto issue_E = [&](int kk, bool first) {
+        const unsigned bar = bar_fullE((kk - ks) & 1);
         const unsigned sb = smem_u32(sm);
-        mbar_expect_tx(bar, (unsigned)(L::stage_bytes + (with_q ? L::q_bytes : 0) + (first ? L::first_extra_bytes : 0)));
+        mbar_expect_tx(bar, (unsigned)(L::e_bytes + (first ? L::first_extra_bytes : 0)));
         if (first) {
-            tma_load_3d(sb + L::ex + (s % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, s + 1);
-            tma_load_3d(sb + L::ey + (s % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, s + 1);
-            tma_load_3d(sb + L::ids + ((s + 3) & 3) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, s);
+            tma_load_3d(sb + L::ex + (kk % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 1);
+            tma_load_3d(sb + L::ey + (kk % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 1);
         }
-        tma_load_3d(sb + L::ex + ((s + 1) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, s + 2);
-        tma_load_3d(sb + L::ey + ((s + 1) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, s + 2);
-        tma_load_3d(sb + L::ez + (s & 1) * L::ez_slot, &maps.E[2], bar, cx, cyy, s + 1);
-        tma_load_3d(sb + L::h + ((s & 1) * 3 + 0) * L::h_slot, &maps.H[0], bar, cx, cyy, s + 1);
-        tma_load_3d(sb + L::h + ((s & 1) * 3 + 1) * L::h_slot, &maps.H[1], bar, cx, cyy, s + 1);
-        tma_load_3d(sb + L::h + ((s & 1) * 3 + 2) * L::h_slot, &maps.H[2], bar, cx, cyy, s + 1);
-        tma_load_3d(sb + L::ids + (s & 3) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, s + 1);
-        if (with_q) tma_load_3d(sb + L::q + ((s + 2) % 3) * L::q_slot, &maps.q, bar, cx + V, cyy + 1, s);
+        tma_load_3d(sb + L::ex + ((kk + 1) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 2);
+        tma_load_3d(sb + L::ey + ((kk + 1) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 2);
+        tma_load_3d(sb + L::ez + (kk & 1) * L::ez_slot, &maps.E[2], bar, cx, cyy, kk + 1);
+        tma_load_3d(sb + L::ids + (kk & 1) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, kk + 1);
     };
-#if defined(EM_SW_STOP) && EM_SW_STOP == 1
-    return;
-#endif
+    auto issue_H = [&](int kk) {
+        const unsigned sb = smem_u32(sm);
+        mbar_expect_tx(bar_fullH, (unsigned)L::h_bytes);
+        tma_load_3d(sb + L::h + 0 * L::h_slot, &maps.H[0], bar_fullH, cx, cyy, kk + 1);
+        tma_load_3d(sb + L::h + 1 * L::h_slot, &maps.H[1], bar_fullH, cx, cyy, kk + 1);
+        tma_load_3d(sb + L::h + 2 * L::h_slot, &maps.H[2], bar_fullH, cx, cyy, kk + 1);
+    };
+    // z geometry of plane kk -> parity kk&1 (cp.async, same group as q)
+    auto issue_z = [&](int kk) {
+        if (tid < (int)sizeof(R) / 4 && kk <= ke)
+            cp_async16(reinterpret_cast<unsigned char *>(&s_z[(kk & 1) * 4]) + 16 * tid,
+                       reinterpret_cast<const unsigned char *>(p.zgeo + 4 * (long long)kk) + 16 * tid);
+    };
     if (tid == 0) {
-        issue_stage(ks, true);
-        if (ks + 1 <= ke) issue_stage(ks + 1, false);
+        issue_E(ks, true);
+        issue_H(ks);
+        if (ks + 1 <= ke) issue_E(ks + 1, false);
     }
-#if defined(EM_SW_STOP) && EM_SW_STOP == 2
-    mbar_wait(bar_full(ks & 1), 0);
-    if (ks + 1 <= ke) mbar_wait(bar_full((ks + 1) & 1), 0);
-    return;
-#endif
-#if defined(EM_SW_STOP) && EM_SW_STOP == 3
-    if (tid == 0) { mbar_wait(bar_full(ks & 1), 0); if (ks + 1 <= ke) mbar_wait(bar_full((ks + 1) & 1), 0); }
+    issue_z(ks); issue_z(ks + 1);
+    cp_async_commit();
+    cp_async_wait<0>();
     __syncthreads();
-    return;
-#endif
 
     const R fy = active ? p.fy[j] : R(0), rdy = active ? p.rdy[j] : R(0), rty = active ? p.rty[j] : R(0);
     const R gq = p.dt * R(0.0625);
-    const long long off0 = (long long)j * PX + i0;    // this thread's vector at plane 0 (stores)
+    const long long off0 = (long long)j * PX + i0;    // this thread's vector at plane 0 (stores, q)
+    // all V cells of an id word hold the same material
     auto id_uniform = [&](unsigned wv) -> bool { return (V == 4) ? (wv == (wv & 0xffu) * 0x01010101u) : (((wv >> 8) & 0xffu) == (wv & 0xffu)); };
-    // ids of the lane's V cells of row `row` (0 = j-2 .. 17) of plane slot `slot`
+    // ids of the lane's V cells of row `row` (0 = j0-2 .. 17) of parity slot `slot`
     auto ld_ids = [&](int slot, int row) -> unsigned {
         const unsigned v = *reinterpret_cast<const IdT *>(sm + L::ids + slot * L::id_slot + row * L::id_row + id_lead + lane * V);
         return (V == 4) ? v : (v | (out_pack & 0xffff0000u));
     };
 
-    unsigned idw_prev = out_pack;                     // set on the first plane from the staged ids of plane ks-1
+    unsigned idw_prev = out_pack;
     bool rowu_prev = false;      // plane k-1: rows j-1 and j of this lane held one material
-    VecR pend;                   // Joule partial sum Sxy(k-1) + Sz(k-1) of layer k-1
-#pragma unroll
-    for (int c = 0; c < V; ++c) pend.v[c] = R(0);
-    bool q_live = false;         // q of layer k-1 must be stored (some sigma != 0 among the lane's cells)
+    bool l_stale = false;        // warp-uniform: the L slots were skipped by the one-material path
+    bool q_live = false;         // q of layer k-1 was fetched (some sigma != 0 among the lane's cells)
+    // source cursor: starts at the tile's first entry with k >= kz0 and may run into the next chunk's
+    // entries on the closing plane k = kz1 (E'(kz1) enters the Joule sum of layer kz1-1)
     int s_cur = fs.tile_sbeg[item];
     const int s_end = fs.tile_sbeg[(tile + 1) * zc.nzs];
     int s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
@@ -230,30 +227,21 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         const int par = k & 1;
         const long long o = off0 + (long long)k * PXY;
         const bool st = own && k >= kz0 && k < kz1;          // this chunk stores H'(k), E'(k)
-        const VecR zg = *reinterpret_cast<const VecR *>(p.zgeo + 4 * (long long)k);   // {fz, 1/dz, 1/dz~, 0} (V = 2: first two)
-        const R fz = zg.v[0], rdz = zg.v[1];
-        const R rtz = (V == 4) ? zg.v[V == 4 ? 2 : 0] : p.zgeo[4 * (long long)k + 2];
+        const R fz = s_z[par * 4 + 0], rdz = s_z[par * 4 + 1], rtz = s_z[par * 4 + 2];
 
-        mbar_wait(bar_full(par), (unsigned)(it >> 1) & 1u);  // the TMA boxes of plane k have landed
-        const unsigned idw = ld_ids(k & 3, w + 1), idj = ld_ids(k & 3, w);
-        if (it == 0) {
-            idw_prev = ld_ids((k + 3) & 3, w + 1);
-            rowu_prev = (idw_prev == ld_ids((k + 3) & 3, w)) && id_uniform(idw_prev);
-        }
+        // ---- phase A: H' = H - nbar * curl E  (PAPER.md L65: inner factor of S = curl mu^-1 curl) ----------
+        mbar_wait(bar_fullE(it & 1), (unsigned)(it >> 1) & 1u);   // E group of plane k has landed
+        const unsigned idw = ld_ids(par, w + 1), idj = ld_ids(par, w);
         // one material over the warp's whole coefficient neighbourhood (rows j-1..j, planes k-1..k)?
         const bool rowu = (idw == idj) && id_uniform(idw);
         const unsigned idw_lane0 = __shfl_sync(0xffffffffu, idw, 0);   // (every lane must execute it)
         const bool hom = __all_sync(0xffffffffu, rowu && rowu_prev && idw == idw_prev && idw == idw_lane0);
-
-        // ---- phase A: H' = H - nbar * curl E  (PAPER.md L65: inner factor of S = curl mu^-1 curl) ----------
         VecR hxn, hyn, hzn;
-        const VecR ex0 = ldsv(L::ex + rk * L::ex_slot + my), ey0 = ldsv(L::ey + rk * L::ey_slot + my);
-        const VecR ez = ldsv(L::ez + par * L::ez_slot + my);
+        const VecR ex0 = staged(L::ex + rk * L::ex_slot), ey0 = staged(L::ey + rk * L::ey_slot);
+        const VecR ez = staged(L::ez + par * L::ez_slot);
         {
-            const VecR ex1 = ldsv(L::ex + rk1 * L::ex_slot + my), ey1 = ldsv(L::ey + rk1 * L::ey_slot + my);
-            const VecR hx = ldsv(L::h + (par * 3 + 0) * L::h_slot + my), hy = ldsv(L::h + (par * 3 + 1) * L::h_slot + my);
-            const VecR hz = ldsv(L::h + (par * 3 + 2) * L::h_slot + my);
-            const VecR exn = ldsv(L::ex + rk * L::ex_slot + my + kSwRow), ezn = ldsv(L::ez + par * L::ez_slot + my + kSwRow);
+            const VecR ex1 = staged(L::ex + rk1 * L::ex_slot), ey1 = staged(L::ey + rk1 * L::ey_slot);
+            const VecR exn = staged(L::ex + rk * L::ex_slot + kSwRow), ezn = staged(L::ez + par * L::ez_slot + kSwRow);
             const R ey0_r = shfl_down1(ey0.v[0]), ez_r = shfl_down1(ez.v[0]);
             const VecR rdxv = s_geo[0 * 32 + lane];
             VecR nbx, nby, nbz;
@@ -276,6 +264,8 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
                     nbz.v[c] = lerp(nk, ncur[c], fz);
                 }
             }
+            mbar_wait(bar_fullH, (unsigned)it & 1u);              // H(k) has landed
+            const VecR hx = staged(L::h + 0 * L::h_slot), hy = staged(L::h + 1 * L::h_slot), hz = staged(L::h + 2 * L::h_slot);
 #pragma unroll
             for (int c = 0; c < V; ++c) {
                 const R eyip = (c < V - 1) ? ey0.v[c < V - 1 ? c + 1 : c] : ey0_r;
@@ -294,72 +284,79 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             *reinterpret_cast<VecR *>(p.Hn[1] + o) = hyn;
             *reinterpret_cast<VecR *>(p.Hn[2] + o) = hzn;
         }
-        stsv(rows_off(0, par, w), hxn); stsv(rows_off(1, par, w), hzn);
-        __syncwarp();
-        if (lane == 0) {
-            mbar_arrive(bar_H(w));                    // H'(k) of this row is visible
-            mbar_arrive(bar_empty(par));              // this warp is done with the staged fields of plane k
-            if (w == 0 && k + 2 <= ke) {              // producer: refill the stage once all 16 warps released it
-                mbar_wait(bar_empty(par), (unsigned)(it >> 1) & 1u);
-                issue_stage(k + 2, false);
-            }
-        }
+        smHx[r][lane] = hxn; smHz[r][lane] = hzn;
+        __syncthreads();                          // B2: H' rows visible; every thread holds H(k) in registers
+        if (tid == 0 && k + 1 <= ke) issue_H(k + 1);
 
+        // ---- phase B: E' = E + r (curl H' - J - sigma E), Joule squares (eq. 2-3) -------------
+        // (warp 0 = halo row -1 only supplies H' to row 0: no E', no Joule)
+        VecR bx, by, bz;         // (2 Ebar)^2
         if (w != 0) {
-            // ---- phase B: E' = E + r (curl H' - J - sigma E), Joule squares (eq. 2-3) --------
-            mbar_wait(bar_H(w - 1), (unsigned)it & 1u);       // H'(k) of row j-1
-            VecR bx, by, bz;         // (2 Ebar)^2
             if (hom && s_next_k > k) {
-#include "em_sweep_phaseb_hom.inc"
-            } else if (s_next_k <= k) {
-#define EM_HAS_J 1
-#include "em_sweep_phaseb.inc"
-#undef EM_HAS_J
-                s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
+#include "em_fused_phaseb_hom.inc"
+                l_stale = true;
             } else {
-#define EM_HAS_J 0
-#include "em_sweep_phaseb.inc"
+                if (l_stale) {   // plane k-1 took the one-material path: its coefficient means are the entry itself
+                    const MatEntry<R> Ap = s_tab[idw_prev & 0xff];
+                    VecR va, vb, vm;
+#pragma unroll
+                    for (int c = 0; c < V; ++c) { va.v[c] = Ap.a; vb.v[c] = Ap.b; vm.v[c] = Ap.m * Ap.m; }
+                    mine[(kSlotL + 0) * NT] = va; mine[(kSlotL + 1) * NT] = vb; mine[(kSlotL + 2) * NT] = vm;
+                    mine[(kSlotL + 3) * NT] = va; mine[(kSlotL + 4) * NT] = vb; mine[(kSlotL + 5) * NT] = vm;
+                    l_stale = false;
+                }
+                if (s_next_k <= k) {
+#define EM_HAS_J 1
+#include "em_fused_phaseb.inc"
 #undef EM_HAS_J
+                    s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
+                } else {
+#define EM_HAS_J 0
+#include "em_fused_phaseb.inc"
+#undef EM_HAS_J
+                }
             }
             if (!active) {
 #pragma unroll
                 for (int c = 0; c < V; ++c) bx.v[c] = by.v[c] = bz.v[c] = R(0);
             }
-            stsv(rows_off(2, par, w), bx); stsv(rows_off(3, par, w), bz);
-            stsv(carry_hy, hyn);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_B(w));             // (2 Ebar)^2 of this row is visible
-
-            // ---- phase C: q(k-1) += dt sigma/16 (pend + Sxy(k)); pend = Sxy(k) + Sz(k) ----------------------
-            if (!is_top) {
-                mbar_wait(bar_B(w + 1), (unsigned)it & 1u);   // row j+1
-                const VecR bxn = ldsv(rows_off(2, par, w + 1)), bzn = ldsv(rows_off(3, par, w + 1));
-                const R by_r = shfl_down1(by.v[0]), bz_r = shfl_down1(bz.v[0]), bzn_r = shfl_down1(bzn.v[0]);
-                const bool have_q = own_q && k > kz0 && q_live;                      // layer k-1 in [kz0, kz1)
-                VecR qv;
-                if (have_q) qv = ldsv(L::q + ((k + 2) % 3) * L::q_slot + (w - 1) * L::q_row + (lane - 1) * 16);
-#pragma unroll
-                for (int c = 0; c < V; ++c) {
-                    const R byip = (c < V - 1) ? by.v[c < V - 1 ? c + 1 : c] : by_r;
-                    const R bzip = (c < V - 1) ? bz.v[c < V - 1 ? c + 1 : c] : bz_r;
-                    const R bznip = (c < V - 1) ? bzn.v[c < V - 1 ? c + 1 : c] : bzn_r;
-                    const R sxy = (bx.v[c] + bxn.v[c]) + (by.v[c] + byip);
-                    const R sz = (bz.v[c] + bzip) + (bzn.v[c] + bznip);
-                    const R sg = s_tab[(idw_prev >> (8 * (hom ? 0 : c))) & 0xff].b;     // sigma of the cell of layer k-1
-                    if (have_q) qv.v[c] = mad(gq * sg, pend.v[c] + sxy, qv.v[c]);
-                    pend.v[c] = sxy + sz;
-                }
-                // q of a lane whose V cells are one lossless material never changes: not stored
-                if (have_q) *reinterpret_cast<VecR *>(p.q + o - PXY) = qv;
-                q_live = !(id_uniform(idw) && s_tab[idw & 0xff].b == R(0));
-            }
-        } else {
-            mbar_wait(bar_B(1), (unsigned)it & 1u);           // throttle: row -1 stays within one plane of row 0
+            smBx[r][lane] = bx; smBz[r][lane] = bz;
+            mine[(kSlotHp + 0) * NT] = hxn; mine[(kSlotHp + 1) * NT] = hyn;
         }
+        cp_async_wait<0>();                       // q(k-1) and the z geometry of plane k+1 have landed
+        __syncthreads();                          // B3: B rows and z geometry visible; the staged E(k), ids(k) are dead
+        if (tid == 0 && k + 2 <= ke) issue_E(k + 2, false);
+
+        // ---- phase C: q(k-1) += dt sigma/16 (pend + Sxy(k)); pend = Sxy(k) + Sz(k) ---------------------------
+        if (w != 0 && !is_top) {
+            const VecR bxn = smBx[r + 1][lane], bzn = smBz[r + 1][lane];
+            const R by_r = shfl_down1(by.v[0]), bz_r = shfl_down1(bz.v[0]), bzn_r = shfl_down1(bzn.v[0]);
+            VecR qv = mine[kSlotQ * NT];
+            VecR pend = mine[kSlotPend * NT];
+#pragma unroll
+            for (int c = 0; c < V; ++c) {
+                const R byip = (c < V - 1) ? by.v[c < V - 1 ? c + 1 : c] : by_r;
+                const R bzip = (c < V - 1) ? bz.v[c < V - 1 ? c + 1 : c] : bz_r;
+                const R bznip = (c < V - 1) ? bzn.v[c < V - 1 ? c + 1 : c] : bzn_r;
+                const R sxy = (bx.v[c] + bxn.v[c]) + (by.v[c] + byip);
+                const R sz = (bz.v[c] + bzip) + (bzn.v[c] + bznip);
+                const R sg = s_tab[(idw_prev >> (8 * (hom ? 0 : c))) & 0xff].b;     // sigma of the cell of layer k-1
+                qv.v[c] = mad(gq * sg, pend.v[c] + sxy, qv.v[c]);
+                pend.v[c] = sxy + sz;
+            }
+            mine[kSlotPend * NT] = pend;
+            // q of a lane whose V cells are one lossless material never changes: neither fetched nor stored
+            if (own_q && k > kz0 && q_live) *reinterpret_cast<VecR *>(p.q + o - PXY) = qv;   // layer k-1 in [kz0, kz1)
+            q_live = !(id_uniform(idw) && s_tab[idw & 0xff].b == R(0));
+            if (own_q && k >= kz0 && k < ke && q_live) cp_async16(mine + kSlotQ * NT, p.q + o);   // q(k)
+        }
+        issue_z(k + 2);
+        cp_async_commit();
         idw_prev = idw;
         rowu_prev = rowu;
         rk = rk1;
     }
+    cp_async_wait<0>();
 }
 
 template <typename R>
