@@ -24,6 +24,8 @@
 
 namespace em {
 
+#define EM_ST(ptr, val) (*reinterpret_cast<VecR *>(ptr) = (val))     // output stores of the phase-B includes
+
 #ifndef EM_FUSED_TY
 #define EM_FUSED_TY 14
 #endif

@@ -361,12 +361,14 @@ int32_t Ctx<R>::make_maps() {
     EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(fn);
     const int V = 16 / (int)sizeof(R);
     const cuuint32_t ones[3] = {1, 1, 1};
+    const char *pe = std::getenv("EM_TMA_L2PROMO");           // tuning knob: 0 none, 1 64 B, 2 128 B (default), 3 256 B
+    const CUtensorMapL2promotion promo = pe ? (CUtensorMapL2promotion)std::atoi(pe) : CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
     auto encode = [&](CUtensorMap *m, CUtensorMapDataType dt, size_t esz, void *base, int bx, int by) -> int32_t {
         const cuuint64_t dims[3] = {(cuuint64_t)g.PX, (cuuint64_t)g.PY, (cuuint64_t)g.PZ};
         const cuuint64_t strides[2] = {(cuuint64_t)g.PX * esz, (cuuint64_t)g.PXY * esz};
         const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
         CUresult r = enc(m, dt, 3, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                         CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(EM_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
         return EM_OK;
     };

@@ -5,7 +5,7 @@
 //
 // Same decomposition, arithmetic and barrier structure as em_fused.cuh (tile = 30V x 14 columns marched in
 // z, warp = one row, lane = V consecutive x, halo lanes/rows recompute, two CTA barriers per plane, phase B
-// shared through em_fused_phaseb*.inc), but the input planes are staged by TMA instead of per-thread
+// as in em_fused_phaseb*.inc), but the input planes are staged by TMA instead of per-thread
 // cp.async:
 //  * every E, H and material-id plane of the tile is ONE cp.async.bulk.tensor.3d box per array, issued by
 //    one thread and counted on an mbarrier: no per-thread address arithmetic, no LDGSTS instructions and
@@ -21,12 +21,19 @@
 
 namespace em {
 
+#undef EM_ST
+#ifdef EM_EXP_NOSTCS
+#define EM_ST(ptr, val) (*reinterpret_cast<VecR *>(ptr) = (val))
+#else
+#define EM_ST(ptr, val) st_stream16((ptr), (val))     // output planes: streaming stores
+#endif
+
 constexpr int kSwTY = kFusedTY;                    // 14 owned rows
 constexpr int kSwWarps = kSwTY + 2;                // rows -1 .. TY
 constexpr int kSwThreads = kSwWarps * 32;          // 512
 constexpr int kSwRow = 512;                        // bytes of one staged row (32 lanes x 16 B)
 constexpr int kSwIdShift = 16;                     // the id map starts 16 B before the row (16-B aligned base)
-constexpr int kSwPriv = 10;                        // private 16-B slots per thread: q, L x 6, H' x 2, pend
+constexpr int kSwPriv = 8;                         // private 16-B slots per thread: q, L x 4, H' x 2, pend
 
 struct alignas(64) SweepMaps { CUtensorMap E[3], H[3], q, mat; };
 
@@ -40,16 +47,16 @@ template <int SZ> struct SweepLayout {
     static constexpr int ey_slot = 16 * kSwRow;
     static constexpr int ez = ey + 3 * ey_slot;                   // Ez, 2 parities, rows -1 .. TY+1
     static constexpr int ez_slot = 17 * kSwRow;
-    static constexpr int h = ez + 2 * ez_slot;                    // Hx, Hy, Hz of plane k, rows -1 .. TY
+    static constexpr int h = ez + 2 * ez_slot;                    // [2 parities][Hx, Hy, Hz], rows -1 .. TY
     static constexpr int h_slot = 16 * kSwRow;
-    static constexpr int ids = h + 3 * h_slot;                    // ids, 2 parities, rows -2 .. TY+1
+    static constexpr int ids = h + 6 * h_slot;                    // ids, 2 parities, rows -2 .. TY+1
     static constexpr int id_row = 32 * V + 16;                    // box starts on a 16-B boundary: up to 15 B of lead-in
     static constexpr int id_slot = (18 * id_row + 127) / 128 * 128;
     static constexpr int priv = ids + 2 * id_slot;                // private slots [kSwPriv][512 threads]
     static constexpr int rows = priv + kSwPriv * 16 * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kFusedRows][32]
     static constexpr int geo = rows + 4 * kFusedRows * kSwRow;    // 1/dx, 1/dx~, fx of the 32 lanes
     static constexpr int zg = geo + 3 * kSwRow;                   // [2 parity]{fz, 1/dz, 1/dz~, 0}
-    static constexpr int bar = zg + 64;                           // fullE[2], fullH
+    static constexpr int bar = zg + 64;                           // fullE[2], fullH[2]
     static constexpr int tab = bar + 64;                          // material table (n_table entries)
     static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + 18 * id_row;
     static constexpr int first_extra_bytes = ex_slot + ey_slot;
@@ -99,7 +106,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     using VecR = Vec<R>;
     using IdT = typename std::conditional<V == 4, unsigned, unsigned short>::type;
     // private slot numbering of this kernel (shadows the cp.async sweep's enum inside em_fused_phaseb*.inc)
-    constexpr int kSlotQ = 0, kSlotL = 1, kSlotHp = 7, kSlotPend = 9;
+    constexpr int kSlotQ = 0, kSlotL = 1, kSlotHp = 5, kSlotPend = 7;
     extern __shared__ __align__(1024) unsigned char sm[];
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -134,21 +141,21 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     auto staged = [&](int byte_off) -> VecR { return *reinterpret_cast<const VecR *>(reinterpret_cast<const unsigned char *>(stg) + byte_off); };
     const unsigned bar0 = smem_u32(sm + L::bar);
     auto bar_fullE = [&](int s) -> unsigned { return bar0 + 8 * s; };
-    const unsigned bar_fullH = bar0 + 16;
+    auto bar_fullH = [&](int s) -> unsigned { return bar0 + 16 + 8 * s; };
 
     // ---- prologue: barriers, table, x geometry, zeroed exchange rows and private slots -------------------
     if (tid == 0) {
-        mbar_init(bar_fullE(0), 1); mbar_init(bar_fullE(1), 1); mbar_init(bar_fullH, 1);
+        mbar_init(bar_fullE(0), 1); mbar_init(bar_fullE(1), 1); mbar_init(bar_fullH(0), 1); mbar_init(bar_fullH(1), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int t = tid; t < p.n_table; t += NT) s_tab[t] = p.table[t];
     {
-        VecR z, one;
+        VecR z, mone;
 #pragma unroll
-        for (int c = 0; c < V; ++c) { z.v[c] = R(0); one.v[c] = R(1); }
+        for (int c = 0; c < V; ++c) { z.v[c] = R(0); mone.v[c] = R(-1); }
         for (int t = tid; t < 4 * kFusedRows * 32; t += NT) s_rows[t] = z;
         for (int t = 0; t < kSwPriv; ++t) mine[t * NT] = z;
-        mine[(kSlotL + 0) * NT] = one; mine[(kSlotL + 3) * NT] = one;
+        mine[(kSlotL + 0) * NT] = mone; mine[(kSlotL + 2) * NT] = mone;     // plane k = -1 is outside: eps/dt = 1, mask 0 (sign)
         if (w == 0) {
             const bool in = (i0 + V <= p.PX);
             s_geo[0 * 32 + lane] = in ? *reinterpret_cast<const VecR *>(p.rdx + i0) : z;
@@ -176,12 +183,13 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         tma_load_3d(sb + L::ez + (kk & 1) * L::ez_slot, &maps.E[2], bar, cx, cyy, kk + 1);
         tma_load_3d(sb + L::ids + (kk & 1) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, kk + 1);
     };
+    // H group of plane kk -> parity kk&1 (two planes in flight)
     auto issue_H = [&](int kk) {
-        const unsigned sb = smem_u32(sm);
-        mbar_expect_tx(bar_fullH, (unsigned)L::h_bytes);
-        tma_load_3d(sb + L::h + 0 * L::h_slot, &maps.H[0], bar_fullH, cx, cyy, kk + 1);
-        tma_load_3d(sb + L::h + 1 * L::h_slot, &maps.H[1], bar_fullH, cx, cyy, kk + 1);
-        tma_load_3d(sb + L::h + 2 * L::h_slot, &maps.H[2], bar_fullH, cx, cyy, kk + 1);
+        const unsigned sb = smem_u32(sm), bar = bar_fullH((kk - ks) & 1);
+        mbar_expect_tx(bar, (unsigned)L::h_bytes);
+        tma_load_3d(sb + L::h + ((kk & 1) * 3 + 0) * L::h_slot, &maps.H[0], bar, cx, cyy, kk + 1);
+        tma_load_3d(sb + L::h + ((kk & 1) * 3 + 1) * L::h_slot, &maps.H[1], bar, cx, cyy, kk + 1);
+        tma_load_3d(sb + L::h + ((kk & 1) * 3 + 2) * L::h_slot, &maps.H[2], bar, cx, cyy, kk + 1);
     };
     // z geometry of plane kk -> parity kk&1 (cp.async, same group as q)
     auto issue_z = [&](int kk) {
@@ -192,7 +200,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     if (tid == 0) {
         issue_E(ks, true);
         issue_H(ks);
-        if (ks + 1 <= ke) issue_E(ks + 1, false);
+        if (ks + 1 <= ke) { issue_E(ks + 1, false); issue_H(ks + 1); }
     }
     issue_z(ks); issue_z(ks + 1);
     cp_async_commit();
@@ -264,8 +272,9 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
                     nbz.v[c] = lerp(nk, ncur[c], fz);
                 }
             }
-            mbar_wait(bar_fullH, (unsigned)it & 1u);              // H(k) has landed
-            const VecR hx = staged(L::h + 0 * L::h_slot), hy = staged(L::h + 1 * L::h_slot), hz = staged(L::h + 2 * L::h_slot);
+            mbar_wait(bar_fullH(it & 1), (unsigned)(it >> 1) & 1u);   // H(k) has landed
+            const VecR hx = staged(L::h + (par * 3 + 0) * L::h_slot), hy = staged(L::h + (par * 3 + 1) * L::h_slot);
+            const VecR hz = staged(L::h + (par * 3 + 2) * L::h_slot);
 #pragma unroll
             for (int c = 0; c < V; ++c) {
                 const R eyip = (c < V - 1) ? ey0.v[c < V - 1 ? c + 1 : c] : ey0_r;
@@ -280,13 +289,13 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             for (int c = 0; c < V; ++c) hxn.v[c] = hyn.v[c] = hzn.v[c] = R(0);
         }
         if (st) {
-            *reinterpret_cast<VecR *>(p.Hn[0] + o) = hxn;
-            *reinterpret_cast<VecR *>(p.Hn[1] + o) = hyn;
-            *reinterpret_cast<VecR *>(p.Hn[2] + o) = hzn;
+            EM_ST(p.Hn[0] + o, hxn);
+            EM_ST(p.Hn[1] + o, hyn);
+            EM_ST(p.Hn[2] + o, hzn);
         }
         smHx[r][lane] = hxn; smHz[r][lane] = hzn;
         __syncthreads();                          // B2: H' rows visible; every thread holds H(k) in registers
-        if (tid == 0 && k + 1 <= ke) issue_H(k + 1);
+        if (tid == 0 && k + 2 <= ke) issue_H(k + 2);
 
         // ---- phase B: E' = E + r (curl H' - J - sigma E), Joule squares (eq. 2-3) -------------
         // (warp 0 = halo row -1 only supplies H' to row 0: no E', no Joule)
@@ -298,21 +307,21 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             } else {
                 if (l_stale) {   // plane k-1 took the one-material path: its coefficient means are the entry itself
                     const MatEntry<R> Ap = s_tab[idw_prev & 0xff];
-                    VecR va, vb, vm;
+                    VecR va, vb;
 #pragma unroll
-                    for (int c = 0; c < V; ++c) { va.v[c] = Ap.a; vb.v[c] = Ap.b; vm.v[c] = Ap.m * Ap.m; }
-                    mine[(kSlotL + 0) * NT] = va; mine[(kSlotL + 1) * NT] = vb; mine[(kSlotL + 2) * NT] = vm;
-                    mine[(kSlotL + 3) * NT] = va; mine[(kSlotL + 4) * NT] = vb; mine[(kSlotL + 5) * NT] = vm;
+                    for (int c = 0; c < V; ++c) { va.v[c] = Ap.m != R(0) ? Ap.a : -Ap.a; vb.v[c] = Ap.b; }
+                    mine[(kSlotL + 0) * NT] = va; mine[(kSlotL + 1) * NT] = vb;
+                    mine[(kSlotL + 2) * NT] = va; mine[(kSlotL + 3) * NT] = vb;
                     l_stale = false;
                 }
                 if (s_next_k <= k) {
 #define EM_HAS_J 1
-#include "em_fused_phaseb.inc"
+#include "em_sweep_phaseb.inc"
 #undef EM_HAS_J
                     s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
                 } else {
 #define EM_HAS_J 0
-#include "em_fused_phaseb.inc"
+#include "em_sweep_phaseb.inc"
 #undef EM_HAS_J
                 }
             }
@@ -346,7 +355,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             }
             mine[kSlotPend * NT] = pend;
             // q of a lane whose V cells are one lossless material never changes: neither fetched nor stored
-            if (own_q && k > kz0 && q_live) *reinterpret_cast<VecR *>(p.q + o - PXY) = qv;   // layer k-1 in [kz0, kz1)
+            if (own_q && k > kz0 && q_live) EM_ST(p.q + o - PXY, qv);   // layer k-1 in [kz0, kz1)
             q_live = !(id_uniform(idw) && s_tab[idw & 0xff].b == R(0));
             if (own_q && k >= kz0 && k < ke && q_live) cp_async16(mine + kSlotQ * NT, p.q + o);   // q(k)
         }
