@@ -89,7 +89,7 @@ def measured_peak():
 
 def ncu_traffic(kernel_name: str, cells: int):
     """dram bytes per launch of the dominant kernel from the committed ncu summary, if any."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    path = os.path.join(ROOT, "profiles", "r1_traffic.txt")     # JSON text written from the ncu summary beside it
     try:
         with open(path) as f:
             t = json.load(f)

@@ -42,23 +42,23 @@ struct alignas(64) SweepMaps { CUtensorMap E[3], H[3], q, mat; };
 template <int SZ> struct SweepLayout {
     static constexpr int V = 16 / SZ;
     static constexpr int ex = 0;                                  // Ex ring of 3 planes, rows -1 .. TY+1
-    static constexpr int ex_slot = 17 * kSwRow;
+    static constexpr int ex_slot = (kSwWarps + 1) * kSwRow;
     static constexpr int ey = ex + 3 * ex_slot;                   // Ey ring of 3 planes, rows -1 .. TY
-    static constexpr int ey_slot = 16 * kSwRow;
+    static constexpr int ey_slot = kSwWarps * kSwRow;
     static constexpr int ez = ey + 3 * ey_slot;                   // Ez, 2 parities, rows -1 .. TY+1
-    static constexpr int ez_slot = 17 * kSwRow;
+    static constexpr int ez_slot = (kSwWarps + 1) * kSwRow;
     static constexpr int h = ez + 2 * ez_slot;                    // [2 parities][Hx, Hy, Hz], rows -1 .. TY
-    static constexpr int h_slot = 16 * kSwRow;
+    static constexpr int h_slot = kSwWarps * kSwRow;
     static constexpr int ids = h + 6 * h_slot;                    // ids, 2 parities, rows -2 .. TY+1
     static constexpr int id_row = 32 * V + 16;                    // box starts on a 16-B boundary: up to 15 B of lead-in
-    static constexpr int id_slot = (18 * id_row + 127) / 128 * 128;
+    static constexpr int id_slot = ((kSwWarps + 2) * id_row + 127) / 128 * 128;
     static constexpr int priv = ids + 2 * id_slot;                // private slots [kSwPriv][512 threads]
-    static constexpr int rows = priv + kSwPriv * 16 * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kFusedRows][32]
+    static constexpr int rows = priv + kSwPriv * kSwWarps * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kFusedRows][32]
     static constexpr int geo = rows + 4 * kFusedRows * kSwRow;    // 1/dx, 1/dx~, fx of the 32 lanes
     static constexpr int zg = geo + 3 * kSwRow;                   // [2 parity]{fz, 1/dz, 1/dz~, 0}
     static constexpr int bar = zg + 64;                           // fullE[2], fullH[2]
     static constexpr int tab = bar + 64;                          // material table (n_table entries)
-    static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + 18 * id_row;
+    static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + (kSwWarps + 2) * id_row;
     static constexpr int first_extra_bytes = ex_slot + ey_slot;
     static constexpr int h_bytes = 3 * h_slot;
 };
