@@ -173,6 +173,7 @@ def run_b200(args):
     import numpy as np
     import torch
     import paper_2603_07038_b200 as P
+    from paper_2603_07038_b200.replicas import aggregate_throughput, max_over_ranks
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -230,11 +231,8 @@ def run_b200(args):
     launches = em.launch_count - l0
     kname, klaunch, kms = em.em_timing_read()
     em.em_timing_enable(False)
-    if dist is not None:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = cells * K * world / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, dev)
+    value = aggregate_throughput(cells * K, ms * 1e-3, world)
 
     # ---- end to end through the C ABI with host buffers -------------------------------------------
     e2e = None
@@ -266,11 +264,8 @@ def run_b200(args):
         tot = em.em_joule(None, None, total=True); d2h += 8
         torch.cuda.synchronize(dev)
         el = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([el], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            el = float(t.item())
-        e2e = {"value": cells * K * world / el, "unit": "cell-updates/s", "h2d_bytes_per_step": h2d / K,
+        el = max_over_ranks(el, dist, dev)
+        e2e = {"value": aggregate_throughput(cells * K, el, world), "unit": "cell-updates/s", "h2d_bytes_per_step": h2d / K,
                "d2h_bytes_per_step": d2h / K,
                "what": "em_set_field x6 from pinned host, %d x em_step with em_probe reads%s, em_get_field x6 + Joule total to host"
                        % (K, " and Joule maps to host every %d steps" % je if je else "")}
