@@ -23,7 +23,9 @@
  * Readings of the paper where it is silent are those of SURVEY.md 8(c) C1-C20 (listed in
  * DESIGN.md).  Pins: tests/test_oracle_*.py (TE101 closed form, energy conservation, Poynting
  * balance, divergence invariants, conductor decay + Joule geometric series, dense eq. (2)-(3)
- * brute force, worked impulse example, axis-permutation symmetry, CFL power iteration).
+ * brute force, worked impulse example, axis-permutation symmetry, CFL power iteration) and
+ * tests/test_oracle_pmc.py for the PMC walls of PAPER.md L142 (mirror-image equivalence with the all-PEC
+ * doubled domain, quarter-wave closed form, energy and Poynting balance with mixed walls, dense eq. (2)-(3)).
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -40,13 +42,18 @@
 
 #define EMO_LOSS_CD 0
 #define EMO_LOSS_EXP 1
-#define EMO_BC_PEC 0
+#define EMO_BC_PEC 0   /* tangential E held at 0 on the wall                                        */
+#define EMO_BC_PMC 1   /* the paper's truncation: tangential H = 0 on the wall.  The
+                          wall's tangential E edges stay unknowns; their dual face is the half face
+                          inside the domain (dual length d/2) and H outside the domain is 0
+                          (SURVEY.md 8(c) C8).  Equivalent to mirroring the domain in the wall
+                          (tangential E even, tangential H odd), which is how the tests pin it. */
 
 typedef struct {
     int32_t nx, ny, nz;
     const double *dx, *dy, *dz;   /* cell sizes, lengths nx, ny, nz */
     int32_t loss_mode;            /* EMO_LOSS_CD (paper eq. 3) or EMO_LOSS_EXP */
-    int32_t bc[6];                /* -x,+x,-y,+y,-z,+z ; only EMO_BC_PEC */
+    int32_t bc[6];                /* -x,+x,-y,+y,-z,+z ; EMO_BC_PEC or EMO_BC_PMC */
 } emo_grid;
 
 typedef struct { double eps, mu, sigma; int32_t flags; } emo_material;   /* flags bit0 = PEC */
@@ -56,6 +63,7 @@ typedef struct { int32_t comp, i, j, k; } emo_probe_pt;
 
 typedef struct emo_ctx {
     int32_t nx, ny, nz, loss_mode;
+    int32_t bc[6];
     double dt;
     double *dx, *dy, *dz;          /* primal lengths */
     double *tx, *ty, *tz;          /* dual lengths d~ (nx+1, ny+1, nz+1) */
@@ -163,7 +171,7 @@ int32_t emo_create(const emo_grid *g, const uint8_t *mat_id, const emo_material 
     if (!g || !mat_id || !tab || !out) return EMO_ERR_INVALID_ARG;
     if (g->nx < 1 || g->ny < 1 || g->nz < 1 || n_mat < 1 || n_mat > 256 || !(dt > 0.0)) return EMO_ERR_INVALID_ARG;
     if (g->loss_mode != EMO_LOSS_CD && g->loss_mode != EMO_LOSS_EXP) return EMO_ERR_INVALID_ARG;
-    for (int b = 0; b < 6; ++b) if (g->bc[b] != EMO_BC_PEC) return EMO_ERR_UNSUPPORTED;
+    for (int b = 0; b < 6; ++b) if (g->bc[b] != EMO_BC_PEC && g->bc[b] != EMO_BC_PMC) return EMO_ERR_INVALID_ARG;
     for (int m = 0; m < n_mat; ++m)
         if (!(tab[m].eps > 0.0) || !(tab[m].mu > 0.0) || !(tab[m].sigma >= 0.0)) return EMO_ERR_INVALID_ARG;
     int nx = g->nx, ny = g->ny, nz = g->nz;
@@ -175,6 +183,10 @@ int32_t emo_create(const emo_grid *g, const uint8_t *mat_id, const emo_material 
 
     emo_ctx *c = (emo_ctx *)calloc(1, sizeof(emo_ctx));
     c->nx = nx; c->ny = ny; c->nz = nz; c->loss_mode = g->loss_mode; c->dt = dt;
+    for (int b = 0; b < 6; ++b) c->bc[b] = g->bc[b];
+    /* wall planes that hold tangential E at 0 */
+    const int wx0 = g->bc[0] == EMO_BC_PEC, wx1 = g->bc[1] == EMO_BC_PEC, wy0 = g->bc[2] == EMO_BC_PEC,
+              wy1 = g->bc[3] == EMO_BC_PEC, wz0 = g->bc[4] == EMO_BC_PEC, wz1 = g->bc[5] == EMO_BC_PEC;
     c->dx = (double *)malloc(sizeof(double) * nx); memcpy(c->dx, g->dx, sizeof(double) * nx);
     c->dy = (double *)malloc(sizeof(double) * ny); memcpy(c->dy, g->dy, sizeof(double) * ny);
     c->dz = (double *)malloc(sizeof(double) * nz); memcpy(c->dz, g->dz, sizeof(double) * nz);
@@ -211,7 +223,7 @@ int32_t emo_create(const emo_grid *g, const uint8_t *mat_id, const emo_material 
             double w = c->dy[jj] * c->dz[kk];
             sw += w; se += w * m->eps; ss += w * m->sigma; pec |= (m->flags & 1);
         }
-        int fx = (j == 0) || (j == ny) || (k == 0) || (k == nz) || pec;   /* PEC walls / PEC material */
+        int fx = (j == 0 && wy0) || (j == ny && wy1) || (k == 0 && wz0) || (k == nz && wz1) || pec;   /* PEC walls / PEC material */
         int64_t e = EX(i, j, k);
         c->fixed[0][e] = (uint8_t)fx;
         if (!fx) loss_coeff(c->loss_mode, se / sw, ss / sw, dt, &c->ca[0][e], &c->cb[0][e]);
@@ -225,7 +237,7 @@ int32_t emo_create(const emo_grid *g, const uint8_t *mat_id, const emo_material 
             double w = c->dx[ii] * c->dz[kk];
             sw += w; se += w * m->eps; ss += w * m->sigma; pec |= (m->flags & 1);
         }
-        int fx = (i == 0) || (i == nx) || (k == 0) || (k == nz) || pec;
+        int fx = (i == 0 && wx0) || (i == nx && wx1) || (k == 0 && wz0) || (k == nz && wz1) || pec;
         int64_t e = EY(i, j, k);
         c->fixed[1][e] = (uint8_t)fx;
         if (!fx) loss_coeff(c->loss_mode, se / sw, ss / sw, dt, &c->ca[1][e], &c->cb[1][e]);
@@ -239,7 +251,7 @@ int32_t emo_create(const emo_grid *g, const uint8_t *mat_id, const emo_material 
             double w = c->dx[ii] * c->dy[jj];
             sw += w; se += w * m->eps; ss += w * m->sigma; pec |= (m->flags & 1);
         }
-        int fx = (i == 0) || (i == nx) || (j == 0) || (j == ny) || pec;
+        int fx = (i == 0 && wx0) || (i == nx && wx1) || (j == 0 && wy0) || (j == ny && wy1) || pec;
         int64_t e = EZ(i, j, k);
         c->fixed[2][e] = (uint8_t)fx;
         if (!fx) loss_coeff(c->loss_mode, se / sw, ss / sw, dt, &c->ca[2][e], &c->cb[2][e]);
@@ -346,29 +358,38 @@ static void one_step(emo_ctx *c) {
         }
     }
 
-    /* a2: E^{n+1} = ca E^n + cb (C_h H^{n+1/2} - J^{n+1/2}) on every non-fixed edge */
+    /* a2: E^{n+1} = ca E^n + cb (C_h H^{n+1/2} - J^{n+1/2}) on every non-fixed edge.
+     * H with an out-of-range index is 0; only reachable from the non-fixed edges of a PMC wall, where
+     * the dual length ty/tz/tx is the half cell (SURVEY.md 8(c) "One step" a2, C8). */
+#define HXG(i, j, k) (((j) >= 0 && (j) < ny && (k) >= 0 && (k) < nz) ? Hx[HX(i, j, k)] : 0.0)
+#define HYG(i, j, k) (((i) >= 0 && (i) < nx && (k) >= 0 && (k) < nz) ? Hy[HY(i, j, k)] : 0.0)
+#define HZG(i, j, k) (((i) >= 0 && (i) < nx && (j) >= 0 && (j) < ny) ? Hz[HZ(i, j, k)] : 0.0)
     double *Exn = c->En[0], *Eyn = c->En[1], *Ezn = c->En[2];
 #pragma omp parallel for schedule(static)
     for (k = 0; k <= nz; ++k) for (int j = 0; j <= ny; ++j) for (int i = 0; i < nx; ++i) {
         int64_t e = EX(i, j, k);
         if (c->fixed[0][e]) { Exn[e] = 0.0; continue; }
         Exn[e] = c->ca[0][e] * Ex[e] + c->cb[0][e] *
-            ((Hz[HZ(i, j, k)] - Hz[HZ(i, j - 1, k)]) / ty[j] - (Hy[HY(i, j, k)] - Hy[HY(i, j, k - 1)]) / tz[k] - c->J[0][e]);
+            ((HZG(i, j, k) - HZG(i, j - 1, k)) / ty[j] - (HYG(i, j, k) - HYG(i, j, k - 1)) / tz[k] - c->J[0][e]);
     }
 #pragma omp parallel for schedule(static)
     for (k = 0; k <= nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i <= nx; ++i) {
         int64_t e = EY(i, j, k);
         if (c->fixed[1][e]) { Eyn[e] = 0.0; continue; }
         Eyn[e] = c->ca[1][e] * Ey[e] + c->cb[1][e] *
-            ((Hx[HX(i, j, k)] - Hx[HX(i, j, k - 1)]) / tz[k] - (Hz[HZ(i, j, k)] - Hz[HZ(i - 1, j, k)]) / tx[i] - c->J[1][e]);
+            ((HXG(i, j, k) - HXG(i, j, k - 1)) / tz[k] - (HZG(i, j, k) - HZG(i - 1, j, k)) / tx[i] - c->J[1][e]);
     }
 #pragma omp parallel for schedule(static)
     for (k = 0; k < nz; ++k) for (int j = 0; j <= ny; ++j) for (int i = 0; i <= nx; ++i) {
         int64_t e = EZ(i, j, k);
         if (c->fixed[2][e]) { Ezn[e] = 0.0; continue; }
         Ezn[e] = c->ca[2][e] * Ez[e] + c->cb[2][e] *
-            ((Hy[HY(i, j, k)] - Hy[HY(i - 1, j, k)]) / tx[i] - (Hx[HX(i, j, k)] - Hx[HX(i, j - 1, k)]) / ty[j] - c->J[2][e]);
+            ((HYG(i, j, k) - HYG(i - 1, j, k)) / tx[i] - (HXG(i, j, k) - HXG(i, j - 1, k)) / ty[j] - c->J[2][e]);
     }
+
+#undef HXG
+#undef HYG
+#undef HZG
 
     /* a4: q_c += dt sigma_c * 1/4 sum over the 12 edges of c of ((E^{n+1} + E^n)/2)^2 */
 #define B2(A, An, idx) ({ double b_ = 0.5 * ((An)[idx] + (A)[idx]); b_ * b_; })

@@ -70,13 +70,13 @@ def _shapes(nx, ny, nz):
             (nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)]
 
 
-def _mk_grid(nx, ny, nz, dx, dy, dz, loss_mode):
+def _mk_grid(nx, ny, nz, dx, dy, dz, loss_mode, bc=(0,) * 6):
     g = _Grid()
     g.nx, g.ny, g.nz = nx, ny, nz
     g.dx, g.dy, g.dz = _dp(dx), _dp(dy), _dp(dz)
     g.loss_mode = loss_mode
     for b in range(6):
-        g.bc[b] = 0
+        g.bc[b] = int(bc[b])
     return g
 
 
@@ -117,7 +117,8 @@ class Oracle:
         self._dz = np.ascontiguousarray(p.dz, np.float64)
         mat = np.ascontiguousarray(p.mat_id, np.uint8)
         assert mat.shape == (self.nz, self.ny, self.nx)
-        g = _mk_grid(self.nx, self.ny, self.nz, self._dx, self._dy, self._dz, int(p.loss_mode))
+        g = _mk_grid(self.nx, self.ny, self.nz, self._dx, self._dy, self._dz, int(p.loss_mode),
+                     tuple(getattr(p, "bc", (0,) * 6)))
         tab = _mk_table(p.table, p.flags)
         self._h = C.c_void_p()
         rc = lib().emo_create(C.byref(g), mat.ctypes.data_as(C.c_void_p), tab, p.table.shape[0],

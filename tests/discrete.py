@@ -71,16 +71,18 @@ def face_mean(cell, dx, dy, dz, comp):
     return num / den
 
 
-def fixed_mask(nx, ny, nz, comp, pec_cell=None):
-    """True on PEC-fixed edges (tangential E on the six walls, or touching a PEC-flagged cell)."""
+def fixed_mask(nx, ny, nz, comp, pec_cell=None, bc=(0,) * 6):
+    """True on PEC-fixed edges (tangential E on the walls whose bc is PEC = 0, or touching a PEC-flagged
+    cell).  bc order: -x, +x, -y, +y, -z, +z; 1 = PMC (the wall's tangential E stays an unknown)."""
     sh = shapes(nx, ny, nz)[comp]
     m = np.zeros(sh, bool)
+    x0, x1, y0, y1, z0, z1 = (b == 0 for b in bc)
     if comp == 0:
-        m[[0, -1], :, :] = True; m[:, [0, -1], :] = True
+        m[0, :, :] |= z0; m[-1, :, :] |= z1; m[:, 0, :] |= y0; m[:, -1, :] |= y1
     elif comp == 1:
-        m[[0, -1], :, :] = True; m[:, :, [0, -1]] = True
+        m[0, :, :] |= z0; m[-1, :, :] |= z1; m[:, :, 0] |= x0; m[:, :, -1] |= x1
     else:
-        m[:, [0, -1], :] = True; m[:, :, [0, -1]] = True
+        m[:, 0, :] |= y0; m[:, -1, :] |= y1; m[:, :, 0] |= x0; m[:, :, -1] |= x1
     if pec_cell is not None and pec_cell.any():
         one = np.ones(1)
         touched = edge_mean(pec_cell.astype(np.float64), np.ones(nx), np.ones(ny), np.ones(nz), comp)

@@ -16,18 +16,21 @@ from oracle import emo
 import discrete as D
 
 
-@pytest.mark.parametrize("dims,seed", [((4, 4, 4), 101), ((3, 5, 4), 102)])
-def test_p7_dense_eq2_eq3(dims, seed):
+@pytest.mark.parametrize("dims,seed,bc", [((4, 4, 4), 101, (0,) * 6), ((3, 5, 4), 102, (0,) * 6),
+                                          ((4, 4, 4), 104, (1, 0, 0, 1, 1, 0)), ((3, 4, 5), 105, (1,) * 6)])
+def test_p7_dense_eq2_eq3(dims, seed, bc):
+    """bc with 1 = PMC walls: their tangential edges stay in the free set; C_h built from
+    the incidence definition already has the half dual faces and no H outside the domain."""
     nx, ny, nz = dims
     steps = 300
-    p = W.random_problem(nx, ny, nz, seed=seed, loss_mode=LOSS_CD, steps=steps, n_ports=2, blocky=False)
+    p = W.random_problem(nx, ny, nz, seed=seed, loss_mode=LOSS_CD, steps=steps, n_ports=2, blocky=False, bc=bc)
     p.init = None                                              # e^0 = e^{-1} = 0, H^{-1/2} = 0
     assert p.n_ports >= 1
     ops = D.Operators(nx, ny, nz, p.dx, p.dy, p.dz)
     eps_e = ops.flat([D.edge_mean(p.table[p.mat_id, 0], p.dx, p.dy, p.dz, a) for a in range(3)])
     sig_e = ops.flat([D.edge_mean(p.table[p.mat_id, 2], p.dx, p.dy, p.dz, a) for a in range(3)])
     nu_f = ops.flat([D.face_mean(1.0 / p.table[p.mat_id, 1], p.dx, p.dy, p.dz, a) for a in range(3)])
-    free = ~ops.flat([D.fixed_mask(nx, ny, nz, a) for a in range(3)]).astype(bool)
+    free = ~ops.flat([D.fixed_mask(nx, ny, nz, a, bc=p.bc) for a in range(3)]).astype(bool)
     Ce = ops.Ce.toarray(); Ch = ops.Ch.toarray()
     if dims == (4, 4, 4):
         assert Ce.shape == (240, 300) and Ch.shape == (300, 240)

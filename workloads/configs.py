@@ -442,10 +442,11 @@ def config5_graded(scale: int = 1, zscale: int = 1, steps: Optional[int] = None,
 def random_problem(nx: int, ny: int, nz: int, seed: int, steps: int = 20, loss_mode: int = LOSS_CD,
                    precision: int = 64, ids=(VAC, SI, SIO2, CU, MAG), uniform: bool = False,
                    n_ports: int = 2, blocky: bool = True, pec_material: bool = False,
-                   lossless: bool = False, init_scale: float = 1.0) -> Problem:
+                   lossless: bool = False, init_scale: float = 1.0, bc=(0,) * 6) -> Problem:
     """Random ids (blocky or per-cell), random spacings (ratio up to ~3), random initial E and H
     (H scaled by 1/eta0 so both carry comparable energy), a few random single-edge or two-edge
-    ports with smooth random waveforms."""
+    ports with smooth random waveforms.  bc: wall truncation (-x,+x,-y,+y,-z,+z; 1 = PMC); with a PMC
+    wall and n_ports > 0 one extra single-edge port sits ON the first PMC wall (a tangential edge)."""
     rng = np.random.default_rng(seed)
     if uniform:
         dx = np.full(nx, 1.0e-6); dy = np.full(ny, 1.5e-6); dz = np.full(nz, 0.75e-6)
@@ -508,7 +509,25 @@ def random_problem(nx: int, ny: int, nz: int, seed: int, steps: int = 20, loss_m
         w = np.sin(2 * math.pi * f * t + rng.uniform(0, 6.28)) * np.exp(-((t - 0.5 * steps * dt) / (0.3 * steps * dt)) ** 2)
         off, ln = src.add_wave(w)
         src.add_port(cands, 1.0e9 * rng.uniform(0.5, 1.5), off, ln)
+    pmc = [b for b in range(6) if bc[b]]
+    if pmc and n_ports > 0 and not pec_material and min(nx, ny, nz) >= 2:
+        b = pmc[0]; a = b // 2                                  # wall normal axis
+        c = (a + 1) % 3                                         # a tangential component
+        lim = [nx, ny, nz]
+        ijk = [0, 0, 0]
+        for ax in range(3):
+            if ax == a:
+                ijk[ax] = 0 if b % 2 == 0 else lim[ax]          # node plane of the wall
+            elif ax == c:
+                ijk[ax] = int(rng.integers(0, lim[ax]))         # along the edge: cell index
+            else:
+                ijk[ax] = int(rng.integers(1, max(lim[ax], 2))) # node strictly inside the other axis
+        f = rng.uniform(0.5, 3.0) / max(steps * dt, 1e-30)
+        w = np.sin(2 * math.pi * f * t + rng.uniform(0, 6.28))
+        off, ln = src.add_wave(w)
+        src.add_port([(c, ijk[0], ijk[1], ijk[2], 1.0)], 1.0e9 * rng.uniform(0.5, 1.5), off, ln)
     src.apply(p)
+    p.bc = tuple(int(v) for v in bc)
     _probes_default(p, rng, 6)
     return p
 

@@ -15,6 +15,8 @@ EPS0 = 1.0 / (MU0 * C0 * C0)
 
 LOSS_CD = 0   # paper eq. (3): M, K = D_eps +- dt/2 D_sigma
 LOSS_EXP = 1  # exponential-loss update (BASELINE.json config 2)
+BC_PEC = 0    # tangential E = 0 on the wall (north_star, configs 1-5; ground plane PAPER.md L134)
+BC_PMC = 1    # the paper's EM truncation: tangential H = 0 on the wall
 
 # Shared 16-entry table: ids 0-4 from BASELINE.json, 5-15 generator constants (handbook-order
 # values, NOT from the paper: PAPER.md L136-L138 prints mechanical constants only).
@@ -86,6 +88,8 @@ class Problem:
     probes: np.ndarray = dataclasses.field(default_factory=lambda: np.zeros((0, 4), np.int32))
     init: Optional[Dict[int, np.ndarray]] = None   # comp (0..5 = Ex,Ey,Ez,Hx,Hy,Hz) -> array
     joule_every: int = 0      # config 4: Joule map output every 100 steps
+    # wall truncation, order -x, +x, -y, +y, -z, +z: BC_PEC (tangential E = 0) or BC_PMC
+    bc: tuple = (0, 0, 0, 0, 0, 0)
     notes: str = ""
 
     @property
