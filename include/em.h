@@ -50,8 +50,11 @@ extern "C" {
 #define EM_LOSS_CD 0  /* paper eq. (3): trapezoidal conduction term, M,K = D_eps +- dt/2 D_sigma */
 #define EM_LOSS_EXP 1 /* exponential-loss update: ca = exp(-s dt/eps), cb = -expm1(-s dt/eps)/s  */
 
-#define EM_BC_PEC 0 /* tangential E = 0 on the wall (the only supported truncation)             */
-#define EM_BC_PMC 1 /* paper's truncation: not implemented -> EM_ERR_UNSUPPORTED */
+#define EM_BC_PEC 0 /* tangential E = 0 on the wall (north_star; ground plane PAPER.md L134)          */
+#define EM_BC_PMC 1 /* the paper's EM truncation: tangential H = 0 on the wall.  The   */
+                    /* wall's tangential E edges stay unknowns, updated with the half dual face inside */
+                    /* the domain and H = 0 outside -- the symmetry plane of the   */
+                    /* mirrored domain.  An edge shared with a PEC wall stays fixed.  Needs n_mat<=254. */
 
 #define EM_MAT_PEC 1 /* em_material.flags bit0: every edge touching such a cell is held at 0      */
 
@@ -72,7 +75,7 @@ typedef struct em_grid {
     const double *dx, *dy, *dz;  /* HOST: cell sizes [m], lengths nx, ny, nz, all > 0                */
     int32_t precision;           /* 32 or 64: working precision of fields, maps and arithmetic      */
     int32_t loss_mode;           /* EM_LOSS_CD or EM_LOSS_EXP                                        */
-    int32_t bc[6];               /* -x,+x,-y,+y,-z,+z: EM_BC_PEC                                     */
+    int32_t bc[6];               /* -x,+x,-y,+y,-z,+z: EM_BC_PEC or EM_BC_PMC                          */
     int32_t kernel;              /* EM_KERNEL_*                                                      */
     int32_t max_ports;           /* capacity reserved in the workspace for em_set_source            */
     int64_t max_source_edges;
@@ -102,7 +105,7 @@ int32_t em_workspace_bytes(const em_grid *g, size_t *out_bytes);
  * workspace: DEVICE, 256-byte aligned, >= em_workspace_bytes.  stream: cudaStream_t (may be 0).
  * Zeroes fields, Joule accumulator and the step counter.  Synchronises the stream before returning
  * (the host inputs may be freed on return).
- * Errors: INVALID_ARG, WORKSPACE_TOO_SMALL, UNSUPPORTED (a bc != EM_BC_PEC), CUDA. */
+ * Errors: INVALID_ARG, WORKSPACE_TOO_SMALL, CUDA (INVALID_ARG also for an unknown bc, or a PMC wall with n_mat > 254). */
 int32_t em_create(const em_grid *g, const uint8_t *mat_id, const em_material *table, int32_t n_mat,
                   double dt, void *workspace, size_t workspace_bytes, void *stream, em_ctx **out);
 

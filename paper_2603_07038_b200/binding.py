@@ -148,7 +148,7 @@ class EM:
     """One em_ctx.  ``p`` is any object with the attributes of workloads.Problem (plain arrays)."""
 
     def __init__(self, p, precision: Optional[int] = None, kernel: int = EM_KERNEL_AUTO, device="cuda:0",
-                 stream=None, bc: Sequence[int] = (0,) * 6, load_sources: bool = True, load_init: bool = True,
+                 stream=None, bc: Optional[Sequence[int]] = None, load_sources: bool = True, load_init: bool = True,
                  max_ports: Optional[int] = None, max_source_edges: Optional[int] = None,
                  max_wave_samples: Optional[int] = None):
         import torch
@@ -171,7 +171,8 @@ class EM:
                               int(p.loss_mode), kernel,
                               max_ports if max_ports is not None else max(n_ports, 1),
                               max_source_edges if max_source_edges is not None else max(n_con, 1),
-                              max_wave_samples if max_wave_samples is not None else max(int(p.wave.shape[0]), 1), bc)
+                              max_wave_samples if max_wave_samples is not None else max(int(p.wave.shape[0]), 1),
+                              tuple(bc) if bc is not None else tuple(getattr(p, "bc", (0,) * 6)))
         nbytes = C.c_size_t()
         _check(self._L.em_workspace_bytes(C.byref(self._grid), C.byref(nbytes)))
         self.workspace_bytes = int(nbytes.value)

@@ -21,6 +21,25 @@ struct DevSources {
     const R *wave;
 };
 
+// PMC walls: a pad cell that lies beyond PMC walls ONLY gets the id of the
+// "outside / PMC" table entry (mask 1, zero weight in every mean because the pad spacings are 0), so the
+// tangential E of a PMC wall stays an unknown; pad cells beyond any PEC wall keep the mask-0 entry.
+// base = the element (i, j, k) = (-1, -1, -1); n = PX * PY * PZ elements; pmc_mask bit b = wall b is PMC.
+__global__ void __launch_bounds__(256) k_pad_pmc(uint8_t *base, int nx, int ny, int nz, int PX, int PY, long long n,
+                                                 int pmc_mask, uint8_t pmc_id) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const long long PXY = (long long)PX * PY;
+    const int k = (int)(t / PXY) - 1;
+    const long long rem = t % PXY;
+    const int j = (int)(rem / PX) - 1, i = (int)(rem % PX) - 1;
+    int beyond = 0;                                   // walls this cell lies beyond
+    if (i < 0) beyond |= 1; if (i >= nx) beyond |= 2;
+    if (j < 0) beyond |= 4; if (j >= ny) beyond |= 8;
+    if (k < 0) beyond |= 16; if (k >= nz) beyond |= 32;
+    if (beyond != 0 && (beyond & ~pmc_mask) == 0) base[t] = pmc_id;
+}
+
 // Zero E[comp] wherever the edge is PEC-fixed (mask product of its 4 cells is 0).
 template <typename R>
 __global__ void __launch_bounds__(256) k_mask_fixed(DevParams<R> p, int comp) {

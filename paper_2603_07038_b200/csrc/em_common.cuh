@@ -36,6 +36,7 @@ struct DevParams {
     const uint8_t *mat;      // material ids, same geometry
     const MatEntry<R> *table;// n_table entries in global memory
     int n_table;
+    int warm_lo;             // 1: the -z wall is PMC, the sweeps also run plane k = -1 as a warm-up plane
     // per-axis arrays indexed [-1 .. n+1] (pointer shifted to index 0):
     //   rd = 1/d (0 outside), rt = 1/d~, f = d[i]/(d[i-1]+d[i]) with d[-1] = d[n] = 0
     const R *rdx, *rtx, *fx, *rdy, *rty, *fy, *rdz, *rtz, *fz;

@@ -172,7 +172,7 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
     const int item = blockIdx.x, tile = item / zc.nzs, chunk = item - tile * zc.nzs;
     const int tx = tile % ntx, ty = tile / ntx;
     const int kz0 = zc.kb[chunk], kz1 = zc.kb[chunk + 1];
-    const int ks = kz0 > 0 ? kz0 - 1 : 0, ke = kz1 <= p.nz ? kz1 : p.nz;
+    const int ks = (kz0 > 0 || p.warm_lo) ? kz0 - 1 : 0, ke = kz1 <= p.nz ? kz1 : p.nz;   // PMC at -z: plane -1 warms up too
     const int cy = w - 1, r = cy + 2;
     const int j = ty * kFusedTY + cy;
     const int i0 = tx * TXo - V + V * lane;
@@ -254,7 +254,7 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
     bool rowu_prev = false;      // plane k-1: rows j-1 and j of this lane held one material
     bool l_stale = false;        // warp-uniform: the L slots were skipped by the one-material path
     bool q_live = false;         // q of layer k-1 was fetched (some sigma != 0 among the lane's cells)
-    int rk = ks % 3;                              // k % 3
+    int rk = (ks + 3) % 3;                            // k % 3
     if (active) {
         cp_async16(mine + (kSlotEx + rk) * NT, p.E[0] + off0 + (long long)ks * PXY);   // plane ks into ring slot ks%3
         cp_async16(mine + (kSlotEy + rk) * NT, p.E[1] + off0 + (long long)ks * PXY);

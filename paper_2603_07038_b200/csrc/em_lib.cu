@@ -253,7 +253,7 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     const size_t need = carve<R>(g, *gr, nullptr, nullptr, max_items);
     if (ws_bytes < need) return fail(EM_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
     carve<R>(g, *gr, workspace, &c, max_items);
-    sweep_smem = em::sweep_smem_bytes((int)sizeof(R), n_mat + 1);
+    sweep_smem = em::sweep_smem_bytes((int)sizeof(R), n_mat + 2);
     if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_TMA;     // measured on config 4: TMA sweep 2.44 ms/step, cp.async sweep 2.71 ms/step
     if (kernel == EM_KERNEL_TMA) {
         int dev = 0, optin = 0;
@@ -265,17 +265,23 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
 
     // ---- material table -> (eps/dt, sigma, mask, dt/mu), built in fp64, rounded once ----------
     table.assign(tab, tab + n_mat);
-    std::vector<em::MatEntry<R>> ht(n_mat + 1);
-    fixed_cell.assign(n_mat + 1, 0);
+    // table = the materials, then (only with a PMC wall) the "outside, beyond PMC walls only" entry whose mask is 1,
+    // then, always last, the "outside / PEC" entry whose mask is 0 (what fixes the tangential E of PEC walls)
+    bool any_pmc = false;
+    for (int b = 0; b < 6; ++b) any_pmc = any_pmc || gr->bc[b] == EM_BC_PMC;
+    const int n_table = n_mat + (any_pmc ? 2 : 1);
+    std::vector<em::MatEntry<R>> ht(n_table);
+    fixed_cell.assign(n_table, 0);
     for (int m = 0; m < n_mat; ++m) {
         const bool pec = (tab[m].flags & EM_MAT_PEC) != 0;
         ht[m].a = (R)(tab[m].eps / dt); ht[m].b = (R)tab[m].sigma;
         ht[m].m = pec ? R(0) : R(1); ht[m].n = (R)(dt / tab[m].mu);
         fixed_cell[m] = pec;
     }
-    ht[n_mat].a = R(1); ht[n_mat].b = R(0); ht[n_mat].m = R(0); ht[n_mat].n = R(0);
-    fixed_cell[n_mat] = 1;
-    CU(cudaMemcpyAsync(c.table, ht.data(), sizeof(em::MatEntry<R>) * (n_mat + 1), cudaMemcpyHostToDevice, stream));
+    if (any_pmc) { ht[n_mat].a = R(1); ht[n_mat].b = R(0); ht[n_mat].m = R(1); ht[n_mat].n = R(0); }
+    ht[n_table - 1].a = R(1); ht[n_table - 1].b = R(0); ht[n_table - 1].m = R(0); ht[n_table - 1].n = R(0);
+    fixed_cell[n_table - 1] = 1;
+    CU(cudaMemcpyAsync(c.table, ht.data(), sizeof(em::MatEntry<R>) * n_table, cudaMemcpyHostToDevice, stream));
 
     // ---- per-axis arrays, index -1 .. n+1 (+ slack), fp64 then rounded once -------------------
     const double *d[3] = {gr->dx, gr->dy, gr->dz};
@@ -305,8 +311,17 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     CU(cudaMemcpyAsync(c.vy, gr->dy, sizeof(double) * g.ny, cudaMemcpyHostToDevice, stream));
     CU(cudaMemcpyAsync(c.vz, gr->dz, sizeof(double) * g.nz, cudaMemcpyHostToDevice, stream));
 
-    // ---- material ids: halo = "outside" id n_mat, interior copied with a pitched 3-D copy ------
-    CU(cudaMemsetAsync(c.mat, n_mat, g.alloc_elems, stream));
+    // ---- material ids: halo = the "outside / PEC" id, interior copied with a pitched 3-D copy; pad cells that
+    // lie beyond PMC walls only get the "outside / PMC" id (em_aux.cuh k_pad_pmc) -----------------------------
+    CU(cudaMemsetAsync(c.mat, n_table - 1, g.alloc_elems, stream));
+    if (any_pmc) {
+        int pmc_mask = 0;
+        for (int b = 0; b < 6; ++b) if (gr->bc[b] == EM_BC_PMC) pmc_mask |= 1 << b;
+        const long long n = g.vol;
+        em::k_pad_pmc<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(c.mat + g.origin - g.PXY - g.PX - 1, g.nx, g.ny, g.nz,
+                                                                        g.PX, g.PY, n, pmc_mask, (uint8_t)n_mat);
+        CU(cudaGetLastError());
+    }
     {
         cudaMemcpy3DParms m = {};
         m.srcPtr = make_cudaPitchedPtr(const_cast<uint8_t *>(mat_id), g.nx, g.nx, g.ny);
@@ -327,7 +342,8 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
 
     // ---- device parameter block -----------------------------------------------------------------
     p.nx = g.nx; p.ny = g.ny; p.nz = g.nz; p.PX = g.PX; p.PY = g.PY; p.PXY = g.PXY;
-    p.q = c.q + g.origin; p.mat = c.mat + g.origin; p.table = c.table; p.n_table = n_mat + 1;
+    p.q = c.q + g.origin; p.mat = c.mat + g.origin; p.table = c.table; p.n_table = n_table;
+    p.warm_lo = gr->bc[4] == EM_BC_PMC ? 1 : 0;
     p.rdx = c.axis[0] + 4; p.rtx = c.axis[1] + 4; p.fx = c.axis[2] + 4;
     p.rdy = c.axis[3] + 4; p.rty = c.axis[4] + 4; p.fy = c.axis[5] + 4;
     p.rdz = c.axis[6] + 4; p.rtz = c.axis[7] + 4; p.fz = c.axis[8] + 4;
@@ -711,8 +727,8 @@ int32_t em_create(const em_grid *gr, const uint8_t *mat_id, const em_material *t
     if (n_mat < 1 || n_mat > 255) return fail(EM_ERR_INVALID_ARG, "n_mat must be 1..255");
     if (!(dt > 0.0) || !std::isfinite(dt)) return fail(EM_ERR_INVALID_ARG, "dt must be > 0");
     for (int b = 0; b < 6; ++b) {
-        if (gr->bc[b] == EM_BC_PMC) return fail(EM_ERR_UNSUPPORTED, "PMC walls are not implemented");
-        if (gr->bc[b] != EM_BC_PEC) return fail(EM_ERR_INVALID_ARG, "unknown boundary condition");
+        if (gr->bc[b] != EM_BC_PEC && gr->bc[b] != EM_BC_PMC) return fail(EM_ERR_INVALID_ARG, "unknown boundary condition");
+        if (gr->bc[b] == EM_BC_PMC && n_mat > 254) return fail(EM_ERR_INVALID_ARG, "n_mat must be <= 254 with a PMC wall");
     }
     for (int m = 0; m < n_mat; ++m)
         if (!(tab[m].eps > 0.0) || !(tab[m].mu > 0.0) || !(tab[m].sigma >= 0.0) || !std::isfinite(tab[m].eps + tab[m].mu + tab[m].sigma))

@@ -115,7 +115,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     const int item = blockIdx.x, tile = item / zc.nzs, chunk = item - tile * zc.nzs;
     const int tx = tile % ntx, ty = tile / ntx;
     const int kz0 = zc.kb[chunk], kz1 = zc.kb[chunk + 1];
-    const int ks = kz0 > 0 ? kz0 - 1 : 0, ke = kz1 <= p.nz ? kz1 : p.nz;
+    const int ks = (kz0 > 0 || p.warm_lo) ? kz0 - 1 : 0, ke = kz1 <= p.nz ? kz1 : p.nz;   // PMC at -z: plane -1 warms up too
     const int cy = w - 1, r = cy + 2;
     const int j = ty * kSwTY + cy;
     const int i0 = tx * TXo - V + V * lane;
@@ -175,8 +175,8 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         const unsigned sb = smem_u32(sm);
         mbar_expect_tx(bar, (unsigned)(L::e_bytes + (first ? L::first_extra_bytes : 0)));
         if (first) {
-            tma_load_3d(sb + L::ex + (kk % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 1);
-            tma_load_3d(sb + L::ey + (kk % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 1);
+            tma_load_3d(sb + L::ex + ((kk + 3) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 1);
+            tma_load_3d(sb + L::ey + ((kk + 3) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 1);
         }
         tma_load_3d(sb + L::ex + ((kk + 1) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 2);
         tma_load_3d(sb + L::ey + ((kk + 1) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 2);
@@ -228,7 +228,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     const int s_end = fs.tile_sbeg[(tile + 1) * zc.nzs];
     int s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
 
-    int rk = ks % 3;                                  // k % 3
+    int rk = (ks + 3) % 3;                                // k % 3
     for (int k = ks; k <= ke; ++k) {
         const int it = k - ks;
         const int rk1 = (rk == 2) ? 0 : rk + 1;

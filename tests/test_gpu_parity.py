@@ -90,6 +90,28 @@ def test_random_grids_exp(dims, precision, kernel):
     run_pair(p, 40, precision, kernel, checkpoints=(1,))
 
 
+# --------------------------------------------------------------------- PMC walls
+PMC_BC = [(1, 1, 1, 1, 1, 1), (1, 0, 0, 1, 0, 1), (0, 1, 1, 0, 1, 0), (1, 1, 1, 1, 0, 1)]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("bc", PMC_BC)
+@pytest.mark.parametrize("dims", [(37, 29, 23), (130, 3, 2), (5, 9, 2), (33, 65, 4)])
+def test_random_grids_pmc_walls(dims, bc, precision, kernel):
+    """per-face PMC walls (tangential E of the wall updated with the half dual face), one port ON a PMC wall,
+    random initial fields that are non-zero on the PMC walls"""
+    p = W.random_problem(*dims, seed=5000 + sum(dims) + sum(bc), loss_mode=LOSS_CD, steps=40, n_ports=3, bc=bc)
+    run_pair(p, 40, precision, kernel, checkpoints=(1, 10))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_pmc_exp_loss_and_z_chunks(kernel, monkeypatch):
+    monkeypatch.setenv("EM_FUSED_ZSPLIT", "3")
+    p = W.random_problem(21, 18, 33, seed=5101, loss_mode=LOSS_EXP, steps=30, n_ports=20, bc=(0, 1, 1, 1, 1, 1))
+    run_pair(p, 30, 64, kernel, checkpoints=(1, 7))
+
+
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_random_grid_percell_ids_and_pec_material(kernel):
     p = W.random_problem(21, 19, 17, seed=3001, blocky=False, steps=30, n_ports=2)

@@ -65,8 +65,11 @@ def test_create_validates_before_touching_the_device():
     assert create(m=bad) == 1
     assert create(w=C.c_void_p(8)) == 1                      # misaligned workspace
     assert create(w=None) == 1
+    gp = B._mk_grid(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, 64, bc=(2, 0, 0, 0, 0, 0))
+    assert create(grid=gp) == 1                              # unknown boundary condition
+    assert b"boundary" in L.em_last_error()
     gp = B._mk_grid(p.nx, p.ny, p.nz, p.dx, p.dy, p.dz, 64, bc=(1, 0, 0, 0, 0, 0))
-    assert create(grid=gp) == 5                              # PMC: EM_ERR_UNSUPPORTED
+    assert create(grid=gp, n_mat=255) == 1                   # a PMC wall needs a table id of its own
     assert b"PMC" in L.em_last_error()
     for fn in (L.em_step, L.em_reset):
         assert fn(None, 1) == 1 if fn is L.em_step else fn(None) == 1
