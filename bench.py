@@ -106,7 +106,7 @@ def make_problem(args):
     kw = {}
     if args.config in (4, 5):
         kw["steps"] = max(args.steps + args.warmup, 1000) if args.scale == 1 else args.steps + args.warmup
-    elif args.config in (2, 3):
+    elif args.config in (2, 3, 6):
         kw["steps"] = args.steps + args.warmup
     if args.config == 1:
         return W.make_config(1)
@@ -298,7 +298,8 @@ def run_b200(args):
         "vs_baseline": None, "dtype": "f32" if precision == 32 else "f64", "data": "synthetic",
         "config": {"workload": "config %d: %s %dx%dx%d cells (%d), %d ports, %s loss, Joule map every %s steps"
                                % (args.config, p.name, p.nx, p.ny, p.nz, cells, p.n_ports,
-                                  "EXP" if p.loss_mode else "CD", je or "-"),
+                                  "EXP" if p.loss_mode else "CD", je or "-")
+                               + (", walls -x+x-y+y-z+z = %s (1 = PMC)" % "".join(str(int(b)) for b in p.bc) if any(p.bc) else ""),
                    "kernel_strategy": args.kernel, "l2": "state %.1f GB >> 126 MB L2 (no flush needed)" % (em.workspace_bytes / 1e9)
                    if em.workspace_bytes > 1e9 else "state fits L2: %.0f MB" % (em.workspace_bytes / 1e6),
                    "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},

@@ -113,6 +113,22 @@ def test_pmc_exp_loss_and_z_chunks(kernel, monkeypatch):
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
+def test_config6_paper_mesh_scaled(kernel):
+    """the paper-shaped run (PAPER.md L160 mesh, 20 fs, PEC ground + PMC walls) at 1/4 of the x, y cell counts"""
+    p = W.make_config(6, scale=4, steps=300)
+    assert p.bc == (1, 1, 1, 1, 0, 1) and p.dt == 20.0e-15
+    run_pair(p, 300, 32, kernel, checkpoints=(10,))
+
+
+def test_config6_paper_mesh_full_size():
+    """376 x 408 x 45 cells = the paper's 21 088 285 EM unknowns, fp32, AUTO strategy, the whole field compared"""
+    p = W.make_config(6, steps=120)
+    ne = p.nx * (p.ny + 1) * (p.nz + 1) + (p.nx + 1) * p.ny * (p.nz + 1) + (p.nx + 1) * (p.ny + 1) * p.nz
+    assert ne == 21088285                                      # PAPER.md L160
+    run_pair(p, 120, 32, P.EM_KERNEL_AUTO, checkpoints=(3,))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
 def test_random_grid_percell_ids_and_pec_material(kernel):
     p = W.random_problem(21, 19, 17, seed=3001, blocky=False, steps=30, n_ports=2)
     run_pair(p, 30, 64, kernel)

@@ -16,6 +16,7 @@ from .configs import (
     config3_interposer,
     config4_package,
     config5_graded,
+    config6_paper_mesh,
     random_problem,
     impulse_problem,
     make_config,
@@ -24,5 +25,5 @@ from .configs import (
 __all__ = [
     "Problem", "EPS0", "MU0", "C0", "material_table", "MATERIAL_NAMES", "cfl_dt",
     "config1_cavity", "config2_slab", "config3_interposer", "config4_package",
-    "config5_graded", "random_problem", "impulse_problem", "make_config",
+    "config5_graded", "config6_paper_mesh", "random_problem", "impulse_problem", "make_config",
 ]

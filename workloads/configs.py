@@ -354,11 +354,12 @@ def _package_layout(nx: int, ny: int, nz: int, rng, n_traces: int, n_ports: int)
     return mat, ports
 
 
-def _package_waveforms(p: Problem, ports, rng, steps: int):
+def _package_waveforms(p: Problem, ports, rng, steps: int, window_steps: Optional[int] = None):
     """The paper's three waveform families with the 300 ps window mapped onto
-    T = steps*dt, and its deterministic jitter."""
+    T = window_steps*dt (default: the run length steps*dt), and its deterministic jitter (PAPER.md L146);
+    `steps` samples are tabulated."""
     src = _Sources()
-    T = steps * p.dt
+    T = (window_steps if window_steps is not None else steps) * p.dt
     u = T / 300.0                                    # "one paper picosecond"
     t = _half_times(steps, p.dt)
     for fam, edges in ports:
@@ -433,6 +434,36 @@ def config5_graded(scale: int = 1, zscale: int = 1, steps: Optional[int] = None,
     _package_waveforms(p, ports, rng, steps)
     _probes_default(p, rng)
     p.notes = "centres x=%s y=%s ports=%d" % (cx, cy, len(ports))
+    return p
+
+
+def config6_paper_mesh(scale: int = 1, steps: Optional[int] = None, n_ports: int = 64, n_traces: int = 96,
+                       precision: int = 32) -> Problem:
+    """NEXT-2 of SURVEY.md 8(f): a run shaped like the paper's own (376 x 408 x 45 cells, EM DOF
+    21 088 285, dt = 20 fs, 300 ps = 15 000 steps; L134: ground plane on z = 0; L142: PMC on the rest of the
+    EM boundary; L144-L146: Ricker / 5 GHz sine / 40 GHz burst ports with jitter, at PHYSICAL time scale).
+    The layout itself (NEC SX-Aurora, Fig. 1) is not public: cfg 4's seeded package generator in index space
+    stands in for it, on a non-uniform grid (x, y: 20 um under the dies graded to 60 um; z: 12 um in the
+    bump / RDL region graded to 80 um) chosen so that the paper's dt = 20 fs is below 0.9 x the CFL bound."""
+    rng = np.random.default_rng(SEED0 + 6)
+    nx, ny, nz = 376 // scale, 408 // scale, 45
+    dx = _graded_axis(nx, [nx // 2], max(2, nx // 4), fine=20.0e-6, coarse=60.0e-6, ratio=1.05) * scale
+    dy = _graded_axis(ny, [ny // 2], max(2, ny // 4), fine=20.0e-6, coarse=60.0e-6, ratio=1.05) * scale
+    dz = _graded_axis(nz, [int(round(nz * 116 / 192.0))], 4, fine=12.0e-6, coarse=80.0e-6, ratio=1.2)
+    if scale > 1:
+        n_traces = max(8, n_traces // scale); n_ports = max(8, n_ports // scale)
+    mat, ports = _package_layout(nx, ny, nz, rng, n_traces, n_ports)
+    table = material_table(16)
+    dt = 20.0e-15                                           # PAPER.md L160
+    assert dt <= cfl_dt(dx, dy, dz, mat, table, 0.9), "20 fs must satisfy the CFL rule on this grid"
+    if steps is None:
+        steps = 15000
+    p = Problem("cfg6_paper_mesh", nx, ny, nz, dx, dy, dz, mat, table, np.zeros(16, np.int32), dt,
+                LOSS_CD, precision, steps)
+    p.bc = (1, 1, 1, 1, 0, 1)                               # PEC ground at z = 0, PMC elsewhere
+    _package_waveforms(p, ports, rng, steps, window_steps=15000)
+    _probes_default(p, rng)
+    p.notes = "ports=%d  Lx=%.2f mm Ly=%.2f mm Lz=%.2f mm" % (len(ports), dx.sum() * 1e3, dy.sum() * 1e3, dz.sum() * 1e3)
     return p
 
 
@@ -563,4 +594,6 @@ def make_config(k: int, scale: int = 1, **kw) -> Problem:
         return config4_package(scale=scale, **kw)
     if k == 5:
         return config5_graded(scale=scale, **kw)
-    raise ValueError("config must be 1..5")
+    if k == 6:
+        return config6_paper_mesh(scale=scale, **kw)
+    raise ValueError("config must be 1..6")
