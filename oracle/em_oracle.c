@@ -26,6 +26,9 @@
  * brute force, worked impulse example, axis-permutation symmetry, CFL power iteration) and
  * tests/test_oracle_pmc.py for the PMC walls of PAPER.md L142 (mirror-image equivalence with the all-PEC
  * doubled domain, quarter-wave closed form, energy and Poynting balance with mixed walls, dense eq. (2)-(3)).
+ * Thermal stage (NEXT-1: PAPER.md eq. (4)-(6)) -- emo_set_thermal & co. at the end of this file -- is pinned by
+ * tests/test_oracle_thermal.py (adiabatic scalar recurrence + exact energy balance, cosine-mode diffusion closed form,
+ * heat conservation == Joule energy, dense V0a^T D_k V0).
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -68,7 +71,14 @@ typedef struct emo_ctx {
     double *dx, *dy, *dz;          /* primal lengths */
     double *tx, *ty, *tz;          /* dual lengths d~ (nx+1, ny+1, nz+1) */
     uint8_t *mat;                  /* [nz][ny][nx] */
-    double *sigma_c;               /* per-cell sigma (from the table) */
+    double *sigma_c;               /* per-cell sigma: the table's, or sigma(T) of eq. (6) when thermal coupling is on */
+    double *eps_c;                 /* per-cell eps (from the table) */
+    uint8_t *pec_c;                /* per-cell PEC-material flag */
+    /* thermal coupling (eq. (4)-(6), L84-L96; NEXT-1 of SURVEY.md 8(f)); off unless emo_set_thermal */
+    int32_t thermal;
+    double *theta, *theta_n;       /* temperature rise T - T0 per cell, and the next level */
+    double *dq;                    /* Joule energy density deposited in the current step [J/m^3] */
+    double *sigma0_c, *rho_cp_c, *kth_c, *alpha_c;
     double *E[3], *H[3];           /* fields */
     double *En[3];                 /* E^{n+1} scratch */
     double *ca[3], *cb[3];         /* per-edge update coefficients (0,0 on fixed edges) */
@@ -155,7 +165,8 @@ static void loss_coeff(int mode, double eps, double sig, double dt, double *ca, 
 static void free_ctx(emo_ctx *c) {
     if (!c) return;
     free(c->dx); free(c->dy); free(c->dz); free(c->tx); free(c->ty); free(c->tz);
-    free(c->mat); free(c->sigma_c); free(c->q);
+    free(c->mat); free(c->sigma_c); free(c->q); free(c->eps_c); free(c->pec_c);
+    free(c->theta); free(c->theta_n); free(c->dq); free(c->sigma0_c); free(c->rho_cp_c); free(c->kth_c); free(c->alpha_c);
     for (int a = 0; a < 3; ++a) {
         free(c->E[a]); free(c->H[a]); free(c->En[a]); free(c->ca[a]); free(c->cb[a]);
         free(c->fixed[a]); free(c->nu[a]); free(c->J[a]);
@@ -165,6 +176,61 @@ static void free_ctx(emo_ctx *c) {
 }
 
 int32_t emo_destroy(emo_ctx *c) { free_ctx(c); return EMO_OK; }
+
+/* D_eps, D_sigma on the edges (SURVEY.md 8(c) "Coefficients", C5) from the per-cell eps, sigma and PEC flags, and
+ * the update coefficients ca, cb of every non-fixed edge.  Called once at create, and again after every step when
+ * sigma depends on the temperature ("D_sigma(T^n) ... updated at each time step"). */
+static void edge_coefficients(emo_ctx *c) {
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    const int wx0 = c->bc[0] == EMO_BC_PEC, wx1 = c->bc[1] == EMO_BC_PEC, wy0 = c->bc[2] == EMO_BC_PEC,
+              wy1 = c->bc[3] == EMO_BC_PEC, wz0 = c->bc[4] == EMO_BC_PEC, wz1 = c->bc[5] == EMO_BC_PEC;
+    /* ---- D_eps, D_sigma on edges: area-weighted mean over the <=4 cells round the edge ------ */
+    /* Ex(i,j,k): cells (i, j', k'), j' in {j-1,j}, k' in {k-1,k}, weight dy[j'] dz[k']            */
+    for (int k = 0; k <= nz; ++k) for (int j = 0; j <= ny; ++j) for (int i = 0; i < nx; ++i) {
+        double sw = 0, se = 0, ss = 0; int pec = 0;
+        for (int kk = k - 1; kk <= k; ++kk) for (int jj = j - 1; jj <= j; ++jj) {
+            if (jj < 0 || jj >= ny || kk < 0 || kk >= nz) continue;
+            const int64_t q = CELL(i, jj, kk);
+            double w = c->dy[jj] * c->dz[kk];
+            sw += w; se += w * c->eps_c[q]; ss += w * c->sigma_c[q]; pec |= c->pec_c[q];
+        }
+        int fx = (j == 0 && wy0) || (j == ny && wy1) || (k == 0 && wz0) || (k == nz && wz1) || pec;   /* PEC walls / PEC material */
+        int64_t e = EX(i, j, k);
+        c->fixed[0][e] = (uint8_t)fx;
+        if (!fx) loss_coeff(c->loss_mode, se / sw, ss / sw, c->dt, &c->ca[0][e], &c->cb[0][e]);
+        else c->ca[0][e] = c->cb[0][e] = 0.0;
+    }
+    /* Ey(i,j,k): cells (i', j, k'), weight dx[i'] dz[k'] */
+    for (int k = 0; k <= nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i <= nx; ++i) {
+        double sw = 0, se = 0, ss = 0; int pec = 0;
+        for (int kk = k - 1; kk <= k; ++kk) for (int ii = i - 1; ii <= i; ++ii) {
+            if (ii < 0 || ii >= nx || kk < 0 || kk >= nz) continue;
+            const int64_t q = CELL(ii, j, kk);
+            double w = c->dx[ii] * c->dz[kk];
+            sw += w; se += w * c->eps_c[q]; ss += w * c->sigma_c[q]; pec |= c->pec_c[q];
+        }
+        int fx = (i == 0 && wx0) || (i == nx && wx1) || (k == 0 && wz0) || (k == nz && wz1) || pec;
+        int64_t e = EY(i, j, k);
+        c->fixed[1][e] = (uint8_t)fx;
+        if (!fx) loss_coeff(c->loss_mode, se / sw, ss / sw, c->dt, &c->ca[1][e], &c->cb[1][e]);
+        else c->ca[1][e] = c->cb[1][e] = 0.0;
+    }
+    /* Ez(i,j,k): cells (i', j', k), weight dx[i'] dy[j'] */
+    for (int k = 0; k < nz; ++k) for (int j = 0; j <= ny; ++j) for (int i = 0; i <= nx; ++i) {
+        double sw = 0, se = 0, ss = 0; int pec = 0;
+        for (int jj = j - 1; jj <= j; ++jj) for (int ii = i - 1; ii <= i; ++ii) {
+            if (ii < 0 || ii >= nx || jj < 0 || jj >= ny) continue;
+            const int64_t q = CELL(ii, jj, k);
+            double w = c->dx[ii] * c->dy[jj];
+            sw += w; se += w * c->eps_c[q]; ss += w * c->sigma_c[q]; pec |= c->pec_c[q];
+        }
+        int fx = (i == 0 && wx0) || (i == nx && wx1) || (j == 0 && wy0) || (j == ny && wy1) || pec;
+        int64_t e = EZ(i, j, k);
+        c->fixed[2][e] = (uint8_t)fx;
+        if (!fx) loss_coeff(c->loss_mode, se / sw, ss / sw, c->dt, &c->ca[2][e], &c->cb[2][e]);
+        else c->ca[2][e] = c->cb[2][e] = 0.0;
+    }
+}
 
 int32_t emo_create(const emo_grid *g, const uint8_t *mat_id, const emo_material *tab, int32_t n_mat,
                    double dt, emo_ctx **out) {
@@ -184,9 +250,7 @@ int32_t emo_create(const emo_grid *g, const uint8_t *mat_id, const emo_material 
     emo_ctx *c = (emo_ctx *)calloc(1, sizeof(emo_ctx));
     c->nx = nx; c->ny = ny; c->nz = nz; c->loss_mode = g->loss_mode; c->dt = dt;
     for (int b = 0; b < 6; ++b) c->bc[b] = g->bc[b];
-    /* wall planes that hold tangential E at 0 */
-    const int wx0 = g->bc[0] == EMO_BC_PEC, wx1 = g->bc[1] == EMO_BC_PEC, wy0 = g->bc[2] == EMO_BC_PEC,
-              wy1 = g->bc[3] == EMO_BC_PEC, wz0 = g->bc[4] == EMO_BC_PEC, wz1 = g->bc[5] == EMO_BC_PEC;
+
     c->dx = (double *)malloc(sizeof(double) * nx); memcpy(c->dx, g->dx, sizeof(double) * nx);
     c->dy = (double *)malloc(sizeof(double) * ny); memcpy(c->dy, g->dy, sizeof(double) * ny);
     c->dz = (double *)malloc(sizeof(double) * nz); memcpy(c->dz, g->dz, sizeof(double) * nz);
@@ -199,7 +263,11 @@ int32_t emo_create(const emo_grid *g, const uint8_t *mat_id, const emo_material 
     for (int k = 0; k <= nz; ++k) c->tz[k] = 0.5 * ((k > 0 ? c->dz[k - 1] : 0.0) + (k < nz ? c->dz[k] : 0.0));
     c->mat = (uint8_t *)malloc(ncell); memcpy(c->mat, mat_id, ncell);
     c->sigma_c = (double *)malloc(sizeof(double) * ncell);
-    for (int64_t q = 0; q < ncell; ++q) c->sigma_c[q] = tab[mat_id[q]].sigma;
+    c->eps_c = (double *)malloc(sizeof(double) * ncell);
+    c->pec_c = (uint8_t *)malloc(ncell);
+    for (int64_t q = 0; q < ncell; ++q) {
+        c->sigma_c[q] = tab[mat_id[q]].sigma; c->eps_c[q] = tab[mat_id[q]].eps; c->pec_c[q] = (uint8_t)(tab[mat_id[q]].flags & 1);
+    }
     c->q = (double *)calloc(ncell, sizeof(double));
     for (int a = 0; a < 3; ++a) {
         int64_t ne = count_of(c, a), nf = count_of(c, 3 + a);
@@ -213,49 +281,7 @@ int32_t emo_create(const emo_grid *g, const uint8_t *mat_id, const emo_material 
         c->nu[a] = (double *)calloc(nf, sizeof(double));
     }
 
-    /* ---- D_eps, D_sigma on edges: area-weighted mean over the <=4 cells round the edge ------ */
-    /* Ex(i,j,k): cells (i, j', k'), j' in {j-1,j}, k' in {k-1,k}, weight dy[j'] dz[k']            */
-    for (int k = 0; k <= nz; ++k) for (int j = 0; j <= ny; ++j) for (int i = 0; i < nx; ++i) {
-        double sw = 0, se = 0, ss = 0; int pec = 0;
-        for (int kk = k - 1; kk <= k; ++kk) for (int jj = j - 1; jj <= j; ++jj) {
-            if (jj < 0 || jj >= ny || kk < 0 || kk >= nz) continue;
-            const emo_material *m = &tab[mat_id[CELL(i, jj, kk)]];
-            double w = c->dy[jj] * c->dz[kk];
-            sw += w; se += w * m->eps; ss += w * m->sigma; pec |= (m->flags & 1);
-        }
-        int fx = (j == 0 && wy0) || (j == ny && wy1) || (k == 0 && wz0) || (k == nz && wz1) || pec;   /* PEC walls / PEC material */
-        int64_t e = EX(i, j, k);
-        c->fixed[0][e] = (uint8_t)fx;
-        if (!fx) loss_coeff(c->loss_mode, se / sw, ss / sw, dt, &c->ca[0][e], &c->cb[0][e]);
-    }
-    /* Ey(i,j,k): cells (i', j, k'), weight dx[i'] dz[k'] */
-    for (int k = 0; k <= nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i <= nx; ++i) {
-        double sw = 0, se = 0, ss = 0; int pec = 0;
-        for (int kk = k - 1; kk <= k; ++kk) for (int ii = i - 1; ii <= i; ++ii) {
-            if (ii < 0 || ii >= nx || kk < 0 || kk >= nz) continue;
-            const emo_material *m = &tab[mat_id[CELL(ii, j, kk)]];
-            double w = c->dx[ii] * c->dz[kk];
-            sw += w; se += w * m->eps; ss += w * m->sigma; pec |= (m->flags & 1);
-        }
-        int fx = (i == 0 && wx0) || (i == nx && wx1) || (k == 0 && wz0) || (k == nz && wz1) || pec;
-        int64_t e = EY(i, j, k);
-        c->fixed[1][e] = (uint8_t)fx;
-        if (!fx) loss_coeff(c->loss_mode, se / sw, ss / sw, dt, &c->ca[1][e], &c->cb[1][e]);
-    }
-    /* Ez(i,j,k): cells (i', j', k), weight dx[i'] dy[j'] */
-    for (int k = 0; k < nz; ++k) for (int j = 0; j <= ny; ++j) for (int i = 0; i <= nx; ++i) {
-        double sw = 0, se = 0, ss = 0; int pec = 0;
-        for (int jj = j - 1; jj <= j; ++jj) for (int ii = i - 1; ii <= i; ++ii) {
-            if (ii < 0 || ii >= nx || jj < 0 || jj >= ny) continue;
-            const emo_material *m = &tab[mat_id[CELL(ii, jj, k)]];
-            double w = c->dx[ii] * c->dy[jj];
-            sw += w; se += w * m->eps; ss += w * m->sigma; pec |= (m->flags & 1);
-        }
-        int fx = (i == 0 && wx0) || (i == nx && wx1) || (j == 0 && wy0) || (j == ny && wy1) || pec;
-        int64_t e = EZ(i, j, k);
-        c->fixed[2][e] = (uint8_t)fx;
-        if (!fx) loss_coeff(c->loss_mode, se / sw, ss / sw, dt, &c->ca[2][e], &c->cb[2][e]);
-    }
+    edge_coefficients(c);
     /* ---- 1/mu on faces: length-weighted mean over the <=2 cells across the face ------------- */
     for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i <= nx; ++i) {
         double sw = 0, sn = 0;
@@ -322,6 +348,41 @@ int32_t emo_get_field(emo_ctx *c, int32_t comp, double *dst) {
     if (!c || comp < 0 || comp > 5 || !dst) return EMO_ERR_INVALID_ARG;
     memcpy(dst, comp < 3 ? c->E[comp] : c->H[comp - 3], sizeof(double) * count_of(c, comp));
     return EMO_OK;
+}
+
+/* Thermal stage (NEXT-1 of SURVEY.md 8(f); eq. (4)-(6), L84-L96), on the temperature RISE theta = T - T0
+ * (M_kk annihilates constants and eq. (6) sees only T - T0, so T0 never enters):
+ *   eq. (5)  theta^{n+1} = theta^n - dt/(rho c_p) (M_kk theta^n) + (dt P^{n+1})/(rho c_p)
+ *   eq. (6)  sigma^{n+1} = sigma_0 / (1 + alpha theta^{n+1}),   then D_sigma(T^{n+1}) for the next E update (L78)
+ * Readings (T1-T5): theta per CELL (the Joule heat is per cell, C7); dt P^{n+1} := the Joule energy density
+ * dq_c this step deposited (time-centred, with the sigma(T^n) the E update used), so that EM loss == heat gained
+ * exactly; M_kk = V0a^T D_k V0 as the cell-centred finite-volume -div k grad: the flux through the face between
+ * cells c and c' is k_f A_f (theta_c - theta_c') / l~_f with the series (harmonic) conductivity
+ * k_f l~_f^-1 = 2 / (d_c/k_c + d_c'/k_c'); no flux through the walls (adiabatic). */
+static void thermal_step(emo_ctx *c) {
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    const double dt = c->dt;
+    const double *dx = c->dx, *dy = c->dy, *dz = c->dz, *th = c->theta, *kt = c->kth_c;
+    int k;
+#define COND(da, ka, db, kb) (((ka) > 0.0 && (kb) > 0.0) ? 2.0 / ((da) / (ka) + (db) / (kb)) : 0.0)   /* k_f / l~_f */
+#pragma omp parallel for schedule(static)
+    for (k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+        const int64_t q = CELL(i, j, k);
+        double out = 0.0;                               /* (M_kk theta)_c V_c : heat leaving cell c per second */
+        if (i > 0)      out += COND(dx[i], kt[q], dx[i - 1], kt[CELL(i - 1, j, k)]) * dy[j] * dz[k] * (th[q] - th[CELL(i - 1, j, k)]);
+        if (i < nx - 1) out += COND(dx[i], kt[q], dx[i + 1], kt[CELL(i + 1, j, k)]) * dy[j] * dz[k] * (th[q] - th[CELL(i + 1, j, k)]);
+        if (j > 0)      out += COND(dy[j], kt[q], dy[j - 1], kt[CELL(i, j - 1, k)]) * dx[i] * dz[k] * (th[q] - th[CELL(i, j - 1, k)]);
+        if (j < ny - 1) out += COND(dy[j], kt[q], dy[j + 1], kt[CELL(i, j + 1, k)]) * dx[i] * dz[k] * (th[q] - th[CELL(i, j + 1, k)]);
+        if (k > 0)      out += COND(dz[k], kt[q], dz[k - 1], kt[CELL(i, j, k - 1)]) * dx[i] * dy[j] * (th[q] - th[CELL(i, j, k - 1)]);
+        if (k < nz - 1) out += COND(dz[k], kt[q], dz[k + 1], kt[CELL(i, j, k + 1)]) * dx[i] * dy[j] * (th[q] - th[CELL(i, j, k + 1)]);
+        const double vol = dx[i] * dy[j] * dz[k];
+        c->theta_n[q] = th[q] - dt / c->rho_cp_c[q] * (out / vol) + c->dq[q] / c->rho_cp_c[q];
+    }
+#undef COND
+    { double *t = c->theta; c->theta = c->theta_n; c->theta_n = t; }
+    const int64_t ncell = (int64_t)nx * ny * nz;
+    for (int64_t q = 0; q < ncell; ++q) c->sigma_c[q] = c->sigma0_c[q] / (1.0 + c->alpha_c[q] * c->theta[q]);   /* eq. (6) */
+    edge_coefficients(c);                               /* D_sigma(T^{n+1}) for the next step */
 }
 
 /* One step n -> n+1 (SURVEY.md 8(c) "One step"): a1 H update, a3 source, a2 E update, a4 Joule. */
@@ -399,7 +460,9 @@ static void one_step(emo_ctx *c) {
             B2(Ex, Exn, EX(i, j, k)) + B2(Ex, Exn, EX(i, j + 1, k)) + B2(Ex, Exn, EX(i, j, k + 1)) + B2(Ex, Exn, EX(i, j + 1, k + 1)) +
             B2(Ey, Eyn, EY(i, j, k)) + B2(Ey, Eyn, EY(i + 1, j, k)) + B2(Ey, Eyn, EY(i, j, k + 1)) + B2(Ey, Eyn, EY(i + 1, j, k + 1)) +
             B2(Ez, Ezn, EZ(i, j, k)) + B2(Ez, Ezn, EZ(i + 1, j, k)) + B2(Ez, Ezn, EZ(i, j + 1, k)) + B2(Ez, Ezn, EZ(i + 1, j + 1, k)));
-        c->q[CELL(i, j, k)] += dt * c->sigma_c[CELL(i, j, k)] * s;
+        const double dq = dt * c->sigma_c[CELL(i, j, k)] * s;     /* heat deposited in this step, sigma = sigma(T^n) */
+        c->q[CELL(i, j, k)] += dq;
+        if (c->thermal) c->dq[CELL(i, j, k)] = dq;
     }
 #undef B2
 
@@ -413,6 +476,7 @@ static void one_step(emo_ctx *c) {
             c->J[ed->comp][IX(sx, sy, ed->i, ed->j, ed->k)] = 0.0;
         }
     }
+    if (c->thermal) thermal_step(c);
     c->step += 1;
 }
 
@@ -473,8 +537,57 @@ int32_t emo_reset(emo_ctx *c) {
         memset(c->H[a], 0, sizeof(double) * count_of(c, 3 + a));
     }
     memset(c->q, 0, sizeof(double) * (int64_t)c->nx * c->ny * c->nz);
+    if (c->thermal) {
+        const int64_t ncell = (int64_t)c->nx * c->ny * c->nz;
+        memset(c->theta, 0, sizeof(double) * ncell);
+        memcpy(c->sigma_c, c->sigma0_c, sizeof(double) * ncell);
+        edge_coefficients(c);
+    }
     c->step = 0;
     return EMO_OK;
 }
 
 int64_t emo_step_index(const emo_ctx *c) { return c ? c->step : -1; }
+
+/* ---- thermal coupling API (NEXT-1) ---------------------------------------------------------------------------- */
+typedef struct { double rho_cp, k, alpha; } emo_thermal_material;   /* J/(m^3 K), W/(m K), 1/K */
+
+/* Switches the coupling on: per-material volumetric heat capacity, thermal conductivity and temperature coefficient
+ * of resistance; theta = 0, sigma = sigma_0 (the table's).  rho_cp > 0, k >= 0 (0 = no conduction through the cell). */
+int32_t emo_set_thermal(emo_ctx *c, const emo_thermal_material *tt, int32_t n_mat) {
+    if (!c || !tt || n_mat < 1) return EMO_ERR_INVALID_ARG;
+    const int64_t ncell = (int64_t)c->nx * c->ny * c->nz;
+    for (int64_t q = 0; q < ncell; ++q) if (c->mat[q] >= n_mat) return EMO_ERR_INVALID_ARG;
+    for (int m = 0; m < n_mat; ++m) if (!(tt[m].rho_cp > 0.0) || !(tt[m].k >= 0.0)) return EMO_ERR_INVALID_ARG;
+    if (!c->thermal) {
+        c->theta = (double *)calloc(ncell, sizeof(double)); c->theta_n = (double *)calloc(ncell, sizeof(double));
+        c->dq = (double *)calloc(ncell, sizeof(double));
+        c->sigma0_c = (double *)malloc(sizeof(double) * ncell); c->rho_cp_c = (double *)malloc(sizeof(double) * ncell);
+        c->kth_c = (double *)malloc(sizeof(double) * ncell); c->alpha_c = (double *)malloc(sizeof(double) * ncell);
+        memcpy(c->sigma0_c, c->sigma_c, sizeof(double) * ncell);
+        c->thermal = 1;
+    }
+    for (int64_t q = 0; q < ncell; ++q) {
+        c->rho_cp_c[q] = tt[c->mat[q]].rho_cp; c->kth_c[q] = tt[c->mat[q]].k; c->alpha_c[q] = tt[c->mat[q]].alpha;
+        c->theta[q] = 0.0; c->sigma_c[q] = c->sigma0_c[q];
+    }
+    edge_coefficients(c);
+    return EMO_OK;
+}
+
+int32_t emo_get_temperature_rise(emo_ctx *c, double *dst) {
+    if (!c || !dst || !c->thermal) return EMO_ERR_INVALID_ARG;
+    memcpy(dst, c->theta, sizeof(double) * (int64_t)c->nx * c->ny * c->nz);
+    return EMO_OK;
+}
+
+/* sets theta and refreshes sigma(T) (eq. 6) and the edge coefficients */
+int32_t emo_set_temperature_rise(emo_ctx *c, const double *src) {
+    if (!c || !src || !c->thermal) return EMO_ERR_INVALID_ARG;
+    const int64_t ncell = (int64_t)c->nx * c->ny * c->nz;
+    for (int64_t q = 0; q < ncell; ++q) if (!(1.0 + c->alpha_c[q] * src[q] > 0.0)) return EMO_ERR_INVALID_ARG;
+    memcpy(c->theta, src, sizeof(double) * ncell);
+    for (int64_t q = 0; q < ncell; ++q) c->sigma_c[q] = c->sigma0_c[q] / (1.0 + c->alpha_c[q] * c->theta[q]);
+    edge_coefficients(c);
+    return EMO_OK;
+}

@@ -130,6 +130,8 @@ class Oracle:
         if load_init and p.init:
             for comp, arr in p.init.items():
                 self.set_field(comp, arr)
+        if getattr(p, "thermal", None) is not None:
+            self.set_thermal(p.thermal)
 
     def close(self):
         if self._h:
@@ -206,6 +208,28 @@ class Oracle:
 
     def reset(self):
         lib().emo_reset(self._h)
+
+    # ---- thermal coupling (NEXT-1; eq. (4)-(6)) --------------------------------------
+    def set_thermal(self, thermal):
+        """thermal: (n_mat, 3) float64 rows (rho_cp [J/m^3/K], k [W/m/K], alpha [1/K])"""
+        t = np.ascontiguousarray(thermal, np.float64)
+        rc = lib().emo_set_thermal(self._h, _dp(t), int(t.shape[0]))
+        if rc:
+            raise RuntimeError("emo_set_thermal rc=%d" % rc)
+
+    def temperature_rise(self) -> np.ndarray:
+        out = np.empty((self.nz, self.ny, self.nx), np.float64)
+        rc = lib().emo_get_temperature_rise(self._h, _dp(out))
+        if rc:
+            raise RuntimeError("emo_get_temperature_rise rc=%d" % rc)
+        return out
+
+    def set_temperature_rise(self, theta):
+        a = np.ascontiguousarray(theta, np.float64)
+        assert a.shape == (self.nz, self.ny, self.nx)
+        rc = lib().emo_set_temperature_rise(self._h, _dp(a))
+        if rc:
+            raise RuntimeError("emo_set_temperature_rise rc=%d" % rc)
 
     @property
     def step_index(self) -> int:

@@ -9,7 +9,7 @@ The five configurations are the synthetic stand-ins named in BASELINE.json ``con
 follows SURVEY.md section 8(d) and is restated in DESIGN.md.  The paper's own layout (PAPER.md
 L130-L138, Fig. 1) is not public, so these inputs stand in for its structure.
 """
-from .problem import Problem, EPS0, MU0, C0, material_table, MATERIAL_NAMES, cfl_dt
+from .problem import Problem, EPS0, MU0, C0, material_table, thermal_table, MATERIAL_NAMES, cfl_dt
 from .configs import (
     config1_cavity,
     config2_slab,
@@ -23,7 +23,7 @@ from .configs import (
 )
 
 __all__ = [
-    "Problem", "EPS0", "MU0", "C0", "material_table", "MATERIAL_NAMES", "cfl_dt",
+    "Problem", "EPS0", "MU0", "C0", "material_table", "thermal_table", "MATERIAL_NAMES", "cfl_dt",
     "config1_cavity", "config2_slab", "config3_interposer", "config4_package",
     "config5_graded", "config6_paper_mesh", "random_problem", "impulse_problem", "make_config",
 ]

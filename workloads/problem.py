@@ -43,6 +43,33 @@ MATERIAL_NAMES = [m[0] for m in _MATERIALS]
 VAC, SI, SIO2, CU, ORG, UF, PI, EMC, BT, SOLDER, LOWK, SIN, DSI, LINER, AL, MAG = range(16)
 
 
+# Thermal constants of the same 16 materials (handbook-order values, NOT from the paper, which prints mechanical
+# constants only): rho*c_p [J/m^3/K], k [W/m/K], alpha = temperature coefficient of resistance [1/K]
+_THERMAL = [
+    (1.2e3,   0.026, 0.0),      # vacuum / air
+    (1.63e6, 148.0,  0.0),      # silicon
+    (1.61e6,   1.4,  0.0),      # sio2
+    (3.45e6, 400.0,  3.9e-3),   # copper
+    (1.8e6,    0.3,  0.0),      # organic substrate
+    (1.9e6,    0.5,  0.0),      # underfill
+    (1.55e6,   0.2,  0.0),      # polyimide
+    (1.7e6,    0.8,  0.0),      # epoxy mould
+    (1.8e6,    0.35, 0.0),      # BT resin
+    (1.67e6,  50.0,  4.0e-3),   # solder
+    (1.4e6,    0.6,  0.0),      # low-k oxide
+    (2.2e6,   20.0,  0.0),      # SiN
+    (1.63e6, 130.0,  0.0),      # doped Si
+    (1.61e6,   1.4,  0.0),      # TSV liner
+    (2.42e6, 237.0,  4.3e-3),   # aluminium
+    (2.0e6,    1.0,  0.0),      # test magnetic
+]
+
+
+def thermal_table(n: int = 16) -> np.ndarray:
+    """(n, 3) float64 array of (rho*c_p, k, alpha)."""
+    return np.asarray(_THERMAL[:n], np.float64).copy()
+
+
 def material_table(n: int = 16) -> np.ndarray:
     """(n, 3) float64 array of absolute (eps, mu, sigma)."""
     t = np.empty((n, 3), dtype=np.float64)
@@ -90,6 +117,9 @@ class Problem:
     joule_every: int = 0      # config 4: Joule map output every 100 steps
     # wall truncation, order -x, +x, -y, +y, -z, +z: BC_PEC (tangential E = 0) or BC_PMC
     bc: tuple = (0, 0, 0, 0, 0, 0)
+    # thermal coupling (eq. (4)-(6)): None = EM only; else (n_mat, 3) float64 rows
+    # (rho*c_p [J/m^3/K], k [W/m/K], alpha [1/K]) -> temperature rise per cell and sigma(T) feedback
+    thermal: Optional[np.ndarray] = None
     notes: str = ""
 
     @property
