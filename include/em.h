@@ -80,6 +80,8 @@ typedef struct em_grid {
     int32_t max_ports;           /* capacity reserved in the workspace for em_set_source            */
     int64_t max_source_edges;
     int64_t max_wave_samples;
+    int32_t thermal;             /* 1: reserve workspace for the thermal stage (em_set_thermal); forces the    */
+    int32_t pad_;                /*    SPLIT strategy (EM_ERR_UNSUPPORTED with kernel = FUSED / TMA).  0: EM only */
 } em_grid;
 
 typedef struct em_material { double eps, mu, sigma; int32_t flags; int32_t pad_; } em_material;
@@ -148,6 +150,24 @@ int32_t em_probe(em_ctx *ctx, int32_t n_pts, const em_probe_pt *pts, double *out
 
 /* Zero the six fields, q and the step counter; keep grid, materials and sources. */
 int32_t em_reset(em_ctx *ctx);
+
+/* ---- two-way thermal coupling (eq. (4)-(6), L84-L96; NEXT-1 of SURVEY.md 8(f)) ------------------------
+ * State: the temperature RISE theta = T - T0 per cell [K] (eq. (4) and (6) see only T - T0), dense [nz][ny][nx] maps
+ * in the working precision.  Per step, after a1-a4:
+ *   eq. (5)  theta' = theta - dt/(rho c_p) (M_kk theta) + dq/(rho c_p),  dq = the Joule energy density of the step (a4)
+ *   eq. (6)  sigma' = sigma_0 / (1 + alpha theta'), used by the next step's E update ("D_sigma(T^n)", L78)
+ * M_kk = V0a^T D_k V0: cell-centred -div k grad with the series conductivity of the two half cells on each face,
+ * adiabatic walls (L142).  sigma_0 = the em_material.sigma given to em_create.  em_joule's power density then uses
+ * the current sigma(T).  em_reset also zeroes theta.  Runs on the split kernels (first CUDA path of this stage). */
+typedef struct em_thermal_material { double rho_cp /* J/(m^3 K) > 0 */, k /* W/(m K) >= 0 */, alpha /* 1/K */; } em_thermal_material;
+
+/* Switches the coupling on (theta = 0).  table: HOST, n_mat entries (the n_mat of em_create).
+ * Errors: STATE (ctx created with em_grid.thermal = 0), INVALID_ARG, CUDA. */
+int32_t em_set_thermal(em_ctx *ctx, const em_thermal_material *table, int32_t n_mat);
+/* theta out / in (in: also refreshes sigma(T)); device or host pointer; host copies synchronise.
+ * Errors: STATE (coupling not switched on), INVALID_ARG, CUDA. */
+int32_t em_get_temperature_rise(em_ctx *ctx, void *dst, int32_t dst_is_device);
+int32_t em_set_temperature_rise(em_ctx *ctx, const void *src, int32_t src_is_device);
 
 /* Absolute step index n (host bookkeeping). */
 int32_t em_step_index(em_ctx *ctx, int64_t *n);

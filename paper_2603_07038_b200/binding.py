@@ -30,7 +30,12 @@ class em_grid(C.Structure):
                 ("dx", C.POINTER(C.c_double)), ("dy", C.POINTER(C.c_double)), ("dz", C.POINTER(C.c_double)),
                 ("precision", C.c_int32), ("loss_mode", C.c_int32), ("bc", C.c_int32 * 6),
                 ("kernel", C.c_int32), ("max_ports", C.c_int32),
-                ("max_source_edges", C.c_int64), ("max_wave_samples", C.c_int64)]
+                ("max_source_edges", C.c_int64), ("max_wave_samples", C.c_int64),
+                ("thermal", C.c_int32), ("pad_", C.c_int32)]
+
+
+class em_thermal_material(C.Structure):
+    _fields_ = [("rho_cp", C.c_double), ("k", C.c_double), ("alpha", C.c_double)]
 
 
 class em_material(C.Structure):
@@ -82,6 +87,9 @@ def load():
     L.em_joule.argtypes = [vp, vp, vp, C.POINTER(C.c_double), i32]
     L.em_probe.argtypes = [vp, i32, C.POINTER(em_probe_pt), C.POINTER(C.c_double)]
     L.em_reset.argtypes = [vp]
+    L.em_set_thermal.argtypes = [vp, C.POINTER(em_thermal_material), i32]
+    L.em_get_temperature_rise.argtypes = [vp, vp, i32]
+    L.em_set_temperature_rise.argtypes = [vp, vp, i32]
     L.em_step_index.argtypes = [vp, C.POINTER(i64)]
     L.em_launch_count.argtypes = [vp, C.POINTER(i64)]
     L.em_timing_enable.argtypes = [vp, i32]
@@ -100,7 +108,7 @@ def _dp(a: np.ndarray):
 
 
 def _mk_grid(nx, ny, nz, dx, dy, dz, precision=64, loss_mode=0, kernel=0, max_ports=0,
-             max_source_edges=0, max_wave_samples=0, bc=(0,) * 6) -> em_grid:
+             max_source_edges=0, max_wave_samples=0, bc=(0,) * 6, thermal=0) -> em_grid:
     g = em_grid()
     g.nx, g.ny, g.nz = int(nx), int(ny), int(nz)
     g.dx, g.dy, g.dz = _dp(dx), _dp(dy), _dp(dz)
@@ -108,6 +116,7 @@ def _mk_grid(nx, ny, nz, dx, dy, dz, precision=64, loss_mode=0, kernel=0, max_po
     for b in range(6):
         g.bc[b] = int(bc[b])
     g.max_ports, g.max_source_edges, g.max_wave_samples = int(max_ports), int(max_source_edges), int(max_wave_samples)
+    g.thermal = int(thermal)
     return g
 
 
@@ -172,7 +181,8 @@ class EM:
                               max_ports if max_ports is not None else max(n_ports, 1),
                               max_source_edges if max_source_edges is not None else max(n_con, 1),
                               max_wave_samples if max_wave_samples is not None else max(int(p.wave.shape[0]), 1),
-                              tuple(bc) if bc is not None else tuple(getattr(p, "bc", (0,) * 6)))
+                              tuple(bc) if bc is not None else tuple(getattr(p, "bc", (0,) * 6)),
+                              1 if getattr(p, "thermal", None) is not None else 0)
         nbytes = C.c_size_t()
         _check(self._L.em_workspace_bytes(C.byref(self._grid), C.byref(nbytes)))
         self.workspace_bytes = int(nbytes.value)
@@ -194,6 +204,8 @@ class EM:
         if load_init and getattr(p, "init", None):
             for comp, arr in p.init.items():
                 self.em_set_field(comp, arr)
+        if getattr(p, "thermal", None) is not None:
+            self.em_set_thermal(p.thermal)
 
     # -- lifetime ---------------------------------------------------------------------------
     def close(self):
@@ -250,6 +262,33 @@ class EM:
 
     def fields(self):
         return [self.em_get_field(c) for c in range(6)]
+
+    # thermal coupling (eq. (4)-(6)); the context must come from a problem with p.thermal set
+    def em_set_thermal(self, thermal):
+        t = np.ascontiguousarray(thermal, np.float64)
+        arr = (em_thermal_material * t.shape[0])()
+        for m in range(t.shape[0]):
+            arr[m].rho_cp, arr[m].k, arr[m].alpha = float(t[m, 0]), float(t[m, 1]), float(t[m, 2])
+        _check(self._L.em_set_thermal(self._h, arr, int(t.shape[0])))
+
+    def em_get_temperature_rise(self, out=None, device: bool = False):
+        shape = (self.nz, self.ny, self.nx)
+        if device:
+            t = out if out is not None else self._torch.empty(shape, dtype=self.dtype, device=self.device)
+            _check(self._L.em_get_temperature_rise(self._h, C.c_void_p(t.data_ptr()), 1))
+            return t
+        a = out if out is not None else np.empty(shape, self.np_dtype)
+        _check(self._L.em_get_temperature_rise(self._h, a.ctypes.data_as(C.c_void_p), 0))
+        return a
+
+    def em_set_temperature_rise(self, theta):
+        if self._torch.is_tensor(theta):
+            t = theta.to(device=self.device, dtype=self.dtype).contiguous()
+            _check(self._L.em_set_temperature_rise(self._h, C.c_void_p(t.data_ptr()), 1))
+            return
+        a = np.ascontiguousarray(theta, self.np_dtype)
+        assert a.shape == (self.nz, self.ny, self.nx)
+        _check(self._L.em_set_temperature_rise(self._h, a.ctypes.data_as(C.c_void_p), 0))
 
     def em_step(self, n: int = 1):
         _check(self._L.em_step(self._h, int(n)))

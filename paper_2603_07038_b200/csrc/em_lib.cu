@@ -16,6 +16,7 @@
 #include "em_fused.cuh"
 #include "em_split.cuh"
 #include "em_sweep.cuh"
+#include "em_thermal.cuh"
 
 namespace {
 
@@ -85,6 +86,8 @@ struct Carved {
     int *con_port; R *con_scale; long long *port_woff, *port_wlen; R *wave;
     // fused-sweep tile source index
     int *tile_sbeg; int4 *tile_ent;
+    // thermal coupling (only when em_grid.thermal != 0): theta ping-pong, sigma(T) per cell, thermal table
+    R *theta[2]; R *sig; em::ThEntry<R> *ttable;
 };
 
 template <typename R>
@@ -111,6 +114,11 @@ size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int
     o.wave = w.take<R>((size_t)std::max<int64_t>(gr.max_wave_samples, 1));
     o.tile_sbeg = w.take<int>((size_t)n_items + 1);
     o.tile_ent = w.take<int4>(4 * me);
+    o.theta[0] = o.theta[1] = o.sig = nullptr; o.ttable = nullptr;
+    if (gr.thermal) {
+        o.theta[0] = w.take<R>(g.alloc_elems); o.theta[1] = w.take<R>(g.alloc_elems); o.sig = w.take<R>(g.alloc_elems);
+        o.ttable = w.take<em::ThEntry<R>>(em::kMaxTable);
+    }
     return align_up(w.off);
 }
 
@@ -133,6 +141,8 @@ struct em_ctx {
     virtual int32_t joule(void *, void *, double *, int32_t) = 0;
     virtual int32_t probe(int32_t, const em_probe_pt *, double *) = 0;
     virtual int32_t reset() = 0;
+    virtual int32_t set_thermal(const em_thermal_material *, int32_t) = 0;
+    virtual int32_t temperature_rise(void *, const void *, int32_t) = 0;
     int64_t step_index = 0, launches = 0;
     Timing timing;
     const char *main_kernel = "";
@@ -190,6 +200,19 @@ struct Ctx final : em_ctx {
     int32_t joule(void *, void *, double *, int32_t) override;
     int32_t probe(int32_t, const em_probe_pt *, double *) override;
     int32_t reset() override { return zero_state(); }
+    int32_t set_thermal(const em_thermal_material *, int32_t) override;
+    int32_t temperature_rise(void *dst, const void *src, int32_t is_dev) override;
+    int32_t step_thermal();
+    int32_t refresh_sigma();
+    bool thermal_on = false;            // em_set_thermal was called
+    int th_cur = 0;
+    int n_mat_ = 0;
+    em::ThermalParams<R> tp() const {
+        em::ThermalParams<R> t;
+        t.theta = c.theta[th_cur] + g.origin; t.theta_n = c.theta[1 - th_cur] + g.origin;
+        t.sig = c.sig + g.origin; t.ttable = c.ttable;
+        return t;
+    }
     int32_t step_split();
     int32_t step_fused();
     int32_t step_tma();
@@ -220,6 +243,9 @@ int32_t validate_grid(const em_grid *g) {
     if (g->precision != 32 && g->precision != 64) return fail(EM_ERR_INVALID_ARG, "precision must be 32 or 64");
     if (g->loss_mode != EM_LOSS_CD && g->loss_mode != EM_LOSS_EXP) return fail(EM_ERR_INVALID_ARG, "bad loss_mode");
     if (g->kernel < EM_KERNEL_AUTO || g->kernel > EM_KERNEL_TMA) return fail(EM_ERR_INVALID_ARG, "bad kernel strategy");
+    if (g->thermal != 0 && g->thermal != 1) return fail(EM_ERR_INVALID_ARG, "thermal must be 0 or 1");
+    if (g->thermal && (g->kernel == EM_KERNEL_FUSED || g->kernel == EM_KERNEL_TMA))
+        return fail(EM_ERR_UNSUPPORTED, "thermal coupling runs on the split kernels (kernel = AUTO or SPLIT)");
     if (g->max_ports < 0 || g->max_source_edges < 0 || g->max_wave_samples < 0)
         return fail(EM_ERR_INVALID_ARG, "negative source capacity");
     return EM_OK;
@@ -231,6 +257,12 @@ int32_t Ctx<R>::zero_state() {
     CU(cudaMemsetAsync(c.q, 0, sizeof(R) * g.alloc_elems, stream));
     e_cur = h_cur = 0; bind();
     step_index = 0;
+    if (grid.thermal) {
+        CU(cudaMemsetAsync(c.theta[0], 0, sizeof(R) * g.alloc_elems, stream));
+        CU(cudaMemsetAsync(c.theta[1], 0, sizeof(R) * g.alloc_elems, stream));
+        th_cur = 0;
+        if (thermal_on) return refresh_sigma();
+    }
     return EM_OK;
 }
 
@@ -254,6 +286,8 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     if (ws_bytes < need) return fail(EM_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
     carve<R>(g, *gr, workspace, &c, max_items);
     sweep_smem = em::sweep_smem_bytes((int)sizeof(R), n_mat + 2);
+    n_mat_ = n_mat;
+    if (gr->thermal) kernel = EM_KERNEL_SPLIT;                // sigma(T) lives in a per-cell array: split kernels (em_thermal.cuh)
     if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_TMA;     // measured on config 4: TMA sweep 2.44 ms/step, cp.async sweep 2.71 ms/step
     if (kernel == EM_KERNEL_TMA) {
         int dev = 0, optin = 0;
@@ -585,6 +619,85 @@ int32_t Ctx<R>::step_split() {
     return EM_OK;
 }
 
+// ---- thermal coupling (NEXT-1; eq. (4)-(6); em_thermal.cuh) ---------------------------------------
+template <typename R>
+int32_t Ctx<R>::refresh_sigma() {
+    dim3 b(32, 8);
+    em::k_sigma_refresh<R><<<node_grid(b, 0), b, 0, stream>>>(p, tp());
+    CU(cudaGetLastError());
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::set_thermal(const em_thermal_material *tt, int32_t n_mat) {
+    if (!grid.thermal) return fail(EM_ERR_STATE, "the context was created with em_grid.thermal = 0");
+    if (!tt || n_mat != n_mat_) return fail(EM_ERR_INVALID_ARG, "thermal table must have the n_mat entries of em_create");
+    for (int m = 0; m < n_mat; ++m)
+        if (!(tt[m].rho_cp > 0.0) || !(tt[m].k >= 0.0)) return fail(EM_ERR_INVALID_ARG, "need rho_cp > 0 and k >= 0");
+    std::vector<em::ThEntry<R>> ht(p.n_table);          // the outside entries stay 0: no heat, no conduction
+    for (auto &e : ht) { e.irc = R(0); e.k = R(0); e.alpha = R(0); e.sigma0 = R(0); }
+    for (int m = 0; m < n_mat; ++m) {
+        ht[m].irc = (R)(1.0 / tt[m].rho_cp); ht[m].k = (R)tt[m].k; ht[m].alpha = (R)tt[m].alpha; ht[m].sigma0 = (R)table[m].sigma;
+    }
+    CU(cudaMemcpyAsync(c.ttable, ht.data(), sizeof(em::ThEntry<R>) * ht.size(), cudaMemcpyHostToDevice, stream));
+    CU(cudaMemsetAsync(c.theta[0], 0, sizeof(R) * g.alloc_elems, stream));
+    CU(cudaMemsetAsync(c.theta[1], 0, sizeof(R) * g.alloc_elems, stream));
+    CU(cudaMemsetAsync(c.sig, 0, sizeof(R) * g.alloc_elems, stream));
+    th_cur = 0;
+    thermal_on = true;
+    int32_t rc = refresh_sigma(); if (rc) return rc;
+    CU(cudaStreamSynchronize(stream));                   // ht is a local
+    return EM_OK;
+}
+
+// dst != null: copy theta out; src != null: copy theta in and refresh sigma(T).  Dense [nz][ny][nx] maps.
+template <typename R>
+int32_t Ctx<R>::temperature_rise(void *dst, const void *srcp, int32_t is_dev) {
+    if (!thermal_on) return fail(EM_ERR_STATE, "thermal coupling is not switched on (em_set_thermal)");
+    R *th = c.theta[th_cur] + g.origin;
+    cudaMemcpy3DParms m = {};
+    m.extent = make_cudaExtent(sizeof(R) * g.nx, g.ny, g.nz);
+    if (dst) {
+        m.srcPtr = make_cudaPitchedPtr(th, sizeof(R) * g.PX, g.PX, g.PY);
+        m.dstPtr = make_cudaPitchedPtr(dst, sizeof(R) * g.nx, g.nx, g.ny);
+        m.kind = is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+        CU(cudaMemcpy3DAsync(&m, stream));
+    } else {
+        m.srcPtr = make_cudaPitchedPtr(const_cast<void *>(srcp), sizeof(R) * g.nx, g.nx, g.ny);
+        m.dstPtr = make_cudaPitchedPtr(th, sizeof(R) * g.PX, g.PX, g.PY);
+        m.kind = is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+        CU(cudaMemcpy3DAsync(&m, stream));
+        int32_t rc = refresh_sigma(); if (rc) return rc;
+    }
+    if (!is_dev) CU(cudaStreamSynchronize(stream));
+    return EM_OK;
+}
+
+// One coupled step: a1, a2 with D_sigma(T^n), a3 with r_e(sigma(T^n)), then a4 + eq. (5) + eq. (6) in one kernel.
+template <typename R>
+int32_t Ctx<R>::step_thermal() {
+    dim3 b(32, 8);
+    const R *sig = c.sig + g.origin;
+    em::k_split_h<R><<<node_grid(b, 1), b, 0, stream>>>(p);
+    int32_t rc = record_begin(); if (rc) return rc;
+    if (loss == EM_LOSS_CD) em::k_split_e_sig<R, 0><<<node_grid(b, 1), b, 0, stream>>>(p, sig);
+    else                    em::k_split_e_sig<R, 1><<<node_grid(b, 1), b, 0, stream>>>(p, sig);
+    rc = record_end(); if (rc) return rc;
+    launches += 2;
+    if (n_unique) {
+        const int gs = (n_unique + 127) / 128;
+        if (loss == EM_LOSS_CD) em::k_source_coef_sig<R, 0><<<gs, 128, 0, stream>>>(p, src, sig);
+        else                    em::k_source_coef_sig<R, 1><<<gs, 128, 0, stream>>>(p, src, sig);
+        em::k_apply_source<R><<<gs, 128, 0, stream>>>(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
+        launches += 2;
+    }
+    em::k_joule_thermal<R><<<node_grid(b, 0), b, 0, stream>>>(p, tp());
+    launches += 1;
+    CU(cudaGetLastError());
+    e_cur ^= 1; th_cur ^= 1; bind();
+    return EM_OK;
+}
+
 template <typename R>
 int32_t Ctx<R>::step_fused() {
     int32_t rc = record_begin(); if (rc) return rc;
@@ -616,7 +729,7 @@ template <typename R>
 int32_t Ctx<R>::step(int64_t n) {
     if (n < 0) return fail(EM_ERR_INVALID_ARG, "n < 0");
     for (int64_t s = 0; s < n; ++s) {
-        int32_t rc = kernel == EM_KERNEL_TMA ? step_tma() : kernel == EM_KERNEL_FUSED ? step_fused() : step_split();
+        int32_t rc = thermal_on ? step_thermal() : kernel == EM_KERNEL_TMA ? step_tma() : kernel == EM_KERNEL_FUSED ? step_fused() : step_split();
         if (rc) return rc;
         step_index += 1;
     }
@@ -628,7 +741,8 @@ template <typename R>
 int32_t Ctx<R>::joule(void *power, void *energy, double *total, int32_t do_reset) {
     dim3 b(32, 8);
     if (power) {
-        em::k_power<R><<<node_grid(b, 0), b, 0, stream>>>(p, static_cast<R *>(power));
+        if (thermal_on) em::k_power_sig<R><<<node_grid(b, 0), b, 0, stream>>>(p, c.sig + g.origin, static_cast<R *>(power));
+        else            em::k_power<R><<<node_grid(b, 0), b, 0, stream>>>(p, static_cast<R *>(power));
         CU(cudaGetLastError()); launches += 1;
     }
     if (energy) {
@@ -775,6 +889,14 @@ int32_t em_step(em_ctx *ctx, int64_t n) { EM_CHECK_CTX; return ctx->step(n); }
 int32_t em_joule(em_ctx *ctx, void *p, void *q, double *t, int32_t reset) { EM_CHECK_CTX; return ctx->joule(p, q, t, reset); }
 int32_t em_probe(em_ctx *ctx, int32_t n, const em_probe_pt *pts, double *out) { EM_CHECK_CTX; return ctx->probe(n, pts, out); }
 int32_t em_reset(em_ctx *ctx) { EM_CHECK_CTX; return ctx->reset(); }
+
+int32_t em_set_thermal(em_ctx *ctx, const em_thermal_material *table, int32_t n_mat) { EM_CHECK_CTX; return ctx->set_thermal(table, n_mat); }
+int32_t em_get_temperature_rise(em_ctx *ctx, void *dst, int32_t dst_is_device) {
+    EM_CHECK_CTX; if (!dst) return fail(EM_ERR_INVALID_ARG, "null"); return ctx->temperature_rise(dst, nullptr, dst_is_device);
+}
+int32_t em_set_temperature_rise(em_ctx *ctx, const void *src, int32_t src_is_device) {
+    EM_CHECK_CTX; if (!src) return fail(EM_ERR_INVALID_ARG, "null"); return ctx->temperature_rise(nullptr, src, src_is_device);
+}
 int32_t em_step_index(em_ctx *ctx, int64_t *n) { EM_CHECK_CTX; if (!n) return fail(EM_ERR_INVALID_ARG, "null"); *n = ctx->step_index; return EM_OK; }
 int32_t em_launch_count(em_ctx *ctx, int64_t *n) { EM_CHECK_CTX; if (!n) return fail(EM_ERR_INVALID_ARG, "null"); *n = ctx->launches; return EM_OK; }
 

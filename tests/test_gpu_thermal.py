@@ -1,0 +1,96 @@
+"""GPU-vs-oracle parity of the two-way EM-thermal coupling (NEXT-1; eq. (4)-(6)) through the C ABI:
+fields, Joule maps AND the temperature rise, element by element, same seeded inputs, tolerances of north_star."""
+import numpy as np
+import pytest
+
+import workloads as W
+from workloads.problem import LOSS_CD, LOSS_EXP
+import paper_2603_07038_b200 as P
+from oracle import emo
+from parity import compare_state, rel_l2, TOL
+
+pytestmark = pytest.mark.gpu
+
+
+def _coupled(dims, seed, k_scale=2.0e5, tcr_scale=1.0e4, **kw):
+    """random heterogeneous non-uniform grid with the thermal table; conduction and the temperature coefficient
+    exaggerated so that both matter within a few dozen EM steps (see tests/test_oracle_thermal.py)"""
+    p = W.random_problem(*dims, seed=seed, **kw)
+    th = W.thermal_table()
+    th[:, 1] *= k_scale; th[:, 2] *= tcr_scale
+    p.thermal = th
+    return p
+
+
+def _run(p, steps, precision, checkpoints=()):
+    g = P.EM(p, precision=precision)
+    o = emo.Oracle(p)
+    tol = TOL[precision]
+    done = 0
+    for cp in list(checkpoints) + [steps]:
+        g.em_step(cp - done); o.step(cp - done); done = cp
+        res = compare_state(g, o, tol)
+        tg, to = g.em_get_temperature_rise(), o.temperature_rise()
+        res["theta"] = rel_l2([tg], [to])
+        assert np.max(np.abs(to)) > 0
+        assert res["theta"] <= tol, res
+    g.close(); o.close()
+    return res, to
+
+
+CASES = [((37, 29, 23), LOSS_CD), ((9, 7, 6), LOSS_CD), ((130, 3, 2), LOSS_CD), ((1, 5, 7), LOSS_CD),
+         ((37, 29, 23), LOSS_EXP), ((9, 7, 6), LOSS_EXP)]     # EXP on the non-degenerate grids, as in test_gpu_parity.py
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("dims,mode", CASES)
+def test_coupled_random_grids(dims, mode, precision):
+    p = _coupled(dims, 8000 + sum(dims), loss_mode=mode, steps=60, n_ports=3, init_scale=4.0e6)
+    res, theta = _run(p, 60, precision, checkpoints=(1, 10))
+    # the feedback is not a perturbation below the tolerance: alpha * theta reaches the per-cent range
+    assert (p.thermal[p.mat_id, 2] * theta).max() > 1e-3
+
+
+def test_coupled_with_pmc_walls_and_wall_port():
+    p = _coupled((21, 18, 12), 8101, steps=40, n_ports=4, init_scale=4.0e6, bc=(1, 1, 0, 1, 0, 1))
+    _run(p, 40, 64, checkpoints=(1,))
+
+
+def test_pure_diffusion_and_set_get_temperature():
+    p = _coupled((12, 9, 8), 8102, steps=30, n_ports=0, lossless=True)
+    p.init = None
+    rng = np.random.default_rng(9)
+    th0 = rng.uniform(0.0, 1.0, size=(p.nz, p.ny, p.nx))
+    for precision in (64, 32):
+        g = P.EM(p, precision=precision); o = emo.Oracle(p)
+        g.em_set_temperature_rise(th0); o.set_temperature_rise(th0)
+        assert rel_l2([g.em_get_temperature_rise()], [th0]) <= (0 if precision == 64 else 1e-7)
+        g.em_step(30); o.step(30)
+        to = o.temperature_rise()
+        assert np.linalg.norm(to - th0) > 1e-3 * np.linalg.norm(th0)
+        assert rel_l2([g.em_get_temperature_rise()], [to]) <= TOL[precision]
+        g.em_reset()
+        assert not np.any(g.em_get_temperature_rise())
+        g.close(); o.close()
+
+
+def test_coupled_config4_scaled():
+    """the package layout with the handbook-order thermal table as it stands (no exaggeration): tiny temperature
+    rises, the coupled path must still match to tolerance"""
+    p = W.make_config(4, scale=16, zscale=4, steps=80)
+    p.thermal = W.thermal_table()
+    for precision in (64, 32):
+        _run(p, 80, precision)
+
+
+def test_thermal_needs_flag_and_split_strategy():
+    p = W.random_problem(6, 5, 4, seed=8103, n_ports=0)
+    g = P.EM(p)
+    with pytest.raises(P.EMError):
+        g.em_set_thermal(W.thermal_table())                   # created with em_grid.thermal = 0
+    with pytest.raises(P.EMError):
+        g.em_get_temperature_rise()
+    g.close()
+    p.thermal = W.thermal_table()
+    with pytest.raises(P.EMError):
+        P.EM(p, kernel=P.EM_KERNEL_TMA)                       # the sweeps take sigma from the table
