@@ -38,6 +38,8 @@ def parse():
     ap.add_argument("--kernel", default="auto", choices=["auto", "split", "fused", "tma"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--thermal", action="store_true",
+                    help="two-way EM-thermal coupling (PAPER.md eq. (4)-(6)) with the handbook-order thermal table")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     return ap.parse_args()
 
@@ -108,9 +110,10 @@ def make_problem(args):
         kw["steps"] = max(args.steps + args.warmup, 1000) if args.scale == 1 else args.steps + args.warmup
     elif args.config in (2, 3, 6):
         kw["steps"] = args.steps + args.warmup
-    if args.config == 1:
-        return W.make_config(1)
-    return W.make_config(args.config, scale=args.scale, **kw)
+    p = W.make_config(1) if args.config == 1 else W.make_config(args.config, scale=args.scale, **kw)
+    if getattr(args, "thermal", False):
+        p.thermal = W.thermal_table(p.table.shape[0])
+    return p
 
 
 # ------------------------------------------------------------------------------------------------
@@ -279,8 +282,18 @@ def run_b200(args):
 
     peak, peak_src = measured_peak()
     bmin = B_MIN[precision]
+    if args.thermal:                 # + theta read/write + sigma(T) read/write per cell-update
+        bmin += 4 * (precision // 8)
     avg_ms = kms / max(klaunch, 1)
     achieved = bmin * cells / (avg_ms * 1e-3) / 1e9 if klaunch else None
+    if kname.startswith("k_split"):
+        # split strategy (and the thermal coupling that runs on it): the step is several kernels, each moving only
+        # part of B_min, so the honest roofline figure is the whole step's, not one kernel's
+        step_ms = ms / K
+        achieved = bmin * cells / (step_ms * 1e-3) / 1e9
+        avg_ms = step_ms
+        kname = "split step: k_split_h + %s + %s" % ("k_split_e_sig" if args.thermal else "k_split_e",
+                                                     "k_joule_thermal" if args.thermal else "k_split_joule")
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak if achieved else None, "traffic": ncu_traffic(kname, cells),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bmin * cells,
@@ -299,7 +312,8 @@ def run_b200(args):
         "config": {"workload": "config %d: %s %dx%dx%d cells (%d), %d ports, %s loss, Joule map every %s steps"
                                % (args.config, p.name, p.nx, p.ny, p.nz, cells, p.n_ports,
                                   "EXP" if p.loss_mode else "CD", je or "-")
-                               + (", walls -x+x-y+y-z+z = %s (1 = PMC)" % "".join(str(int(b)) for b in p.bc) if any(p.bc) else ""),
+                               + (", walls -x+x-y+y-z+z = %s (1 = PMC)" % "".join(str(int(b)) for b in p.bc) if any(p.bc) else "")
+                               + (", two-way thermal coupling (split kernels)" if args.thermal else ""),
                    "kernel_strategy": args.kernel, "l2": "state %.1f GB >> 126 MB L2 (no flush needed)" % (em.workspace_bytes / 1e9)
                    if em.workspace_bytes > 1e9 else "state fits L2: %.0f MB" % (em.workspace_bytes / 1e6),
                    "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},
