@@ -38,6 +38,9 @@ def parse():
     ap.add_argument("--kernel", default="auto", choices=["auto", "split", "fused", "tma"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: independent replicas (default, weak scaling) or ONE problem cut into z slabs with a "
+                         "two-plane halo exchange per step over NCCL (strong scaling; paper_2603_07038_b200/slabs.py)")
     ap.add_argument("--thermal", action="store_true",
                     help="two-way EM-thermal coupling (PAPER.md eq. (4)-(6)) with the handbook-order thermal table")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -195,7 +198,15 @@ def run_b200(args):
     precision = args.precision or p.precision
     kernel = {"auto": P.EM_KERNEL_AUTO, "split": P.EM_KERNEL_SPLIT, "fused": P.EM_KERNEL_FUSED, "tma": P.EM_KERNEL_TMA}[args.kernel]
     K, Wm = args.steps, args.warmup
+    slab = None
+    p_global = p
+    if args.decomp == "slabs" and world > 1:
+        from paper_2603_07038_b200 import slabs
+        p, meta = slabs.sub_problem(p_global, rank, world)       # this rank's extended slab (PMC on the artificial walls)
     em = P.EM(p, precision=precision, kernel=kernel, device=dev)
+    if args.decomp == "slabs" and world > 1:
+        slab = slabs.SlabRank(em, meta)
+        args.no_e2e = True                                       # the end-to-end leg is defined for whole problems
     cells = p.n_cells
     je = p.joule_every if p.joule_every else 0
     pw_map = torch.empty((p.nz, p.ny, p.nx), dtype=em.dtype, device=dev) if je else None
@@ -214,7 +225,13 @@ def run_b200(args):
             if je:
                 to_out = je - ((start + done) % je)
                 nxt = min(nxt, to_out)
-            em.em_step(nxt); done += nxt
+            if slab is None:
+                em.em_step(nxt)
+            else:                                                # one halo exchange after every step
+                for _ in range(nxt):
+                    em.em_step(1)
+                    slabs.exchange_dist(slab, dist)
+            done += nxt
             if je and (start + done) % je == 0:
                 em.em_joule(pw_map, q_map, total=False)
 
@@ -235,7 +252,12 @@ def run_b200(args):
     kname, klaunch, kms = em.em_timing_read()
     em.em_timing_enable(False)
     ms = max_over_ranks(ms, dist, dev)
-    value = aggregate_throughput(cells * K, ms * 1e-3, world)
+    kcells = p.n_cells
+    if slab is None:
+        value = aggregate_throughput(cells * K, ms * 1e-3, world)
+    else:                                                        # one problem over all ranks: its own cells / max time
+        cells = p_global.n_cells
+        value = aggregate_throughput(cells * K, ms * 1e-3, 1)
 
     # ---- end to end through the C ABI with host buffers -------------------------------------------
     e2e = None
@@ -285,18 +307,18 @@ def run_b200(args):
     if args.thermal:                 # + theta read/write + sigma(T) read/write per cell-update
         bmin += 4 * (precision // 8)
     avg_ms = kms / max(klaunch, 1)
-    achieved = bmin * cells / (avg_ms * 1e-3) / 1e9 if klaunch else None
+    achieved = bmin * kcells / (avg_ms * 1e-3) / 1e9 if klaunch else None
     if kname.startswith("k_split"):
         # split strategy (and the thermal coupling that runs on it): the step is several kernels, each moving only
         # part of B_min, so the honest roofline figure is the whole step's, not one kernel's
         step_ms = ms / K
-        achieved = bmin * cells / (step_ms * 1e-3) / 1e9
+        achieved = bmin * kcells / (step_ms * 1e-3) / 1e9
         avg_ms = step_ms
         kname = "split step: k_split_h + %s + %s" % ("k_split_e_sig" if args.thermal else "k_split_e",
                                                      "k_joule_thermal" if args.thermal else "k_split_joule")
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak if achieved else None, "traffic": ncu_traffic(kname, cells),
-                "peak_source": peak_src, "algorithmic_bytes_per_launch": bmin * cells,
+                "frac": achieved / peak if achieved else None, "traffic": ncu_traffic(kname, kcells),
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": bmin * kcells,
                 "avg_launch_ms": avg_ms, "launches_timed": klaunch,
                 "step_effective_GBps": bmin * value / world / 1e9, "step_frac_of_peak": bmin * value / world / 1e9 / peak,
                 "frac_of_8TBps_nominal": (achieved / 8000.0) if achieved else None}
@@ -307,16 +329,18 @@ def run_b200(args):
                "ms_per_step_on_sample": ms_cpu}
     line = {
         "metric": "EM cell-updates/sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
-        "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+        "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True,
+        "scaling": "strong" if slab is not None else "weak",
         "vs_baseline": None, "dtype": "f32" if precision == 32 else "f64", "data": "synthetic",
         "config": {"workload": "config %d: %s %dx%dx%d cells (%d), %d ports, %s loss, Joule map every %s steps"
-                               % (args.config, p.name, p.nx, p.ny, p.nz, cells, p.n_ports,
+                               % (args.config, p_global.name, p_global.nx, p_global.ny, p_global.nz, cells, p_global.n_ports,
                                   "EXP" if p.loss_mode else "CD", je or "-")
                                + (", walls -x+x-y+y-z+z = %s (1 = PMC)" % "".join(str(int(b)) for b in p.bc) if any(p.bc) else "")
                                + (", two-way thermal coupling (split kernels)" if args.thermal else ""),
                    "kernel_strategy": args.kernel, "l2": "state %.1f GB >> 126 MB L2 (no flush needed)" % (em.workspace_bytes / 1e9)
                    if em.workspace_bytes > 1e9 else "state fits L2: %.0f MB" % (em.workspace_bytes / 1e6),
-                   "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},
+                   "parallelism": ("z-slabs x%d, 2-plane halo exchange per step" % world if slab is not None else
+                                   "replicas x%d" % world) if world > 1 else "single GPU"},
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
         "clocks": sampler.summary(),
     }

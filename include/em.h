@@ -132,6 +132,13 @@ int32_t em_set_source(em_ctx *ctx, int32_t n_ports, const em_port *ports, const 
 int32_t em_set_field(em_ctx *ctx, int32_t comp, const void *src, int32_t src_is_device);
 int32_t em_get_field(em_ctx *ctx, int32_t comp, void *dst, int32_t dst_is_device);
 
+/* One z plane k of a component (dense [sy][sx] of that component's logical shape, working precision) out of / into
+ * the context: the halo exchange of a z-slab decomposition (paper_2603_07038_b200/slabs.py), where the
+ * artificial slab walls are PMC walls whose tangential E is refreshed from the neighbouring slab after every step.
+ * Errors: INVALID_ARG (component, k out of range, null), CUDA.  Host transfers synchronise the stream. */
+int32_t em_get_plane(em_ctx *ctx, int32_t comp, int32_t k, void *dst, int32_t dst_is_device);
+int32_t em_set_plane(em_ctx *ctx, int32_t comp, int32_t k, const void *src, int32_t src_is_device);
+
 /* Advance n >= 0 steps (n = 0 is a no-op).  Per step: H^{n+1/2} = H^{n-1/2} - dt nu (C_e E^n);
  * E^{n+1} = ca E^n + cb (C_h H^{n+1/2} - J^{n+1/2}) on non-fixed edges; Joule energy density
  * q_c += dt sigma_c 1/4 sum over the 12 edges of c of ((E^{n+1} + E^n)/2)^2.  Asynchronous. */

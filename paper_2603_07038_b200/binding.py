@@ -83,6 +83,8 @@ def load():
     L.em_set_source.argtypes = [vp, i32, C.POINTER(em_port), C.POINTER(em_edge), i64, C.POINTER(C.c_double), i64]
     L.em_set_field.argtypes = [vp, i32, vp, i32]
     L.em_get_field.argtypes = [vp, i32, vp, i32]
+    L.em_get_plane.argtypes = [vp, i32, i32, vp, i32]
+    L.em_set_plane.argtypes = [vp, i32, i32, vp, i32]
     L.em_step.argtypes = [vp, i64]
     L.em_joule.argtypes = [vp, vp, vp, C.POINTER(C.c_double), i32]
     L.em_probe.argtypes = [vp, i32, C.POINTER(em_probe_pt), C.POINTER(C.c_double)]
@@ -262,6 +264,17 @@ class EM:
 
     def fields(self):
         return [self.em_get_field(c) for c in range(6)]
+
+    def em_get_plane(self, comp: int, k: int, out=None):
+        """device tensor [sy][sx] holding plane k of component comp"""
+        sh = self.shapes[comp][1:]
+        t = out if out is not None else self._torch.empty(sh, dtype=self.dtype, device=self.device)
+        _check(self._L.em_get_plane(self._h, comp, int(k), C.c_void_p(t.data_ptr()), 1))
+        return t
+
+    def em_set_plane(self, comp: int, k: int, t):
+        assert tuple(t.shape) == tuple(self.shapes[comp][1:]) and t.dtype == self.dtype and t.is_contiguous()
+        _check(self._L.em_set_plane(self._h, comp, int(k), C.c_void_p(t.data_ptr()), 1 if t.is_cuda else 0))
 
     # thermal coupling (PAPER.md eq. (4)-(6)); the context must come from a problem with p.thermal set
     def em_set_thermal(self, thermal):

@@ -42,12 +42,12 @@ __global__ void __launch_bounds__(256) k_pad_pmc(uint8_t *base, int nx, int ny, 
 
 // Zero E[comp] wherever the edge is PEC-fixed (mask product of its 4 cells is 0).
 template <typename R>
-__global__ void __launch_bounds__(256) k_mask_fixed(DevParams<R> p, int comp) {
+__global__ void __launch_bounds__(256) k_mask_fixed(DevParams<R> p, int comp, int k0) {
     __shared__ MatEntry<R> s_tab[kMaxTable];
     load_table(s_tab, p);
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k = blockIdx.z;
+    const int k = blockIdx.z + k0;
     if (i > p.nx || j > p.ny) return;
     const long long PX = p.PX, PXY = p.PXY;
     const long long o = ((long long)k * p.PY + j) * PX + i;

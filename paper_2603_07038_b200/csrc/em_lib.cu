@@ -137,6 +137,7 @@ struct em_ctx {
     virtual int32_t set_source(int32_t, const em_port *, const em_edge *, int64_t, const double *, int64_t) = 0;
     virtual int32_t set_field(int32_t, const void *, int32_t) = 0;
     virtual int32_t get_field(int32_t, void *, int32_t) = 0;
+    virtual int32_t plane(int32_t comp, int32_t k, void *dst, const void *src, int32_t is_dev) = 0;
     virtual int32_t step(int64_t) = 0;
     virtual int32_t joule(void *, void *, double *, int32_t) = 0;
     virtual int32_t probe(int32_t, const em_probe_pt *, double *) = 0;
@@ -196,6 +197,7 @@ struct Ctx final : em_ctx {
     int32_t set_source(int32_t, const em_port *, const em_edge *, int64_t, const double *, int64_t) override;
     int32_t set_field(int32_t, const void *, int32_t) override;
     int32_t get_field(int32_t, void *, int32_t) override;
+    int32_t plane(int32_t comp, int32_t k, void *dst, const void *src, int32_t is_dev) override;
     int32_t step(int64_t) override;
     int32_t joule(void *, void *, double *, int32_t) override;
     int32_t probe(int32_t, const em_probe_pt *, double *) override;
@@ -562,8 +564,33 @@ int32_t Ctx<R>::set_field(int32_t comp, const void *srcp, int32_t is_dev) {
     CU(cudaMemcpy3DAsync(&m, stream));
     if (comp < 3) {
         dim3 b(32, 8);
-        em::k_mask_fixed<R><<<node_grid(b, 1), b, 0, stream>>>(p, comp);
+        em::k_mask_fixed<R><<<node_grid(b, 1), b, 0, stream>>>(p, comp, 0);
         CU(cudaGetLastError());
+    }
+    if (!is_dev) CU(cudaStreamSynchronize(stream));
+    return EM_OK;
+}
+
+// One z plane of a component out (dst) or in (src): the halo exchange of a z-slab decomposition.
+template <typename R>
+int32_t Ctx<R>::plane(int32_t comp, int32_t k, void *dst, const void *srcp, int32_t is_dev) {
+    if (comp < 0 || comp > 5) return fail(EM_ERR_INVALID_ARG, "plane: bad component");
+    int sx, sy, sz; comp_dims(comp, &sx, &sy, &sz);
+    if (k < 0 || k >= sz) return fail(EM_ERR_INVALID_ARG, "plane: k out of range");
+    R *base = comp_ptr(comp) + (long long)k * g.PXY;
+    const size_t wbytes = sizeof(R) * sx;
+    if (dst) {
+        CU(cudaMemcpy2DAsync(dst, wbytes, base, sizeof(R) * g.PX, wbytes, sy,
+                             is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, stream));
+    } else {
+        CU(cudaMemcpy2DAsync(base, sizeof(R) * g.PX, srcp, wbytes, wbytes, sy,
+                             is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, stream));
+        if (comp < 3) {                                   // PEC-fixed edges of this plane stay 0
+            dim3 b(32, 8);
+            dim3 gr((g.nx + 1 + b.x - 1) / b.x, (g.ny + 1 + b.y - 1) / b.y, 1);
+            em::k_mask_fixed<R><<<gr, b, 0, stream>>>(p, comp, k);
+            CU(cudaGetLastError());
+        }
     }
     if (!is_dev) CU(cudaStreamSynchronize(stream));
     return EM_OK;
@@ -885,6 +912,12 @@ int32_t em_set_source(em_ctx *ctx, int32_t n_ports, const em_port *ports, const 
 }
 int32_t em_set_field(em_ctx *ctx, int32_t comp, const void *src, int32_t is_dev) { EM_CHECK_CTX; return ctx->set_field(comp, src, is_dev); }
 int32_t em_get_field(em_ctx *ctx, int32_t comp, void *dst, int32_t is_dev) { EM_CHECK_CTX; return ctx->get_field(comp, dst, is_dev); }
+int32_t em_get_plane(em_ctx *ctx, int32_t comp, int32_t k, void *dst, int32_t is_dev) {
+    EM_CHECK_CTX; if (!dst) return fail(EM_ERR_INVALID_ARG, "null"); return ctx->plane(comp, k, dst, nullptr, is_dev);
+}
+int32_t em_set_plane(em_ctx *ctx, int32_t comp, int32_t k, const void *src, int32_t is_dev) {
+    EM_CHECK_CTX; if (!src) return fail(EM_ERR_INVALID_ARG, "null"); return ctx->plane(comp, k, nullptr, src, is_dev);
+}
 int32_t em_step(em_ctx *ctx, int64_t n) { EM_CHECK_CTX; return ctx->step(n); }
 int32_t em_joule(em_ctx *ctx, void *p, void *q, double *t, int32_t reset) { EM_CHECK_CTX; return ctx->joule(p, q, t, reset); }
 int32_t em_probe(em_ctx *ctx, int32_t n, const em_probe_pt *pts, double *out) { EM_CHECK_CTX; return ctx->probe(n, pts, out); }
