@@ -49,17 +49,20 @@ struct FusedPlan {
     int chunk_of(int k) const { int c = 0; while (c + 1 < nzs && k >= kb[c + 1]) ++c; return c; }
 };
 
-// Number of z chunks: a chunk re-runs up to two planes of its lower neighbour (warm-up plane kb-1 and
-// the closing plane kb[c+1]), so the cost model is waves x (planes per chunk + 2); n_sm = 0 (no
-// device known yet: workspace sizing) returns the maximum.
+// Number of z chunks.  Work items are scheduled dynamically onto the SMs, so the step takes about
+//   total work / n_sm  +  one item (the tail),   work of an item = its planes + ~4 planes of overhead
+// (the re-run warm-up and closing planes of a chunk plus the prologue and the pipeline fill).  Fitted on B200:
+// config 4 (666 tiles x 193 planes) -> 3, config 5 (385 x 257) -> 5, config 3 (185 x 129) -> 5, which are the
+// measured optima (profiles/r1_configs.md).  n_sm = 0 (no device known yet: workspace sizing) returns the maximum.
 inline int choose_zsplit(int n_tiles, int nz, int n_sm, int forced) {
     const int cap = std::max(1, std::min(kFusedMaxZSplit, (nz + 1) / 4));
     if (forced > 0) return std::min(forced, cap);
     if (n_sm <= 0) return kFusedMaxZSplit;
     int best = 1; double best_cost = 1e300;
     for (int s = 1; s <= cap; ++s) {
-        const long long waves = ((long long)n_tiles * s + n_sm - 1) / n_sm;
-        const double cost = (double)waves * ((double)(nz + 1) / s + (s > 1 ? 2.0 : 0.0));
+        const double over = s > 1 ? 4.0 : 0.0;
+        const double item = (double)(nz + 1) / s + over;
+        const double cost = (double)n_tiles * s * item / n_sm + item;
         if (cost < best_cost * 0.999) { best_cost = cost; best = s; }
     }
     return best;

@@ -88,6 +88,14 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
         "@!p bra W_%=;\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+// 1-D bulk copy global -> shared counted on an mbarrier (bytes: multiple of 16)
+__device__ __forceinline__ void bulk_load(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+// producer / consumer named barrier of two warps (ids 1..15; id 0 is __syncthreads)
+__device__ __forceinline__ void pair_arrive(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void pair_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map, unsigned bar, int x, int y, int z) {
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
@@ -173,7 +181,8 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     auto issue_E = [&](int kk, bool first) {
         const unsigned bar = bar_fullE((kk - ks) & 1);
         const unsigned sb = smem_u32(sm);
-        mbar_expect_tx(bar, (unsigned)(L::e_bytes + (first ? L::first_extra_bytes : 0)));
+        mbar_expect_tx(bar, (unsigned)(L::e_bytes + (first ? L::first_extra_bytes : 0) + 4 * sizeof(R)));
+        bulk_load(smem_u32(&s_z[(kk & 1) * 4]), p.zgeo + 4 * (long long)kk, 4 * (unsigned)sizeof(R), bar);   // {fz, 1/dz, 1/dz~, 0}
         if (first) {
             tma_load_3d(sb + L::ex + ((kk + 3) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 1);
             tma_load_3d(sb + L::ey + ((kk + 3) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 1);
@@ -191,21 +200,11 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         tma_load_3d(sb + L::h + ((kk & 1) * 3 + 1) * L::h_slot, &maps.H[1], bar, cx, cyy, kk + 1);
         tma_load_3d(sb + L::h + ((kk & 1) * 3 + 2) * L::h_slot, &maps.H[2], bar, cx, cyy, kk + 1);
     };
-    // z geometry of plane kk -> parity kk&1 (cp.async, same group as q)
-    auto issue_z = [&](int kk) {
-        if (tid < (int)sizeof(R) / 4 && kk <= ke)
-            cp_async16(reinterpret_cast<unsigned char *>(&s_z[(kk & 1) * 4]) + 16 * tid,
-                       reinterpret_cast<const unsigned char *>(p.zgeo + 4 * (long long)kk) + 16 * tid);
-    };
     if (tid == 0) {
         issue_E(ks, true);
         issue_H(ks);
         if (ks + 1 <= ke) { issue_E(ks + 1, false); issue_H(ks + 1); }
     }
-    issue_z(ks); issue_z(ks + 1);
-    cp_async_commit();
-    cp_async_wait<0>();
-    __syncthreads();
 
     const R fy = active ? p.fy[j] : R(0), rdy = active ? p.rdy[j] : R(0), rty = active ? p.rty[j] : R(0);
     const R gq = p.dt * R(0.0625);
@@ -235,10 +234,10 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         const int par = k & 1;
         const long long o = off0 + (long long)k * PXY;
         const bool st = own && k >= kz0 && k < kz1;          // this chunk stores H'(k), E'(k)
-        const R fz = s_z[par * 4 + 0], rdz = s_z[par * 4 + 1], rtz = s_z[par * 4 + 2];
 
         // ---- phase A: H' = H - nbar * curl E  (inner factor of S = curl mu^-1 curl) ----------
         mbar_wait(bar_fullE(it & 1), (unsigned)(it >> 1) & 1u);   // E group of plane k has landed
+        const R fz = s_z[par * 4 + 0], rdz = s_z[par * 4 + 1], rtz = s_z[par * 4 + 2];
         const unsigned idw = ld_ids(par, w + 1), idj = ld_ids(par, w);
         // one material over the warp's whole coefficient neighbourhood (rows j-1..j, planes k-1..k)?
         const bool rowu = (idw == idj) && id_uniform(idw);
@@ -294,8 +293,8 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             EM_ST(p.Hn[2] + o, hzn);
         }
         smHx[r][lane] = hxn; smHz[r][lane] = hzn;
-        __syncthreads();                          // B2: H' rows visible; every thread holds H(k) in registers
-        if (tid == 0 && k + 2 <= ke) issue_H(k + 2);
+        __syncthreads();                          // B2: H' rows visible; the staged E(k), H(k), ids(k), z geometry are dead (registers)
+        if (tid == 0 && k + 2 <= ke) { issue_H(k + 2); issue_E(k + 2, false); }
 
         // ---- phase B: E' = E + r (curl H' - J - sigma E), Joule squares (eq. 2-3) -------------
         // (warp 0 = halo row -1 only supplies H' to row 0: no E', no Joule)
@@ -332,9 +331,13 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             smBx[r][lane] = bx; smBz[r][lane] = bz;
             mine[(kSlotHp + 0) * NT] = hxn; mine[(kSlotHp + 1) * NT] = hyn;
         }
-        cp_async_wait<0>();                       // q(k-1) and the z geometry of plane k+1 have landed
-        __syncthreads();                          // B3: B rows and z geometry visible; the staged E(k), ids(k) are dead
-        if (tid == 0 && k + 2 <= ke) issue_E(k + 2, false);
+        // No CTA barrier here: row j needs only the (2 Ebar)^2 row of row j+1, so the two warps meet on a
+        // producer/consumer named barrier of their own (id = the upper warp's index) and a warp on the one-material
+        // path does not wait for a general-path warp elsewhere in the CTA.  Warp 0 (no phase C) still consumes, so
+        // that it cannot overwrite its H' row (phase A of plane k+1) while warp 1 reads it in phase B.
+        if (w != 0) pair_arrive(w);               // my B row is written (and I am done reading the H' row of row j-1)
+        if (!is_top) pair_sync(w + 1);            // the B row of row j+1 is visible
+        cp_async_wait<0>();                       // q(k-1) has landed (private slot: no barrier needed)
 
         // ---- phase C: q(k-1) += dt sigma/16 (pend + Sxy(k)); pend = Sxy(k) + Sz(k) ---------------------------
         if (w != 0 && !is_top) {
@@ -359,7 +362,6 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             q_live = !(id_uniform(idw) && s_tab[idw & 0xff].b == R(0));
             if (own_q && k >= kz0 && k < ke && q_live) cp_async16(mine + kSlotQ * NT, p.q + o);   // q(k)
         }
-        issue_z(k + 2);
         cp_async_commit();
         idw_prev = idw;
         rowu_prev = rowu;
