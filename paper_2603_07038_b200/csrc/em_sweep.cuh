@@ -56,8 +56,8 @@ template <int SZ> struct SweepLayout {
     static constexpr int rows = priv + kSwPriv * kSwWarps * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kFusedRows][32]
     static constexpr int geo = rows + 4 * kFusedRows * kSwRow;    // 1/dx, 1/dx~, fx of the 32 lanes
     static constexpr int zg = geo + 3 * kSwRow;                   // [2 parity]{fz, 1/dz, 1/dz~, 0}
-    static constexpr int bar = zg + 64;                           // fullE[2], fullH[2]
-    static constexpr int tab = bar + 64;                          // material table (n_table entries)
+    static constexpr int bar = zg + 64;                           // fullE[2], fullH[2], empty[2], rowH[kSwWarps]
+    static constexpr int tab = bar + 64 + 8 * kSwWarps;                          // material table (n_table entries)
     static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + (kSwWarps + 2) * id_row;
     static constexpr int first_extra_bytes = ex_slot + ey_slot;
     static constexpr int h_bytes = 3 * h_slot;
@@ -150,10 +150,14 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     const unsigned bar0 = smem_u32(sm + L::bar);
     auto bar_fullE = [&](int s) -> unsigned { return bar0 + 8 * s; };
     auto bar_fullH = [&](int s) -> unsigned { return bar0 + 16 + 8 * s; };
+    auto bar_empty = [&](int s) -> unsigned { return bar0 + 32 + 8 * s; };     // every warp has consumed the staged plane
+    auto bar_rowH = [&](int ww) -> unsigned { return bar0 + 64 + 8 * ww; };    // H'(k) row of warp ww is published
 
     // ---- prologue: barriers, table, x geometry, zeroed exchange rows and private slots -------------------
     if (tid == 0) {
         mbar_init(bar_fullE(0), 1); mbar_init(bar_fullE(1), 1); mbar_init(bar_fullH(0), 1); mbar_init(bar_fullH(1), 1);
+        mbar_init(bar_empty(0), kSwWarps); mbar_init(bar_empty(1), kSwWarps);
+        for (int ww = 0; ww < kSwWarps; ++ww) mbar_init(bar_rowH(ww), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int t = tid; t < p.n_table; t += NT) s_tab[t] = p.table[t];
@@ -293,8 +297,16 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             EM_ST(p.Hn[2] + o, hzn);
         }
         smHx[r][lane] = hxn; smHz[r][lane] = hzn;
-        __syncthreads();                          // B2: H' rows visible; the staged E(k), H(k), ids(k), z geometry are dead (registers)
-        if (tid == 0 && k + 2 <= ke) { issue_H(k + 2); issue_E(k + 2, false); }
+        // No CTA barrier in the plane loop.  Row j+1 waits only for THIS row's H' (mbarrier rowH), and the producer
+        // thread refills the staged slots once every warp has pulled plane k into registers (mbarrier empty).
+        // WAR on the exchange rows is ordered by the chain  B(k) of row j+1 done -> pair barrier -> C(k), A(k+1) of row j.
+        __syncwarp();
+        if (lane == 0) { mbar_arrive(bar_rowH(w)); mbar_arrive(bar_empty(it & 1)); }
+        if (tid == 0 && k + 2 <= ke) {
+            mbar_wait(bar_empty(it & 1), (unsigned)(it >> 1) & 1u);
+            issue_H(k + 2); issue_E(k + 2, false);
+        }
+        if (w != 0) mbar_wait(bar_rowH(w - 1), (unsigned)it & 1u);   // H'(k) of row j-1 is visible
 
         // ---- phase B: E' = E + r (curl H' - J - sigma E), Joule squares (eq. 2-3) -------------
         // (warp 0 = halo row -1 only supplies H' to row 0: no E', no Joule)
