@@ -82,6 +82,33 @@ def test_fused_z_chunks(zsplit, monkeypatch):
     run_pair(p, 30, 64, P.EM_KERNEL_FUSED, checkpoints=(1, 7))
 
 
+@pytest.mark.parametrize("zsplit", [1, 2, 3, 5, 8])
+def test_tma_sweep_z_chunks(zsplit, monkeypatch):
+    monkeypatch.setenv("EM_FUSED_ZSPLIT", str(zsplit))
+    p = W.random_problem(21, 18, 33, seed=78, loss_mode=LOSS_CD, steps=30, n_ports=60, bc=(0, 0, 1, 0, 1, 1))
+    run_pair(p, 30, 64, P.EM_KERNEL_TMA, checkpoints=(1, 7))
+
+
+def test_tma_sweep_is_deterministic_across_runs_and_chunkings(monkeypatch):
+    """The TMA sweep has no CTA barrier in its plane loop (mbarrier / named-barrier hand-offs between rows): a missing
+    ordering would show up as run-to-run or chunking-dependent bits.  256 x 256 x 192 package slice, 228 work items
+    and more, 40 steps, fp32: every run must give IDENTICAL bits."""
+    p = W.make_config(4, scale=4, steps=40)
+    ref = None
+    for zsplit in ("3", "3", "1", "8", "3"):
+        monkeypatch.setenv("EM_FUSED_ZSPLIT", zsplit)
+        g = P.EM(p, precision=32, kernel=P.EM_KERNEL_TMA)
+        g.em_step(40)
+        out = [g.em_get_field(c) for c in range(6)] + [g.joule_maps()[1]]
+        g.close()
+        if ref is None:
+            ref = out
+            assert all(np.isfinite(a).all() for a in out) and np.abs(out[0]).max() > 0
+        else:
+            for a, b in zip(out, ref):
+                assert np.array_equal(a, b), zsplit
+
+
 @pytest.mark.parametrize("kernel", KERNELS)
 @pytest.mark.parametrize("precision", [64, 32])
 @pytest.mark.parametrize("dims", [(37, 29, 23), (9, 4, 70)])
