@@ -92,9 +92,11 @@ __global__ void k_source_coef_sig(DevParams<R> p, DevSources<R> s, const R *sig)
     s.r[u] = r[s.comp[u]];
 }
 
-// series conductance per unit face area of the two half cells: k_f / l~_f = 2 / (d_a/k_a + d_b/k_b); 0 if either is 0
-template <typename R> __device__ __forceinline__ R half_cell_cond(R rda, R ka, R rdb, R kb) {
-    return (ka > R(0) && kb > R(0)) ? R(2) / (R(1) / (rda * ka) + R(1) / (rdb * kb)) : R(0);
+// series conductance per unit face area of the two half cells: k_f / l~_f = 2 / (d_a/k_a + d_b/k_b) = 2 g_a g_b / (g_a + g_b)
+// with the half-cell conductances g = k/d; 0 if either cell does not conduct (k = 0, or a pad cell: 1/d = 0)
+template <typename R> __device__ __forceinline__ R half_cell_cond(R ga, R gb) {
+    const R den = ga + gb;
+    return den > R(0) ? R(2) * ga * gb * rcp<R>(den) : R(0);
 }
 
 // a4 + eq. (5) + eq. (6): Joule heat of the step into q and into the cell's temperature rise, conduction to the six
@@ -128,16 +130,17 @@ __global__ void __launch_bounds__(256) k_joule_thermal(DevParams<R> p, ThermalPa
     }
     const R th = t.theta[o];
     const R rdx = p.rdx[i], rdy = p.rdy[j], rdz = p.rdz[k];
+    const R gx = rdx * me.k, gy = rdy * me.k, gz = rdz * me.k;     // own half-cell conductances k/d
     R lap = R(0);                                        // (M_kk theta)_c
-    lap = mad(rdx, half_cell_cond(rdx, me.k, p.rdx[i - 1], s_th[p.mat[o - 1]].k) * (th - t.theta[o - 1]), lap);
-    lap = mad(rdx, half_cell_cond(rdx, me.k, p.rdx[i + 1], s_th[p.mat[o + 1]].k) * (th - t.theta[o + 1]), lap);
-    lap = mad(rdy, half_cell_cond(rdy, me.k, p.rdy[j - 1], s_th[p.mat[o - PX]].k) * (th - t.theta[o - PX]), lap);
-    lap = mad(rdy, half_cell_cond(rdy, me.k, p.rdy[j + 1], s_th[p.mat[o + PX]].k) * (th - t.theta[o + PX]), lap);
-    lap = mad(rdz, half_cell_cond(rdz, me.k, p.rdz[k - 1], s_th[p.mat[o - PXY]].k) * (th - t.theta[o - PXY]), lap);
-    lap = mad(rdz, half_cell_cond(rdz, me.k, p.rdz[k + 1], s_th[p.mat[o + PXY]].k) * (th - t.theta[o + PXY]), lap);
+    lap = mad(rdx, half_cell_cond(gx, p.rdx[i - 1] * s_th[p.mat[o - 1]].k) * (th - t.theta[o - 1]), lap);
+    lap = mad(rdx, half_cell_cond(gx, p.rdx[i + 1] * s_th[p.mat[o + 1]].k) * (th - t.theta[o + 1]), lap);
+    lap = mad(rdy, half_cell_cond(gy, p.rdy[j - 1] * s_th[p.mat[o - PX]].k) * (th - t.theta[o - PX]), lap);
+    lap = mad(rdy, half_cell_cond(gy, p.rdy[j + 1] * s_th[p.mat[o + PX]].k) * (th - t.theta[o + PX]), lap);
+    lap = mad(rdz, half_cell_cond(gz, p.rdz[k - 1] * s_th[p.mat[o - PXY]].k) * (th - t.theta[o - PXY]), lap);
+    lap = mad(rdz, half_cell_cond(gz, p.rdz[k + 1] * s_th[p.mat[o + PXY]].k) * (th - t.theta[o + PXY]), lap);
     const R thn = th - p.dt * me.irc * lap + dq * me.irc;
     t.theta_n[o] = thn;
-    t.sig[o] = me.sigma0 / (R(1) + me.alpha * thn);
+    t.sig[o] = me.sigma0 * rcp<R>(R(1) + me.alpha * thn);
 }
 
 // sigma = sigma_0 / (1 + alpha theta) on every cell (after em_set_thermal / em_set_temperature_rise / em_reset)
