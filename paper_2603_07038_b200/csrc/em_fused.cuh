@@ -32,17 +32,26 @@ namespace em {
 #ifndef EM_FUSED_OCC
 #define EM_FUSED_OCC 1
 #endif
-constexpr int kFusedTY = EM_FUSED_TY;               // owned rows per tile (16 warps x 128 regs)
+#ifndef EM_FUSED_TY64
+#define EM_FUSED_TY64 10
+#endif
 constexpr int kFusedOcc = EM_FUSED_OCC;             // resident CTAs per SM
-constexpr int kFusedWarps = kFusedTY + 2;          // rows -1 .. TY
-constexpr int kFusedThreads = kFusedWarps * 32;    // 576
-constexpr int kFusedRows = kFusedTY + 4;           // exchange rows, r = cy + 2 (row 0 and last: dummies)
+// Tile rows per working precision.  fp32: 14 owned rows = 16 warps x 128 registers.  fp64 needs ~170 registers per
+// thread to stay spill-free (a spill is very expensive here: the 227 KB carve-out leaves almost no L1), so its tiles
+// own 10 rows = 12 warps (measured on config 3 fp64: 1.22 -> 0.87 ms/step).
+template <int SZ> struct Tile {
+    static constexpr int TY = SZ == 8 ? EM_FUSED_TY64 : EM_FUSED_TY;   // owned rows per tile
+    static constexpr int warps = TY + 2;                                // rows -1 .. TY
+    static constexpr int threads = warps * 32;
+    static constexpr int rows = TY + 4;                                 // exchange rows, r = cy + 2 (row 0 and last: dummies)
+};
+inline int tile_rows(int sizeof_real) { return sizeof_real == 8 ? Tile<8>::TY : Tile<4>::TY; }
 constexpr int kFusedSlots = 21;                    // private 16-B slots per thread (see enum below)
 
 constexpr int kFusedMaxZSplit = 8;                // z chunks per tile column (work items = tiles x chunks)
 
 struct FusedPlan {
-    int V, TXo, ntx, nty, n_tiles;
+    int V, TXo, TY, ntx, nty, n_tiles;
     int nzs;                         // z chunks; chunk c owns the planes kb[c] <= k < kb[c+1], kb[nzs] = nz+1
     int kb[kFusedMaxZSplit + 1];
     size_t smem_bytes;
@@ -73,7 +82,9 @@ inline FusedPlan make_fused_plan(int nx, int ny, int nz, int sizeof_real, int n_
     f.V = 16 / sizeof_real;
     f.TXo = 30 * f.V;
     f.ntx = (nx + 1 + f.TXo - 1) / f.TXo;
-    f.nty = (ny + 1 + kFusedTY - 1) / kFusedTY;
+    f.TY = tile_rows(sizeof_real);
+    const int kFusedRows = f.TY + 4, kFusedThreads = (f.TY + 2) * 32;
+    f.nty = (ny + 1 + f.TY - 1) / f.TY;
     f.n_tiles = f.ntx * f.nty;
     f.nzs = choose_zsplit(f.n_tiles, nz, n_sm * kFusedOcc, forced_zsplit);
     for (int c = 0; c <= kFusedMaxZSplit; ++c) f.kb[c] = nz + 1;
@@ -92,8 +103,8 @@ inline int tiles_of_node(const FusedPlan &f, int i, int j, int out[4]) {
     int txs[2], tys[2], nxs = 0, nys = 0;
     txs[nxs++] = i / f.TXo;
     if (i % f.TXo == 0 && i > 0) txs[nxs++] = i / f.TXo - 1;
-    tys[nys++] = j / kFusedTY;
-    if (j % kFusedTY == 0 && j > 0) tys[nys++] = j / kFusedTY - 1;
+    tys[nys++] = j / f.TY;
+    if (j % f.TY == 0 && j > 0) tys[nys++] = j / f.TY - 1;
     int n = 0;
     for (int a = 0; a < nys; ++a)
         for (int b = 0; b < nxs; ++b)
@@ -149,11 +160,12 @@ enum : int {
 };
 
 template <typename R, int LOSS, bool UMU>
-__global__ void __launch_bounds__(kFusedThreads, kFusedOcc)
+__global__ void __launch_bounds__(Tile<sizeof(R)>::threads, kFusedOcc)
 k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc, int ntx, long long step) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TXo = 30 * V;
-    constexpr int NT = kFusedThreads;
+    constexpr int kFusedTY = Tile<sizeof(R)>::TY, kFusedRows = Tile<sizeof(R)>::rows;
+    constexpr int NT = Tile<sizeof(R)>::threads;
     using VecR = Vec<R>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     MatEntry<R> *s_tab = reinterpret_cast<MatEntry<R> *>(smem_raw);
@@ -437,7 +449,7 @@ cudaError_t launch_fused(const FusedPlan &plan, const DevParams<R> &p, const Dev
         if (e != cudaSuccess) return e;
         for (auto &c : configured) if (!c) { c = (const void *)kern; break; }
     }
-    kern<<<plan.n_tiles * plan.nzs, kFusedThreads, plan.smem_bytes, stream>>>(p, src, fs, zc, plan.ntx, step);
+    kern<<<plan.n_tiles * plan.nzs, Tile<sizeof(R)>::threads, plan.smem_bytes, stream>>>(p, src, fs, zc, plan.ntx, step);
     return cudaGetLastError();
 }
 

@@ -427,13 +427,13 @@ int32_t Ctx<R>::make_maps() {
     const CUtensorMapDataType fdt = sizeof(R) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
     for (int a = 0; a < 12; ++a) {
         const int comp = a % 3, is_e = a < 6;
-        const int rows = (is_e && comp != 1) ? em::kSwWarps + 1 : em::kSwWarps;         // Ex, Ez carry row TY+1
+        const int rows = (is_e && comp != 1) ? em::Tile<sizeof(R)>::warps + 1 : em::Tile<sizeof(R)>::warps;         // Ex, Ez carry row TY+1
         int32_t rc = encode(&map_field[a], fdt, sizeof(R), c.field[a] + g.PX - V, 32 * V, rows);
         if (rc) return rc;
     }
-    int32_t rc = encode(&map_q, fdt, sizeof(R), c.q + g.PX - V, 30 * V, em::kSwTY);
+    int32_t rc = encode(&map_q, fdt, sizeof(R), c.q + g.PX - V, 30 * V, em::Tile<sizeof(R)>::TY);
     if (rc) return rc;
-    return encode(&map_mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, c.mat + g.PX - em::kSwIdShift, 32 * V + 16, em::kSwWarps + 2);
+    return encode(&map_mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, c.mat + g.PX - em::kSwIdShift, 32 * V + 16, em::Tile<sizeof(R)>::warps + 2);
 }
 
 // ---- sources ------------------------------------------------------------------------------------

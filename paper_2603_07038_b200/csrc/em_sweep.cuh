@@ -28,9 +28,6 @@ namespace em {
 #define EM_ST(ptr, val) st_stream16((ptr), (val))     // output planes: streaming stores
 #endif
 
-constexpr int kSwTY = kFusedTY;                    // 14 owned rows
-constexpr int kSwWarps = kSwTY + 2;                // rows -1 .. TY
-constexpr int kSwThreads = kSwWarps * 32;          // 512
 constexpr int kSwRow = 512;                        // bytes of one staged row (32 lanes x 16 B)
 constexpr int kSwIdShift = 16;                     // the id map starts 16 B before the row (16-B aligned base)
 constexpr int kSwPriv = 8;                         // private 16-B slots per thread: q, L x 4, H' x 2, pend
@@ -41,6 +38,7 @@ struct alignas(64) SweepMaps { CUtensorMap E[3], H[3], q, mat; };
 // because its size is only known at run time)
 template <int SZ> struct SweepLayout {
     static constexpr int V = 16 / SZ;
+    static constexpr int kSwWarps = Tile<SZ>::warps, kFusedRows = Tile<SZ>::rows;
     static constexpr int ex = 0;                                  // Ex ring of 3 planes, rows -1 .. TY+1
     static constexpr int ex_slot = (kSwWarps + 1) * kSwRow;
     static constexpr int ey = ex + 3 * ex_slot;                   // Ey ring of 3 planes, rows -1 .. TY
@@ -110,12 +108,13 @@ __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map
 
 // ---- the kernel ------------------------------------------------------------------------------------------
 template <typename R, int LOSS, bool UMU>
-__global__ void __launch_bounds__(kSwThreads, 1)
+__global__ void __launch_bounds__(Tile<sizeof(R)>::threads, 1)
 k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R> src, FusedSources fs,
             FusedChunks zc, int ntx, long long step) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TXo = 30 * V;
-    constexpr int NT = kSwThreads;
+    constexpr int kSwTY = Tile<sizeof(R)>::TY, kSwWarps = Tile<sizeof(R)>::warps, kFusedRows = Tile<sizeof(R)>::rows;
+    constexpr int NT = Tile<sizeof(R)>::threads;
     using L = SweepLayout<(int)sizeof(R)>;
     using VecR = Vec<R>;
     using IdT = typename std::conditional<V == 4, unsigned, unsigned short>::type;
@@ -401,7 +400,7 @@ cudaError_t launch_sweep_tma(const FusedPlan &plan, size_t smem_bytes, const Swe
     else           kern = uniform_mu ? (K)k_sweep_tma<R, 1, true> : (K)k_sweep_tma<R, 1, false>;
     cudaError_t e = cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
-    kern<<<plan.n_tiles * plan.nzs, kSwThreads, smem_bytes, stream>>>(maps, p, src, fs, zc, plan.ntx, step);
+    kern<<<plan.n_tiles * plan.nzs, Tile<sizeof(R)>::threads, smem_bytes, stream>>>(maps, p, src, fs, zc, plan.ntx, step);
     return cudaGetLastError();
 }
 
