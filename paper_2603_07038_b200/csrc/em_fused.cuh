@@ -301,11 +301,7 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
         // one material over the warp's whole coefficient neighbourhood (rows j-1..j, planes k-1..k)?
         const bool rowu = (idw == idj) && id_uniform(idw);
         const unsigned idw_lane0 = __shfl_sync(0xffffffffu, idw, 0);     // (not inside the && chain: every lane must execute it)
-#ifdef EM_EXP_NOHOM
-        const bool hom = false;
-#else
         const bool hom = __all_sync(0xffffffffu, rowu && rowu_prev && idw == idw_prev && idw == idw_lane0);
-#endif
         VecR hxn, hyn, hzn;
         const VecR ex0 = mine[(kSlotEx + rk) * NT], ey0 = mine[(kSlotEy + rk) * NT], ez = mine[(kSlotEz + par) * NT];
         {
@@ -415,11 +411,7 @@ k_fused_sweep(DevParams<R> p, DevSources<R> src, FusedSources fs, FusedChunks zc
             mine[kSlotPend * NT] = pend;
             // q of a lane whose V cells are one lossless material never changes: neither fetched nor stored
             if (own_q && k > kz0 && q_live) *reinterpret_cast<VecR *>(p.q + o - PXY) = qv;   // layer k-1 in [kz0, kz1)
-#ifdef EM_EXP_NOQSKIP
-            q_live = true;
-#else
             q_live = !(id_uniform(idw) && s_tab[idw & 0xff].b == R(0));
-#endif
             if (own_q && k >= kz0 && k < ke && q_live) cp_async16(mine + kSlotQ * NT, p.q + o);   // G_q(k)
         }
         cp_async_commit();

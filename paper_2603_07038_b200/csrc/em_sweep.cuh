@@ -22,11 +22,7 @@
 namespace em {
 
 #undef EM_ST
-#ifdef EM_EXP_NOSTCS
-#define EM_ST(ptr, val) (*reinterpret_cast<VecR *>(ptr) = (val))
-#else
-#define EM_ST(ptr, val) st_stream16((ptr), (val))     // output planes: streaming stores
-#endif
+#define EM_ST(ptr, val) st_stream16((ptr), (val))     // output planes: streaming (evict-first) stores
 
 constexpr int kSwRow = 512;                        // bytes of one staged row (32 lanes x 16 B)
 constexpr int kSwIdShift = 16;                     // the id map starts 16 B before the row (16-B aligned base)
