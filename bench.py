@@ -138,6 +138,11 @@ def cpu_oracle_rate(args, seconds: float):
             break
     rate = p.n_cells * n / el
     sample = "%s at %dx%dx%d cells (scale 1/%d in x,y), %d steps, fp64" % (p.name, p.nx, p.ny, p.nz, scale, n)
+    # the same oracle on ONE thread (2 steps), for the single-core figure SURVEY.md 8(d) asks for
+    emo.set_threads(1)
+    t1 = time.perf_counter(); o.step(2)
+    cpu_oracle_rate.single_thread = p.n_cells * 2 / (time.perf_counter() - t1)
+    emo.set_threads(threads)
     o.close()
     return rate, threads, sample, el / n * 1e3, p
 
@@ -308,14 +313,17 @@ def run_b200(args):
         bmin += 4 * (precision // 8)
     avg_ms = kms / max(klaunch, 1)
     achieved = bmin * kcells / (avg_ms * 1e-3) / 1e9 if klaunch else None
-    if kname.startswith("k_split"):
+    if kname.startswith("k_split") or args.thermal:
         # split strategy (and the thermal coupling that runs on it): the step is several kernels, each moving only
         # part of B_min, so the honest roofline figure is the whole step's, not one kernel's
         step_ms = ms / K
         achieved = bmin * kcells / (step_ms * 1e-3) / 1e9
         avg_ms = step_ms
-        kname = "split step: k_split_h + %s + %s" % ("k_split_e_sig" if args.thermal else "k_split_e",
-                                                     "k_joule_thermal" if args.thermal else "k_split_joule")
+        if kname.startswith("k_split"):
+            kname = "split step: k_split_h + %s + %s" % ("k_split_e_sig" if args.thermal else "k_split_e",
+                                                         "k_joule_thermal" if args.thermal else "k_split_joule")
+        else:
+            kname = "coupled step: k_diffuse + k_sweep_tma<TH> (sweep alone %.3f ms)" % (kms / max(klaunch, 1))
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak if achieved else None, "traffic": ncu_traffic(kname, kcells),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bmin * kcells,
@@ -326,6 +334,7 @@ def run_b200(args):
     if not args.no_cpu_baseline:
         rate, threads, sample, ms_cpu, _ = cpu_oracle_rate(args, args.cpu_seconds)
         cpu = {"value": rate, "unit": "cell-updates/s", "cores": threads, "kind": "oracle", "sample": sample,
+               "single_thread_value": getattr(cpu_oracle_rate, "single_thread", None),
                "ms_per_step_on_sample": ms_cpu}
     line = {
         "metric": "EM cell-updates/sec", "value": value, "unit": "cell-updates/s", "n_gpus": world,
@@ -336,7 +345,7 @@ def run_b200(args):
                                % (args.config, p_global.name, p_global.nx, p_global.ny, p_global.nz, cells, p_global.n_ports,
                                   "EXP" if p.loss_mode else "CD", je or "-")
                                + (", walls -x+x-y+y-z+z = %s (1 = PMC)" % "".join(str(int(b)) for b in p.bc) if any(p.bc) else "")
-                               + (", two-way thermal coupling (split kernels)" if args.thermal else ""),
+                               + (", two-way thermal coupling (%s)" % ("split kernels" if args.kernel == "split" else "coupled TMA sweep + conduction kernel") if args.thermal else ""),
                    "kernel_strategy": args.kernel, "l2": "state %.1f GB >> 126 MB L2 (no flush needed)" % (em.workspace_bytes / 1e9)
                    if em.workspace_bytes > 1e9 else "state fits L2: %.0f MB" % (em.workspace_bytes / 1e6),
                    "parallelism": ("z-slabs x%d, 2-plane halo exchange per step" % world if slab is not None else

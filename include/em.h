@@ -80,8 +80,8 @@ typedef struct em_grid {
     int32_t max_ports;           /* capacity reserved in the workspace for em_set_source            */
     int64_t max_source_edges;
     int64_t max_wave_samples;
-    int32_t thermal;             /* 1: reserve workspace for the thermal stage (em_set_thermal); forces the    */
-    int32_t pad_;                /*    SPLIT strategy (EM_ERR_UNSUPPORTED with kernel = FUSED / TMA).  0: EM only */
+    int32_t thermal;             /* 1: reserve workspace for the thermal stage (em_set_thermal): AUTO / TMA run */
+    int32_t pad_;                /*    the coupled TMA sweep, SPLIT the split kernels; FUSED -> EM_ERR_UNSUPPORTED */
 } em_grid;
 
 typedef struct em_material { double eps, mu, sigma; int32_t flags; int32_t pad_; } em_material;
@@ -165,7 +165,10 @@ int32_t em_reset(em_ctx *ctx);
  *   eq. (6)  sigma' = sigma_0 / (1 + alpha theta'), used by the next step's E update ("D_sigma(T^n)", L78)
  * M_kk = V0a^T D_k V0: cell-centred -div k grad with the series conductivity of the two half cells on each face,
  * adiabatic walls (L142).  sigma_0 = the em_material.sigma given to em_create.  em_joule's power density then uses
- * the current sigma(T).  em_reset also zeroes theta.  Runs on the split kernels (first CUDA path of this stage). */
+ * the current sigma(T).  em_reset also zeroes theta.  Per step: one conduction kernel (theta^n -> theta - dt/(rho c_p)
+ * M_kk theta) and the coupled TMA sweep (sigma(T^n) staged as one more plane per step plane, Joule heat added to theta
+ * and sigma(T^{n+1}) written in its Joule phase); kernel = SPLIT runs the same step on the split kernels.  Until
+ * em_set_thermal is called such a context steps EM-only on the split kernels. */
 typedef struct em_thermal_material { double rho_cp /* J/(m^3 K) > 0 */, k /* W/(m K) >= 0 */, alpha /* 1/K */; } em_thermal_material;
 
 /* Switches the coupling on (theta = 0).  table: HOST, n_mat entries (the n_mat of em_create).

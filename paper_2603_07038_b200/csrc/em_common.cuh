@@ -44,6 +44,18 @@ struct DevParams {
     R dt;
 };
 
+// Thermal coupling (eq. (4)-(6)).  Per material: 1/(rho c_p), k, alpha, sigma_0; the "outside" entries are all
+// 0 (no heat, no conduction).
+template <typename R> struct alignas(4 * sizeof(R)) ThEntry { R irc, k, alpha, sigma0; };
+
+// Extra arguments of the thermally coupled sweep (em_sweep.cuh, TH = true); unused otherwise.
+template <typename R>
+struct ThermalSweep {
+    R *theta;                    // temperature rise after the conduction kernel (theta_d); the sweep adds dq/(rho c_p) in place
+    R *sig_out;                  // sigma(T^{n+1}) (the sigma(T^n) array is read through its tensor map)
+    const ThEntry<R> *ttable;    // n_table entries
+};
+
 __device__ __forceinline__ float  mad(float a, float b, float c)    { return ::fmaf(a, b, c); }
 __device__ __forceinline__ double mad(double a, double b, double c) { return ::fma(a, b, c); }
 template <typename R> __device__ __forceinline__ R lerp(R lo, R hi, R f) { return mad(f, hi - lo, lo); }

@@ -39,13 +39,15 @@ constexpr int kFusedOcc = EM_FUSED_OCC;             // resident CTAs per SM
 // Tile rows per working precision.  fp32: 14 owned rows = 16 warps x 128 registers.  fp64 needs ~170 registers per
 // thread to stay spill-free (a spill is very expensive here: the 227 KB carve-out leaves almost no L1), so its tiles
 // own 10 rows = 12 warps (measured on config 3 fp64: 1.22 -> 0.87 ms/step).
-template <int SZ> struct Tile {
-    static constexpr int TY = SZ == 8 ? EM_FUSED_TY64 : EM_FUSED_TY;   // owned rows per tile
+// TH = the thermally coupled sweep (em_sweep.cuh, sigma(T) planes + theta in the sweep): it also takes the 10-row tile
+// (room in registers and shared memory for the extra state).
+template <int SZ, bool TH = false> struct Tile {
+    static constexpr int TY = (SZ == 8 || TH) ? EM_FUSED_TY64 : EM_FUSED_TY;   // owned rows per tile
     static constexpr int warps = TY + 2;                                // rows -1 .. TY
     static constexpr int threads = warps * 32;
     static constexpr int rows = TY + 4;                                 // exchange rows, r = cy + 2 (row 0 and last: dummies)
 };
-inline int tile_rows(int sizeof_real) { return sizeof_real == 8 ? Tile<8>::TY : Tile<4>::TY; }
+inline int tile_rows(int sizeof_real, bool thermal = false) { return (sizeof_real == 8 || thermal) ? Tile<8>::TY : Tile<4>::TY; }
 constexpr int kFusedSlots = 21;                    // private 16-B slots per thread (see enum below)
 
 constexpr int kFusedMaxZSplit = 8;                // z chunks per tile column (work items = tiles x chunks)
@@ -77,12 +79,13 @@ inline int choose_zsplit(int n_tiles, int nz, int n_sm, int forced) {
     return best;
 }
 
-inline FusedPlan make_fused_plan(int nx, int ny, int nz, int sizeof_real, int n_sm = 0, int forced_zsplit = 0) {
+inline FusedPlan make_fused_plan(int nx, int ny, int nz, int sizeof_real, int n_sm = 0, int forced_zsplit = 0,
+                                 bool thermal = false) {
     FusedPlan f;
     f.V = 16 / sizeof_real;
     f.TXo = 30 * f.V;
     f.ntx = (nx + 1 + f.TXo - 1) / f.TXo;
-    f.TY = tile_rows(sizeof_real);
+    f.TY = tile_rows(sizeof_real, thermal);
     const int kFusedRows = f.TY + 4, kFusedThreads = (f.TY + 2) * 32;
     f.nty = (ny + 1 + f.TY - 1) / f.TY;
     f.n_tiles = f.ntx * f.nty;

@@ -87,7 +87,7 @@ struct Carved {
     // fused-sweep tile source index
     int *tile_sbeg; int4 *tile_ent;
     // thermal coupling (only when em_grid.thermal != 0): theta ping-pong, sigma(T) per cell, thermal table
-    R *theta[2]; R *sig; em::ThEntry<R> *ttable;
+    R *theta[2]; R *sig, *sig2; em::ThEntry<R> *ttable;
 };
 
 template <typename R>
@@ -114,9 +114,10 @@ size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int
     o.wave = w.take<R>((size_t)std::max<int64_t>(gr.max_wave_samples, 1));
     o.tile_sbeg = w.take<int>((size_t)n_items + 1);
     o.tile_ent = w.take<int4>(4 * me);
-    o.theta[0] = o.theta[1] = o.sig = nullptr; o.ttable = nullptr;
+    o.theta[0] = o.theta[1] = o.sig = o.sig2 = nullptr; o.ttable = nullptr;
     if (gr.thermal) {
         o.theta[0] = w.take<R>(g.alloc_elems); o.theta[1] = w.take<R>(g.alloc_elems); o.sig = w.take<R>(g.alloc_elems);
+        o.sig2 = w.take<R>(g.alloc_elems);
         o.ttable = w.take<em::ThEntry<R>>(em::kMaxTable);
     }
     return align_up(w.off);
@@ -205,6 +206,10 @@ struct Ctx final : em_ctx {
     int32_t set_thermal(const em_thermal_material *, int32_t) override;
     int32_t temperature_rise(void *dst, const void *src, int32_t is_dev) override;
     int32_t step_thermal();
+    int32_t step_thermal_sweep();
+    int sg_cur = 0;                     // which sigma(T) buffer is current (the coupled sweep ping-pongs them)
+    R *sig_buf(int which) const { return (which ? c.sig2 : c.sig) + g.origin; }
+    CUtensorMap map_sig[2];
     int32_t refresh_sigma();
     bool thermal_on = false;            // em_set_thermal was called
     int th_cur = 0;
@@ -212,7 +217,7 @@ struct Ctx final : em_ctx {
     em::ThermalParams<R> tp() const {
         em::ThermalParams<R> t;
         t.theta = c.theta[th_cur] + g.origin; t.theta_n = c.theta[1 - th_cur] + g.origin;
-        t.sig = c.sig + g.origin; t.ttable = c.ttable;
+        t.sig = sig_buf(sg_cur); t.ttable = c.ttable;
         return t;
     }
     int32_t step_split();
@@ -246,8 +251,8 @@ int32_t validate_grid(const em_grid *g) {
     if (g->loss_mode != EM_LOSS_CD && g->loss_mode != EM_LOSS_EXP) return fail(EM_ERR_INVALID_ARG, "bad loss_mode");
     if (g->kernel < EM_KERNEL_AUTO || g->kernel > EM_KERNEL_TMA) return fail(EM_ERR_INVALID_ARG, "bad kernel strategy");
     if (g->thermal != 0 && g->thermal != 1) return fail(EM_ERR_INVALID_ARG, "thermal must be 0 or 1");
-    if (g->thermal && (g->kernel == EM_KERNEL_FUSED || g->kernel == EM_KERNEL_TMA))
-        return fail(EM_ERR_UNSUPPORTED, "thermal coupling runs on the split kernels (kernel = AUTO or SPLIT)");
+    if (g->thermal && g->kernel == EM_KERNEL_FUSED)
+        return fail(EM_ERR_UNSUPPORTED, "thermal coupling runs on the TMA sweep or the split kernels (kernel = AUTO, TMA or SPLIT)");
     if (g->max_ports < 0 || g->max_source_edges < 0 || g->max_wave_samples < 0)
         return fail(EM_ERR_INVALID_ARG, "negative source capacity");
     return EM_OK;
@@ -280,7 +285,7 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
         const char *forced = std::getenv("EM_FUSED_ZSPLIT");      // tuning/test knob: force the z chunk count
-        plan = em::make_fused_plan(g.nx, g.ny, g.nz, (int)sizeof(R), n_sm, forced ? std::atoi(forced) : 0);
+        plan = em::make_fused_plan(g.nx, g.ny, g.nz, (int)sizeof(R), n_sm, forced ? std::atoi(forced) : 0, gr->thermal != 0);
     }
     kernel = gr->kernel;
     const int max_items = plan.n_tiles * em::kFusedMaxZSplit;
@@ -289,13 +294,18 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     carve<R>(g, *gr, workspace, &c, max_items);
     sweep_smem = em::sweep_smem_bytes((int)sizeof(R), n_mat + 2);
     n_mat_ = n_mat;
-    if (gr->thermal) kernel = EM_KERNEL_SPLIT;                // sigma(T) lives in a per-cell array: split kernels (em_thermal.cuh)
+    // thermal coupling: the coupled TMA sweep (sigma(T) planes staged beside the ids) or, if its shared-memory layout
+    // does not fit / on request, the split kernels (em_thermal.cuh)
+    if (gr->thermal) {
+        sweep_smem = em::sweep_smem_bytes((int)sizeof(R), n_mat + 2, true);
+        if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_TMA;
+    }
     if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_TMA;     // measured on config 4: TMA sweep 2.44 ms/step, cp.async sweep 2.71 ms/step
     if (kernel == EM_KERNEL_TMA) {
         int dev = 0, optin = 0;
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-        if (sweep_smem > (size_t)optin) kernel = EM_KERNEL_FUSED;   // very large tables: cp.async sweep
+        if (sweep_smem > (size_t)optin) kernel = gr->thermal ? EM_KERNEL_SPLIT : EM_KERNEL_FUSED;   // very large tables
     }
     main_kernel = kernel == EM_KERNEL_TMA ? "k_sweep_tma" : kernel == EM_KERNEL_FUSED ? "k_fused_sweep" : "k_split_e";
 
@@ -424,16 +434,23 @@ int32_t Ctx<R>::make_maps() {
         if (r != CUDA_SUCCESS) return fail(EM_ERR_CUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
         return EM_OK;
     };
+    const int sw_warps = grid.thermal ? em::Tile<sizeof(R), true>::warps : em::Tile<sizeof(R)>::warps;
     const CUtensorMapDataType fdt = sizeof(R) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
     for (int a = 0; a < 12; ++a) {
         const int comp = a % 3, is_e = a < 6;
-        const int rows = (is_e && comp != 1) ? em::Tile<sizeof(R)>::warps + 1 : em::Tile<sizeof(R)>::warps;         // Ex, Ez carry row TY+1
+        const int rows = (is_e && comp != 1) ? sw_warps + 1 : sw_warps;         // Ex, Ez carry row TY+1
         int32_t rc = encode(&map_field[a], fdt, sizeof(R), c.field[a] + g.PX - V, 32 * V, rows);
         if (rc) return rc;
     }
-    int32_t rc = encode(&map_q, fdt, sizeof(R), c.q + g.PX - V, 30 * V, em::Tile<sizeof(R)>::TY);
+    int32_t rc = encode(&map_q, fdt, sizeof(R), c.q + g.PX - V, 30 * V, sw_warps - 2);
     if (rc) return rc;
-    return encode(&map_mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, c.mat + g.PX - em::kSwIdShift, 32 * V + 16, em::Tile<sizeof(R)>::warps + 2);
+    rc = encode(&map_mat, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, c.mat + g.PX - em::kSwIdShift, 32 * V + 16, sw_warps + 2);
+    if (rc) return rc;
+    if (grid.thermal) {                                   // sigma(T) planes of the coupled sweep: rows -2 .. TY
+        rc = encode(&map_sig[0], fdt, sizeof(R), c.sig + g.PX - V, 32 * V, sw_warps + 1); if (rc) return rc;
+        rc = encode(&map_sig[1], fdt, sizeof(R), c.sig2 + g.PX - V, 32 * V, sw_warps + 1); if (rc) return rc;
+    }
+    return EM_OK;
 }
 
 // ---- sources ------------------------------------------------------------------------------------
@@ -650,7 +667,10 @@ int32_t Ctx<R>::step_split() {
 template <typename R>
 int32_t Ctx<R>::refresh_sigma() {
     dim3 b(32, 8);
-    em::k_sigma_refresh<R><<<node_grid(b, 0), b, 0, stream>>>(p, tp());
+    em::ThermalParams<R> t = tp();
+    em::k_sigma_refresh<R><<<node_grid(b, 0), b, 0, stream>>>(p, t);
+    t.sig = sig_buf(1 - sg_cur);                        // both buffers: the coupled sweep rewrites only the lossy lanes
+    em::k_sigma_refresh<R><<<node_grid(b, 0), b, 0, stream>>>(p, t);
     CU(cudaGetLastError());
     return EM_OK;
 }
@@ -670,6 +690,8 @@ int32_t Ctx<R>::set_thermal(const em_thermal_material *tt, int32_t n_mat) {
     CU(cudaMemsetAsync(c.theta[0], 0, sizeof(R) * g.alloc_elems, stream));
     CU(cudaMemsetAsync(c.theta[1], 0, sizeof(R) * g.alloc_elems, stream));
     CU(cudaMemsetAsync(c.sig, 0, sizeof(R) * g.alloc_elems, stream));
+    CU(cudaMemsetAsync(c.sig2, 0, sizeof(R) * g.alloc_elems, stream));
+    sg_cur = 0;
     th_cur = 0;
     thermal_on = true;
     int32_t rc = refresh_sigma(); if (rc) return rc;
@@ -704,7 +726,7 @@ int32_t Ctx<R>::temperature_rise(void *dst, const void *srcp, int32_t is_dev) {
 template <typename R>
 int32_t Ctx<R>::step_thermal() {
     dim3 b(32, 8);
-    const R *sig = c.sig + g.origin;
+    const R *sig = sig_buf(sg_cur);
     em::k_split_h<R><<<node_grid(b, 1), b, 0, stream>>>(p);
     int32_t rc = record_begin(); if (rc) return rc;
     if (loss == EM_LOSS_CD) em::k_split_e_sig<R, 0><<<node_grid(b, 1), b, 0, stream>>>(p, sig);
@@ -722,6 +744,29 @@ int32_t Ctx<R>::step_thermal() {
     launches += 1;
     CU(cudaGetLastError());
     e_cur ^= 1; th_cur ^= 1; bind();
+    return EM_OK;
+}
+
+// One coupled step on the TMA sweep: conduction first (theta_d = theta^n - dt/(rho c_p) M_kk theta^n into the other theta
+// buffer), then the sweep with D_sigma(T^n) from the current sigma buffer; its phase C adds the Joule heat of the step to
+// theta_d in place and writes sigma(T^{n+1}) of the lossy lanes to the other sigma buffer.  Buffers are swapped.
+template <typename R>
+int32_t Ctx<R>::step_thermal_sweep() {
+    dim3 b(32, 8);
+    R *th_in = c.theta[th_cur] + g.origin, *th_out = c.theta[1 - th_cur] + g.origin;
+    em::k_diffuse<R><<<node_grid(b, 0), b, 0, stream>>>(p, c.ttable, th_in, th_out);
+    launches += 1;
+    int32_t rc = record_begin(); if (rc) return rc;
+    em::FusedSources fsrc{c.tile_sbeg, c.tile_ent};
+    em::SweepMaps maps;
+    for (int a = 0; a < 3; ++a) { maps.E[a] = map_field[e_cur * 3 + a]; maps.H[a] = map_field[6 + h_cur * 3 + a]; }
+    maps.q = map_q; maps.mat = map_mat; maps.sig = map_sig[sg_cur];
+    em::ThermalSweep<R> tsw{th_out, sig_buf(1 - sg_cur), c.ttable};
+    cudaError_t e = em::launch_sweep_tma<R>(plan, sweep_smem, maps, p, src, fsrc, loss, uniform_mu, (long long)step_index, stream, &tsw);
+    if (e != cudaSuccess) return fail(EM_ERR_CUDA, std::string("coupled TMA sweep launch: ") + cudaGetErrorString(e));
+    rc = record_end(); if (rc) return rc;
+    launches += 1;
+    e_cur ^= 1; h_cur ^= 1; th_cur ^= 1; sg_cur ^= 1; bind();
     return EM_OK;
 }
 
@@ -756,7 +801,9 @@ template <typename R>
 int32_t Ctx<R>::step(int64_t n) {
     if (n < 0) return fail(EM_ERR_INVALID_ARG, "n < 0");
     for (int64_t s = 0; s < n; ++s) {
-        int32_t rc = thermal_on ? step_thermal() : kernel == EM_KERNEL_TMA ? step_tma() : kernel == EM_KERNEL_FUSED ? step_fused() : step_split();
+        int32_t rc = thermal_on ? (kernel == EM_KERNEL_TMA ? step_thermal_sweep() : step_thermal())
+                   : grid.thermal ? step_split()            // (tile geometry of the coupled sweep: EM-only steps run split)
+                   : kernel == EM_KERNEL_TMA ? step_tma() : kernel == EM_KERNEL_FUSED ? step_fused() : step_split();
         if (rc) return rc;
         step_index += 1;
     }
@@ -768,7 +815,7 @@ template <typename R>
 int32_t Ctx<R>::joule(void *power, void *energy, double *total, int32_t do_reset) {
     dim3 b(32, 8);
     if (power) {
-        if (thermal_on) em::k_power_sig<R><<<node_grid(b, 0), b, 0, stream>>>(p, c.sig + g.origin, static_cast<R *>(power));
+        if (thermal_on) em::k_power_sig<R><<<node_grid(b, 0), b, 0, stream>>>(p, sig_buf(sg_cur), static_cast<R *>(power));
         else            em::k_power<R><<<node_grid(b, 0), b, 0, stream>>>(p, static_cast<R *>(power));
         CU(cudaGetLastError()); launches += 1;
     }
@@ -830,7 +877,7 @@ int32_t em_workspace_bytes(const em_grid *gr, size_t *out) {
     if (!out) return fail(EM_ERR_INVALID_ARG, "out is null");
     int32_t rc = validate_grid(gr); if (rc) return rc;
     const Geometry g = make_geometry(gr->nx, gr->ny, gr->nz);
-    const em::FusedPlan plan = em::make_fused_plan(g.nx, g.ny, g.nz, gr->precision / 8);
+    const em::FusedPlan plan = em::make_fused_plan(g.nx, g.ny, g.nz, gr->precision / 8, 0, 0, gr->thermal != 0);
     const int max_items = plan.n_tiles * em::kFusedMaxZSplit;
     *out = gr->precision == 32 ? carve<float>(g, *gr, nullptr, nullptr, max_items)
                                : carve<double>(g, *gr, nullptr, nullptr, max_items);

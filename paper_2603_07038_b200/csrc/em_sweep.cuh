@@ -28,13 +28,14 @@ constexpr int kSwRow = 512;                        // bytes of one staged row (3
 constexpr int kSwIdShift = 16;                     // the id map starts 16 B before the row (16-B aligned base)
 constexpr int kSwPriv = 8;                         // private 16-B slots per thread: q, L x 4, H' x 2, pend
 
-struct alignas(64) SweepMaps { CUtensorMap E[3], H[3], q, mat; };
+struct alignas(64) SweepMaps { CUtensorMap E[3], H[3], q, mat, sig; };   // sig: the sigma(T^n) array (coupled sweep only)
 
 // Shared-memory layout (bytes; identical for fp32 and fp64 except the id rows; the table comes last
 // because its size is only known at run time)
-template <int SZ> struct SweepLayout {
+template <int SZ, bool TH = false> struct SweepLayout {
     static constexpr int V = 16 / SZ;
-    static constexpr int kSwWarps = Tile<SZ>::warps, kFusedRows = Tile<SZ>::rows;
+    static constexpr int kSwWarps = Tile<SZ, TH>::warps, kFusedRows = Tile<SZ, TH>::rows;
+    static constexpr int n_priv = kSwPriv + (TH ? 1 : 0);          // + theta of layer k-1 (coupled sweep)
     static constexpr int ex = 0;                                  // Ex ring of 3 planes, rows -1 .. TY+1
     static constexpr int ex_slot = (kSwWarps + 1) * kSwRow;
     static constexpr int ey = ex + 3 * ex_slot;                   // Ey ring of 3 planes, rows -1 .. TY
@@ -47,19 +48,23 @@ template <int SZ> struct SweepLayout {
     static constexpr int id_row = 32 * V + 16;                    // box starts on a 16-B boundary: up to 15 B of lead-in
     static constexpr int id_slot = ((kSwWarps + 2) * id_row + 127) / 128 * 128;
     static constexpr int priv = ids + 2 * id_slot;                // private slots [kSwPriv][512 threads]
-    static constexpr int rows = priv + kSwPriv * kSwWarps * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kFusedRows][32]
+    static constexpr int rows = priv + n_priv * kSwWarps * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kFusedRows][32]
     static constexpr int geo = rows + 4 * kFusedRows * kSwRow;    // 1/dx, 1/dx~, fx of the 32 lanes
     static constexpr int zg = geo + 3 * kSwRow;                   // [2 parity]{fz, 1/dz, 1/dz~, 0}
-    static constexpr int bar = zg + 64;                           // fullE[2], fullH[2], empty[2], rowH[kSwWarps]
+    static constexpr int sig = zg + 128;                          // coupled sweep: sigma(T^n), 2 parities, rows -2 .. TY (TMA: 128-B aligned)
+    static constexpr int sig_slot = TH ? (kSwWarps + 1) * kSwRow : 0;
+    static constexpr int bar = sig + 2 * sig_slot;                // fullE[2], fullH[2], empty[2], rowH[kSwWarps]
     static constexpr int tab = bar + 64 + 8 * kSwWarps;                          // material table (n_table entries)
-    static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + (kSwWarps + 2) * id_row;
+    static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + (kSwWarps + 2) * id_row + sig_slot;
     static constexpr int first_extra_bytes = ex_slot + ey_slot;
     static constexpr int h_bytes = 3 * h_slot;
 };
 
-inline size_t sweep_smem_bytes(int sizeof_real, int n_table) {
-    const size_t tab = sizeof_real == 4 ? SweepLayout<4>::tab : SweepLayout<8>::tab;
-    return tab + (size_t)n_table * 4 * sizeof_real;
+// the material table, and for the coupled sweep the thermal table (ThEntry, same size) behind it
+inline size_t sweep_smem_bytes(int sizeof_real, int n_table, bool thermal = false) {
+    const size_t tab = thermal ? (sizeof_real == 4 ? SweepLayout<4, true>::tab : SweepLayout<8, true>::tab)
+                               : (sizeof_real == 4 ? SweepLayout<4>::tab : SweepLayout<8>::tab);
+    return tab + (size_t)n_table * 4 * sizeof_real * (thermal ? 2 : 1);
 }
 
 // ---- mbarrier / TMA PTX wrappers ---------------------------------------------------------------------
@@ -103,19 +108,23 @@ __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------------
-template <typename R, int LOSS, bool UMU>
-__global__ void __launch_bounds__(Tile<sizeof(R)>::threads, 1)
+// TH = true: the thermally coupled sweep (eq. (4)-(6); DESIGN.md section 9 NEXT-1).  The per-cell sigma(T^n)
+// is staged as one more TMA plane per step plane (rows -2 .. TY) and replaces the table's sigma in the coefficient
+// gather; phase C adds the Joule heat of the step to theta (already advanced by the conduction kernel k_diffuse) and
+// writes sigma(T^{n+1}) to the other sigma buffer.  The one-material path is taken only for materials with alpha = 0.
+template <typename R, int LOSS, bool UMU, bool TH = false>
+__global__ void __launch_bounds__(Tile<sizeof(R), TH>::threads, 1)
 k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R> src, FusedSources fs,
-            FusedChunks zc, int ntx, long long step) {
+            FusedChunks zc, int ntx, long long step, ThermalSweep<R> th) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TXo = 30 * V;
-    constexpr int kSwTY = Tile<sizeof(R)>::TY, kSwWarps = Tile<sizeof(R)>::warps, kFusedRows = Tile<sizeof(R)>::rows;
-    constexpr int NT = Tile<sizeof(R)>::threads;
-    using L = SweepLayout<(int)sizeof(R)>;
+    constexpr int kSwTY = Tile<sizeof(R), TH>::TY, kSwWarps = Tile<sizeof(R), TH>::warps, kFusedRows = Tile<sizeof(R), TH>::rows;
+    constexpr int NT = Tile<sizeof(R), TH>::threads;
+    using L = SweepLayout<(int)sizeof(R), TH>;
     using VecR = Vec<R>;
     using IdT = typename std::conditional<V == 4, unsigned, unsigned short>::type;
     // private slot numbering of this kernel (shadows the cp.async sweep's enum inside em_fused_phaseb*.inc)
-    constexpr int kSlotQ = 0, kSlotL = 1, kSlotHp = 5, kSlotPend = 7;
+    constexpr int kSlotQ = 0, kSlotL = 1, kSlotHp = 5, kSlotPend = 7, kSlotTheta = 8;
     extern __shared__ __align__(1024) unsigned char sm[];
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -162,12 +171,14 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int t = tid; t < p.n_table; t += NT) s_tab[t] = p.table[t];
+    ThEntry<R> *s_th = reinterpret_cast<ThEntry<R> *>(s_tab + p.n_table);     // coupled sweep only
+    if (TH) for (int t = tid; t < p.n_table; t += NT) s_th[t] = th.ttable[t];
     {
         VecR z, mone;
 #pragma unroll
         for (int c = 0; c < V; ++c) { z.v[c] = R(0); mone.v[c] = R(-1); }
         for (int t = tid; t < 4 * kFusedRows * 32; t += NT) s_rows[t] = z;
-        for (int t = 0; t < kSwPriv; ++t) mine[t * NT] = z;
+        for (int t = 0; t < L::n_priv; ++t) mine[t * NT] = z;
         mine[(kSlotL + 0) * NT] = mone; mine[(kSlotL + 2) * NT] = mone;     // plane k = -1 is outside: eps/dt = 1, mask 0 (sign)
         if (w == 0) {
             const bool in = (i0 + V <= p.PX);
@@ -196,6 +207,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         tma_load_3d(sb + L::ey + ((kk + 1) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 2);
         tma_load_3d(sb + L::ez + (kk & 1) * L::ez_slot, &maps.E[2], bar, cx, cyy, kk + 1);
         tma_load_3d(sb + L::ids + (kk & 1) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, kk + 1);
+        if (TH) tma_load_3d(sb + L::sig + (kk & 1) * L::sig_slot, &maps.sig, bar, cx, cyy - 1, kk + 1);   // rows -2 .. TY
     };
     // H group of plane kk -> parity kk&1 (two planes in flight)
     auto issue_H = [&](int kk) {
@@ -226,6 +238,9 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     bool rowu_prev = false;      // plane k-1: rows j-1 and j of this lane held one material
     bool l_stale = false;        // warp-uniform: the L slots were skipped by the one-material path
     bool q_live = false;         // q of layer k-1 was fetched (some sigma != 0 among the lane's cells)
+    VecR sig_prev;               // coupled sweep: sigma(T^n) of the lane's cells of layer k-1 (Joule sum of phase C)
+#pragma unroll
+    for (int c = 0; c < V; ++c) sig_prev.v[c] = R(0);
     // source cursor: starts at the tile's first entry with k >= kz0 and may run into the next chunk's
     // entries on the closing plane k = kz1 (E'(kz1) enters the Joule sum of layer kz1-1)
     int s_cur = fs.tile_sbeg[item];
@@ -247,7 +262,12 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         // one material over the warp's whole coefficient neighbourhood (rows j-1..j, planes k-1..k)?
         const bool rowu = (idw == idj) && id_uniform(idw);
         const unsigned idw_lane0 = __shfl_sync(0xffffffffu, idw, 0);   // (every lane must execute it)
-        const bool hom = __all_sync(0xffffffffu, rowu && rowu_prev && idw == idw_prev && idw == idw_lane0);
+        bool hom = __all_sync(0xffffffffu, rowu && rowu_prev && idw == idw_prev && idw == idw_lane0);
+        VecR sigw, sigj;             // coupled sweep: sigma(T^n) of rows j and j-1 of plane k (box rows start at j0-2)
+        if (TH) {
+            hom = hom && s_th[idw_lane0 & 0xff].alpha == R(0);     // sigma of the material does not depend on T
+            sigw = staged(L::sig + par * L::sig_slot + kSwRow); sigj = staged(L::sig + par * L::sig_slot);
+        }
         VecR hxn, hyn, hzn;
         const VecR ex0 = staged(L::ex + rk * L::ex_slot), ey0 = staged(L::ey + rk * L::ey_slot);
         const VecR ez = staged(L::ez + par * L::ez_slot);
@@ -358,6 +378,8 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             const R by_r = shfl_down1(by.v[0]), bz_r = shfl_down1(bz.v[0]), bzn_r = shfl_down1(bzn.v[0]);
             VecR qv = mine[kSlotQ * NT];
             VecR pend = mine[kSlotPend * NT];
+            VecR thv, sgn;           // coupled sweep: theta and sigma(T^{n+1}) of the cells of layer k-1
+            if (TH) thv = mine[kSlotTheta * NT];
 #pragma unroll
             for (int c = 0; c < V; ++c) {
                 const R byip = (c < V - 1) ? by.v[c < V - 1 ? c + 1 : c] : by_r;
@@ -365,19 +387,35 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
                 const R bznip = (c < V - 1) ? bzn.v[c < V - 1 ? c + 1 : c] : bzn_r;
                 const R sxy = (bx.v[c] + bxn.v[c]) + (by.v[c] + byip);
                 const R sz = (bz.v[c] + bzip) + (bzn.v[c] + bznip);
-                const R sg = s_tab[(idw_prev >> (8 * (hom ? 0 : c))) & 0xff].b;     // sigma of the cell of layer k-1
-                qv.v[c] = mad(gq * sg, pend.v[c] + sxy, qv.v[c]);
+                if (TH) {            // eq. (5) source term and eq. (6), with sigma(T^n) as used by the E update
+                    const ThEntry<R> te = s_th[(idw_prev >> (8 * c)) & 0xff];
+                    const R dq = gq * sig_prev.v[c] * (pend.v[c] + sxy);
+                    qv.v[c] += dq;
+                    thv.v[c] = mad(dq, te.irc, thv.v[c]);
+                    sgn.v[c] = te.sigma0 * rcp<R>(mad(te.alpha, thv.v[c], R(1)));
+                } else {
+                    const R sg = s_tab[(idw_prev >> (8 * (hom ? 0 : c))) & 0xff].b;     // sigma of the cell of layer k-1
+                    qv.v[c] = mad(gq * sg, pend.v[c] + sxy, qv.v[c]);
+                }
                 pend.v[c] = sxy + sz;
             }
             mine[kSlotPend * NT] = pend;
             // q of a lane whose V cells are one lossless material never changes: neither fetched nor stored
-            if (own_q && k > kz0 && q_live) EM_ST(p.q + o - PXY, qv);   // layer k-1 in [kz0, kz1)
+            // (coupled sweep: the same holds for theta -- only conduction moves it -- and for sigma = 0)
+            if (own_q && k > kz0 && q_live) {                            // layer k-1 in [kz0, kz1)
+                EM_ST(p.q + o - PXY, qv);
+                if (TH) { EM_ST(th.theta + o - PXY, thv); EM_ST(th.sig_out + o - PXY, sgn); }
+            }
             q_live = !(id_uniform(idw) && s_tab[idw & 0xff].b == R(0));
-            if (own_q && k >= kz0 && k < ke && q_live) cp_async16(mine + kSlotQ * NT, p.q + o);   // q(k)
+            if (own_q && k >= kz0 && k < ke && q_live) {
+                cp_async16(mine + kSlotQ * NT, p.q + o);                 // q(k)
+                if (TH) cp_async16(mine + kSlotTheta * NT, th.theta + o);   // theta_d(k)
+            }
         }
         cp_async_commit();
         idw_prev = idw;
         rowu_prev = rowu;
+        if (TH) sig_prev = sigw;
         rk = rk1;
     }
     cp_async_wait<0>();
@@ -386,17 +424,22 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
 template <typename R>
 cudaError_t launch_sweep_tma(const FusedPlan &plan, size_t smem_bytes, const SweepMaps &maps, const DevParams<R> &p,
                              const DevSources<R> &src, const FusedSources &fs, int loss, bool uniform_mu,
-                             long long step, cudaStream_t stream) {
-    using K = void (*)(const SweepMaps, DevParams<R>, DevSources<R>, FusedSources, FusedChunks, int, long long);
+                             long long step, cudaStream_t stream, const ThermalSweep<R> *thermal = nullptr) {
+    using K = void (*)(const SweepMaps, DevParams<R>, DevSources<R>, FusedSources, FusedChunks, int, long long, ThermalSweep<R>);
     FusedChunks zc;
     zc.nzs = plan.nzs;
     for (int c = 0; c <= kFusedMaxZSplit; ++c) zc.kb[c] = plan.kb[c];
     K kern;
-    if (loss == 0) kern = uniform_mu ? (K)k_sweep_tma<R, 0, true> : (K)k_sweep_tma<R, 0, false>;
-    else           kern = uniform_mu ? (K)k_sweep_tma<R, 1, true> : (K)k_sweep_tma<R, 1, false>;
+    ThermalSweep<R> th{};
+    int threads = Tile<sizeof(R)>::threads;
+    if (thermal) {           // coupled sweep: sigma(T) planes, general mu path only (one instantiation per loss mode)
+        th = *thermal; threads = Tile<sizeof(R), true>::threads;
+        kern = loss == 0 ? (K)k_sweep_tma<R, 0, false, true> : (K)k_sweep_tma<R, 1, false, true>;
+    } else if (loss == 0) kern = uniform_mu ? (K)k_sweep_tma<R, 0, true> : (K)k_sweep_tma<R, 0, false>;
+    else                  kern = uniform_mu ? (K)k_sweep_tma<R, 1, true> : (K)k_sweep_tma<R, 1, false>;
     cudaError_t e = cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
-    kern<<<plan.n_tiles * plan.nzs, Tile<sizeof(R)>::threads, smem_bytes, stream>>>(maps, p, src, fs, zc, plan.ntx, step);
+    kern<<<plan.n_tiles * plan.nzs, threads, smem_bytes, stream>>>(maps, p, src, fs, zc, plan.ntx, step, th);
     return cudaGetLastError();
 }
 

@@ -13,8 +13,7 @@
 
 namespace em {
 
-// per material: 1/(rho c_p), k, alpha, sigma_0; the "outside" entries are all 0 (no heat, no conduction)
-template <typename R> struct alignas(4 * sizeof(R)) ThEntry { R irc, k, alpha, sigma0; };
+// (ThEntry: em_common.cuh)
 
 template <typename R>
 struct ThermalParams {
@@ -141,6 +140,36 @@ __global__ void __launch_bounds__(256) k_joule_thermal(DevParams<R> p, ThermalPa
     const R thn = th - p.dt * me.irc * lap + dq * me.irc;
     t.theta_n[o] = thn;
     t.sig[o] = me.sigma0 * rcp<R>(R(1) + me.alpha * thn);
+}
+
+// Conduction half of eq. (5) for the coupled sweep: theta_d = theta^n - dt/(rho c_p) (M_kk theta^n), all cells, into the
+// other theta buffer (the sweep then adds the Joule heat of the step in place).
+template <typename R>
+__global__ void __launch_bounds__(256) k_diffuse(DevParams<R> p, const ThEntry<R> *ttable, const R *theta, R *theta_d) {
+    __shared__ ThEntry<R> s_th[kMaxTable];
+    {
+        const int tid = threadIdx.y * blockDim.x + threadIdx.x, nth = blockDim.x * blockDim.y;
+        for (int m = tid; m < p.n_table; m += nth) s_th[m] = ttable[m];
+        __syncthreads();
+    }
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= p.nx || j >= p.ny) return;
+    const long long PX = p.PX, PXY = p.PXY;
+    const long long o = ((long long)k * p.PY + j) * PX + i;
+    const ThEntry<R> me = s_th[p.mat[o]];
+    const R th = theta[o];
+    const R rdx = p.rdx[i], rdy = p.rdy[j], rdz = p.rdz[k];
+    const R gx = rdx * me.k, gy = rdy * me.k, gz = rdz * me.k;
+    R lap = R(0);
+    lap = mad(rdx, half_cell_cond(gx, p.rdx[i - 1] * s_th[p.mat[o - 1]].k) * (th - theta[o - 1]), lap);
+    lap = mad(rdx, half_cell_cond(gx, p.rdx[i + 1] * s_th[p.mat[o + 1]].k) * (th - theta[o + 1]), lap);
+    lap = mad(rdy, half_cell_cond(gy, p.rdy[j - 1] * s_th[p.mat[o - PX]].k) * (th - theta[o - PX]), lap);
+    lap = mad(rdy, half_cell_cond(gy, p.rdy[j + 1] * s_th[p.mat[o + PX]].k) * (th - theta[o + PX]), lap);
+    lap = mad(rdz, half_cell_cond(gz, p.rdz[k - 1] * s_th[p.mat[o - PXY]].k) * (th - theta[o - PXY]), lap);
+    lap = mad(rdz, half_cell_cond(gz, p.rdz[k + 1] * s_th[p.mat[o + PXY]].k) * (th - theta[o + PXY]), lap);
+    theta_d[o] = th - p.dt * me.irc * lap;
 }
 
 // sigma = sigma_0 / (1 + alpha theta) on every cell (after em_set_thermal / em_set_temperature_rise / em_reset)

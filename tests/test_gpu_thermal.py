@@ -22,8 +22,11 @@ def _coupled(dims, seed, k_scale=2.0e5, tcr_scale=1.0e4, **kw):
     return p
 
 
-def _run(p, steps, precision, checkpoints=()):
-    g = P.EM(p, precision=precision)
+STRATEGIES = [pytest.param(P.EM_KERNEL_AUTO, id="coupled-sweep"), pytest.param(P.EM_KERNEL_SPLIT, id="split")]
+
+
+def _run(p, steps, precision, checkpoints=(), kernel=P.EM_KERNEL_AUTO):
+    g = P.EM(p, precision=precision, kernel=kernel)
     o = emo.Oracle(p)
     tol = TOL[precision]
     done = 0
@@ -42,18 +45,27 @@ CASES = [((37, 29, 23), LOSS_CD), ((9, 7, 6), LOSS_CD), ((130, 3, 2), LOSS_CD), 
          ((37, 29, 23), LOSS_EXP), ((9, 7, 6), LOSS_EXP)]     # EXP on the non-degenerate grids, as in test_gpu_parity.py
 
 
+@pytest.mark.parametrize("kernel", STRATEGIES)
 @pytest.mark.parametrize("precision", [64, 32])
 @pytest.mark.parametrize("dims,mode", CASES)
-def test_coupled_random_grids(dims, mode, precision):
+def test_coupled_random_grids(dims, mode, precision, kernel):
     p = _coupled(dims, 8000 + sum(dims), loss_mode=mode, steps=60, n_ports=3, init_scale=4.0e6)
-    res, theta = _run(p, 60, precision, checkpoints=(1, 10))
+    res, theta = _run(p, 60, precision, checkpoints=(1, 10), kernel=kernel)
     # the feedback is not a perturbation below the tolerance: alpha * theta reaches the per-cent range
     assert (p.thermal[p.mat_id, 2] * theta).max() > 1e-3
 
 
-def test_coupled_with_pmc_walls_and_wall_port():
-    p = _coupled((21, 18, 12), 8101, steps=40, n_ports=4, init_scale=4.0e6, bc=(1, 1, 0, 1, 0, 1))
-    _run(p, 40, 64, checkpoints=(1,))
+@pytest.mark.parametrize("kernel", STRATEGIES)
+def test_coupled_with_pmc_walls_and_wall_port(kernel):
+    p = _coupled((21, 18, 12), 8101, steps=40, n_ports=4, init_scale=4.0e6, bc=(1, 1, 0, 1, 1, 1))
+    _run(p, 40, 64, checkpoints=(1,), kernel=kernel)
+
+
+@pytest.mark.parametrize("zsplit", [1, 3, 8])
+def test_coupled_sweep_z_chunks(zsplit, monkeypatch):
+    monkeypatch.setenv("EM_FUSED_ZSPLIT", str(zsplit))
+    p = _coupled((21, 18, 33), 8104, steps=30, n_ports=40, init_scale=4.0e6)
+    _run(p, 30, 64, checkpoints=(1, 7))
 
 
 def test_pure_diffusion_and_set_get_temperature():
@@ -61,8 +73,8 @@ def test_pure_diffusion_and_set_get_temperature():
     p.init = None
     rng = np.random.default_rng(9)
     th0 = rng.uniform(0.0, 1.0, size=(p.nz, p.ny, p.nx))
-    for precision in (64, 32):
-        g = P.EM(p, precision=precision); o = emo.Oracle(p)
+    for precision, kernel in ((64, P.EM_KERNEL_AUTO), (32, P.EM_KERNEL_AUTO), (64, P.EM_KERNEL_SPLIT)):
+        g = P.EM(p, precision=precision, kernel=kernel); o = emo.Oracle(p)
         g.em_set_temperature_rise(th0); o.set_temperature_rise(th0)
         assert rel_l2([g.em_get_temperature_rise()], [th0]) <= (0 if precision == 64 else 1e-7)
         g.em_step(30); o.step(30)
@@ -81,9 +93,10 @@ def test_coupled_config4_scaled():
     p.thermal = W.thermal_table()
     for precision in (64, 32):
         _run(p, 80, precision)
+    _run(p, 80, 32, kernel=P.EM_KERNEL_SPLIT)
 
 
-def test_thermal_needs_flag_and_split_strategy():
+def test_thermal_needs_flag_and_a_coupled_strategy():
     p = W.random_problem(6, 5, 4, seed=8103, n_ports=0)
     g = P.EM(p)
     with pytest.raises(P.EMError):
@@ -93,4 +106,4 @@ def test_thermal_needs_flag_and_split_strategy():
     g.close()
     p.thermal = W.thermal_table()
     with pytest.raises(P.EMError):
-        P.EM(p, kernel=P.EM_KERNEL_TMA)                       # the sweeps take sigma from the table
+        P.EM(p, kernel=P.EM_KERNEL_FUSED)                     # the cp.async sweep takes sigma from the table only
