@@ -754,7 +754,11 @@ template <typename R>
 int32_t Ctx<R>::step_thermal_sweep() {
     dim3 b(32, 8);
     R *th_in = c.theta[th_cur] + g.origin, *th_out = c.theta[1 - th_cur] + g.origin;
-    em::k_diffuse<R><<<node_grid(b, 0), b, 0, stream>>>(p, c.ttable, th_in, th_out);
+    {
+        constexpr int V = 16 / (int)sizeof(R);
+        dim3 gd(((g.nx + V - 1) / V + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, g.nz);
+        em::k_diffuse<R><<<gd, b, 0, stream>>>(p, c.ttable, th_in, th_out);
+    }
     launches += 1;
     int32_t rc = record_begin(); if (rc) return rc;
     em::FusedSources fsrc{c.tile_sbeg, c.tile_ent};

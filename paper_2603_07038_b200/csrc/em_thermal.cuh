@@ -10,6 +10,7 @@
 // an array of the common padded geometry (0 in the pad), so the E update gathers it exactly like the table's sigma.
 #pragma once
 #include "em_split.cuh"
+#include <type_traits>
 
 namespace em {
 
@@ -143,33 +144,61 @@ __global__ void __launch_bounds__(256) k_joule_thermal(DevParams<R> p, ThermalPa
 }
 
 // Conduction half of eq. (5) for the coupled sweep: theta_d = theta^n - dt/(rho c_p) (M_kk theta^n), all cells, into the
-// other theta buffer (the sweep then adds the Joule heat of the step in place).
+// other theta buffer (the sweep then adds the Joule heat of the step in place).  A thread owns V = 16 B / sizeof(R)
+// consecutive cells in x: 128-bit loads of the centre, the +-y and +-z neighbour vectors, V + 1 x-face conductances
+// shared between neighbouring cells.  Vectors past nx only touch pad cells (k = 0, theta = 0) and are not stored.
 template <typename R>
 __global__ void __launch_bounds__(256) k_diffuse(DevParams<R> p, const ThEntry<R> *ttable, const R *theta, R *theta_d) {
+    constexpr int V = 16 / sizeof(R);
+    struct alignas(16) VR { R v[V]; };
     __shared__ ThEntry<R> s_th[kMaxTable];
     {
         const int tid = threadIdx.y * blockDim.x + threadIdx.x, nth = blockDim.x * blockDim.y;
         for (int m = tid; m < p.n_table; m += nth) s_th[m] = ttable[m];
         __syncthreads();
     }
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
-    if (i >= p.nx || j >= p.ny) return;
+    if (i0 >= p.nx || j >= p.ny) return;
     const long long PX = p.PX, PXY = p.PXY;
-    const long long o = ((long long)k * p.PY + j) * PX + i;
-    const ThEntry<R> me = s_th[p.mat[o]];
-    const R th = theta[o];
-    const R rdx = p.rdx[i], rdy = p.rdy[j], rdz = p.rdz[k];
-    const R gx = rdx * me.k, gy = rdy * me.k, gz = rdz * me.k;
-    R lap = R(0);
-    lap = mad(rdx, half_cell_cond(gx, p.rdx[i - 1] * s_th[p.mat[o - 1]].k) * (th - theta[o - 1]), lap);
-    lap = mad(rdx, half_cell_cond(gx, p.rdx[i + 1] * s_th[p.mat[o + 1]].k) * (th - theta[o + 1]), lap);
-    lap = mad(rdy, half_cell_cond(gy, p.rdy[j - 1] * s_th[p.mat[o - PX]].k) * (th - theta[o - PX]), lap);
-    lap = mad(rdy, half_cell_cond(gy, p.rdy[j + 1] * s_th[p.mat[o + PX]].k) * (th - theta[o + PX]), lap);
-    lap = mad(rdz, half_cell_cond(gz, p.rdz[k - 1] * s_th[p.mat[o - PXY]].k) * (th - theta[o - PXY]), lap);
-    lap = mad(rdz, half_cell_cond(gz, p.rdz[k + 1] * s_th[p.mat[o + PXY]].k) * (th - theta[o + PXY]), lap);
-    theta_d[o] = th - p.dt * me.irc * lap;
+    const long long o = ((long long)k * p.PY + j) * PX + i0;
+    auto ldv = [&](long long off) -> VR { return *reinterpret_cast<const VR *>(theta + off); };
+    const VR th = ldv(o), tym = ldv(o - PX), typ = ldv(o + PX), tzm = ldv(o - PXY), tzp = ldv(o + PXY);
+    const R txm = theta[o - 1], txp = theta[o + V];
+    const R rdy = p.rdy[j], rdz = p.rdz[k];
+    const R rdym = p.rdy[j - 1], rdyp = p.rdy[j + 1], rdzm = p.rdz[k - 1], rdzp = p.rdz[k + 1];
+    // the V material ids of a vector as one aligned word (i0 is a multiple of V and the array origin is 128-B aligned)
+    using IdT = typename std::conditional<V == 4, unsigned, unsigned short>::type;
+    auto ldid = [&](long long off) -> unsigned { return *reinterpret_cast<const IdT *>(p.mat + off); };
+    const unsigned idc = ldid(o), idym = ldid(o - PX), idyp = ldid(o + PX), idzm = ldid(o - PXY), idzp = ldid(o + PXY);
+    R kc[V + 2], rdx[V + 2];                                  // cells i0-1 .. i0+V
+    kc[0] = s_th[p.mat[o - 1]].k; kc[V + 1] = s_th[p.mat[o + V]].k;
+#pragma unroll
+    for (int c = 0; c < V; ++c) kc[c + 1] = s_th[(idc >> (8 * c)) & 0xff].k;
+#pragma unroll
+    for (int c = 0; c < V + 2; ++c) rdx[c] = p.rdx[i0 + c - 1];
+    R gxf[V + 1];                                             // x faces between cells c-1 and c (c = 0 .. V)
+#pragma unroll
+    for (int c = 0; c < V + 1; ++c) gxf[c] = half_cell_cond(rdx[c] * kc[c], rdx[c + 1] * kc[c + 1]);
+    VR out;
+#pragma unroll
+    for (int c = 0; c < V; ++c) {
+        const R kme = kc[c + 1], t0 = th.v[c];
+        const R gy = rdy * kme, gz = rdz * kme;
+        const R tl = c > 0 ? th.v[c > 0 ? c - 1 : 0] : txm, tr = c < V - 1 ? th.v[c < V - 1 ? c + 1 : c] : txp;
+        R lap = rdx[c + 1] * (gxf[c] * (t0 - tl) + gxf[c + 1] * (t0 - tr));
+        lap = mad(rdy, half_cell_cond(gy, rdym * s_th[(idym >> (8 * c)) & 0xff].k) * (t0 - tym.v[c]), lap);
+        lap = mad(rdy, half_cell_cond(gy, rdyp * s_th[(idyp >> (8 * c)) & 0xff].k) * (t0 - typ.v[c]), lap);
+        lap = mad(rdz, half_cell_cond(gz, rdzm * s_th[(idzm >> (8 * c)) & 0xff].k) * (t0 - tzm.v[c]), lap);
+        lap = mad(rdz, half_cell_cond(gz, rdzp * s_th[(idzp >> (8 * c)) & 0xff].k) * (t0 - tzp.v[c]), lap);
+        out.v[c] = t0 - p.dt * s_th[(idc >> (8 * c)) & 0xff].irc * lap;
+    }
+    if (i0 + V <= p.nx) {
+        *reinterpret_cast<VR *>(theta_d + o) = out;
+    } else {
+        for (int c = 0; c < V && i0 + c < p.nx; ++c) theta_d[o + c] = out.v[c];
+    }
 }
 
 // sigma = sigma_0 / (1 + alpha theta) on every cell (after em_set_thermal / em_set_temperature_rise / em_reset)
