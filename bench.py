@@ -128,6 +128,8 @@ def cpu_oracle_rate(args, seconds: float):
     scale = max(args.scale, 4) if args.config in (3, 4, 5) else 1
     kw = {"steps": 64} if args.config != 1 else {}
     p = W.make_config(args.config, scale=scale, **kw) if args.config != 1 else W.make_config(1)
+    if getattr(args, "thermal", False):
+        p.thermal = W.thermal_table(p.table.shape[0])
     o = emo.Oracle(p)
     o.step(1)                                        # warm the pages
     t0 = time.perf_counter(); n = 0
@@ -137,7 +139,8 @@ def cpu_oracle_rate(args, seconds: float):
         if el >= seconds or n >= 60:
             break
     rate = p.n_cells * n / el
-    sample = "%s at %dx%dx%d cells (scale 1/%d in x,y), %d steps, fp64" % (p.name, p.nx, p.ny, p.nz, scale, n)
+    sample = "%s at %dx%dx%d cells (scale 1/%d in x,y), %d steps, fp64%s" % (
+        p.name, p.nx, p.ny, p.nz, scale, n, ", thermal coupling on" if getattr(args, "thermal", False) else "")
     # the same oracle on ONE thread (2 steps), for the single-core figure SURVEY.md 8(d) asks for
     emo.set_threads(1)
     t1 = time.perf_counter(); o.step(2)
