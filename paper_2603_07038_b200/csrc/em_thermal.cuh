@@ -172,8 +172,31 @@ __global__ void __launch_bounds__(256) k_diffuse(DevParams<R> p, const ThEntry<R
     using IdT = typename std::conditional<V == 4, unsigned, unsigned short>::type;
     auto ldid = [&](long long off) -> unsigned { return *reinterpret_cast<const IdT *>(p.mat + off); };
     const unsigned idc = ldid(o), idym = ldid(o - PX), idyp = ldid(o + PX), idzm = ldid(o - PXY), idzp = ldid(o + PXY);
+    const unsigned idl = p.mat[o - 1], idr = p.mat[o + V];
+    // One material over the whole 7-point neighbourhood of the vector (the common case): the series conductance of two
+    // equal half cells is k * 2/(d + d') = k / d~, i.e. k times the dual-length reciprocals the E update already uses.
+    const unsigned rep_id = (idc & 0xffu) * (V == 4 ? 0x01010101u : 0x0101u);
+    if (idc == rep_id && idym == rep_id && idyp == rep_id && idzm == rep_id && idzp == rep_id &&
+        idl == (idc & 0xffu) && idr == (idc & 0xffu) && i0 + V <= p.nx) {
+        const ThEntry<R> me = s_th[idc & 0xffu];
+        const R cy0 = rdy * p.rty[j], cy1 = rdy * p.rty[j + 1], cz0 = rdz * p.rtz[k], cz1 = rdz * p.rtz[k + 1];
+        const R scale = p.dt * me.irc * me.k;
+        VR out;
+#pragma unroll
+        for (int c = 0; c < V; ++c) {
+            const R t0 = th.v[c];
+            const R tl = c > 0 ? th.v[c > 0 ? c - 1 : 0] : txm, tr = c < V - 1 ? th.v[c < V - 1 ? c + 1 : c] : txp;
+            const R rdxc = p.rdx[i0 + c];
+            R lap = rdxc * (p.rtx[i0 + c] * (t0 - tl) + p.rtx[i0 + c + 1] * (t0 - tr));
+            lap = mad(cy0, t0 - tym.v[c], lap); lap = mad(cy1, t0 - typ.v[c], lap);
+            lap = mad(cz0, t0 - tzm.v[c], lap); lap = mad(cz1, t0 - tzp.v[c], lap);
+            out.v[c] = mad(-scale, lap, t0);
+        }
+        *reinterpret_cast<VR *>(theta_d + o) = out;
+        return;
+    }
     R kc[V + 2], rdx[V + 2];                                  // cells i0-1 .. i0+V
-    kc[0] = s_th[p.mat[o - 1]].k; kc[V + 1] = s_th[p.mat[o + V]].k;
+    kc[0] = s_th[idl].k; kc[V + 1] = s_th[idr].k;
 #pragma unroll
     for (int c = 0; c < V; ++c) kc[c + 1] = s_th[(idc >> (8 * c)) & 0xff].k;
 #pragma unroll
