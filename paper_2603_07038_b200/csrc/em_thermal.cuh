@@ -151,12 +151,7 @@ template <typename R>
 __global__ void __launch_bounds__(256) k_diffuse(DevParams<R> p, const ThEntry<R> *ttable, const R *theta, R *theta_d) {
     constexpr int V = 16 / sizeof(R);
     struct alignas(16) VR { R v[V]; };
-    __shared__ ThEntry<R> s_th[kMaxTable];
-    {
-        const int tid = threadIdx.y * blockDim.x + threadIdx.x, nth = blockDim.x * blockDim.y;
-        for (int m = tid; m < p.n_table; m += nth) s_th[m] = ttable[m];
-        __syncthreads();
-    }
+    const ThEntry<R> *s_th = ttable;       // a few 16/32-B entries: read through L1, no shared-memory copy and no barrier
     const int i0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = blockIdx.z;
@@ -181,13 +176,15 @@ __global__ void __launch_bounds__(256) k_diffuse(DevParams<R> p, const ThEntry<R
         const ThEntry<R> me = s_th[idc & 0xffu];
         const R cy0 = rdy * p.rty[j], cy1 = rdy * p.rty[j + 1], cz0 = rdz * p.rtz[k], cz1 = rdz * p.rtz[k + 1];
         const R scale = p.dt * me.irc * me.k;
+        const VR rdxv = *reinterpret_cast<const VR *>(p.rdx + i0), rtxv = *reinterpret_cast<const VR *>(p.rtx + i0);
+        const R rtxe = p.rtx[i0 + V];
         VR out;
 #pragma unroll
         for (int c = 0; c < V; ++c) {
             const R t0 = th.v[c];
             const R tl = c > 0 ? th.v[c > 0 ? c - 1 : 0] : txm, tr = c < V - 1 ? th.v[c < V - 1 ? c + 1 : c] : txp;
-            const R rdxc = p.rdx[i0 + c];
-            R lap = rdxc * (p.rtx[i0 + c] * (t0 - tl) + p.rtx[i0 + c + 1] * (t0 - tr));
+            const R rtx1 = c < V - 1 ? rtxv.v[c < V - 1 ? c + 1 : c] : rtxe;
+            R lap = rdxv.v[c] * (rtxv.v[c] * (t0 - tl) + rtx1 * (t0 - tr));
             lap = mad(cy0, t0 - tym.v[c], lap); lap = mad(cy1, t0 - typ.v[c], lap);
             lap = mad(cz0, t0 - tzm.v[c], lap); lap = mad(cz1, t0 - tzp.v[c], lap);
             out.v[c] = mad(-scale, lap, t0);
