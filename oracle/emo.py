@@ -17,13 +17,29 @@ _SRC = os.path.join(_HERE, "em_oracle.c")
 _LIB = os.path.join(_HERE, "libemo.so")
 
 
+_SRC2 = os.path.join(_HERE, "em_oracle_eonly.c")
+_LIB2 = os.path.join(_HERE, "libemo_eonly.so")
+# EMO_SANITIZE=1: both oracles built with -fsanitize=address,undefined into separate files (run the CPU pins with
+# LD_PRELOAD=$(gcc -print-file-name=libasan.so))
+_SAN = os.environ.get("EMO_SANITIZE", "") == "1"
+if _SAN:
+    _LIB, _LIB2 = _LIB.replace(".so", "_san.so"), _LIB2.replace(".so", "_san.so")
+
+
+def _gcc(src: str, lib: str, force: bool) -> str:
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
+        cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off"]
+        if _SAN:
+            cmd += ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+        subprocess.check_call(cmd + ["-o", lib, src, "-lm"])
+    return lib
+
+
 def build(force: bool = False) -> str:
-    """gcc -O2 -fopenmp -shared; rebuilt when the source is newer than the library."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-fPIC", "-shared", "-ffp-contract=off",
-               "-o", _LIB, _SRC, "-lm"]
-        subprocess.check_call(cmd)
-    return _LIB
+    """gcc -O2 -fopenmp -shared of both oracles (the E/H leapfrog and the literal E-only recurrence of eq. (2));
+    rebuilt when a source is newer than its library.  Returns the path of the leapfrog oracle."""
+    _gcc(_SRC2, _LIB2, force)
+    return _gcc(_SRC, _LIB, force)
 
 
 class _Grid(C.Structure):
@@ -234,3 +250,137 @@ class Oracle:
     @property
     def step_index(self) -> int:
         return int(lib().emo_step_index(self._h))
+
+
+# =====================================================================================================================
+_lib2 = None
+
+
+def lib_eonly():
+    global _lib2
+    if _lib2 is None:
+        build()
+        _lib2 = C.CDLL(_LIB2)
+        _lib2.emo2_step_index.restype = C.c_int64
+    return _lib2
+
+
+class OracleEOnly:
+    """fp64 CPU oracle of the paper's literal E-only three-level recurrence, eq. (2)-(3) (oracle/em_oracle_eonly.c;
+    NEXT-4 of SURVEY.md 8(f)).  State: e^n (level 0) and e^{n-1} (level 1); p.init entries 0..2 set e^0, entries
+    "m0".."m2" (or the argument e_prev) set e^{-1}."""
+
+    def __init__(self, p, load_sources: bool = True, load_init: bool = True, e_prev=None):
+        self.nx, self.ny, self.nz = int(p.nx), int(p.ny), int(p.nz)
+        self.shapes = _shapes(self.nx, self.ny, self.nz)[:3]
+        self._dx = np.ascontiguousarray(p.dx, np.float64)
+        self._dy = np.ascontiguousarray(p.dy, np.float64)
+        self._dz = np.ascontiguousarray(p.dz, np.float64)
+        mat = np.ascontiguousarray(p.mat_id, np.uint8)
+        assert mat.shape == (self.nz, self.ny, self.nx)
+        g = _mk_grid(self.nx, self.ny, self.nz, self._dx, self._dy, self._dz, int(p.loss_mode),
+                     tuple(getattr(p, "bc", (0,) * 6)))
+        tab = _mk_table(p.table, p.flags)
+        self._h = C.c_void_p()
+        rc = lib_eonly().emo2_create(C.byref(g), mat.ctypes.data_as(C.c_void_p), tab, p.table.shape[0],
+                                     C.c_double(p.dt), C.byref(self._h))
+        if rc:
+            raise RuntimeError("emo2_create rc=%d" % rc)
+        if load_sources and p.n_ports > 0:
+            self.set_source(p)
+        if load_init and p.init:
+            for comp, arr in p.init.items():
+                if comp in (0, 1, 2):
+                    self.set_field(0, comp, arr)
+        if e_prev is not None:
+            for comp in range(3):
+                self.set_field(1, comp, e_prev[comp])
+
+    def close(self):
+        if self._h:
+            lib_eonly().emo2_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_source(self, p):
+        np_ = p.n_ports
+        ports = (_Port * max(np_, 1))()
+        for q in range(np_):
+            ports[q].edge_begin = int(p.port_edge_begin[q]); ports[q].edge_end = int(p.port_edge_end[q])
+            ports[q].amplitude = float(p.port_amplitude[q])
+            ports[q].wave_offset = int(p.port_wave_offset[q]); ports[q].wave_len = int(p.port_wave_len[q])
+        ne = int(p.edge_comp.shape[0])
+        edges = (_Edge * max(ne, 1))()
+        for e in range(ne):
+            edges[e].comp = int(p.edge_comp[e])
+            edges[e].i, edges[e].j, edges[e].k = (int(v) for v in p.edge_ijk[e])
+            edges[e].weight = float(p.edge_weight[e])
+        wave = np.ascontiguousarray(p.wave, np.float64)
+        rc = lib_eonly().emo2_set_source(self._h, np_, ports, edges, C.c_int64(ne), _dp(wave), C.c_int64(wave.shape[0]))
+        if rc:
+            raise RuntimeError("emo2_set_source rc=%d" % rc)
+
+    def set_field(self, level: int, comp: int, arr):
+        a = np.ascontiguousarray(arr, np.float64)
+        assert a.shape == self.shapes[comp], (a.shape, self.shapes[comp])
+        rc = lib_eonly().emo2_set_field(self._h, int(level), int(comp), _dp(a))
+        if rc:
+            raise RuntimeError("emo2_set_field rc=%d" % rc)
+
+    def get_field(self, level: int, comp: int) -> np.ndarray:
+        out = np.empty(self.shapes[comp], np.float64)
+        rc = lib_eonly().emo2_get_field(self._h, int(level), int(comp), _dp(out))
+        if rc:
+            raise RuntimeError("emo2_get_field rc=%d" % rc)
+        return out
+
+    def fields(self, level: int = 0):
+        return [self.get_field(level, c) for c in range(3)]
+
+    def step(self, n: int = 1):
+        rc = lib_eonly().emo2_step(self._h, C.c_int64(n))
+        if rc:
+            raise RuntimeError("emo2_step rc=%d" % rc)
+
+    def joule(self, power: bool = True, energy: bool = True, total: bool = True, reset: bool = False):
+        ncell = (self.nz, self.ny, self.nx)
+        p = np.empty(ncell, np.float64) if power else None
+        q = np.empty(ncell, np.float64) if energy else None
+        t = C.c_double()
+        rc = lib_eonly().emo2_joule(self._h, _dp(p) if power else None, _dp(q) if energy else None,
+                                    C.byref(t) if total else None, int(reset))
+        if rc:
+            raise RuntimeError("emo2_joule rc=%d" % rc)
+        return p, q, (t.value if total else None)
+
+    def probe(self, pts) -> np.ndarray:
+        pts = np.asarray(pts, np.int32).reshape(-1, 4)
+        arr = (_ProbePt * max(len(pts), 1))()
+        for n, (c, i, j, k) in enumerate(pts):
+            arr[n].comp, arr[n].i, arr[n].j, arr[n].k = int(c), int(i), int(j), int(k)
+        out = np.empty(len(pts), np.float64)
+        rc = lib_eonly().emo2_probe(self._h, len(pts), arr, _dp(out))
+        if rc:
+            raise RuntimeError("emo2_probe rc=%d" % rc)
+        return out
+
+    def reset(self):
+        lib_eonly().emo2_reset(self._h)
+
+    def set_step_index(self, n: int):
+        rc = lib_eonly().emo2_set_step_index(self._h, C.c_int64(int(n)))
+        if rc:
+            raise RuntimeError("emo2_set_step_index rc=%d" % rc)
+
+    @property
+    def step_index(self) -> int:
+        return int(lib_eonly().emo2_step_index(self._h))
+
+
+def set_threads_eonly(n: int) -> int:
+    return int(lib_eonly().emo2_set_threads(int(n)))

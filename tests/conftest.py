@@ -11,9 +11,15 @@ sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+    config.addinivalue_line("markers", "slow: minutes of host-side oracle time per test; runs only with EM_RUN_SLOW=1")
 
 
 def pytest_collection_modifyitems(config, items):
+    if os.environ.get("EM_RUN_SLOW", "") != "1":
+        slow = pytest.mark.skip(reason="slow: set EM_RUN_SLOW=1")
+        for it in items:
+            if "slow" in it.keywords:
+                it.add_marker(slow)
     try:
         import torch
         has_gpu = torch.cuda.is_available()

@@ -15,18 +15,36 @@ def rel_l2(got, want):
     return (num / den) ** 0.5
 
 
+def max_norm_err(got, want):
+    """max |got - want| over a list of arrays / max |want| over the same list (the group's max-norm); 0/0 -> 0.
+    A single wrong edge on a tile or chunk seam is invisible in a whole-field rel-L2 but not here."""
+    num = den = 0.0
+    for g, w in zip(got, want):
+        w = np.asarray(w, np.float64)
+        step = max(1, (1 << 24) // max(1, int(np.prod(w.shape[1:]))))       # slabs of <= 16 M values
+        for k in range(0, w.shape[0], step):
+            num = max(num, float(np.max(np.abs(np.asarray(g[k:k + step], np.float64) - w[k:k + step]), initial=0.0)))
+            den = max(den, float(np.max(np.abs(w[k:k + step]), initial=0.0)))
+    if den == 0.0:
+        return 0.0 if num == 0.0 else float("inf")
+    return num / den
+
+
 def compare_state(gpu, orc, tol, check_zero_groups=True):
     """gpu: paper_2603_07038_b200.EM, orc: oracle.emo.Oracle, both after the same number of steps.
-    Returns dict of the four parity numbers and asserts them."""
+    Returns dict of the parity numbers (rel-L2 per group and the max-abs-diff / max-norm beside each) and asserts them."""
     Fg, Fo = gpu.fields(), orc.fields()
     eE = rel_l2(Fg[:3], Fo[:3]); eH = rel_l2(Fg[3:], Fo[3:])
+    mE = max_norm_err(Fg[:3], Fo[:3]); mH = max_norm_err(Fg[3:], Fo[3:])
     pg, qg, Qg = gpu.joule_maps()
     po, qo, Qo = orc.joule()
     eq = rel_l2([qg], [qo]); ep = rel_l2([pg], [po])
+    mq = max_norm_err([qg], [qo])
     eQ = abs(Qg - Qo) / abs(Qo) if Qo != 0 else abs(Qg)
-    res = dict(E=eE, H=eH, q=eq, p=ep, Q=eQ)
+    res = dict(E=eE, H=eH, q=eq, p=ep, Q=eQ, Emax=mE, Hmax=mH, qmax=mq)
     assert eE <= tol and eH <= tol, res
     assert eq <= tol and eQ <= tol and ep <= 2 * tol, res
+    assert mE <= tol and mH <= tol and mq <= tol, res     # max |diff| / max |field|: a wrong seam edge shows here
     if check_zero_groups:      # components identically zero in the oracle stay (relatively) zero
         for grp in (range(0, 3), range(3, 6)):
             mx = max(float(np.max(np.abs(Fo[c]))) for c in grp)

@@ -1,0 +1,109 @@
+"""Parity at the STATED size for the STATED step count (BASELINE.json north_star: "oracle-matching fields and Joule maps
+for all five configs ... after the stated step count"): configs 3 (fp32 and fp64, 2000 steps), 4 (1000 steps, the Joule
+maps compared at each of the ten outputs) and 5 (1000 steps), whole field, against the fp64 oracle on the host cores.
+
+The oracle needs minutes per config (0.4 G cell-updates/s on 16 cores: config 3 ~3 min, 4 ~8 min, 5 ~6 min) and ~40 GB of
+host memory for config 4, so these tests are marked `slow` and run only with EM_RUN_SLOW=1:
+
+    EM_RUN_SLOW=1 python -m pytest tests/test_gpu_full_parity.py -m gpu -x -q -s
+
+Each test appends one JSON line with its numbers (rel-L2 of E, H, q, |dQ|/Q and max-abs-diff / max-norm per component)
+to gpurun_out/full_parity.jsonl; profiles/r2_full_parity.md is a copy of those lines from a gpurun call.
+Metric: SURVEY.md 8(c) C16; equations PAPER.md L69-L76 eq. (2)-(3), Joule heat L86.
+"""
+import json
+import os
+import time
+
+import numpy as np
+import pytest
+
+import workloads as W
+import paper_2603_07038_b200 as P
+from oracle import emo
+from parity import TOL, max_norm_err, rel_l2
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+NAMES = ("Ex", "Ey", "Ez", "Hx", "Hy", "Hz")
+
+
+def _record(rec):
+    out = os.path.join(ROOT, "gpurun_out")
+    os.makedirs(out, exist_ok=True)
+    with open(os.path.join(out, "full_parity.jsonl"), "a") as f:
+        f.write(json.dumps(rec) + "\n")
+    print(json.dumps(rec), flush=True)
+
+
+def _joule_numbers(g, o):
+    """rel-L2 and max-norm error of the q and p maps and the relative error of the total, GPU g vs oracle o"""
+    pg, qg, Qg = g.joule_maps()
+    po, qo, Qo = o.joule()
+    return dict(q=rel_l2([qg], [qo]), qmax=max_norm_err([qg], [qo]), p=rel_l2([pg], [po]),
+                Q=abs(Qg - Qo) / abs(Qo) if Qo != 0 else abs(Qg), Q_oracle=Qo)
+
+
+def _field_numbers(g, o):
+    res = {}
+    Fo = o.fields()
+    grp_max = [max(float(np.max(np.abs(Fo[c]))) for c in grp) for grp in ((0, 1, 2), (3, 4, 5))]
+    num = [0.0, 0.0]; den = [0.0, 0.0]
+    for c in range(6):
+        fg = g.em_get_field(c)
+        d = np.asarray(fg, np.float64); d -= Fo[c]
+        num[c // 3] += float(np.sum(d * d)); den[c // 3] += float(np.sum(Fo[c] * Fo[c]))
+        res[NAMES[c] + "_max"] = float(np.max(np.abs(d))) / grp_max[c // 3]      # max |diff| / max-norm of the group
+        del d, fg
+    res["E"] = (num[0] / den[0]) ** 0.5; res["H"] = (num[1] / den[1]) ** 0.5
+    return res
+
+
+def _run(cfg, precisions, steps, outputs_every=0, **kw):
+    t0 = time.time()
+    p = W.make_config(cfg, steps=steps, **kw)
+    assert p.steps == steps
+    threads = emo.set_threads(os.cpu_count() or 1)
+    o = emo.Oracle(p)
+    gs = {pr: P.EM(p, precision=pr, kernel=P.EM_KERNEL_AUTO) for pr in precisions}
+    rec = {"config": cfg, "name": p.name, "cells": [p.nx, p.ny, p.nz], "steps": steps, "oracle_threads": threads,
+           "ports": p.n_ports, "outputs": []}
+    done = 0
+    chunk = outputs_every or steps
+    while done < steps:
+        n = min(chunk, steps - done)
+        for g in gs.values():
+            g.em_step(n)
+        o.step(n); done += n
+        if outputs_every:                         # config 4: Joule map output every 100 steps, each compared
+            for pr, g in gs.items():
+                jn = _joule_numbers(g, o)
+                rec["outputs"].append({"step": done, "precision": pr, **jn})
+                assert jn["q"] <= TOL[pr] and jn["Q"] <= TOL[pr] and jn["qmax"] <= TOL[pr] and jn["p"] <= 2 * TOL[pr], (done, jn)
+    rec["oracle_seconds"] = time.time() - t0
+    for pr, g in gs.items():
+        assert g.step_index == steps
+        res = {**_field_numbers(g, o), **_joule_numbers(g, o)}
+        rec["fp%d" % pr] = res
+        _record({"partial": "fp%d" % pr, "config": cfg, **res})     # (kept even if a later assert fails)
+        tol = TOL[pr]
+        assert res["E"] <= tol and res["H"] <= tol and res["q"] <= tol and res["Q"] <= tol, res
+        assert all(res[n + "_max"] <= tol for n in NAMES) and res["qmax"] <= tol, res
+        g.close()
+    o.close()
+    rec["wall_seconds"] = time.time() - t0
+    _record(rec)
+    return rec
+
+
+def test_config3_full_size_2000_steps_fp32_fp64():
+    _run(3, (32, 64), 2000)
+
+
+def test_config4_full_size_1000_steps_with_joule_outputs():
+    _run(4, (32,), 1000, outputs_every=100)
+
+
+def test_config5_full_size_1000_steps():
+    _run(5, (32,), 1000)
