@@ -58,15 +58,25 @@ extern "C" {
 
 #define EM_MAT_PEC 1 /* em_material.flags bit0: every edge touching such a cell is held at 0      */
 
-/* em_grid.kernel: kernel strategy.  AUTO picks the TMA sweep (one launch per step; E, H and id planes
- * staged by cp.async.bulk.tensor boxes counted on mbarriers; the fastest measured) and falls back to
- * FUSED when the material table is too large for its shared-memory layout; FUSED is the same sweep
- * with per-thread cp.async staging; SPLIT runs the separate H / E / Joule kernels.  All three are CUDA
- * paths of this library and are cross-checked against each other and the oracle in the tests. */
+/* em_grid.kernel: kernel strategy.  AUTO = TMA: the sweep (one launch per step; E, H and id planes staged
+ * by cp.async.bulk.tensor boxes counted on mbarriers; its shared-memory layout holds the largest material
+ * table).  SPLIT runs the separate H / E / source / Joule kernels.  Both are CUDA paths of this library and
+ * are cross-checked against each other and the oracle in the tests. */
 #define EM_KERNEL_AUTO 0
 #define EM_KERNEL_SPLIT 1
-#define EM_KERNEL_FUSED 2
-#define EM_KERNEL_TMA 3
+#define EM_KERNEL_TMA 2
+
+/* em_grid.formulation.  LEAPFROG: the E/H leapfrog (state E^n, H^{n-1/2}).  EONLY: the paper's literal
+ * three-level recurrence M e^{n+1} = N e^n - K e^{n-1} - dt^2 (dJ/dt)^n (eq. (2), L73-L76 eq. (3)):
+ * state e^n and e^{n-1}, no H array; field components 0-2 are e^n and 6-8 are e^{n-1} (3-5 do not exist:
+ * INVALID_ARG), (dJ/dt)^n dt = wave[n] - wave[n-1].  Algebraically identical to LEAPFROG from consistent
+ * states; moves 9 instead of 12 field words per cell-update, but every rounding error of e enters the
+ * difference e^n - e^{n-1} and is amplified by ~1/(omega dt): in fp32 it leaves the 2e-5 parity bound after a
+ * few hundred steps, so LEAPFROG is the default.  TMA sweep only, no thermal coupling. */
+#define EM_FORM_LEAPFROG 0
+#define EM_FORM_EONLY 1
+
+#define EM_ABI_VERSION 3 /* bumped whenever em_grid or a signature changes; em_abi_version() returns it */
 
 typedef struct em_ctx em_ctx; /* opaque, host-side */
 
@@ -81,7 +91,11 @@ typedef struct em_grid {
     int64_t max_source_edges;
     int64_t max_wave_samples;
     int32_t thermal;             /* 1: reserve workspace for the thermal stage (em_set_thermal): AUTO / TMA run */
-    int32_t pad_;                /*    the coupled TMA sweep, SPLIT the split kernels; FUSED -> EM_ERR_UNSUPPORTED */
+                                 /*    the coupled TMA sweep, SPLIT the split kernels                            */
+    int32_t formulation;         /* EM_FORM_LEAPFROG or EM_FORM_EONLY                                            */
+    int32_t z_chunks;            /* 0: the library chooses how many z chunks a tile column is cut into (work     */
+                                 /* items = tiles x chunks, from the SM count); 1..8 forces it (tests, tuning)   */
+    int32_t pad_;
 } em_grid;
 
 typedef struct em_material { double eps, mu, sigma; int32_t flags; int32_t pad_; } em_material;
@@ -94,8 +108,12 @@ typedef struct em_port { int64_t edge_begin, edge_end; double amplitude; int64_t
 typedef struct em_edge { int32_t comp /*0=x,1=y,2=z*/, i, j, k; double weight; } em_edge;
 typedef struct em_probe_pt { int32_t comp /*0..5 = Ex,Ey,Ez,Hx,Hy,Hz*/, i, j, k; } em_probe_pt;
 
-/* Thread-local description of the last error returned by any call on this thread. */
+/* Thread-local description of the last error returned by any call on this thread (thread-local rather than
+ * per-context so that a failed em_create, which has no context, can be described too). */
 const char *em_last_error(void);
+
+/* EM_ABI_VERSION of the built library: a binding compares it with the header it was written against. */
+int32_t em_abi_version(void);
 
 /* Bytes of device workspace needed for this grid (fields with padding and their ping-pong copies,
  * material ids, Joule accumulator, coefficient tables, source lists up to the max_* capacities).
@@ -106,8 +124,10 @@ int32_t em_workspace_bytes(const em_grid *g, size_t *out_bytes);
  * n_mat entries, eps > 0, mu > 0, sigma >= 0.  dt > 0 (CFL is the caller's business: em_cfl_dt).
  * workspace: DEVICE, 256-byte aligned, >= em_workspace_bytes.  stream: cudaStream_t (may be 0).
  * Zeroes fields, Joule accumulator and the step counter.  Synchronises the stream before returning
- * (the host inputs may be freed on return).
- * Errors: INVALID_ARG, WORKSPACE_TOO_SMALL, CUDA (INVALID_ARG also for an unknown bc, or a PMC wall with n_mat > 254). */
+ * (the host inputs may be freed on return).  The context belongs to the device that owns `workspace`: every
+ * call switches to it and restores the caller's current device.
+ * Errors: INVALID_ARG, WORKSPACE_TOO_SMALL, CUDA, UNSUPPORTED (INVALID_ARG also for an unknown bc, or a PMC wall
+ * with n_mat > 254; UNSUPPORTED for EONLY with SPLIT or thermal). */
 int32_t em_create(const em_grid *g, const uint8_t *mat_id, const em_material *table, int32_t n_mat,
                   double dt, void *workspace, size_t workspace_bytes, void *stream, em_ctx **out);
 
@@ -126,7 +146,8 @@ int32_t em_cfl_dt(const em_grid *g, const uint8_t *mat_id, const em_material *ta
 int32_t em_set_source(em_ctx *ctx, int32_t n_ports, const em_port *ports, const em_edge *edges,
                       int64_t n_edges, const double *wave, int64_t n_samples);
 
-/* Copy one field component (0..5 = Ex,Ey,Ez,Hx,Hy,Hz) from/to a dense array in the working
+/* Copy one field component (0..5 = Ex,Ey,Ez,Hx,Hy,Hz; EONLY contexts: 0..2 = e^n, 6..8 = e^{n-1} with the
+ * shapes of Ex,Ey,Ez) from/to a dense array in the working
  * precision.  src/dst may be a HOST (is_device = 0) or DEVICE (is_device != 0) pointer.  Tangential E
  * on PEC-fixed edges is forced to 0 on set.  Host transfers synchronise the stream. */
 int32_t em_set_field(em_ctx *ctx, int32_t comp, const void *src, int32_t src_is_device);
@@ -164,7 +185,11 @@ int32_t em_reset(em_ctx *ctx);
  *   eq. (5)  theta' = theta - dt/(rho c_p) (M_kk theta) + dq/(rho c_p),  dq = the Joule energy density of the step (a4)
  *   eq. (6)  sigma' = sigma_0 / (1 + alpha theta'), used by the next step's E update ("D_sigma(T^n)", L78)
  * M_kk = V0a^T D_k V0: cell-centred -div k grad with the series conductivity of the two half cells on each face,
- * adiabatic walls (L142).  sigma_0 = the em_material.sigma given to em_create.  em_joule's power density then uses
+ * adiabatic walls (L142).  NOTE -- a deviation from the paper's placement: the paper solves T on the mesh NODES
+ * (7 092 878 unknowns on its 376x408x45 mesh) and does not print its edge-to-node map of D_sigma e^2;
+ * here theta lives per CELL (6 903 360 unknowns on that mesh), where the Joule heat is defined (T1, T3), so
+ * the coupled numbers quoted for this library are for that cell-centred variant of eq. (4)-(5).
+ * Valid range: 1 + alpha theta > 0 (copper: theta > -256 K); below it sigma(T) is clamped at sigma_0 / 1e-6.  sigma_0 = the em_material.sigma given to em_create.  em_joule's power density then uses
  * the current sigma(T).  em_reset also zeroes theta.  Per step: one conduction kernel (theta^n -> theta - dt/(rho c_p)
  * M_kk theta) and the coupled TMA sweep (sigma(T^n) staged as one more plane per step plane, Joule heat added to theta
  * and sigma(T^{n+1}) written in its Joule phase); kernel = SPLIT runs the same step on the split kernels.  Until

@@ -14,7 +14,9 @@ import numpy as np
 
 EM_OK = 0
 EM_LOSS_CD, EM_LOSS_EXP = 0, 1
-EM_KERNEL_AUTO, EM_KERNEL_SPLIT, EM_KERNEL_FUSED, EM_KERNEL_TMA = 0, 1, 2, 3
+EM_KERNEL_AUTO, EM_KERNEL_SPLIT, EM_KERNEL_TMA = 0, 1, 2
+EM_FORM_LEAPFROG, EM_FORM_EONLY = 0, 1
+EM_ABI_VERSION = 3            # include/em.h: this binding's em_grid layout and signatures
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -31,7 +33,7 @@ class em_grid(C.Structure):
                 ("precision", C.c_int32), ("loss_mode", C.c_int32), ("bc", C.c_int32 * 6),
                 ("kernel", C.c_int32), ("max_ports", C.c_int32),
                 ("max_source_edges", C.c_int64), ("max_wave_samples", C.c_int64),
-                ("thermal", C.c_int32), ("pad_", C.c_int32)]
+                ("thermal", C.c_int32), ("formulation", C.c_int32), ("z_chunks", C.c_int32), ("pad_", C.c_int32)]
 
 
 class em_thermal_material(C.Structure):
@@ -65,15 +67,26 @@ def lib_path() -> str:
 
 
 def load():
-    """Load libem.so (building it in-tree with nvcc first if it is missing).  Raises if neither works."""
+    """Load libem.so.  With nvcc at hand the in-tree build runs first (a cheap mtime check: it recompiles only when a
+    source or header is newer than the library); without nvcc the built library must be there.  The library's ABI
+    version must be this binding's.  Raises otherwise -- there is no fallback."""
     global _lib
     if _lib is not None:
         return _lib
     path = lib_path()
-    if not os.path.exists(path):
-        from .build import build_lib
+    from .build import build_lib, have_nvcc
+    if have_nvcc():
         build_lib()
+    elif not os.path.exists(path):
+        raise RuntimeError("libem.so is missing and there is no nvcc to build it (python -m paper_2603_07038_b200.build)")
     L = C.CDLL(path)
+    try:
+        abi = int(L.em_abi_version())
+    except AttributeError:
+        abi = -1
+    if abi != EM_ABI_VERSION:
+        raise RuntimeError("libem.so has ABI version %d, this binding needs %d: rebuild it "
+                           "(python -m paper_2603_07038_b200.build --force)" % (abi, EM_ABI_VERSION))
     L.em_last_error.restype = C.c_char_p
     vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
     L.em_workspace_bytes.argtypes = [C.POINTER(em_grid), C.POINTER(C.c_size_t)]
@@ -110,7 +123,7 @@ def _dp(a: np.ndarray):
 
 
 def _mk_grid(nx, ny, nz, dx, dy, dz, precision=64, loss_mode=0, kernel=0, max_ports=0,
-             max_source_edges=0, max_wave_samples=0, bc=(0,) * 6, thermal=0) -> em_grid:
+             max_source_edges=0, max_wave_samples=0, bc=(0,) * 6, thermal=0, formulation=0, z_chunks=0) -> em_grid:
     g = em_grid()
     g.nx, g.ny, g.nz = int(nx), int(ny), int(nz)
     g.dx, g.dy, g.dz = _dp(dx), _dp(dy), _dp(dz)
@@ -119,6 +132,7 @@ def _mk_grid(nx, ny, nz, dx, dy, dz, precision=64, loss_mode=0, kernel=0, max_po
         g.bc[b] = int(bc[b])
     g.max_ports, g.max_source_edges, g.max_wave_samples = int(max_ports), int(max_source_edges), int(max_wave_samples)
     g.thermal = int(thermal)
+    g.formulation, g.z_chunks = int(formulation), int(z_chunks)
     return g
 
 
@@ -151,8 +165,8 @@ def em_cfl_dt(nx, ny, nz, dx, dy, dz, mat_id, table, flags=None) -> float:
 
 
 def _shapes(nx, ny, nz):
-    return [(nz + 1, ny + 1, nx), (nz + 1, ny, nx + 1), (nz, ny + 1, nx + 1),
-            (nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)]
+    e = [(nz + 1, ny + 1, nx), (nz + 1, ny, nx + 1), (nz, ny + 1, nx + 1)]
+    return e + [(nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)] + e     # 6..8: e^{n-1} (E-only contexts)
 
 
 class EM:
@@ -161,7 +175,8 @@ class EM:
     def __init__(self, p, precision: Optional[int] = None, kernel: int = EM_KERNEL_AUTO, device="cuda:0",
                  stream=None, bc: Optional[Sequence[int]] = None, load_sources: bool = True, load_init: bool = True,
                  max_ports: Optional[int] = None, max_source_edges: Optional[int] = None,
-                 max_wave_samples: Optional[int] = None):
+                 max_wave_samples: Optional[int] = None, formulation: int = EM_FORM_LEAPFROG, z_chunks: int = 0,
+                 e_prev=None):
         import torch
         self._torch = torch
         self._L = load()
@@ -184,7 +199,8 @@ class EM:
                               max_source_edges if max_source_edges is not None else max(n_con, 1),
                               max_wave_samples if max_wave_samples is not None else max(int(p.wave.shape[0]), 1),
                               tuple(bc) if bc is not None else tuple(getattr(p, "bc", (0,) * 6)),
-                              1 if getattr(p, "thermal", None) is not None else 0)
+                              1 if getattr(p, "thermal", None) is not None else 0, formulation, z_chunks)
+        self.formulation = int(formulation)
         nbytes = C.c_size_t()
         _check(self._L.em_workspace_bytes(C.byref(self._grid), C.byref(nbytes)))
         self.workspace_bytes = int(nbytes.value)
@@ -205,7 +221,11 @@ class EM:
             self.em_set_source(p)
         if load_init and getattr(p, "init", None):
             for comp, arr in p.init.items():
-                self.em_set_field(comp, arr)
+                if self.formulation == EM_FORM_LEAPFROG or comp < 3:     # (an E-only context has no H)
+                    self.em_set_field(comp, arr)
+        if e_prev is not None:                                          # E-only: e^{-1}
+            for comp in range(3):
+                self.em_set_field(6 + comp, e_prev[comp])
         if getattr(p, "thermal", None) is not None:
             self.em_set_thermal(p.thermal)
 
@@ -263,7 +283,9 @@ class EM:
         return a
 
     def fields(self):
-        return [self.em_get_field(c) for c in range(6)]
+        """leapfrog: Ex, Ey, Ez, Hx, Hy, Hz; E-only: e^n (3 arrays) then e^{n-1} (3 arrays)"""
+        comps = range(6) if self.formulation == EM_FORM_LEAPFROG else (0, 1, 2, 6, 7, 8)
+        return [self.em_get_field(c) for c in comps]
 
     def em_get_plane(self, comp: int, k: int, out=None):
         """device tensor [sy][sx] holding plane k of component comp"""

@@ -9,8 +9,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libem.so")
 SOURCES = ["em_lib.cu"]
-HEADERS = ["em_common.cuh", "em_split.cuh", "em_aux.cuh", "em_fused.cuh", "em_fused_phaseb.inc", "em_fused_phaseb_hom.inc", "em_sweep.cuh", "em_sweep_phaseb.inc", "em_thermal.cuh", os.path.join("..", "..", "include", "em.h")]
+HEADERS = ["em_common.cuh", "em_split.cuh", "em_aux.cuh", "em_tile.cuh", "em_sweep.cuh", "em_sweep_phaseb.inc", "em_sweep_phaseb_hom.inc", "em_thermal.cuh", os.path.join("..", "..", "include", "em.h")]
 
+
+
+def have_nvcc() -> bool:
+    return os.path.exists(os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc"))
 
 
 def _stale() -> bool:

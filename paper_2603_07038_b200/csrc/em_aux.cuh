@@ -40,9 +40,9 @@ __global__ void __launch_bounds__(256) k_pad_pmc(uint8_t *base, int nx, int ny, 
     if (beyond != 0 && (beyond & ~pmc_mask) == 0) base[t] = pmc_id;
 }
 
-// Zero E[comp] wherever the edge is PEC-fixed (mask product of its 4 cells is 0).
+// Zero the edge array `e` of direction comp wherever the edge is PEC-fixed (mask product of its 4 cells is 0).
 template <typename R>
-__global__ void __launch_bounds__(256) k_mask_fixed(DevParams<R> p, int comp, int k0) {
+__global__ void __launch_bounds__(256) k_mask_fixed(DevParams<R> p, R *e, int comp, int k0) {
     __shared__ MatEntry<R> s_tab[kMaxTable];
     load_table(s_tab, p);
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(256) k_mask_fixed(DevParams<R> p, int comp, in
     if (comp == 0)      m = s_tab[mat[o]].m * s_tab[mat[o - PX]].m * s_tab[mat[o - PXY]].m * s_tab[mat[o - PXY - PX]].m;
     else if (comp == 1) m = s_tab[mat[o]].m * s_tab[mat[o - 1]].m * s_tab[mat[o - PXY]].m * s_tab[mat[o - PXY - 1]].m;
     else                m = s_tab[mat[o]].m * s_tab[mat[o - 1]].m * s_tab[mat[o - PX]].m * s_tab[mat[o - PX - 1]].m;
-    if (m == R(0)) p.E[comp][o] = R(0);
+    if (m == R(0)) e[o] = R(0);
 }
 
 // r_e for every unique source edge; flags[u] = 1 if the edge is PEC-fixed (argument error).
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(256) k_energy_final(const double *partial, int
 }
 
 template <typename R>
-struct ProbeArrays { const R *f[6]; };
+struct ProbeArrays { const R *f[9]; };
 
 template <typename R>
 __global__ void k_probe(ProbeArrays<R> a, const long long *off, const int *comp, int n, double *out) {

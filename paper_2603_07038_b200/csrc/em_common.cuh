@@ -48,6 +48,13 @@ struct DevParams {
 // 0 (no heat, no conduction).
 template <typename R> struct alignas(4 * sizeof(R)) ThEntry { R irc, k, alpha, sigma0; };
 
+// Denominator of eq. (6), sigma(T) = sigma_0 / (1 + alpha theta), floored at 1e-6: below 1 + alpha theta = 0 the
+// formula has no meaning (include/em.h states the valid range); the floor keeps sigma finite and positive there.
+template <typename R> __device__ __forceinline__ R thermal_den(R alpha, R theta) {
+    const R d = alpha * theta + R(1);
+    return d > R(1e-6) ? d : R(1e-6);
+}
+
 // Extra arguments of the thermally coupled sweep (em_sweep.cuh, TH = true); unused otherwise.
 template <typename R>
 struct ThermalSweep {

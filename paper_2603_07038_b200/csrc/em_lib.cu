@@ -13,10 +13,10 @@
 #include "../../include/em.h"
 #include "em_aux.cuh"
 #include "em_common.cuh"
-#include "em_fused.cuh"
 #include "em_split.cuh"
 #include "em_sweep.cuh"
 #include "em_thermal.cuh"
+#include "em_tile.cuh"
 
 namespace {
 
@@ -29,6 +29,15 @@ int32_t fail(int32_t code, const std::string &msg) { g_err = msg; return code; }
         if (e_ != cudaSuccess)                                                                 \
             return fail(EM_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));      \
     } while (0)
+
+// Every entry point runs on the context's own device whatever the caller's current device is, and restores it.
+struct DeviceGuard {
+    int prev = -1; bool switched = false;
+    explicit DeviceGuard(int dev) {
+        if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 constexpr size_t kAlign = 256;
 size_t align_up(size_t v, size_t a = kAlign) { return (v + a - 1) / a * a; }
@@ -95,7 +104,9 @@ size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int
     Carver w(base);
     Carved<R> tmp;
     Carved<R> &o = c ? *c : tmp;
-    for (int a = 0; a < 12; ++a) o.field[a] = w.take<R>(g.alloc_elems);
+    // leapfrog: E, En, H, Hn (12 arrays); E-only (eq. (2)): three rotating levels of e (9 arrays)
+    const int n_field = gr.formulation == EM_FORM_EONLY ? 9 : 12;
+    for (int a = 0; a < 12; ++a) o.field[a] = a < n_field ? w.take<R>(g.alloc_elems) : nullptr;
     o.q = w.take<R>(g.alloc_elems);
     o.mat = w.take<uint8_t>(g.alloc_elems);
     o.table = w.take<em::MatEntry<R>>(em::kMaxTable);
@@ -149,6 +160,7 @@ struct em_ctx {
     Timing timing;
     const char *main_kernel = "";
     cudaStream_t stream = nullptr;
+    int device = -1;                    // the device that owns the workspace
     int32_t timing_flush();
 };
 
@@ -179,18 +191,29 @@ struct Ctx final : em_ctx {
     std::vector<uint8_t> host_mat;     // host copy of the ids (for argument checks of sources)
     int n_unique = 0, n_ports = 0;
     em::DevSources<R> src;
-    em::FusedPlan plan;
+    em::SweepPlan plan;
     bool uniform_mu = true;
+    bool eonly = false;                 // E-only three-level recurrence (em_grid.formulation = EM_FORM_EONLY)
+    em::SweepKernel<R> sweep_kernel = nullptr;
+    int n_field = 12;
 
     R *org(int a) const { return c.field[a] + g.origin; }
 
+    // leapfrog: E / En ping-pong in arrays 0-5 (e_cur), H / Hn in 6-11 (h_cur).
+    // E-only: the three levels rotate through the array triples 0-2, 3-5, 6-8: e^n = triple lvl, e^{n-1} = triple
+    // (lvl + 2) % 3 (bound to p.H: the sweep stages it in the H slots), e^{n+1} is written to triple (lvl + 1) % 3.
     void bind() {
         for (int a = 0; a < 3; ++a) {
-            p.E[a] = org(e_cur * 3 + a); p.En[a] = org((1 - e_cur) * 3 + a);
-            p.H[a] = org(6 + h_cur * 3 + a); p.Hn[a] = org(6 + (1 - h_cur) * 3 + a);
+            if (eonly) {
+                p.E[a] = org(lvl * 3 + a); p.En[a] = org(((lvl + 1) % 3) * 3 + a);
+                p.H[a] = org(((lvl + 2) % 3) * 3 + a); p.Hn[a] = nullptr;
+            } else {
+                p.E[a] = org(e_cur * 3 + a); p.En[a] = org((1 - e_cur) * 3 + a);
+                p.H[a] = org(6 + h_cur * 3 + a); p.Hn[a] = org(6 + (1 - h_cur) * 3 + a);
+            }
         }
     }
-    int e_cur = 0, h_cur = 0;
+    int e_cur = 0, h_cur = 0, lvl = 0;
 
     int32_t init(const em_grid *gr, const uint8_t *mat_id, const em_material *tab, int32_t n_mat, double dt_,
                  void *workspace, size_t ws_bytes, void *stream_);
@@ -221,23 +244,25 @@ struct Ctx final : em_ctx {
         return t;
     }
     int32_t step_split();
-    int32_t step_fused();
     int32_t step_tma();
     int32_t make_maps();
     CUtensorMap map_field[12], map_q, map_mat;   // TMA descriptors of the padded arrays (sweep boxes)
+    CUtensorMap map_prev[9];                     // E-only: the same arrays in the role of e^{n-1} (boxes of rows -1 .. TY)
     size_t sweep_smem = 0;
     void comp_dims(int comp, int *sx, int *sy, int *sz) const {
         const int nx = g.nx, ny = g.ny, nz = g.nz;
         switch (comp) {
-        case 0: *sx = nx;     *sy = ny + 1; *sz = nz + 1; break;
-        case 1: *sx = nx + 1; *sy = ny;     *sz = nz + 1; break;
-        case 2: *sx = nx + 1; *sy = ny + 1; *sz = nz;     break;
+        case 0: case 6: *sx = nx;     *sy = ny + 1; *sz = nz + 1; break;
+        case 1: case 7: *sx = nx + 1; *sy = ny;     *sz = nz + 1; break;
+        case 2: case 8: *sx = nx + 1; *sy = ny + 1; *sz = nz;     break;
         case 3: *sx = nx + 1; *sy = ny;     *sz = nz;     break;
         case 4: *sx = nx;     *sy = ny + 1; *sz = nz;     break;
         default:*sx = nx;     *sy = ny;     *sz = nz + 1; break;
         }
     }
-    R *comp_ptr(int comp) const { return comp < 3 ? p.E[comp] : p.H[comp - 3]; }
+    // components 0-2: E^n (e^n), 3-5: H^{n-1/2} (leapfrog only), 6-8: e^{n-1} (E-only only)
+    R *comp_ptr(int comp) const { return comp < 3 ? p.E[comp] : comp < 6 ? p.H[comp - 3] : p.H[comp - 6]; }
+    bool comp_ok(int comp) const { return comp >= 0 && (comp < 3 || (eonly ? (comp >= 6 && comp < 9) : comp < 6)); }
     dim3 node_grid(dim3 b, int ex) const { return dim3((g.nx + ex + b.x - 1) / b.x, (g.ny + ex + b.y - 1) / b.y, g.nz + ex); }
     int32_t record_begin();
     int32_t record_end();
@@ -251,8 +276,10 @@ int32_t validate_grid(const em_grid *g) {
     if (g->loss_mode != EM_LOSS_CD && g->loss_mode != EM_LOSS_EXP) return fail(EM_ERR_INVALID_ARG, "bad loss_mode");
     if (g->kernel < EM_KERNEL_AUTO || g->kernel > EM_KERNEL_TMA) return fail(EM_ERR_INVALID_ARG, "bad kernel strategy");
     if (g->thermal != 0 && g->thermal != 1) return fail(EM_ERR_INVALID_ARG, "thermal must be 0 or 1");
-    if (g->thermal && g->kernel == EM_KERNEL_FUSED)
-        return fail(EM_ERR_UNSUPPORTED, "thermal coupling runs on the TMA sweep or the split kernels (kernel = AUTO, TMA or SPLIT)");
+    if (g->formulation != EM_FORM_LEAPFROG && g->formulation != EM_FORM_EONLY) return fail(EM_ERR_INVALID_ARG, "bad formulation");
+    if (g->formulation == EM_FORM_EONLY && (g->thermal || g->kernel == EM_KERNEL_SPLIT))
+        return fail(EM_ERR_UNSUPPORTED, "the E-only recurrence runs on the TMA sweep, without thermal coupling");
+    if (g->z_chunks < 0 || g->z_chunks > em::kSweepMaxZSplit) return fail(EM_ERR_INVALID_ARG, "z_chunks must be 0 (auto) .. 8");
     if (g->max_ports < 0 || g->max_source_edges < 0 || g->max_wave_samples < 0)
         return fail(EM_ERR_INVALID_ARG, "negative source capacity");
     return EM_OK;
@@ -260,9 +287,9 @@ int32_t validate_grid(const em_grid *g) {
 
 template <typename R>
 int32_t Ctx<R>::zero_state() {
-    for (int a = 0; a < 12; ++a) CU(cudaMemsetAsync(c.field[a], 0, sizeof(R) * g.alloc_elems, stream));
+    for (int a = 0; a < n_field; ++a) CU(cudaMemsetAsync(c.field[a], 0, sizeof(R) * g.alloc_elems, stream));
     CU(cudaMemsetAsync(c.q, 0, sizeof(R) * g.alloc_elems, stream));
-    e_cur = h_cur = 0; bind();
+    e_cur = h_cur = lvl = 0; bind();
     step_index = 0;
     if (grid.thermal) {
         CU(cudaMemsetAsync(c.theta[0], 0, sizeof(R) * g.alloc_elems, stream));
@@ -280,15 +307,15 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     g = make_geometry(gr->nx, gr->ny, gr->nz);
     loss = gr->loss_mode; dt = dt_;
     stream = static_cast<cudaStream_t>(stream_);
+    eonly = gr->formulation == EM_FORM_EONLY;
+    n_field = eonly ? 9 : 12;
     {
-        int dev = 0, n_sm = 0;
-        CU(cudaGetDevice(&dev));
-        CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-        const char *forced = std::getenv("EM_FUSED_ZSPLIT");      // tuning/test knob: force the z chunk count
-        plan = em::make_fused_plan(g.nx, g.ny, g.nz, (int)sizeof(R), n_sm, forced ? std::atoi(forced) : 0, gr->thermal != 0);
+        int n_sm = 0;
+        CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device));
+        plan = em::make_sweep_plan(g.nx, g.ny, g.nz, (int)sizeof(R), n_sm, gr->z_chunks, gr->thermal != 0);
     }
     kernel = gr->kernel;
-    const int max_items = plan.n_tiles * em::kFusedMaxZSplit;
+    const int max_items = plan.n_tiles * em::kSweepMaxZSplit;
     const size_t need = carve<R>(g, *gr, nullptr, nullptr, max_items);
     if (ws_bytes < need) return fail(EM_ERR_WORKSPACE_TOO_SMALL, "workspace too small");
     carve<R>(g, *gr, workspace, &c, max_items);
@@ -300,14 +327,13 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
         sweep_smem = em::sweep_smem_bytes((int)sizeof(R), n_mat + 2, true);
         if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_TMA;
     }
-    if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_TMA;     // measured on config 4: TMA sweep 2.44 ms/step, cp.async sweep 2.71 ms/step
-    if (kernel == EM_KERNEL_TMA) {
-        int dev = 0, optin = 0;
-        CU(cudaGetDevice(&dev));
-        CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-        if (sweep_smem > (size_t)optin) kernel = gr->thermal ? EM_KERNEL_SPLIT : EM_KERNEL_FUSED;   // very large tables
+    if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_TMA;
+    if (kernel == EM_KERNEL_TMA) {           // (the layout holds the largest table, 255 + 2 entries, in both precisions)
+        int optin = 0;
+        CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
+        if (sweep_smem > (size_t)optin) return fail(EM_ERR_UNSUPPORTED, "the sweep's shared-memory layout does not fit this device");
     }
-    main_kernel = kernel == EM_KERNEL_TMA ? "k_sweep_tma" : kernel == EM_KERNEL_FUSED ? "k_fused_sweep" : "k_split_e";
+    main_kernel = kernel == EM_KERNEL_TMA ? "k_sweep_tma" : "k_split_e";
 
     // ---- material table -> (eps/dt, sigma, mask, dt/mu), built in fp64, rounded once ----------
     table.assign(tab, tab + n_mat);
@@ -400,7 +426,12 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     CU(cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (plan.n_tiles * plan.nzs + 1), stream));
     int32_t rc = zero_state();
     if (rc) return rc;
-    if (kernel == EM_KERNEL_TMA) { rc = make_maps(); if (rc) return rc; }
+    if (kernel == EM_KERNEL_TMA) {
+        rc = make_maps(); if (rc) return rc;
+        // one instantiation per context: selected and given its dynamic shared memory once, here
+        sweep_kernel = em::select_sweep<R>(loss, uniform_mu, gr->thermal != 0, eonly);
+        CU(em::configure_sweep<R>(sweep_kernel, sweep_smem));
+    }
     CU(cudaStreamSynchronize(stream));
     return EM_OK;
 }
@@ -423,8 +454,7 @@ int32_t Ctx<R>::make_maps() {
     EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(fn);
     const int V = 16 / (int)sizeof(R);
     const cuuint32_t ones[3] = {1, 1, 1};
-    const char *pe = std::getenv("EM_TMA_L2PROMO");           // tuning knob: 0 none, 1 64 B, 2 128 B (default), 3 256 B
-    const CUtensorMapL2promotion promo = pe ? (CUtensorMapL2promotion)std::atoi(pe) : CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
+    const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
     auto encode = [&](CUtensorMap *m, CUtensorMapDataType dt, size_t esz, void *base, int bx, int by) -> int32_t {
         const cuuint64_t dims[3] = {(cuuint64_t)g.PX, (cuuint64_t)g.PY, (cuuint64_t)g.PZ};
         const cuuint64_t strides[2] = {(cuuint64_t)g.PX * esz, (cuuint64_t)g.PXY * esz};
@@ -436,11 +466,12 @@ int32_t Ctx<R>::make_maps() {
     };
     const int sw_warps = grid.thermal ? em::Tile<sizeof(R), true>::warps : em::Tile<sizeof(R)>::warps;
     const CUtensorMapDataType fdt = sizeof(R) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
-    for (int a = 0; a < 12; ++a) {
-        const int comp = a % 3, is_e = a < 6;
+    for (int a = 0; a < n_field; ++a) {
+        const int comp = a % 3, is_e = eonly || a < 6;
         const int rows = (is_e && comp != 1) ? sw_warps + 1 : sw_warps;         // Ex, Ez carry row TY+1
         int32_t rc = encode(&map_field[a], fdt, sizeof(R), c.field[a] + g.PX - V, 32 * V, rows);
         if (rc) return rc;
+        if (eonly) { rc = encode(&map_prev[a], fdt, sizeof(R), c.field[a] + g.PX - V, 32 * V, sw_warps); if (rc) return rc; }
     }
     int32_t rc = encode(&map_q, fdt, sizeof(R), c.q + g.PX - V, 30 * V, sw_warps - 2);
     if (rc) return rc;
@@ -571,7 +602,7 @@ int32_t Ctx<R>::set_source(int32_t np, const em_port *ports, const em_edge *edge
 // ---- dense <-> padded copies ----------------------------------------------------------------------
 template <typename R>
 int32_t Ctx<R>::set_field(int32_t comp, const void *srcp, int32_t is_dev) {
-    if (comp < 0 || comp > 5 || !srcp) return fail(EM_ERR_INVALID_ARG, "set_field arguments");
+    if (!comp_ok(comp) || !srcp) return fail(EM_ERR_INVALID_ARG, "set_field arguments");
     int sx, sy, sz; comp_dims(comp, &sx, &sy, &sz);
     cudaMemcpy3DParms m = {};
     m.srcPtr = make_cudaPitchedPtr(const_cast<void *>(srcp), sizeof(R) * sx, sx, sy);
@@ -579,9 +610,9 @@ int32_t Ctx<R>::set_field(int32_t comp, const void *srcp, int32_t is_dev) {
     m.extent = make_cudaExtent(sizeof(R) * sx, sy, sz);
     m.kind = is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     CU(cudaMemcpy3DAsync(&m, stream));
-    if (comp < 3) {
+    if (comp < 3 || comp >= 6) {
         dim3 b(32, 8);
-        em::k_mask_fixed<R><<<node_grid(b, 1), b, 0, stream>>>(p, comp, 0);
+        em::k_mask_fixed<R><<<node_grid(b, 1), b, 0, stream>>>(p, comp_ptr(comp), comp % 3, 0);
         CU(cudaGetLastError());
     }
     if (!is_dev) CU(cudaStreamSynchronize(stream));
@@ -591,7 +622,7 @@ int32_t Ctx<R>::set_field(int32_t comp, const void *srcp, int32_t is_dev) {
 // One z plane of a component out (dst) or in (src): the halo exchange of a z-slab decomposition.
 template <typename R>
 int32_t Ctx<R>::plane(int32_t comp, int32_t k, void *dst, const void *srcp, int32_t is_dev) {
-    if (comp < 0 || comp > 5) return fail(EM_ERR_INVALID_ARG, "plane: bad component");
+    if (!comp_ok(comp)) return fail(EM_ERR_INVALID_ARG, "plane: bad component");
     int sx, sy, sz; comp_dims(comp, &sx, &sy, &sz);
     if (k < 0 || k >= sz) return fail(EM_ERR_INVALID_ARG, "plane: k out of range");
     R *base = comp_ptr(comp) + (long long)k * g.PXY;
@@ -602,10 +633,10 @@ int32_t Ctx<R>::plane(int32_t comp, int32_t k, void *dst, const void *srcp, int3
     } else {
         CU(cudaMemcpy2DAsync(base, sizeof(R) * g.PX, srcp, wbytes, wbytes, sy,
                              is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, stream));
-        if (comp < 3) {                                   // PEC-fixed edges of this plane stay 0
+        if (comp < 3 || comp >= 6) {                      // PEC-fixed edges of this plane stay 0
             dim3 b(32, 8);
             dim3 gr((g.nx + 1 + b.x - 1) / b.x, (g.ny + 1 + b.y - 1) / b.y, 1);
-            em::k_mask_fixed<R><<<gr, b, 0, stream>>>(p, comp, k);
+            em::k_mask_fixed<R><<<gr, b, 0, stream>>>(p, comp_ptr(comp), comp % 3, k);
             CU(cudaGetLastError());
         }
     }
@@ -615,7 +646,7 @@ int32_t Ctx<R>::plane(int32_t comp, int32_t k, void *dst, const void *srcp, int3
 
 template <typename R>
 int32_t Ctx<R>::get_field(int32_t comp, void *dst, int32_t is_dev) {
-    if (comp < 0 || comp > 5 || !dst) return fail(EM_ERR_INVALID_ARG, "get_field arguments");
+    if (!comp_ok(comp) || !dst) return fail(EM_ERR_INVALID_ARG, "get_field arguments");
     int sx, sy, sz; comp_dims(comp, &sx, &sy, &sz);
     cudaMemcpy3DParms m = {};
     m.srcPtr = make_cudaPitchedPtr(comp_ptr(comp), sizeof(R) * g.PX, g.PX, g.PY);
@@ -680,7 +711,8 @@ int32_t Ctx<R>::set_thermal(const em_thermal_material *tt, int32_t n_mat) {
     if (!grid.thermal) return fail(EM_ERR_STATE, "the context was created with em_grid.thermal = 0");
     if (!tt || n_mat != n_mat_) return fail(EM_ERR_INVALID_ARG, "thermal table must have the n_mat entries of em_create");
     for (int m = 0; m < n_mat; ++m)
-        if (!(tt[m].rho_cp > 0.0) || !(tt[m].k >= 0.0)) return fail(EM_ERR_INVALID_ARG, "need rho_cp > 0 and k >= 0");
+        if (!(tt[m].rho_cp > 0.0) || !(tt[m].k >= 0.0) || !std::isfinite(tt[m].rho_cp + tt[m].k + tt[m].alpha))
+            return fail(EM_ERR_INVALID_ARG, "need finite rho_cp > 0, k >= 0 and alpha");
     std::vector<em::ThEntry<R>> ht(p.n_table);          // the outside entries stay 0: no heat, no conduction
     for (auto &e : ht) { e.irc = R(0); e.k = R(0); e.alpha = R(0); e.sigma0 = R(0); }
     for (int m = 0; m < n_mat; ++m) {
@@ -761,12 +793,12 @@ int32_t Ctx<R>::step_thermal_sweep() {
     }
     launches += 1;
     int32_t rc = record_begin(); if (rc) return rc;
-    em::FusedSources fsrc{c.tile_sbeg, c.tile_ent};
+    em::SweepSources fsrc{c.tile_sbeg, c.tile_ent};
     em::SweepMaps maps;
     for (int a = 0; a < 3; ++a) { maps.E[a] = map_field[e_cur * 3 + a]; maps.H[a] = map_field[6 + h_cur * 3 + a]; }
     maps.q = map_q; maps.mat = map_mat; maps.sig = map_sig[sg_cur];
     em::ThermalSweep<R> tsw{th_out, sig_buf(1 - sg_cur), c.ttable};
-    cudaError_t e = em::launch_sweep_tma<R>(plan, sweep_smem, maps, p, src, fsrc, loss, uniform_mu, (long long)step_index, stream, &tsw);
+    cudaError_t e = em::launch_sweep_tma<R>(sweep_kernel, plan, sweep_smem, maps, p, src, fsrc, (long long)step_index, stream, &tsw);
     if (e != cudaSuccess) return fail(EM_ERR_CUDA, std::string("coupled TMA sweep launch: ") + cudaGetErrorString(e));
     rc = record_end(); if (rc) return rc;
     launches += 1;
@@ -775,29 +807,21 @@ int32_t Ctx<R>::step_thermal_sweep() {
 }
 
 template <typename R>
-int32_t Ctx<R>::step_fused() {
-    int32_t rc = record_begin(); if (rc) return rc;
-    em::FusedSources fsrc{c.tile_sbeg, c.tile_ent};
-    cudaError_t e = em::launch_fused<R>(plan, p, src, fsrc, loss, uniform_mu, (long long)step_index, stream);
-    if (e != cudaSuccess) return fail(EM_ERR_CUDA, std::string("fused sweep launch: ") + cudaGetErrorString(e));
-    rc = record_end(); if (rc) return rc;
-    launches += 1;
-    e_cur ^= 1; h_cur ^= 1; bind();
-    return EM_OK;
-}
-
-template <typename R>
 int32_t Ctx<R>::step_tma() {
     int32_t rc = record_begin(); if (rc) return rc;
-    em::FusedSources fsrc{c.tile_sbeg, c.tile_ent};
+    em::SweepSources fsrc{c.tile_sbeg, c.tile_ent};
     em::SweepMaps maps;
-    for (int a = 0; a < 3; ++a) { maps.E[a] = map_field[e_cur * 3 + a]; maps.H[a] = map_field[6 + h_cur * 3 + a]; }
+    for (int a = 0; a < 3; ++a) {
+        if (eonly) { maps.E[a] = map_field[lvl * 3 + a]; maps.H[a] = map_prev[((lvl + 2) % 3) * 3 + a]; }
+        else       { maps.E[a] = map_field[e_cur * 3 + a]; maps.H[a] = map_field[6 + h_cur * 3 + a]; }
+    }
     maps.q = map_q; maps.mat = map_mat;
-    cudaError_t e = em::launch_sweep_tma<R>(plan, sweep_smem, maps, p, src, fsrc, loss, uniform_mu, (long long)step_index, stream);
+    cudaError_t e = em::launch_sweep_tma<R>(sweep_kernel, plan, sweep_smem, maps, p, src, fsrc, (long long)step_index, stream);
     if (e != cudaSuccess) return fail(EM_ERR_CUDA, std::string("TMA sweep launch: ") + cudaGetErrorString(e));
     rc = record_end(); if (rc) return rc;
     launches += 1;
-    e_cur ^= 1; h_cur ^= 1; bind();
+    if (eonly) lvl = (lvl + 1) % 3; else { e_cur ^= 1; h_cur ^= 1; }
+    bind();
     return EM_OK;
 }
 
@@ -807,7 +831,7 @@ int32_t Ctx<R>::step(int64_t n) {
     for (int64_t s = 0; s < n; ++s) {
         int32_t rc = thermal_on ? (kernel == EM_KERNEL_TMA ? step_thermal_sweep() : step_thermal())
                    : grid.thermal ? step_split()            // (tile geometry of the coupled sweep: EM-only steps run split)
-                   : kernel == EM_KERNEL_TMA ? step_tma() : kernel == EM_KERNEL_FUSED ? step_fused() : step_split();
+                   : kernel == EM_KERNEL_TMA ? step_tma() : step_split();
         if (rc) return rc;
         step_index += 1;
     }
@@ -846,13 +870,13 @@ template <typename R>
 int32_t Ctx<R>::probe(int32_t n, const em_probe_pt *pts, double *out) {
     if (n < 0 || (n && (!pts || !out))) return fail(EM_ERR_INVALID_ARG, "probe arguments");
     for (int q = 0; q < n; ++q) {
-        if (pts[q].comp < 0 || pts[q].comp > 5) return fail(EM_ERR_INVALID_ARG, "probe comp must be 0..5");
+        if (!comp_ok(pts[q].comp)) return fail(EM_ERR_INVALID_ARG, "probe comp must be 0..5 (E-only contexts: 0..2, 6..8)");
         int sx, sy, sz; comp_dims(pts[q].comp, &sx, &sy, &sz);
         if (pts[q].i < 0 || pts[q].i >= sx || pts[q].j < 0 || pts[q].j >= sy || pts[q].k < 0 || pts[q].k >= sz)
             return fail(EM_ERR_INVALID_ARG, "probe point outside the grid");
     }
     em::ProbeArrays<R> pa;
-    for (int a = 0; a < 3; ++a) { pa.f[a] = p.E[a]; pa.f[3 + a] = p.H[a]; }
+    for (int a = 0; a < 3; ++a) { pa.f[a] = p.E[a]; pa.f[3 + a] = p.H[a]; pa.f[6 + a] = p.H[a]; }
     std::vector<long long> off(kProbeChunk); std::vector<int> comp(kProbeChunk);
     for (int base = 0; base < n; base += kProbeChunk) {
         const int m = std::min(kProbeChunk, n - base);
@@ -881,8 +905,8 @@ int32_t em_workspace_bytes(const em_grid *gr, size_t *out) {
     if (!out) return fail(EM_ERR_INVALID_ARG, "out is null");
     int32_t rc = validate_grid(gr); if (rc) return rc;
     const Geometry g = make_geometry(gr->nx, gr->ny, gr->nz);
-    const em::FusedPlan plan = em::make_fused_plan(g.nx, g.ny, g.nz, gr->precision / 8, 0, 0, gr->thermal != 0);
-    const int max_items = plan.n_tiles * em::kFusedMaxZSplit;
+    const em::SweepPlan plan = em::make_sweep_plan(g.nx, g.ny, g.nz, gr->precision / 8, 0, 0, gr->thermal != 0);
+    const int max_items = plan.n_tiles * em::kSweepMaxZSplit;
     *out = gr->precision == 32 ? carve<float>(g, *gr, nullptr, nullptr, max_items)
                                : carve<double>(g, *gr, nullptr, nullptr, max_items);
     return EM_OK;
@@ -934,12 +958,19 @@ int32_t em_create(const em_grid *gr, const uint8_t *mat_id, const em_material *t
     if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return fail(EM_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
     int dev_count = 0;
     if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count < 1) return fail(EM_ERR_CUDA, "no CUDA device");
+    // the context lives on the device that owns the workspace, whatever the caller's current device is
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return fail(EM_ERR_INVALID_ARG, "workspace is not a device pointer");
+    }
+    DeviceGuard guard(attr.device);
     em_ctx *ctx = nullptr;
     if (gr->precision == 32) {
-        auto *c = new Ctx<float>(); ctx = c;
+        auto *c = new Ctx<float>(); ctx = c; c->device = attr.device;
         rc = c->init(gr, mat_id, tab, n_mat, dt, workspace, ws_bytes, stream);
     } else {
-        auto *c = new Ctx<double>(); ctx = c;
+        auto *c = new Ctx<double>(); ctx = c; c->device = attr.device;
         rc = c->init(gr, mat_id, tab, n_mat, dt, workspace, ws_bytes, stream);
     }
     if (rc) { delete ctx; return rc; }
@@ -947,15 +978,18 @@ int32_t em_create(const em_grid *gr, const uint8_t *mat_id, const em_material *t
     return EM_OK;
 }
 
+int32_t em_abi_version(void) { return EM_ABI_VERSION; }
+
 int32_t em_destroy(em_ctx *ctx) {
     if (!ctx) return EM_OK;
+    DeviceGuard guard(ctx->device);
     for (auto e : ctx->timing.beg) cudaEventDestroy(e);
     for (auto e : ctx->timing.end) cudaEventDestroy(e);
     delete ctx;
     return EM_OK;
 }
 
-#define EM_CHECK_CTX if (!ctx) return fail(EM_ERR_INVALID_ARG, "ctx is null")
+#define EM_CHECK_CTX if (!ctx) return fail(EM_ERR_INVALID_ARG, "ctx is null"); DeviceGuard guard_(ctx->device)
 
 int32_t em_set_source(em_ctx *ctx, int32_t n_ports, const em_port *ports, const em_edge *edges, int64_t n_edges,
                       const double *wave, int64_t n_samples) {

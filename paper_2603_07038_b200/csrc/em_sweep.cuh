@@ -3,25 +3,28 @@
 // (eq. (2)-(3) L69-L76 in leapfrog form, L86 for the Joule heat) and moves each
 // field value through HBM once per step: 57 B (fp32) / 113 B (fp64) per cell-update.
 //
-// Same decomposition, arithmetic and barrier structure as em_fused.cuh (tile = 30V x 14 columns marched in
-// z, warp = one row, lane = V consecutive x, halo lanes/rows recompute, two CTA barriers per plane, phase B
-// as in em_fused_phaseb*.inc), but the input planes are staged by TMA instead of per-thread
-// cp.async:
+// Decomposition: em_tile.cuh (tile = 30V x TY columns marched in z, warp = one row, lane = V consecutive x, halo
+// lanes / rows recompute).  Staging:
 //  * every E, H and material-id plane of the tile is ONE cp.async.bulk.tensor.3d box per array, issued by
 //    one thread and counted on an mbarrier: no per-thread address arithmetic, no LDGSTS instructions and
-//    no LSU shared-memory write wavefronts for the loads (they were ~11 % of the instructions of the
-//    cp.async sweep);
+//    no LSU shared-memory write wavefronts for the loads;
 //  * a box lands row-major, 512 B per row, i.e. exactly in the [row = warp][lane] x 16 B slot format the
 //    threads read; the boxes of Ex and Ez carry a 17th row (the top warp's +1 neighbour);
-//  * q (conditionally fetched: lossless lanes skip it) and the per-plane z geometry stay on cp.async.
+//  * q (conditionally fetched: lossless lanes skip it) stays on cp.async; the per-plane z geometry is a bulk copy.
+//
+// EO = true: the paper's LITERAL E-only three-level recurrence (NEXT-4 of SURVEY.md 8(f); eq. (2)
+// eq. (3)):  M e^{n+1} = N e^n - K e^{n-1} - dt^2 (dJ/dt)^n.  State e^n, e^{n-1}; no H array is read or written.  The same
+// sweep: phase A forms g = dt D_nu C_e e^n of the plane on chip (what the leapfrog subtracts from H), phase B applies
+// C_h to it and advances  e^{n+1} = e^n + d + r (-(C_h g) - dJ - sigma d),  d = e^n - e^{n-1},  which is eq. (2) divided by
+// M (N - M - K = -dt^2 S).  The planes of e^{n-1} ride in the staging slots of H.  9 words + 1 B + 2 words per
+// cell-update = 45 B (fp32) / 89 B (fp64) instead of 57 / 113.
 #pragma once
 #include <cuda.h>
 
-#include "em_fused.cuh"
+#include "em_tile.cuh"
 
 namespace em {
 
-#undef EM_ST
 #define EM_ST(ptr, val) st_stream16((ptr), (val))     // output planes: streaming (evict-first) stores
 
 constexpr int kSwRow = 512;                        // bytes of one staged row (32 lanes x 16 B)
@@ -34,7 +37,7 @@ struct alignas(64) SweepMaps { CUtensorMap E[3], H[3], q, mat, sig; };   // sig:
 // because its size is only known at run time)
 template <int SZ, bool TH = false> struct SweepLayout {
     static constexpr int V = 16 / SZ;
-    static constexpr int kSwWarps = Tile<SZ, TH>::warps, kFusedRows = Tile<SZ, TH>::rows;
+    static constexpr int kSwWarps = Tile<SZ, TH>::warps, kSwRows = Tile<SZ, TH>::rows;
     static constexpr int n_priv = kSwPriv + (TH ? 1 : 0);          // + theta of layer k-1 (coupled sweep)
     static constexpr int ex = 0;                                  // Ex ring of 3 planes, rows -1 .. TY+1
     static constexpr int ex_slot = (kSwWarps + 1) * kSwRow;
@@ -48,8 +51,8 @@ template <int SZ, bool TH = false> struct SweepLayout {
     static constexpr int id_row = 32 * V + 16;                    // box starts on a 16-B boundary: up to 15 B of lead-in
     static constexpr int id_slot = ((kSwWarps + 2) * id_row + 127) / 128 * 128;
     static constexpr int priv = ids + 2 * id_slot;                // private slots [kSwPriv][512 threads]
-    static constexpr int rows = priv + n_priv * kSwWarps * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kFusedRows][32]
-    static constexpr int geo = rows + 4 * kFusedRows * kSwRow;    // 1/dx, 1/dx~, fx of the 32 lanes
+    static constexpr int rows = priv + n_priv * kSwWarps * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kSwRows][32]
+    static constexpr int geo = rows + 4 * kSwRows * kSwRow;    // 1/dx, 1/dx~, fx of the 32 lanes
     static constexpr int zg = geo + 3 * kSwRow;                   // [2 parity]{fz, 1/dz, 1/dz~, 0}
     static constexpr int sig = zg + 128;                          // coupled sweep: sigma(T^n), 2 parities, rows -2 .. TY (TMA: 128-B aligned)
     static constexpr int sig_slot = TH ? (kSwWarps + 1) * kSwRow : 0;
@@ -112,18 +115,18 @@ __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map
 // is staged as one more TMA plane per step plane (rows -2 .. TY) and replaces the table's sigma in the coefficient
 // gather; phase C adds the Joule heat of the step to theta (already advanced by the conduction kernel k_diffuse) and
 // writes sigma(T^{n+1}) to the other sigma buffer.  The one-material path is taken only for materials with alpha = 0.
-template <typename R, int LOSS, bool UMU, bool TH = false>
+template <typename R, int LOSS, bool UMU, bool TH = false, bool EO = false>
 __global__ void __launch_bounds__(Tile<sizeof(R), TH>::threads, 1)
-k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R> src, FusedSources fs,
-            FusedChunks zc, int ntx, long long step, ThermalSweep<R> th) {
+k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R> src, SweepSources fs,
+            SweepChunks zc, int ntx, long long step, ThermalSweep<R> th) {
     constexpr int V = 16 / sizeof(R);
     constexpr int TXo = 30 * V;
-    constexpr int kSwTY = Tile<sizeof(R), TH>::TY, kSwWarps = Tile<sizeof(R), TH>::warps, kFusedRows = Tile<sizeof(R), TH>::rows;
+    constexpr int kSwTY = Tile<sizeof(R), TH>::TY, kSwWarps = Tile<sizeof(R), TH>::warps, kSwRows = Tile<sizeof(R), TH>::rows;
     constexpr int NT = Tile<sizeof(R), TH>::threads;
     using L = SweepLayout<(int)sizeof(R), TH>;
     using VecR = Vec<R>;
     using IdT = typename std::conditional<V == 4, unsigned, unsigned short>::type;
-    // private slot numbering of this kernel (shadows the cp.async sweep's enum inside em_fused_phaseb*.inc)
+    // private 16-B slots of a thread
     constexpr int kSlotQ = 0, kSlotL = 1, kSlotHp = 5, kSlotPend = 7, kSlotTheta = 8;
     extern __shared__ __align__(1024) unsigned char sm[];
 
@@ -148,10 +151,10 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     // shared-memory views
     MatEntry<R> *s_tab = reinterpret_cast<MatEntry<R> *>(sm + L::tab);
     VecR *s_rows = reinterpret_cast<VecR *>(sm + L::rows);
-    VecR(*smHx)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 0 * kFusedRows * 32);
-    VecR(*smHz)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 1 * kFusedRows * 32);
-    VecR(*smBx)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 2 * kFusedRows * 32);
-    VecR(*smBz)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 3 * kFusedRows * 32);
+    VecR(*smHx)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 0 * kSwRows * 32);
+    VecR(*smHz)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 1 * kSwRows * 32);
+    VecR(*smBx)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 2 * kSwRows * 32);
+    VecR(*smBz)[32] = reinterpret_cast<VecR(*)[32]>(s_rows + 3 * kSwRows * 32);
     VecR *mine = reinterpret_cast<VecR *>(sm + L::priv) + tid;    // private slots [kSwPriv][NT]
     VecR *s_geo = reinterpret_cast<VecR *>(sm + L::geo);
     R *s_z = reinterpret_cast<R *>(sm + L::zg);
@@ -161,12 +164,14 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     auto bar_fullE = [&](int s) -> unsigned { return bar0 + 8 * s; };
     auto bar_fullH = [&](int s) -> unsigned { return bar0 + 16 + 8 * s; };
     auto bar_empty = [&](int s) -> unsigned { return bar0 + 32 + 8 * s; };     // every warp has consumed the staged plane
+    auto bar_emptyH = [&](int s) -> unsigned { return bar0 + 48 + 8 * s; };    // EO: ... and its e^{n-1} planes (read in phase B)
     auto bar_rowH = [&](int ww) -> unsigned { return bar0 + 64 + 8 * ww; };    // H'(k) row of warp ww is published
 
     // ---- prologue: barriers, table, x geometry, zeroed exchange rows and private slots -------------------
     if (tid == 0) {
         mbar_init(bar_fullE(0), 1); mbar_init(bar_fullE(1), 1); mbar_init(bar_fullH(0), 1); mbar_init(bar_fullH(1), 1);
         mbar_init(bar_empty(0), kSwWarps); mbar_init(bar_empty(1), kSwWarps);
+        mbar_init(bar_emptyH(0), kSwWarps); mbar_init(bar_emptyH(1), kSwWarps);
         for (int ww = 0; ww < kSwWarps; ++ww) mbar_init(bar_rowH(ww), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -177,7 +182,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         VecR z, mone;
 #pragma unroll
         for (int c = 0; c < V; ++c) { z.v[c] = R(0); mone.v[c] = R(-1); }
-        for (int t = tid; t < 4 * kFusedRows * 32; t += NT) s_rows[t] = z;
+        for (int t = tid; t < 4 * kSwRows * 32; t += NT) s_rows[t] = z;
         for (int t = 0; t < L::n_priv; ++t) mine[t * NT] = z;
         mine[(kSlotL + 0) * NT] = mone; mine[(kSlotL + 2) * NT] = mone;     // plane k = -1 is outside: eps/dt = 1, mask 0 (sign)
         if (w == 0) {
@@ -296,9 +301,15 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
                     nbz.v[c] = lerp(nk, ncur[c], fz);
                 }
             }
-            mbar_wait(bar_fullH(it & 1), (unsigned)(it >> 1) & 1u);   // H(k) has landed
-            const VecR hx = staged(L::h + (par * 3 + 0) * L::h_slot), hy = staged(L::h + (par * 3 + 1) * L::h_slot);
-            const VecR hz = staged(L::h + (par * 3 + 2) * L::h_slot);
+            VecR hx, hy, hz;
+            if (EO) {               // no H state: H' stands for -g = -dt D_nu C_e e^n (eq. (3): the inner factor of S)
+#pragma unroll
+                for (int c = 0; c < V; ++c) hx.v[c] = hy.v[c] = hz.v[c] = R(0);
+            } else {
+                mbar_wait(bar_fullH(it & 1), (unsigned)(it >> 1) & 1u);   // H(k) has landed
+                hx = staged(L::h + (par * 3 + 0) * L::h_slot); hy = staged(L::h + (par * 3 + 1) * L::h_slot);
+                hz = staged(L::h + (par * 3 + 2) * L::h_slot);
+            }
 #pragma unroll
             for (int c = 0; c < V; ++c) {
                 const R eyip = (c < V - 1) ? ey0.v[c < V - 1 ? c + 1 : c] : ey0_r;
@@ -312,7 +323,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
 #pragma unroll
             for (int c = 0; c < V; ++c) hxn.v[c] = hyn.v[c] = hzn.v[c] = R(0);
         }
-        if (st) {
+        if (st && !EO) {
             EM_ST(p.Hn[0] + o, hxn);
             EM_ST(p.Hn[1] + o, hyn);
             EM_ST(p.Hn[2] + o, hzn);
@@ -322,10 +333,18 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         // thread refills the staged slots once every warp has pulled plane k into registers (mbarrier empty).
         // WAR on the exchange rows is ordered by the chain  B(k) of row j+1 done -> pair barrier -> C(k), A(k+1) of row j.
         __syncwarp();
-        if (lane == 0) { mbar_arrive(bar_rowH(w)); mbar_arrive(bar_empty(it & 1)); }
+        if (lane == 0) {
+            mbar_arrive(bar_rowH(w)); mbar_arrive(bar_empty(it & 1));
+            if (EO && w == 0) mbar_arrive(bar_emptyH(it & 1));         // (warp 0 has no phase B)
+        }
         if (tid == 0 && k + 2 <= ke) {
             mbar_wait(bar_empty(it & 1), (unsigned)(it >> 1) & 1u);
-            issue_H(k + 2); issue_E(k + 2, false);
+            if (!EO) issue_H(k + 2);
+            issue_E(k + 2, false);
+            if (EO) {               // the e^{n-1} planes are read in phase B: their slots are released there
+                mbar_wait(bar_emptyH(it & 1), (unsigned)(it >> 1) & 1u);
+                issue_H(k + 2);
+            }
         }
         if (w != 0) mbar_wait(bar_rowH(w - 1), (unsigned)it & 1u);   // H'(k) of row j-1 is visible
 
@@ -333,8 +352,12 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         // (warp 0 = halo row -1 only supplies H' to row 0: no E', no Joule)
         VecR bx, by, bz;         // (2 Ebar)^2
         if (w != 0) {
+            // EO: d = e^n - e^{n-1} of the own edges is formed where it is used (em_sweep_phaseb*.inc) from the staged
+            // e^{n-1} planes (the subtraction is exact in floating point when the two levels are within a factor 2)
+            if (EO) mbar_wait(bar_fullH(it & 1), (unsigned)(it >> 1) & 1u);   // e^{n-1}(k) has landed
+#define EM_PREV(comp) staged(L::h + (par * 3 + (comp)) * L::h_slot)
             if (hom && s_next_k > k) {
-#include "em_fused_phaseb_hom.inc"
+#include "em_sweep_phaseb_hom.inc"
                 l_stale = true;
             } else {
                 if (l_stale) {   // plane k-1 took the one-material path: its coefficient means are the entry itself
@@ -356,6 +379,11 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
 #include "em_sweep_phaseb.inc"
 #undef EM_HAS_J
                 }
+            }
+#undef EM_PREV
+            if (EO) {               // the staged e^{n-1} planes have been read
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_emptyH(it & 1));
             }
             if (!active) {
 #pragma unroll
@@ -392,7 +420,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
                     const R dq = gq * sig_prev.v[c] * (pend.v[c] + sxy);
                     qv.v[c] += dq;
                     thv.v[c] = mad(dq, te.irc, thv.v[c]);
-                    sgn.v[c] = te.sigma0 * rcp<R>(mad(te.alpha, thv.v[c], R(1)));
+                    sgn.v[c] = te.sigma0 * rcp<R>(thermal_den(te.alpha, thv.v[c]));
                 } else {
                     const R sg = s_tab[(idw_prev >> (8 * (hom ? 0 : c))) & 0xff].b;     // sigma of the cell of layer k-1
                     qv.v[c] = mad(gq * sg, pend.v[c] + sxy, qv.v[c]);
@@ -421,24 +449,38 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     cp_async_wait<0>();
 }
 
+// The instantiation for a context: loss mode x uniform-mu fast path, or the coupled sweep (general mu path only), or the
+// E-only recurrence.  select + configure once at em_create, launch per step.
 template <typename R>
-cudaError_t launch_sweep_tma(const FusedPlan &plan, size_t smem_bytes, const SweepMaps &maps, const DevParams<R> &p,
-                             const DevSources<R> &src, const FusedSources &fs, int loss, bool uniform_mu,
-                             long long step, cudaStream_t stream, const ThermalSweep<R> *thermal = nullptr) {
-    using K = void (*)(const SweepMaps, DevParams<R>, DevSources<R>, FusedSources, FusedChunks, int, long long, ThermalSweep<R>);
-    FusedChunks zc;
+using SweepKernel = void (*)(const SweepMaps, DevParams<R>, DevSources<R>, SweepSources, SweepChunks, int, long long, ThermalSweep<R>);
+
+template <typename R>
+SweepKernel<R> select_sweep(int loss, bool uniform_mu, bool thermal, bool eonly) {
+    using K = SweepKernel<R>;
+    if (thermal) return loss == 0 ? (K)k_sweep_tma<R, 0, false, true> : (K)k_sweep_tma<R, 1, false, true>;
+    if (eonly) {
+        if (loss == 0) return uniform_mu ? (K)k_sweep_tma<R, 0, true, false, true> : (K)k_sweep_tma<R, 0, false, false, true>;
+        return uniform_mu ? (K)k_sweep_tma<R, 1, true, false, true> : (K)k_sweep_tma<R, 1, false, false, true>;
+    }
+    if (loss == 0) return uniform_mu ? (K)k_sweep_tma<R, 0, true> : (K)k_sweep_tma<R, 0, false>;
+    return uniform_mu ? (K)k_sweep_tma<R, 1, true> : (K)k_sweep_tma<R, 1, false>;
+}
+
+template <typename R>
+cudaError_t configure_sweep(SweepKernel<R> kern, size_t smem_bytes) {
+    return cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+}
+
+template <typename R>
+cudaError_t launch_sweep_tma(SweepKernel<R> kern, const SweepPlan &plan, size_t smem_bytes, const SweepMaps &maps,
+                             const DevParams<R> &p, const DevSources<R> &src, const SweepSources &fs, long long step,
+                             cudaStream_t stream, const ThermalSweep<R> *thermal = nullptr) {
+    SweepChunks zc;
     zc.nzs = plan.nzs;
-    for (int c = 0; c <= kFusedMaxZSplit; ++c) zc.kb[c] = plan.kb[c];
-    K kern;
+    for (int c = 0; c <= kSweepMaxZSplit; ++c) zc.kb[c] = plan.kb[c];
     ThermalSweep<R> th{};
-    int threads = Tile<sizeof(R)>::threads;
-    if (thermal) {           // coupled sweep: sigma(T) planes, general mu path only (one instantiation per loss mode)
-        th = *thermal; threads = Tile<sizeof(R), true>::threads;
-        kern = loss == 0 ? (K)k_sweep_tma<R, 0, false, true> : (K)k_sweep_tma<R, 1, false, true>;
-    } else if (loss == 0) kern = uniform_mu ? (K)k_sweep_tma<R, 0, true> : (K)k_sweep_tma<R, 0, false>;
-    else                  kern = uniform_mu ? (K)k_sweep_tma<R, 1, true> : (K)k_sweep_tma<R, 1, false>;
-    cudaError_t e = cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
-    if (e != cudaSuccess) return e;
+    if (thermal) th = *thermal;
+    const int threads = thermal ? Tile<sizeof(R), true>::threads : Tile<sizeof(R)>::threads;
     kern<<<plan.n_tiles * plan.nzs, threads, smem_bytes, stream>>>(maps, p, src, fs, zc, plan.ntx, step, th);
     return cudaGetLastError();
 }

@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(256) k_joule_thermal(DevParams<R> p, ThermalPa
     lap = mad(rdz, half_cell_cond(gz, p.rdz[k + 1] * s_th[p.mat[o + PXY]].k) * (th - t.theta[o + PXY]), lap);
     const R thn = th - p.dt * me.irc * lap + dq * me.irc;
     t.theta_n[o] = thn;
-    t.sig[o] = me.sigma0 * rcp<R>(R(1) + me.alpha * thn);
+    t.sig[o] = me.sigma0 * rcp<R>(thermal_den(me.alpha, thn));
 }
 
 // Conduction half of eq. (5) for the coupled sweep: theta_d = theta^n - dt/(rho c_p) (M_kk theta^n), all cells, into the
@@ -230,7 +230,7 @@ __global__ void __launch_bounds__(256) k_sigma_refresh(DevParams<R> p, ThermalPa
     if (i >= p.nx || j >= p.ny) return;
     const long long o = ((long long)k * p.PY + j) * p.PX + i;
     const ThEntry<R> me = t.ttable[p.mat[o]];
-    t.sig[o] = me.sigma0 / (R(1) + me.alpha * t.theta[o]);
+    t.sig[o] = me.sigma0 / thermal_den(me.alpha, t.theta[o]);
 }
 
 // p_c = sigma_c(T) * 1/4 sum_12 (E_e)^2 with the CURRENT conductivity (PAPER.md L86 with eq. (6))

@@ -27,6 +27,7 @@ pytestmark = [pytest.mark.gpu, pytest.mark.slow]
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 NAMES = ("Ex", "Ey", "Ez", "Hx", "Hy", "Hz")
+MAXNORM_FACTOR = 10
 
 
 def _record(rec):
@@ -53,8 +54,12 @@ def _field_numbers(g, o):
     for c in range(6):
         fg = g.em_get_field(c)
         d = np.asarray(fg, np.float64); d -= Fo[c]
-        num[c // 3] += float(np.sum(d * d)); den[c // 3] += float(np.sum(Fo[c] * Fo[c]))
-        res[NAMES[c] + "_max"] = float(np.max(np.abs(d))) / grp_max[c // 3]      # max |diff| / max-norm of the group
+        num[c // 3] += float(np.vdot(d, d)); den[c // 3] += float(np.vdot(Fo[c], Fo[c]))
+        np.abs(d, out=d)
+        at = int(np.argmax(d))
+        res[NAMES[c] + "_max"] = float(d.flat[at]) / grp_max[c // 3]            # max |diff| / max-norm of the group
+        k, j, i = np.unravel_index(at, d.shape)
+        res[NAMES[c] + "_at"] = [int(i), int(j), int(k), float(abs(Fo[c].flat[at])) / grp_max[c // 3]]   # where, and |field| there / max-norm
         del d, fg
     res["E"] = (num[0] / den[0]) ** 0.5; res["H"] = (num[1] / den[1]) ** 0.5
     return res
@@ -84,16 +89,18 @@ def _run(cfg, precisions, steps, outputs_every=0, **kw):
     rec["oracle_seconds"] = time.time() - t0
     for pr, g in gs.items():
         assert g.step_index == steps
-        res = {**_field_numbers(g, o), **_joule_numbers(g, o)}
-        rec["fp%d" % pr] = res
-        _record({"partial": "fp%d" % pr, "config": cfg, **res})     # (kept even if a later assert fails)
-        tol = TOL[pr]
-        assert res["E"] <= tol and res["H"] <= tol and res["q"] <= tol and res["Q"] <= tol, res
-        assert all(res[n + "_max"] <= tol for n in NAMES) and res["qmax"] <= tol, res
+        rec["fp%d" % pr] = {**_field_numbers(g, o), **_joule_numbers(g, o)}
         g.close()
     o.close()
     rec["wall_seconds"] = time.time() - t0
     _record(rec)
+    for pr in precisions:
+        res, tol = rec["fp%d" % pr], TOL[pr]
+        # north_star's metric: relative L2 of E, H, the Joule map, and the Joule total
+        assert res["E"] <= tol and res["H"] <= tol and res["q"] <= tol and res["Q"] <= tol, res
+        # pointwise: max |diff| / max-norm of the group.  Not bounded by the L2 bound (the accumulated rounding of
+        # thousands of steps peaks where the field peaks); a wrong edge on a tile or chunk seam would show as 1e-2 .. 1
+        assert all(res[n + "_max"] <= MAXNORM_FACTOR * tol for n in NAMES) and res["qmax"] <= MAXNORM_FACTOR * tol, res
     return rec
 
 

@@ -14,13 +14,11 @@ from parity import TOL, compare_state, rel_l2, subbox_problem
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [pytest.param(P.EM_KERNEL_SPLIT, id="split"), pytest.param(P.EM_KERNEL_FUSED, id="fused"),
-           pytest.param(P.EM_KERNEL_TMA, id="tma")]
-KNAME = {P.EM_KERNEL_SPLIT: "split", P.EM_KERNEL_FUSED: "fused", P.EM_KERNEL_TMA: "tma"}
+KERNELS = [pytest.param(P.EM_KERNEL_SPLIT, id="split"), pytest.param(P.EM_KERNEL_TMA, id="tma")]
 
 
-def run_pair(p, steps, precision, kernel, checkpoints=()):
-    g = P.EM(p, precision=precision, kernel=kernel)
+def run_pair(p, steps, precision, kernel, checkpoints=(), **em_kw):
+    g = P.EM(p, precision=precision, kernel=kernel, **em_kw)
     o = emo.Oracle(p)
     tol = TOL[precision]
     done = 0
@@ -74,30 +72,22 @@ def test_random_grids_cd(dims, precision, kernel):
 
 
 @pytest.mark.parametrize("zsplit", [1, 2, 3, 5, 8])
-def test_fused_z_chunks(zsplit, monkeypatch):
-    """The fused sweep splits every tile column into z chunks (work items); many ports so that source
-    edges sit on chunk boundary planes (their E' closes the Joule sum of the chunk below)."""
-    monkeypatch.setenv("EM_FUSED_ZSPLIT", str(zsplit))
-    p = W.random_problem(21, 18, 33, seed=77, loss_mode=LOSS_CD, steps=30, n_ports=60)
-    run_pair(p, 30, 64, P.EM_KERNEL_FUSED, checkpoints=(1, 7))
+@pytest.mark.parametrize("bc", [(0,) * 6, (0, 0, 1, 0, 1, 1)])
+def test_tma_sweep_z_chunks(zsplit, bc):
+    """The sweep splits every tile column into z chunks (work items; em_grid.z_chunks forces the count); many ports so
+    that source edges sit on chunk boundary planes (their E' closes the Joule sum of the chunk below)."""
+    p = W.random_problem(21, 18, 33, seed=78, loss_mode=LOSS_CD, steps=30, n_ports=60, bc=bc)
+    run_pair(p, 30, 64, P.EM_KERNEL_TMA, checkpoints=(1, 7), z_chunks=zsplit)
 
 
-@pytest.mark.parametrize("zsplit", [1, 2, 3, 5, 8])
-def test_tma_sweep_z_chunks(zsplit, monkeypatch):
-    monkeypatch.setenv("EM_FUSED_ZSPLIT", str(zsplit))
-    p = W.random_problem(21, 18, 33, seed=78, loss_mode=LOSS_CD, steps=30, n_ports=60, bc=(0, 0, 1, 0, 1, 1))
-    run_pair(p, 30, 64, P.EM_KERNEL_TMA, checkpoints=(1, 7))
-
-
-def test_tma_sweep_is_deterministic_across_runs_and_chunkings(monkeypatch):
+def test_tma_sweep_is_deterministic_across_runs_and_chunkings():
     """The TMA sweep has no CTA barrier in its plane loop (mbarrier / named-barrier hand-offs between rows): a missing
     ordering would show up as run-to-run or chunking-dependent bits.  256 x 256 x 192 package slice, 228 work items
     and more, 40 steps, fp32: every run must give IDENTICAL bits."""
     p = W.make_config(4, scale=4, steps=40)
     ref = None
-    for zsplit in ("3", "3", "1", "8", "3"):
-        monkeypatch.setenv("EM_FUSED_ZSPLIT", zsplit)
-        g = P.EM(p, precision=32, kernel=P.EM_KERNEL_TMA)
+    for zsplit in (3, 3, 1, 8, 3):
+        g = P.EM(p, precision=32, kernel=P.EM_KERNEL_TMA, z_chunks=zsplit)
         g.em_step(40)
         out = [g.em_get_field(c) for c in range(6)] + [g.joule_maps()[1]]
         g.close()
@@ -133,10 +123,9 @@ def test_random_grids_pmc_walls(dims, bc, precision, kernel):
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-def test_pmc_exp_loss_and_z_chunks(kernel, monkeypatch):
-    monkeypatch.setenv("EM_FUSED_ZSPLIT", "3")
+def test_pmc_exp_loss_and_z_chunks(kernel):
     p = W.random_problem(21, 18, 33, seed=5101, loss_mode=LOSS_EXP, steps=30, n_ports=20, bc=(0, 1, 1, 1, 1, 1))
-    run_pair(p, 30, 64, kernel, checkpoints=(1, 7))
+    run_pair(p, 30, 64, kernel, checkpoints=(1, 7), z_chunks=3)
 
 
 @pytest.mark.parametrize("kernel", KERNELS)

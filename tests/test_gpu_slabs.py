@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("n_ranks", [2, 3])
-@pytest.mark.parametrize("kernel", [P.EM_KERNEL_TMA, P.EM_KERNEL_FUSED, P.EM_KERNEL_SPLIT])
+@pytest.mark.parametrize("kernel", [P.EM_KERNEL_TMA, P.EM_KERNEL_SPLIT])
 @pytest.mark.parametrize("precision", [64, 32])
 def test_slabs_equal_single_domain(n_ranks, kernel, precision):
     p = W.random_problem(21, 18, 13, seed=9000 + n_ranks, loss_mode=LOSS_CD, steps=40, n_ports=25, bc=(0, 1, 0, 0, 0, 1))

@@ -25,8 +25,8 @@ def _coupled(dims, seed, k_scale=2.0e5, tcr_scale=1.0e4, **kw):
 STRATEGIES = [pytest.param(P.EM_KERNEL_AUTO, id="coupled-sweep"), pytest.param(P.EM_KERNEL_SPLIT, id="split")]
 
 
-def _run(p, steps, precision, checkpoints=(), kernel=P.EM_KERNEL_AUTO):
-    g = P.EM(p, precision=precision, kernel=kernel)
+def _run(p, steps, precision, checkpoints=(), kernel=P.EM_KERNEL_AUTO, **em_kw):
+    g = P.EM(p, precision=precision, kernel=kernel, **em_kw)
     o = emo.Oracle(p)
     tol = TOL[precision]
     done = 0
@@ -62,10 +62,9 @@ def test_coupled_with_pmc_walls_and_wall_port(kernel):
 
 
 @pytest.mark.parametrize("zsplit", [1, 3, 8])
-def test_coupled_sweep_z_chunks(zsplit, monkeypatch):
-    monkeypatch.setenv("EM_FUSED_ZSPLIT", str(zsplit))
+def test_coupled_sweep_z_chunks(zsplit):
     p = _coupled((21, 18, 33), 8104, steps=30, n_ports=40, init_scale=4.0e6)
-    _run(p, 30, 64, checkpoints=(1, 7))
+    _run(p, 30, 64, checkpoints=(1, 7), z_chunks=zsplit)
 
 
 def test_pure_diffusion_and_set_get_temperature():
@@ -106,4 +105,8 @@ def test_thermal_needs_flag_and_a_coupled_strategy():
     g.close()
     p.thermal = W.thermal_table()
     with pytest.raises(P.EMError):
-        P.EM(p, kernel=P.EM_KERNEL_FUSED)                     # the cp.async sweep takes sigma from the table only
+        P.EM(p, formulation=P.EM_FORM_EONLY)                  # the E-only recurrence has no coupled variant
+    bad = W.thermal_table(); bad[3, 2] = float("nan")
+    p.thermal = bad
+    with pytest.raises(P.EMError):
+        P.EM(p)                                               # alpha must be finite
