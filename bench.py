@@ -6,9 +6,9 @@ accumulation + PEC masks, one em_step) on the full-package config of BASELINE.js
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--scale 1] [--impl reference]
 
-N > 1 (torchrun): every rank runs an independent replica of the same problem ("replicas only":
-the path has no data-parallel split inside one problem that would not need a halo exchange; see
-DESIGN.md "Multi-GPU"); value = cells * steps * N / max-over-ranks time.
+N > 1 (torchrun): ONE problem cut into z slabs, one rank per slab (strong scaling; the halo of SURVEY.md 8(e) is
+fused into the sweep as peer stores, --halo p2p uses NCCL send/recv instead); --decomp replicas runs N independent
+replicas (weak scaling).  value = whole-job cell-updates / max-over-ranks device time.
 """
 from __future__ import annotations
 
@@ -24,6 +24,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 B_MIN = {32: 57, 64: 113}     # algorithmic bytes per cell-update (DESIGN.md / SURVEY.md 8(d))
+B_EONLY = {32: 45, 64: 89}    # E-only recurrence of eq. (2): 9 field words + 1 B id + 2 words of q
 
 
 def parse():
@@ -35,12 +36,22 @@ def parse():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--scale", type=int, default=1)
     ap.add_argument("--precision", type=int, default=0, help="0 = the config's own")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "split", "fused", "tma"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "split", "tma"])
+    ap.add_argument("--formulation", default="leapfrog", choices=["leapfrog", "eonly"],
+                    help="eonly: the paper's literal three-level recurrence of eq. (2) (state e^n, e^{n-1}; 45 B fp32 / "
+                         "89 B fp64 per cell-update; fp32 leaves the 2e-5 parity bound on long runs, see DESIGN.md)")
+    ap.add_argument("--force-joule-output", action="store_true",
+                    help="one Joule-map output at the end of every timed repetition even when K is below the config's "
+                         "cadence (default: outputs fall where the cadence puts them; their count is stated in config)")
+    ap.add_argument("--reps", type=int, default=3, help="timed repetitions of the K steps (each after em_reset); the median is reported")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slabs"],
-                    help="N > 1: independent replicas (default, weak scaling) or ONE problem cut into z slabs with a "
-                         "two-plane halo exchange per step over NCCL (strong scaling; paper_2603_07038_b200/slabs.py)")
+    ap.add_argument("--decomp", default="slabs", choices=["slabs", "replicas"],
+                    help="N > 1: ONE problem cut into z slabs (default; strong scaling; SURVEY.md 8(e); "
+                         "paper_2603_07038_b200/slabs.py) or N independent replicas (weak scaling, no data plane)")
+    ap.add_argument("--halo", default="peer", choices=["peer", "p2p"],
+                    help="slabs: halo stores fused into the sweep over a CUDA IPC / NVLink peer mapping + one tiny all-reduce "
+                         "per step (default), or pack kernel -> NCCL send/recv -> unpack kernel")
     ap.add_argument("--thermal", action="store_true",
                     help="two-way EM-thermal coupling (PAPER.md eq. (4)-(6)) with the handbook-order thermal table")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -94,15 +105,15 @@ def measured_peak():
 
 def ncu_traffic(kernel_name: str, cells: int):
     """dram bytes per launch of the dominant kernel from the committed ncu summary, if any."""
-    path = os.path.join(ROOT, "profiles", "r1_traffic.txt")     # JSON text written from the ncu summary beside it
-    try:
-        with open(path) as f:
-            t = json.load(f)
-        ent = t.get(kernel_name)
-        if ent and ent.get("cells") == cells:
-            return float(ent["dram_bytes_per_launch"])
-    except Exception:
-        pass
+    for name in ("r2_traffic.txt", "r1_traffic.txt"):            # JSON text written from the ncu summary beside it
+        try:
+            with open(os.path.join(ROOT, "profiles", name)) as f:
+                t = json.load(f)
+            ent = t.get(kernel_name)
+            if ent and ent.get("cells") == cells:
+                return float(ent["dram_bytes_per_launch"])
+        except Exception:
+            pass
     return None
 
 
@@ -204,16 +215,22 @@ def run_b200(args):
 
     p = make_problem(args)
     precision = args.precision or p.precision
-    kernel = {"auto": P.EM_KERNEL_AUTO, "split": P.EM_KERNEL_SPLIT, "fused": P.EM_KERNEL_FUSED, "tma": P.EM_KERNEL_TMA}[args.kernel]
+    kernel = {"auto": P.EM_KERNEL_AUTO, "split": P.EM_KERNEL_SPLIT, "tma": P.EM_KERNEL_TMA}[args.kernel]
+    form = P.EM_FORM_EONLY if args.formulation == "eonly" else P.EM_FORM_LEAPFROG
+    comps = (0, 1, 2, 6, 7, 8) if form == P.EM_FORM_EONLY else tuple(range(6))
     K, Wm = args.steps, args.warmup
     slab = None
     p_global = p
     if args.decomp == "slabs" and world > 1:
         from paper_2603_07038_b200 import slabs
+        if form == P.EM_FORM_EONLY:
+            raise SystemExit("the z-slab halo covers the leapfrog formulation: use --decomp replicas with --formulation eonly")
         p, meta = slabs.sub_problem(p_global, rank, world)       # this rank's extended slab (PMC on the artificial walls)
-    em = P.EM(p, precision=precision, kernel=kernel, device=dev)
+    em = P.EM(p, precision=precision, kernel=kernel, device=dev, formulation=form)
     if args.decomp == "slabs" and world > 1:
         slab = slabs.SlabRank(em, meta)
+        if args.halo == "peer" and not args.thermal and form == P.EM_FORM_LEAPFROG and kernel != P.EM_KERNEL_SPLIT:
+            slabs.connect_peers_dist(slab, dist)
         args.no_e2e = True                                       # the end-to-end leg is defined for whole problems
     cells = p.n_cells
     je = p.joule_every if p.joule_every else 0
@@ -225,9 +242,12 @@ def run_b200(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    def run_steps(n, start):
-        """n steps with the config's Joule-map outputs (to device buffers) inside."""
-        done = 0
+    outputs = [0]
+
+    def run_steps(n, start, force_output=False):
+        """n steps with the config's Joule-map outputs (energy + power maps to device buffers) inside: every
+        joule_every steps, and (force_output) once at the end if the run is too short to reach one."""
+        done = 0; made = 0
         while done < n:
             nxt = n - done
             if je:
@@ -236,30 +256,42 @@ def run_b200(args):
             if slab is None:
                 em.em_step(nxt)
             else:                                                # one halo exchange after every step
-                for _ in range(nxt):
-                    em.em_step(1)
-                    slabs.exchange_dist(slab, dist)
+                slab.step(nxt, dist)
             done += nxt
             if je and (start + done) % je == 0:
-                em.em_joule(pw_map, q_map, total=False)
+                em.em_joule(pw_map, q_map, total=False); made += 1
+        if je and force_output and made == 0:
+            em.em_joule(pw_map, q_map, total=False); made += 1
+        outputs[0] = made
 
-    # ---- device-resident timing ------------------------------------------------------------------
+    # ---- device-resident timing: W warm-up steps, then `reps` repetitions of [em_reset, K steps]; the MEDIAN repetition
+    # is reported.  Every repetition contains at least one Joule-map output when the config has them.
     run_steps(Wm, 0)
     em.em_timing_enable(True)
     sampler = ClockSampler(local); sampler.start()
     l0 = em.launch_count
-    barrier()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record()
-    run_steps(K, Wm)
-    ev1.record()
-    barrier()
+    rep_ms = []
+    for _ in range(max(args.reps, 1)):
+        em.em_reset() if slab is None else slab.reset()
+        barrier()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        run_steps(K, 0, force_output=args.force_joule_output)
+        ev1.record()
+        barrier()
+        rep_ms.append(max_over_ranks(ev0.elapsed_time(ev1), dist, dev))
     sampler.stop_flag = True
-    ms = ev0.elapsed_time(ev1)
-    launches = em.launch_count - l0
+    out_ms = None
+    if je:                               # one Joule-map output (energy + power maps to device buffers), timed on its own
+        barrier()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(); em.em_joule(pw_map, q_map, total=False); ev1.record()
+        barrier()
+        out_ms = ev0.elapsed_time(ev1)
+    ms = sorted(rep_ms)[len(rep_ms) // 2]
+    launches = (em.launch_count - l0) // max(args.reps, 1)
     kname, klaunch, kms = em.em_timing_read()
     em.em_timing_enable(False)
-    ms = max_over_ranks(ms, dist, dev)
     kcells = p.n_cells
     if slab is None:
         value = aggregate_throughput(cells * K, ms * 1e-3, world)
@@ -273,17 +305,20 @@ def run_b200(args):
         shapes = em.shapes
         host_in = [torch.zeros(s, dtype=em.dtype).pin_memory() for s in shapes]
         rng = np.random.default_rng(7)
-        for c, h in enumerate(host_in):                      # small seeded seed field, not all zeros
-            h.view(-1)[:: max(1, h.numel() // 4096)] = float(rng.standard_normal()) * (1.0 if c < 3 else 1 / 376.73)
-        host_out = [torch.empty(s, dtype=em.dtype).pin_memory() for s in shapes]
+        host_in = [host_in[c] for c in comps]
+        for c, h in zip(comps, host_in):                     # small seeded seed field, not all zeros
+            h.view(-1)[:: max(1, h.numel() // 4096)] = float(rng.standard_normal()) * (1 / 376.73 if 3 <= c < 6 else 1.0)
+        host_out = [torch.empty(shapes[c], dtype=em.dtype).pin_memory() for c in comps]
         host_q = torch.empty((p.nz, p.ny, p.nx), dtype=em.dtype).pin_memory()
         probes = p.probes if len(p.probes) else np.asarray([[0, 0, 1, 1]], np.int32)
+        if form == P.EM_FORM_EONLY:                          # (an E-only context has no H to probe)
+            probes = probes[probes[:, 0] < 3] if (probes[:, 0] < 3).any() else np.asarray([[0, 0, 1, 1]], np.int32)
         em.em_reset()
         barrier()
         t0 = time.perf_counter()
         h2d = d2h = 0
-        for c in range(6):
-            em.em_set_field(c, host_in[c].numpy()); h2d += host_in[c].numel() * host_in[c].element_size()
+        for n, c in enumerate(comps):
+            em.em_set_field(c, host_in[n].numpy()); h2d += host_in[n].numel() * host_in[n].element_size()
         done = 0
         while done < K:
             nxt = min(K - done, (je - (done % je)) if je else 64)
@@ -292,8 +327,8 @@ def run_b200(args):
             if je and done % je == 0:
                 em.em_joule(pw_map, q_map, total=False)
                 host_q.copy_(q_map, non_blocking=False); d2h += host_q.numel() * host_q.element_size()
-        for c in range(6):
-            em.em_get_field(c, host_out[c].numpy()); d2h += host_out[c].numel() * host_out[c].element_size()
+        for n, c in enumerate(comps):
+            em.em_get_field(c, host_out[n].numpy()); d2h += host_out[n].numel() * host_out[n].element_size()
         tot = em.em_joule(None, None, total=True); d2h += 8
         torch.cuda.synchronize(dev)
         el = time.perf_counter() - t0
@@ -304,6 +339,7 @@ def run_b200(args):
                        % (K, " and Joule maps to host every %d steps" % je if je else "")}
         del host_in, host_out, host_q
 
+    q_total = slab.joule_total(dist) if slab is not None else None     # all-reduce of the owned layers' Joule totals
     if rank != 0:
         em.close()
         if dist is not None:
@@ -311,7 +347,7 @@ def run_b200(args):
         return
 
     peak, peak_src = measured_peak()
-    bmin = B_MIN[precision]
+    bmin = B_EONLY[precision] if form == P.EM_FORM_EONLY else B_MIN[precision]
     if args.thermal:                 # + theta read/write + sigma(T) read/write per cell-update
         bmin += 4 * (precision // 8)
     avg_ms = kms / max(klaunch, 1)
@@ -332,7 +368,10 @@ def run_b200(args):
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bmin * kcells,
                 "avg_launch_ms": avg_ms, "launches_timed": klaunch,
                 "step_effective_GBps": bmin * value / world / 1e9, "step_frac_of_peak": bmin * value / world / 1e9 / peak,
-                "frac_of_8TBps_nominal": (achieved / 8000.0) if achieved else None}
+                "frac_of_8TBps_nominal": (achieved / 8000.0) if achieved else None,
+                "algorithmic_bytes_per_cell_update": bmin}
+    if form == P.EM_FORM_EONLY:      # the same cell-updates/s expressed in the leapfrog's B_min: may exceed 1, not clipped
+        roofline["frac_in_leapfrog_bytes"] = B_MIN[precision] * kcells / (avg_ms * 1e-3) / 1e9 / peak
     cpu = None
     if not args.no_cpu_baseline:
         rate, threads, sample, ms_cpu, _ = cpu_oracle_rate(args, args.cpu_seconds)
@@ -348,12 +387,19 @@ def run_b200(args):
                                % (args.config, p_global.name, p_global.nx, p_global.ny, p_global.nz, cells, p_global.n_ports,
                                   "EXP" if p.loss_mode else "CD", je or "-")
                                + (", walls -x+x-y+y-z+z = %s (1 = PMC)" % "".join(str(int(b)) for b in p.bc) if any(p.bc) else "")
+                               + (", E-only three-level recurrence of eq. (2)" if form == P.EM_FORM_EONLY else "")
+                               + (", %d Joule-map output(s) inside each timed repetition of %d steps (one output = %.2f ms, "
+                                  "i.e. +%.3f ms/step at the config's cadence)" % (outputs[0], K, out_ms, out_ms / je) if je else "")
                                + (", two-way thermal coupling (%s)" % ("split kernels" if args.kernel == "split" else "coupled TMA sweep + conduction kernel") if args.thermal else ""),
                    "kernel_strategy": args.kernel, "l2": "state %.1f GB >> 126 MB L2 (no flush needed)" % (em.workspace_bytes / 1e9)
                    if em.workspace_bytes > 1e9 else "state fits L2: %.0f MB" % (em.workspace_bytes / 1e6),
-                   "parallelism": ("z-slabs x%d, 2-plane halo exchange per step" % world if slab is not None else
+                   "parallelism": ("z-slabs x%d, halo per step: %s" % (world, "Ex, Ey wall planes stored by the sweep into the "
+                                   "neighbour's memory (peer mapping) + one 4-byte all-reduce" if slab.mode == "peer" else
+                                   "pack kernel, NCCL send/recv, unpack kernel") if slab is not None else
                                    "replicas x%d" % world) if world > 1 else "single GPU"},
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
+        "joule_total_J": q_total,
+        "timing": {"reps": len(rep_ms), "ms_per_rep": rep_ms, "reported": "median", "reset_before_each_rep": True},
         "clocks": sampler.summary(),
     }
     print(json.dumps(line))

@@ -160,6 +160,34 @@ int32_t em_get_field(em_ctx *ctx, int32_t comp, void *dst, int32_t dst_is_device
 int32_t em_get_plane(em_ctx *ctx, int32_t comp, int32_t k, void *dst, int32_t dst_is_device);
 int32_t em_set_plane(em_ctx *ctx, int32_t comp, int32_t k, const void *src, int32_t src_is_device);
 
+/* ---- z-slab halo in two calls (paper_2603_07038_b200/slabs.py) -------------------------------------
+ * The halo of a slab after a step is the tangential E of ONE node plane per neighbour -- and, in a thermally coupled
+ * context, the temperature rise of the cell layer behind it (the ghost layer's theta and sigma(T) feed the owned layer's
+ * conduction and edge conductivities).  Packed DEVICE buffer of em_halo_elems values in the working precision:
+ * [Ex plane (ny+1) x nx | Ey plane ny x (nx+1) | theta layer ny x nx (coupled contexts only)].
+ * em_get_halo packs node plane k_plane (and cell layer k_layer) with one kernel; em_set_halo unpacks with one kernel,
+ * keeping PEC-fixed edges at 0 and refreshing sigma(T) of the layer.  stream: cudaStream_t to enqueue on (NULL: the
+ * context's stream); ordering between streams is the caller's.  Leapfrog contexts only (UNSUPPORTED otherwise). */
+int32_t em_halo_elems(em_ctx *ctx, int64_t *n);
+int32_t em_get_halo(em_ctx *ctx, int32_t k_plane, int32_t k_layer, void *dst_device, void *stream);
+int32_t em_set_halo(em_ctx *ctx, int32_t k_plane, int32_t k_layer, const void *src_device, void *stream);
+
+/* The same halo FUSED into the sweep: direct stores into the neighbouring slab's memory (NVLink peer mapping, CUDA IPC
+ * or the same device).  em_wall_offset: byte offset, from this context's workspace base, of element (0, 0) of its wall
+ * plane (side 0: the -z wall, plane 0; side 1: the +z wall, plane nz) in the E array of ping-pong parity 0/1, comp
+ * 0 = Ex, 1 = Ey.  The NEIGHBOUR adds that offset to its mapping of this workspace and passes the four addresses
+ * (dst[parity * 2 + comp]) to em_set_peer_halo(side, k_send, dst) on ITS context: from then on its sweep also stores
+ * E'x, E'y of its node plane k_send there, and no longer stores its own wall plane on that side (the neighbour feeds it).
+ * Both contexts must step in lockstep (same number of steps since em_create / em_reset) with one cross-rank barrier
+ * between steps; dst = NULL switches the side off.  Leapfrog TMA sweep only, no thermal coupling (UNSUPPORTED).
+ * Errors: INVALID_ARG, STATE (the wall on that side is not an artificial PMC wall), UNSUPPORTED. */
+int32_t em_wall_offset(em_ctx *ctx, int32_t side, int32_t parity, int32_t comp, size_t *byte_offset);
+int32_t em_set_peer_halo(em_ctx *ctx, int32_t side, int32_t k_send, void *const dst[4]);
+
+/* Joule energy of the cell layers k0 <= k < k1 only: sum q_c V_c [J] (HOST scalar; synchronises).  A slab reports its
+ * OWNED layers with this and the ranks all-reduce the sum. */
+int32_t em_joule_layers(em_ctx *ctx, int32_t k0, int32_t k1, double *total_energy);
+
 /* Advance n >= 0 steps (n = 0 is a no-op).  Per step: H^{n+1/2} = H^{n-1/2} - dt nu (C_e E^n);
  * E^{n+1} = ca E^n + cb (C_h H^{n+1/2} - J^{n+1/2}) on non-fixed edges; Joule energy density
  * q_c += dt sigma_c 1/4 sum over the 12 edges of c of ((E^{n+1} + E^n)/2)^2.  Asynchronous. */

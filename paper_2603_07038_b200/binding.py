@@ -98,6 +98,12 @@ def load():
     L.em_get_field.argtypes = [vp, i32, vp, i32]
     L.em_get_plane.argtypes = [vp, i32, i32, vp, i32]
     L.em_set_plane.argtypes = [vp, i32, i32, vp, i32]
+    L.em_halo_elems.argtypes = [vp, C.POINTER(i64)]
+    L.em_get_halo.argtypes = [vp, i32, i32, vp, vp]
+    L.em_set_halo.argtypes = [vp, i32, i32, vp, vp]
+    L.em_joule_layers.argtypes = [vp, i32, i32, C.POINTER(C.c_double)]
+    L.em_wall_offset.argtypes = [vp, i32, i32, i32, C.POINTER(C.c_size_t)]
+    L.em_set_peer_halo.argtypes = [vp, i32, i32, C.POINTER(vp)]
     L.em_step.argtypes = [vp, i64]
     L.em_joule.argtypes = [vp, vp, vp, C.POINTER(C.c_double), i32]
     L.em_probe.argtypes = [vp, i32, C.POINTER(em_probe_pt), C.POINTER(C.c_double)]
@@ -297,6 +303,53 @@ class EM:
     def em_set_plane(self, comp: int, k: int, t):
         assert tuple(t.shape) == tuple(self.shapes[comp][1:]) and t.dtype == self.dtype and t.is_contiguous()
         _check(self._L.em_set_plane(self._h, comp, int(k), C.c_void_p(t.data_ptr()), 1 if t.is_cuda else 0))
+
+    # z-slab halo (include/em.h): packed [Ex | Ey (| theta)] of one node plane (and the cell layer behind it)
+    @property
+    def halo_elems(self) -> int:
+        n = C.c_int64()
+        _check(self._L.em_halo_elems(self._h, C.byref(n)))
+        return int(n.value)
+
+    def em_get_halo(self, k_plane: int, k_layer: int, out, stream=None):
+        assert out.is_cuda and out.dtype == self.dtype and out.is_contiguous() and out.numel() >= self.halo_elems
+        _check(self._L.em_get_halo(self._h, int(k_plane), int(k_layer), C.c_void_p(out.data_ptr()),
+                                   C.c_void_p(stream.cuda_stream) if stream is not None else None))
+        return out
+
+    def em_set_halo(self, k_plane: int, k_layer: int, src, stream=None):
+        assert src.is_cuda and src.dtype == self.dtype and src.is_contiguous() and src.numel() >= self.halo_elems
+        _check(self._L.em_set_halo(self._h, int(k_plane), int(k_layer), C.c_void_p(src.data_ptr()),
+                                   C.c_void_p(stream.cuda_stream) if stream is not None else None))
+
+    def em_joule_layers(self, k0: int, k1: int) -> float:
+        tot = C.c_double()
+        _check(self._L.em_joule_layers(self._h, int(k0), int(k1), C.byref(tot)))
+        return tot.value
+
+    def new_halo_buffer(self):
+        return self._torch.empty(self.halo_elems, dtype=self.dtype, device=self.device)
+
+    @property
+    def workspace_ptr(self) -> int:
+        return self._ws_ptr
+
+    def em_wall_offset(self, side: int, parity: int, comp: int) -> int:
+        off = C.c_size_t()
+        _check(self._L.em_wall_offset(self._h, int(side), int(parity), int(comp), C.byref(off)))
+        return int(off.value)
+
+    def wall_offsets(self, side: int):
+        """[parity * 2 + comp] byte offsets of this context's wall plane (what a neighbour needs for em_set_peer_halo)"""
+        return [self.em_wall_offset(side, q, c) for q in (0, 1) for c in (0, 1)]
+
+    def em_set_peer_halo(self, side: int, k_send: int, addresses):
+        """addresses: four device addresses [parity * 2 + comp] valid in this process, or None to switch the side off"""
+        if addresses is None:
+            _check(self._L.em_set_peer_halo(self._h, int(side), 0, None))
+            return
+        arr = (C.c_void_p * 4)(*[C.c_void_p(int(a)) for a in addresses])
+        _check(self._L.em_set_peer_halo(self._h, int(side), int(k_send), arr))
 
     # thermal coupling (PAPER.md eq. (4)-(6)); the context must come from a problem with p.thermal set
     def em_set_thermal(self, thermal):

@@ -59,6 +59,60 @@ __global__ void __launch_bounds__(256) k_mask_fixed(DevParams<R> p, R *e, int co
     if (m == R(0)) e[o] = R(0);
 }
 
+// Halo of a z-slab decomposition: the tangential E of node plane kp, packed [Ex (ny+1) x nx | Ey ny x (nx+1)],
+// and -- thermally coupled contexts -- the temperature rise of cell layer kl behind it [ny x nx].  One kernel each way.
+template <typename R>
+__global__ void __launch_bounds__(256) k_pack_halo(DevParams<R> p, const R *ex, const R *ey, const R *theta, int kp, int kl, R *dst) {
+    const long long n0 = (long long)(p.ny + 1) * p.nx, n1 = (long long)p.ny * (p.nx + 1), n2 = theta ? (long long)p.ny * p.nx : 0;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n0) {
+        const int j = (int)(t / p.nx), i = (int)(t % p.nx);
+        dst[t] = ex[((long long)kp * p.PY + j) * p.PX + i];
+    } else if (t < n0 + n1) {
+        const long long u = t - n0;
+        const int j = (int)(u / (p.nx + 1)), i = (int)(u % (p.nx + 1));
+        dst[t] = ey[((long long)kp * p.PY + j) * p.PX + i];
+    } else if (t < n0 + n1 + n2) {
+        const long long u = t - n0 - n1;
+        const int j = (int)(u / p.nx), i = (int)(u % p.nx);
+        dst[t] = theta[((long long)kl * p.PY + j) * p.PX + i];
+    }
+}
+
+// The reverse: PEC-fixed edges of the plane stay 0 (the mask product of the edge's four cells, as in k_mask_fixed); the
+// temperature rise goes into the layer and sigma(T) of the layer's cells is refreshed in both sigma buffers (eq. (6)).
+template <typename R>
+__global__ void __launch_bounds__(256) k_unpack_halo(DevParams<R> p, R *ex, R *ey, R *theta, R *sig_a, R *sig_b,
+                                                     const ThEntry<R> *ttable, int kp, int kl, const R *src) {
+    __shared__ MatEntry<R> s_tab[kMaxTable];
+    load_table(s_tab, p);
+    const long long n0 = (long long)(p.ny + 1) * p.nx, n1 = (long long)p.ny * (p.nx + 1), n2 = theta ? (long long)p.ny * p.nx : 0;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long PX = p.PX, PXY = p.PXY;
+    const uint8_t *mat = p.mat;
+    if (t < n0) {
+        const int j = (int)(t / p.nx), i = (int)(t % p.nx);
+        const long long o = ((long long)kp * p.PY + j) * PX + i;
+        const R m = s_tab[mat[o]].m * s_tab[mat[o - PX]].m * s_tab[mat[o - PXY]].m * s_tab[mat[o - PXY - PX]].m;
+        ex[o] = m == R(0) ? R(0) : src[t];
+    } else if (t < n0 + n1) {
+        const long long u = t - n0;
+        const int j = (int)(u / (p.nx + 1)), i = (int)(u % (p.nx + 1));
+        const long long o = ((long long)kp * p.PY + j) * PX + i;
+        const R m = s_tab[mat[o]].m * s_tab[mat[o - 1]].m * s_tab[mat[o - PXY]].m * s_tab[mat[o - PXY - 1]].m;
+        ey[o] = m == R(0) ? R(0) : src[t];
+    } else if (t < n0 + n1 + n2) {
+        const long long u = t - n0 - n1;
+        const int j = (int)(u / p.nx), i = (int)(u % p.nx);
+        const long long o = ((long long)kl * p.PY + j) * PX + i;
+        const ThEntry<R> me = ttable[mat[o]];
+        const R th = src[t];
+        theta[o] = th;
+        const R sg = me.sigma0 * rcp<R>(thermal_den(me.alpha, th));     // the expression of the stepping kernels (bit-identical slabs)
+        sig_a[o] = sg; sig_b[o] = sg;
+    }
+}
+
 // r_e for every unique source edge; flags[u] = 1 if the edge is PEC-fixed (argument error).
 template <typename R, int LOSS>
 __global__ void k_source_coef(DevParams<R> p, DevSources<R> s, int *fixed_flags) {
@@ -112,13 +166,13 @@ __global__ void __launch_bounds__(256) k_power(DevParams<R> p, R *out) {
 // Q = sum_c q_c V_c in fp64, fixed order: per-block partials then one block.
 template <typename R>
 __global__ void __launch_bounds__(256) k_energy_partial(DevParams<R> p, const double *vx, const double *vy,
-                                                        const double *vz, double *partial) {
+                                                        const double *vz, int k0, int k1, double *partial) {
     __shared__ double sh[256];
-    const long long ncell = (long long)p.nx * p.ny * p.nz;
+    const long long ncell = (long long)p.nx * p.ny * (k1 - k0);           // cell layers k0 <= k < k1
     double acc = 0.0;
     for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += (long long)gridDim.x * blockDim.x) {
         const int i = (int)(c % p.nx); const long long t = c / p.nx;
-        const int j = (int)(t % p.ny); const int k = (int)(t / p.ny);
+        const int j = (int)(t % p.ny); const int k = k0 + (int)(t / p.ny);
         acc += (double)p.q[((long long)k * p.PY + j) * p.PX + i] * (vx[i] * vy[j] * vz[k]);
     }
     sh[threadIdx.x] = acc;

@@ -40,8 +40,15 @@ struct DevParams {
     // per-axis arrays indexed [-1 .. n+1] (pointer shifted to index 0):
     //   rd = 1/d (0 outside), rt = 1/d~, f = d[i]/(d[i-1]+d[i]) with d[-1] = d[n] = 0
     const R *rdx, *rtx, *fx, *rdy, *rty, *fy, *rdz, *rtz, *fz;
-    const R *zgeo;           // interleaved {fz, 1/dz, 1/dz~, 0} per plane (one 4-vector fetch per plane in the fused sweep)
+    const R *zgeo;           // interleaved {fz, 1/dz, 1/dz~, 0} per plane (one bulk copy per plane in the sweep)
     R dt;
+    // z-slab halo fused into the sweep (em_set_peer_halo; SURVEY.md 8(e) "direct peer stores over NVLink"): E'x, E'y of
+    // node plane peer_k[s] are ALSO stored into the neighbouring slab's wall plane -- peer_e[s][comp] is the address of
+    // element (0, 0) of that plane in the neighbour's E^{n+1} array, a peer-mapped pointer -- and the own wall planes
+    // fed by a neighbour are not stored (peer_skip bit 0: plane 0, bit 1: plane nz).  peer_k = -1000: side unused.
+    R *peer_e[2][2];
+    int peer_k[2];
+    int peer_skip;
 };
 
 // Thermal coupling (eq. (4)-(6)).  Per material: 1/(rho c_p), k, alpha, sigma_0; the "outside" entries are all

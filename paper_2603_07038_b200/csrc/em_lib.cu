@@ -156,6 +156,11 @@ struct em_ctx {
     virtual int32_t reset() = 0;
     virtual int32_t set_thermal(const em_thermal_material *, int32_t) = 0;
     virtual int32_t temperature_rise(void *, const void *, int32_t) = 0;
+    virtual int32_t halo(int32_t kp, int32_t kl, void *dst, const void *src, void *stream) = 0;
+    virtual int32_t halo_elems(int64_t *n) = 0;
+    virtual int32_t joule_layers(int32_t k0, int32_t k1, double *total) = 0;
+    virtual int32_t wall_offset(int32_t side, int32_t parity, int32_t comp, size_t *off) = 0;
+    virtual int32_t set_peer_halo(int32_t side, int32_t k_send, void *const dst[4]) = 0;
     int64_t step_index = 0, launches = 0;
     Timing timing;
     const char *main_kernel = "";
@@ -212,6 +217,8 @@ struct Ctx final : em_ctx {
                 p.H[a] = org(6 + h_cur * 3 + a); p.Hn[a] = org(6 + (1 - h_cur) * 3 + a);
             }
         }
+        // the neighbouring slabs step in lockstep: their E^{n+1} array has the parity of mine
+        for (int sd = 0; sd < 2; ++sd) for (int cc = 0; cc < 2; ++cc) p.peer_e[sd][cc] = peer_dst[sd][1 - e_cur][cc];
     }
     int e_cur = 0, h_cur = 0, lvl = 0;
 
@@ -228,6 +235,16 @@ struct Ctx final : em_ctx {
     int32_t reset() override { return zero_state(); }
     int32_t set_thermal(const em_thermal_material *, int32_t) override;
     int32_t temperature_rise(void *dst, const void *src, int32_t is_dev) override;
+    int32_t halo(int32_t kp, int32_t kl, void *dst, const void *src, void *stream) override;
+    int32_t halo_elems(int64_t *n) override {
+        *n = (int64_t)(g.ny + 1) * g.nx + (int64_t)g.ny * (g.nx + 1) + (thermal_on ? (int64_t)g.ny * g.nx : 0);
+        return EM_OK;
+    }
+    int32_t joule_layers(int32_t k0, int32_t k1, double *total) override;
+    int32_t wall_offset(int32_t side, int32_t parity, int32_t comp, size_t *off) override;
+    int32_t set_peer_halo(int32_t side, int32_t k_send, void *const dst[4]) override;
+    void *ws_base = nullptr;
+    R *peer_dst[2][2][2] = {};          // [side][parity of the neighbour's E array][comp]
     int32_t step_thermal();
     int32_t step_thermal_sweep();
     int sg_cur = 0;                     // which sigma(T) buffer is current (the coupled sweep ping-pongs them)
@@ -421,6 +438,8 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     p.rdz = c.axis[6] + 4; p.rtz = c.axis[7] + 4; p.fz = c.axis[8] + 4;
     p.zgeo = c.zgeo + 16;
     p.dt = (R)dt;
+    p.peer_k[0] = p.peer_k[1] = -1000; p.peer_skip = 0;
+    ws_base = workspace;
     src = em::DevSources<R>{};
     src.n_unique = 0;
     CU(cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (plan.n_tiles * plan.nzs + 1), stream));
@@ -658,6 +677,68 @@ int32_t Ctx<R>::get_field(int32_t comp, void *dst, int32_t is_dev) {
     return EM_OK;
 }
 
+// ---- z-slab halo -------------------------------------------------------------------------
+// dst: pack [Ex | Ey] of node plane kp (+ theta of cell layer kl in a coupled context); src: the reverse, PEC-fixed
+// edges kept at 0 and sigma(T) of the layer refreshed.  One kernel, on `st` (null: the context's stream).
+template <typename R>
+int32_t Ctx<R>::halo(int32_t kp, int32_t kl, void *dst, const void *srcp, void *st) {
+    if (eonly) return fail(EM_ERR_UNSUPPORTED, "the halo calls cover the leapfrog formulation");
+    if (kp < 0 || kp > g.nz) return fail(EM_ERR_INVALID_ARG, "halo: node plane out of range");
+    if (thermal_on && (kl < 0 || kl >= g.nz)) return fail(EM_ERR_INVALID_ARG, "halo: cell layer out of range");
+    cudaStream_t s = st ? static_cast<cudaStream_t>(st) : stream;
+    int64_t n = 0; halo_elems(&n);
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    R *th = thermal_on ? c.theta[th_cur] + g.origin : nullptr;
+    if (dst) em::k_pack_halo<R><<<blocks, 256, 0, s>>>(p, p.E[0], p.E[1], th, kp, kl, static_cast<R *>(dst));
+    else     em::k_unpack_halo<R><<<blocks, 256, 0, s>>>(p, p.E[0], p.E[1], th, thermal_on ? sig_buf(0) : nullptr,
+                                                          thermal_on ? sig_buf(1) : nullptr, c.ttable, kp, kl, static_cast<const R *>(srcp));
+    CU(cudaGetLastError());
+    launches += 1;
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::joule_layers(int32_t k0, int32_t k1, double *total) {
+    if (k0 < 0 || k1 < k0 || k1 > g.nz || !total) return fail(EM_ERR_INVALID_ARG, "joule_layers: need 0 <= k0 <= k1 <= nz");
+    em::k_energy_partial<R><<<kReduceBlocks, 256, 0, stream>>>(p, c.vx, c.vy, c.vz, k0, k1, c.partial);
+    em::k_energy_final<<<1, 256, 0, stream>>>(c.partial, kReduceBlocks, c.scalar);
+    CU(cudaGetLastError()); launches += 2;
+    CU(cudaMemcpyAsync(total, c.scalar, sizeof(double), cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    return EM_OK;
+}
+
+// Byte offset, from the workspace base, of element (0, 0) of the wall plane (side 0: plane 0, side 1: plane nz) of the E
+// array with ping-pong parity `parity`, comp 0 = Ex, 1 = Ey: what a neighbouring slab adds to ITS mapping of this
+// workspace to store into that plane (em_set_peer_halo).
+template <typename R>
+int32_t Ctx<R>::wall_offset(int32_t side, int32_t parity, int32_t comp, size_t *off) {
+    if (side < 0 || side > 1 || parity < 0 || parity > 1 || comp < 0 || comp > 1 || !off) return fail(EM_ERR_INVALID_ARG, "wall_offset arguments");
+    if (eonly) return fail(EM_ERR_UNSUPPORTED, "the halo calls cover the leapfrog formulation");
+    const R *ptr = org(parity * 3 + comp) + (long long)(side ? g.nz : 0) * g.PXY;
+    *off = (size_t)(reinterpret_cast<const char *>(ptr) - static_cast<const char *>(ws_base));
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::set_peer_halo(int32_t side, int32_t k_send, void *const dst[4]) {
+    if (side < 0 || side > 1) return fail(EM_ERR_INVALID_ARG, "side must be 0 (-z) or 1 (+z)");
+    if (eonly || kernel != EM_KERNEL_TMA || grid.thermal) return fail(EM_ERR_UNSUPPORTED, "peer halo stores run in the leapfrog TMA sweep (no thermal coupling)");
+    if (!dst) {
+        for (int q = 0; q < 2; ++q) for (int cc = 0; cc < 2; ++cc) peer_dst[side][q][cc] = nullptr;
+        p.peer_k[side] = -1000; p.peer_skip &= ~(1 << side);
+        bind();
+        return EM_OK;
+    }
+    if (grid.bc[4 + side] != EM_BC_PMC) return fail(EM_ERR_STATE, "the wall on that side is not an artificial (PMC) slab wall");
+    if (k_send < 0 || k_send > g.nz) return fail(EM_ERR_INVALID_ARG, "k_send out of range");
+    for (int q = 0; q < 4; ++q) if (!dst[q]) return fail(EM_ERR_INVALID_ARG, "null peer address");
+    for (int q = 0; q < 2; ++q) for (int cc = 0; cc < 2; ++cc) peer_dst[side][q][cc] = static_cast<R *>(dst[q * 2 + cc]);
+    p.peer_k[side] = k_send; p.peer_skip |= 1 << side;
+    bind();
+    return EM_OK;
+}
+
 // ---- time stepping ----------------------------------------------------------------------------------
 template <typename R>
 int32_t Ctx<R>::record_begin() {
@@ -856,7 +937,7 @@ int32_t Ctx<R>::joule(void *power, void *energy, double *total, int32_t do_reset
         CU(cudaMemcpy3DAsync(&m, stream));
     }
     if (total) {
-        em::k_energy_partial<R><<<kReduceBlocks, 256, 0, stream>>>(p, c.vx, c.vy, c.vz, c.partial);
+        em::k_energy_partial<R><<<kReduceBlocks, 256, 0, stream>>>(p, c.vx, c.vy, c.vz, 0, g.nz, c.partial);
         em::k_energy_final<<<1, 256, 0, stream>>>(c.partial, kReduceBlocks, c.scalar);
         CU(cudaGetLastError()); launches += 2;
         CU(cudaMemcpyAsync(total, c.scalar, sizeof(double), cudaMemcpyDeviceToHost, stream));
@@ -1015,6 +1096,17 @@ int32_t em_get_temperature_rise(em_ctx *ctx, void *dst, int32_t dst_is_device) {
 int32_t em_set_temperature_rise(em_ctx *ctx, const void *src, int32_t src_is_device) {
     EM_CHECK_CTX; if (!src) return fail(EM_ERR_INVALID_ARG, "null"); return ctx->temperature_rise(nullptr, src, src_is_device);
 }
+int32_t em_halo_elems(em_ctx *ctx, int64_t *n) { EM_CHECK_CTX; if (!n) return fail(EM_ERR_INVALID_ARG, "null"); return ctx->halo_elems(n); }
+int32_t em_get_halo(em_ctx *ctx, int32_t k_plane, int32_t k_layer, void *dst, void *stream) {
+    EM_CHECK_CTX; if (!dst) return fail(EM_ERR_INVALID_ARG, "null"); return ctx->halo(k_plane, k_layer, dst, nullptr, stream);
+}
+int32_t em_set_halo(em_ctx *ctx, int32_t k_plane, int32_t k_layer, const void *src, void *stream) {
+    EM_CHECK_CTX; if (!src) return fail(EM_ERR_INVALID_ARG, "null"); return ctx->halo(k_plane, k_layer, nullptr, src, stream);
+}
+int32_t em_joule_layers(em_ctx *ctx, int32_t k0, int32_t k1, double *total) { EM_CHECK_CTX; return ctx->joule_layers(k0, k1, total); }
+int32_t em_wall_offset(em_ctx *ctx, int32_t side, int32_t parity, int32_t comp, size_t *off) { EM_CHECK_CTX; return ctx->wall_offset(side, parity, comp, off); }
+int32_t em_set_peer_halo(em_ctx *ctx, int32_t side, int32_t k_send, void *const dst[4]) { EM_CHECK_CTX; return ctx->set_peer_halo(side, k_send, dst); }
+
 int32_t em_step_index(em_ctx *ctx, int64_t *n) { EM_CHECK_CTX; if (!n) return fail(EM_ERR_INVALID_ARG, "null"); *n = ctx->step_index; return EM_OK; }
 int32_t em_launch_count(em_ctx *ctx, int64_t *n) { EM_CHECK_CTX; if (!n) return fail(EM_ERR_INVALID_ARG, "null"); *n = ctx->launches; return EM_OK; }
 

@@ -351,6 +351,14 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         // ---- phase B: E' = E + r (curl H' - J - sigma E), Joule squares (eq. 2-3) -------------
         // (warp 0 = halo row -1 only supplies H' to row 0: no E', no Joule)
         VecR bx, by, bz;         // (2 Ebar)^2
+        // stores of E'x, E'y (comp 0, 1): own array unless the plane is a wall fed by the neighbouring slab, plus the
+        // neighbour's wall plane when this is the plane it needs (DevParams::peer_*)
+        auto store_exy = [&](int comp, const VecR &v) {
+            if (!st) return;
+            if (!((k == 0 && (p.peer_skip & 1)) || (k == nz && (p.peer_skip & 2)))) EM_ST(p.En[comp] + o, v);
+            if (k == p.peer_k[0]) EM_ST(p.peer_e[0][comp] + (o - (long long)k * PXY), v);
+            if (k == p.peer_k[1]) EM_ST(p.peer_e[1][comp] + (o - (long long)k * PXY), v);
+        };
         if (w != 0) {
             // EO: d = e^n - e^{n-1} of the own edges is formed where it is used (em_sweep_phaseb*.inc) from the staged
             // e^{n-1} planes (the subtraction is exact in floating point when the two levels are within a factor 2)

@@ -3,21 +3,32 @@
 One process per GPU, each with its own em_ctx over its slab of cell layers [a, b) EXTENDED by one ghost cell layer on
 every interior side.  The artificial end walls of the extended slab are PMC walls (include/em.h EM_BC_PMC): their
 tangential E (Ex, Ey on the wall's node plane) is an unknown that the library lets the caller overwrite, and it is
-the ONLY thing a slab cannot compute itself -- everything one plane inside the wall (H', E'z of the ghost layer, the
-Joule sum that closes on the plane above) follows from correct inputs.  So the exchange after every step is
+the ONLY field value a slab cannot compute itself -- everything one plane inside the wall (H', E'z of the ghost layer,
+the Joule sum that closes on the plane above) follows from correct inputs.  So the halo after every step is
     to the slab above : my Ex, Ey at global node plane b-1   -> its lower wall plane
     to the slab below : my Ex, Ey at global node plane a+1   -> its upper wall plane
-i.e. two planes per neighbour per step (2 x nx*ny reals), point-to-point only.  All arithmetic stays
-in the CUDA kernels; this module only slices inputs (host) and moves planes (em_get_plane / em_set_plane + send/recv).
+(2 x nx*ny reals per neighbour), point-to-point only; with the two-way thermal coupling the temperature
+rise of the owned boundary layer rides along (-> the neighbour's ghost layer, whose theta and sigma(T) feed the owned
+layer's conduction and edge conductivities).  Two ways to move it, both with every arithmetic step in the CUDA kernels:
 
-The path of BASELINE.json is one GPU; this is the multi-GPU scale-out of the same kernels, tested on one GPU by running
-the slab contexts one after another (no kernel waits on another) and, for the exchange logic, with gloo on CPU.
+  mode "p2p"  : em_get_halo packs the message with one kernel into a preallocated buffer, torch.distributed moves it
+                (batched isend/irecv: NCCL over NVLink, stream-ordered, no host synchronisation; gloo in the CPU tests),
+                em_set_halo unpacks with one kernel.  Works for the coupled step too.
+  mode "peer" : the halo is FUSED into the sweep: the kernel stores E'x, E'y of the plane the neighbour needs straight
+                into the neighbour's wall plane through a peer mapping of its workspace (em_set_peer_halo; NVLink
+                stores, CUDA IPC between processes), overlapped with the sweep by construction; the only thing left
+                per step is one tiny stream-ordered all-reduce as the cross-rank barrier (step n+1 of a rank may start
+                only when its neighbours finished step n).
+
+The Joule total is the all-reduced sum of the owned layers' totals (em_joule_layers).  The path of BASELINE.json is one
+GPU; this is the scale-out of the same kernels, tested on one GPU (slab contexts run one after another; two processes
+sharing one GPU for the IPC wiring) and, for the exchange logic, with gloo on CPU.
 """
 from __future__ import annotations
 
 import copy
 import dataclasses
-from typing import List, Sequence
+from typing import List, Optional, Sequence
 
 import numpy as np
 
@@ -51,15 +62,16 @@ def slab_ranges(nz: int, n_ranks: int):
     return [(cuts[r], cuts[r + 1]) for r in range(n_ranks)]
 
 
+def slab_meta(nz: int, rank: int, n_ranks: int) -> SlabMeta:
+    a, b = slab_ranges(nz, n_ranks)[rank]
+    return SlabMeta(rank, n_ranks, a, b, a - 1 if rank > 0 else 0, b + 1 if rank < n_ranks - 1 else nz, nz)
+
+
 def sub_problem(p, rank: int, n_ranks: int):
     """The inputs of slab `rank`: a shallow copy of the problem restricted to the extended slab, with PMC on the
     artificial walls, the port edges that fall inside it (k shifted) and the matching slices of the initial fields."""
-    if getattr(p, "thermal", None) is not None:
-        raise ValueError("the slab decomposition covers the EM + Joule path; thermal conduction needs a theta halo")
-    a, b = slab_ranges(p.nz, n_ranks)[rank]
-    lo = a - 1 if rank > 0 else 0
-    hi = b + 1 if rank < n_ranks - 1 else p.nz
-    meta = SlabMeta(rank, n_ranks, a, b, lo, hi, p.nz)
+    meta = slab_meta(p.nz, rank, n_ranks)
+    lo, hi = meta.lo, meta.hi
     s = copy.copy(p)
     s.name = "%s_slab%d_of_%d" % (p.name, rank, n_ranks)
     s.nz = hi - lo
@@ -92,13 +104,20 @@ def sub_problem(p, rank: int, n_ranks: int):
 
 
 class SlabRank:
-    """One slab: its context (anything with em_step / em_get_plane / em_set_plane / em_get_field / joule_maps) and
-    the plane bookkeeping of the exchange."""
+    """One slab: its context (paper_2603_07038_b200.EM, or anything with em_step / em_get_halo / em_set_halo /
+    new_halo_buffer) and the plane bookkeeping of the halo."""
 
-    def __init__(self, em, meta: SlabMeta):
-        self.em, self.meta = em, meta
+    def __init__(self, em, meta: SlabMeta, mode: str = "p2p"):
+        assert mode in ("p2p", "peer")
+        self.em, self.meta, self.mode = em, meta, mode
+        self._buf = {}
+        self._token = None
 
-    # local plane indices ------------------------------------------------------------------------------------
+    # local indices --------------------------------------------------------------------------------------------
+    @property
+    def nz_local(self) -> int:
+        return self.meta.hi - self.meta.lo
+
     @property
     def k_send_up(self) -> int:        # global node plane b - 1
         return self.meta.b - 1 - self.meta.lo
@@ -108,24 +127,60 @@ class SlabRank:
         return self.meta.a + 1 - self.meta.lo
 
     @property
+    def layer_send_up(self) -> int:    # my top owned cell layer b - 1 -> the ghost layer of the slab above
+        return self.meta.b - 1 - self.meta.lo
+
+    @property
+    def layer_send_down(self) -> int:  # my bottom owned cell layer a -> the ghost layer of the slab below
+        return self.meta.a - self.meta.lo
+
+    @property
     def k_wall_lo(self) -> int:
         return 0
 
     @property
     def k_wall_hi(self) -> int:
-        return self.meta.hi - self.meta.lo
+        return self.nz_local
 
-    def planes_up(self):
-        return [self.em.em_get_plane(0, self.k_send_up), self.em.em_get_plane(1, self.k_send_up)]
+    def buf(self, name):
+        if name not in self._buf:
+            self._buf[name] = self.em.new_halo_buffer()
+        return self._buf[name]
 
-    def planes_down(self):
-        return [self.em.em_get_plane(0, self.k_send_down), self.em.em_get_plane(1, self.k_send_down)]
+    # the halo in two kernels per neighbour ---------------------------------------------------------------------------
+    def pack_up(self):
+        return self.em.em_get_halo(self.k_send_up, self.layer_send_up, self.buf("send_up"))
 
-    def set_wall_lo(self, planes):
-        self.em.em_set_plane(0, self.k_wall_lo, planes[0]); self.em.em_set_plane(1, self.k_wall_lo, planes[1])
+    def pack_down(self):
+        return self.em.em_get_halo(self.k_send_down, self.layer_send_down, self.buf("send_down"))
 
-    def set_wall_hi(self, planes):
-        self.em.em_set_plane(0, self.k_wall_hi, planes[0]); self.em.em_set_plane(1, self.k_wall_hi, planes[1])
+    def unpack_lo(self, msg):          # from the slab below: my lower wall plane and my ghost layer 0
+        self.em.em_set_halo(self.k_wall_lo, 0, msg)
+
+    def unpack_hi(self, msg):          # from the slab above: my upper wall plane and my ghost layer nz_local - 1
+        self.em.em_set_halo(self.k_wall_hi, self.nz_local - 1, msg)
+
+    # stepping with torch.distributed (rank == slab rank) ---------------------------------------------------------
+    def step(self, n: int, dist, group=None):
+        for _ in range(n):
+            self.em.em_step(1)
+            if self.mode == "p2p":
+                exchange_dist(self, dist, group)
+            else:
+                barrier_on_stream(self, dist, group)
+
+    def reset(self):
+        self.em.em_reset()
+
+    def joule_total(self, dist=None, group=None) -> float:
+        """Joule energy of the WHOLE problem: the owned layers' total, all-reduced over the ranks."""
+        own = self.em.em_joule_layers(self.meta.a - self.meta.lo, self.meta.b - self.meta.lo)
+        if dist is None:
+            return own
+        import torch
+        t = torch.tensor([own], dtype=torch.float64, device=self.em.device if dist.get_backend(group) == "nccl" else "cpu")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+        return float(t.item())
 
     # owned parts of the results (NumPy, global k order) ---------------------------------------------------------
     def owned_fields(self):
@@ -145,61 +200,110 @@ class SlabRank:
         pw, q, _ = self.em.joule_maps()
         return pw[m.a - m.lo:m.b - m.lo], q[m.a - m.lo:m.b - m.lo]
 
-
-def exchange_inprocess(ranks: Sequence[SlabRank]):
-    """Halo exchange between slab contexts that live in ONE process (one GPU, run one after another): plain device
-    copies through em_get_plane / em_set_plane.  Used by the single-GPU tests of the decomposition."""
-    ups = [r.planes_up() if r.meta.has_above else None for r in ranks]
-    downs = [r.planes_down() if r.meta.has_below else None for r in ranks]
-    for n, r in enumerate(ranks):
-        if r.meta.has_below:
-            r.set_wall_lo(ups[n - 1])
-        if r.meta.has_above:
-            r.set_wall_hi(downs[n + 1])
-
-
-def _pack(planes):
-    import torch
-    return torch.cat([planes[0].reshape(-1), planes[1].reshape(-1)])
-
-
-def _unpack(buf, like):
-    n0 = like[0].numel()
-    return [buf[:n0].reshape(like[0].shape).contiguous(), buf[n0:].reshape(like[1].shape).contiguous()]
+    def owned_theta(self):
+        m = self.meta
+        return self.em.em_get_temperature_rise()[m.a - m.lo:m.b - m.lo]
 
 
 def exchange_dist(rank: SlabRank, dist, group=None):
     """Halo exchange of one process per slab over torch.distributed (nccl on GPUs over NVLink, gloo in the CPU tests):
-    point-to-point only, one packed [Ex plane | Ey plane] message per neighbour and direction, posted as a batch so that
-    the two directions overlap.  torch.distributed rank == slab rank."""
+    point-to-point only, one packed message per neighbour and direction in preallocated buffers, posted as one batch so
+    that the two directions overlap.  With nccl everything is stream-ordered (wait() makes the current stream wait)."""
     m = rank.meta
-    ops, recv = [], {}
+    ops = []
     if m.has_above:
-        up = rank.planes_up()
-        send_up = _pack(up)
-        recv["hi"] = (send_up.new_empty(send_up.shape), up)
-        ops += [dist.P2POp(dist.isend, send_up, m.rank + 1, group), dist.P2POp(dist.irecv, recv["hi"][0], m.rank + 1, group)]
+        ops += [dist.P2POp(dist.isend, rank.pack_up(), m.rank + 1, group),
+                dist.P2POp(dist.irecv, rank.buf("recv_hi"), m.rank + 1, group)]
     if m.has_below:
-        down = rank.planes_down()
-        send_down = _pack(down)
-        recv["lo"] = (send_down.new_empty(send_down.shape), down)
-        ops += [dist.P2POp(dist.isend, send_down, m.rank - 1, group), dist.P2POp(dist.irecv, recv["lo"][0], m.rank - 1, group)]
+        ops += [dist.P2POp(dist.isend, rank.pack_down(), m.rank - 1, group),
+                dist.P2POp(dist.irecv, rank.buf("recv_lo"), m.rank - 1, group)]
     if ops:
         for w in dist.batch_isend_irecv(ops):
             w.wait()
-    if "lo" in recv:
-        rank.set_wall_lo(_unpack(*recv["lo"]))
-    if "hi" in recv:
-        rank.set_wall_hi(_unpack(*recv["hi"]))
+    if m.has_below:
+        rank.unpack_lo(rank.buf("recv_lo"))
+    if m.has_above:
+        rank.unpack_hi(rank.buf("recv_hi"))
 
 
-def make_ranks_inprocess(p, n_ranks: int, **em_kw) -> List[SlabRank]:
+def barrier_on_stream(rank: SlabRank, dist, group=None):
+    """The cross-rank barrier of the peer mode: nccl -- a one-element all-reduce, stream-ordered, no host
+    synchronisation; any other backend -- device synchronise, then a host barrier."""
+    import torch
+    if dist.get_backend(group) == "nccl":
+        if rank._token is None:
+            rank._token = torch.zeros(1, dtype=torch.float32, device=rank.em.device)
+        dist.all_reduce(rank._token, group=group)
+    else:
+        torch.cuda.synchronize(rank.em.device)
+        dist.barrier(group)
+
+
+# ---- peer wiring ------------------------------------------------------------------------------------------------------
+def _peer_addresses(base_ptr: int, offsets):
+    return [base_ptr + int(o) for o in offsets]
+
+
+def connect_peers_inprocess(ranks: Sequence[SlabRank]):
+    """All slab contexts live in this process on one GPU: a neighbour's workspace is directly addressable."""
+    for n, r in enumerate(ranks):
+        if r.meta.has_above:
+            nb = ranks[n + 1]
+            r.em.em_set_peer_halo(1, r.k_send_up, _peer_addresses(nb.em.workspace_ptr, nb.em.wall_offsets(0)))
+        if r.meta.has_below:
+            nb = ranks[n - 1]
+            r.em.em_set_peer_halo(0, r.k_send_down, _peer_addresses(nb.em.workspace_ptr, nb.em.wall_offsets(1)))
+        r.mode = "peer"
+
+
+def connect_peers_dist(rank: SlabRank, dist, group=None):
+    """One process per slab: every rank exports its workspace as a CUDA IPC handle (torch's storage sharing), the
+    neighbours map it (NVLink peer mapping between GPUs of one node) and hand the wall-plane addresses to their sweeps."""
+    import torch
+    em = rank.em
+    storage = em._ws.untyped_storage()
+    info = {"ipc": storage._share_cuda_(), "ws_off": em.workspace_ptr - storage.data_ptr(),
+            "wall_lo": em.wall_offsets(0), "wall_hi": em.wall_offsets(1)}
+    world = dist.get_world_size(group)
+    infos: List[Optional[dict]] = [None] * world
+    dist.all_gather_object(infos, info, group=group)
+    rank._peer_storages = []                                # keep the mappings alive
+    m = rank.meta
+    for side, nb in ((1, m.rank + 1 if m.has_above else None), (0, m.rank - 1 if m.has_below else None)):
+        if nb is None:
+            continue
+        st = torch.UntypedStorage._new_shared_cuda(*infos[nb]["ipc"])
+        rank._peer_storages.append(st)
+        base = st.data_ptr() + infos[nb]["ws_off"]
+        offs = infos[nb]["wall_lo"] if side == 1 else infos[nb]["wall_hi"]       # my +z neighbour's -z wall and vice versa
+        em.em_set_peer_halo(side, rank.k_send_up if side == 1 else rank.k_send_down, _peer_addresses(base, offs))
+    rank.mode = "peer"
+    torch.cuda.synchronize(em.device)
+    dist.barrier(group)
+
+
+# ---- all slabs in one process on one GPU (tests) -----------------------------------------------------------------------
+def exchange_inprocess(ranks: Sequence[SlabRank]):
+    """Halo exchange between slab contexts that live in ONE process (one GPU, run one after another): the packed
+    messages are handed over directly (pack kernel -> unpack kernel)."""
+    ups = [r.pack_up() if r.meta.has_above else None for r in ranks]
+    downs = [r.pack_down() if r.meta.has_below else None for r in ranks]
+    for n, r in enumerate(ranks):
+        if r.meta.has_below:
+            r.unpack_lo(ups[n - 1])
+        if r.meta.has_above:
+            r.unpack_hi(downs[n + 1])
+
+
+def make_ranks_inprocess(p, n_ranks: int, mode: str = "p2p", **em_kw) -> List[SlabRank]:
     """all slab contexts of p in this process, on one GPU (tests; a real run has one process and GPU per slab)"""
     from .binding import EM
     out = []
     for r in range(n_ranks):
         s, meta = sub_problem(p, r, n_ranks)
         out.append(SlabRank(EM(s, **em_kw), meta))
+    if mode == "peer":
+        connect_peers_inprocess(out)
     return out
 
 
@@ -207,7 +311,8 @@ def step_inprocess(ranks: Sequence[SlabRank], n: int = 1):
     for _ in range(n):
         for r in ranks:
             r.em.em_step(1)
-        exchange_inprocess(ranks)
+        if ranks[0].mode == "p2p":
+            exchange_inprocess(ranks)           # (peer mode: the sweeps stored the halos themselves; one stream orders them)
 
 
 def gather_inprocess(ranks: Sequence[SlabRank]):

@@ -1,5 +1,6 @@
 """CPU tests of the z-slab decomposition plumbing (NEXT-3): input slicing, ownership bookkeeping and the
-torch.distributed halo exchange (gloo, world_size 2 and 3) with a stand-in context that only stores planes."""
+torch.distributed halo exchange (gloo, world_size 2 and 3) around a NumPy stand-in context that runs a real recurrence
+with the data dependencies of the sweep (its single-domain run is the closed form the slabs must reproduce)."""
 import os
 import socket
 import sys
@@ -42,23 +43,59 @@ def test_ranges_and_sub_problem_slicing():
     # owned layers tile [0, nz) exactly
     assert [(m.a, m.b) for m in metas] == [(0, 4), (4, 8), (8, 13)]
     p.thermal = W.thermal_table()
-    with pytest.raises(ValueError):
-        slabs.sub_problem(p, 0, 2)
+    s, m = slabs.sub_problem(p, 1, 3)                            # the coupled problem shards too (theta rides in the halo)
+    assert s.thermal is p.thermal
 
 
-class _FakeEM:
-    """stores Ex / Ey planes only; plane k of rank r holds the value 1000 r + 10 k + comp"""
-    def __init__(self, rank, nz, ny=3, nx=4):
-        self.shape = {0: (ny + 1, nx), 1: (ny, nx + 1)}
-        self.planes = {(c, k): torch.full(self.shape[c], 1000.0 * rank + 10.0 * k + c, dtype=torch.float64)
-                       for c in (0, 1) for k in range(nz + 1)}
+class _StandInEM:
+    """A NumPy stand-in for the library with the halo calls of include/em.h and a REAL recurrence with the data
+    dependencies of the sweep: node planes u[k] (Ex and Ey stacks) advance by a 3-point stencil in z, cell layers (theta)
+    by a 3-point diffusion; a real wall plane is held (Dirichlet), a real end layer reflects; an ARTIFICIAL wall plane and
+    a ghost layer compute garbage that only the halo exchange can repair.  The single-domain run of the same class is
+    the closed form the assembled slabs must reproduce bit for bit."""
+    C1, C2 = 0.23, 0.11
 
-    def em_get_plane(self, comp, k):
-        return self.planes[(comp, k)].clone()
+    def __init__(self, u_ex, u_ey, theta, wall_lo_real=True, wall_hi_real=True):
+        self.ex, self.ey, self.th = u_ex.copy(), u_ey.copy(), theta.copy()
+        self.real = (wall_lo_real, wall_hi_real)
+        self.nz = theta.shape[0]
+        self.n0, self.n1, self.n2 = self.ex[0].size, self.ey[0].size, self.th[0].size
+        self.device = "cpu"
 
-    def em_set_plane(self, comp, k, t):
-        assert tuple(t.shape) == self.shape[comp]
-        self.planes[(comp, k)] = t.clone()
+    def new_halo_buffer(self):
+        return torch.empty(self.n0 + self.n1 + self.n2, dtype=torch.float64)
+
+    def em_step(self, n=1):
+        for _ in range(n):
+            for u in (self.ex, self.ey):
+                new = u.copy()
+                new[1:-1] = u[1:-1] + self.C1 * (u[2:] - 2.0 * u[1:-1] + u[:-2])
+                if not self.real[0]:
+                    new[0] = 0.5 * u[0] + 7.0                      # garbage on an artificial wall
+                if not self.real[1]:
+                    new[-1] = -3.0 * u[-1] - 1.0
+                u[...] = new
+            t = self.th
+            lo = np.concatenate([t[:1], t[:-1]]); hi = np.concatenate([t[1:], t[-1:]])     # reflecting ends
+            new = t + self.C2 * (hi - 2.0 * t + lo)
+            if not self.real[0]:
+                new[0] = 1.0e3                                      # garbage in a ghost layer
+            if not self.real[1]:
+                new[-1] = -1.0e3
+            t[...] = new
+
+    def em_get_halo(self, kp, kl, out, stream=None):
+        out[:self.n0] = torch.from_numpy(self.ex[kp].ravel()); out[self.n0:self.n0 + self.n1] = torch.from_numpy(self.ey[kp].ravel())
+        out[self.n0 + self.n1:] = torch.from_numpy(self.th[kl].ravel())
+        return out
+
+    def em_set_halo(self, kp, kl, src, stream=None):
+        a = src.numpy()
+        self.ex[kp] = a[:self.n0].reshape(self.ex[kp].shape); self.ey[kp] = a[self.n0:self.n0 + self.n1].reshape(self.ey[kp].shape)
+        self.th[kl] = a[self.n0 + self.n1:].reshape(self.th[kl].shape)
+
+    def em_joule_layers(self, k0, k1):
+        return float(self.th[k0:k1].sum())
 
 
 def _free_port():
@@ -67,38 +104,40 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _worker(rank, world, port, nz, out):
+def _global_state(nz, ny=3, nx=4, seed=5):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((nz + 1, ny + 1, nx)), rng.standard_normal((nz + 1, ny, nx + 1)), rng.standard_normal((nz, ny, nx))
+
+
+def _worker(rank, world, port, nz, steps, out):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        a, b = slabs.slab_ranges(nz, world)[rank]
-        lo, hi = (a - 1 if rank > 0 else 0), (b + 1 if rank < world - 1 else nz)
-        sr = slabs.SlabRank(_FakeEM(rank, hi - lo), slabs.SlabMeta(rank, world, a, b, lo, hi, nz))
-        slabs.exchange_dist(sr, dist)
-        dist.barrier()
-        res = {"lo": [sr.em.planes[(c, 0)][0, 0].item() for c in (0, 1)],
-               "hi": [sr.em.planes[(c, hi - lo)][0, 0].item() for c in (0, 1)], "a": a, "b": b, "lo_": lo, "hi_": hi}
-        torch.save(res, os.path.join(out, "r%d.pt" % rank))
+        m = slabs.slab_meta(nz, rank, world)
+        ex, ey, th = _global_state(nz)
+        em = _StandInEM(ex[m.lo:m.hi + 1], ey[m.lo:m.hi + 1], th[m.lo:m.hi], not m.has_below, not m.has_above)
+        sr = slabs.SlabRank(em, m)
+        sr.step(steps, dist)
+        total = sr.joule_total(dist)
+        k0, k1 = m.a - m.lo, m.b - m.lo
+        last = 1 if not m.has_above else 0
+        np.savez(os.path.join(out, "r%d.npz" % rank), ex=em.ex[k0:k1 + last], ey=em.ey[k0:k1 + last], th=em.th[k0:k1], total=total)
     finally:
         dist.destroy_process_group()
 
 
 @pytest.mark.parametrize("world", [2, 3])
-def test_exchange_dist_gloo(world, tmp_path):
-    nz = 13
-    mp.spawn(_worker, args=(world, _free_port(), nz, str(tmp_path)), nprocs=world, join=True)
-    res = [torch.load(os.path.join(str(tmp_path), "r%d.pt" % r)) for r in range(world)]
-    for r in range(world):
-        me = res[r]
-        if r > 0:            # my lower wall plane <- the lower neighbour's global node plane b_low - 1 = a - 1
-            nb = res[r - 1]
-            k_local = (nb["b"] - 1) - nb["lo_"]
-            assert me["lo"] == [1000.0 * (r - 1) + 10.0 * k_local + c for c in (0, 1)]
-        else:                # a real wall keeps its own values
-            assert me["lo"] == [0.0, 1.0]
-        if r < world - 1:    # my upper wall plane <- the upper neighbour's global node plane a_up + 1 = b + 1
-            nb = res[r + 1]
-            k_local = (nb["a"] + 1) - nb["lo_"]
-            assert me["hi"] == [1000.0 * (r + 1) + 10.0 * k_local + c for c in (0, 1)]
-        else:
-            assert me["hi"] == [1000.0 * r + 10.0 * (me["hi_"] - me["lo_"]) + c for c in (0, 1)]
+def test_exchange_dist_gloo_reproduces_the_single_domain_recurrence(world, tmp_path):
+    nz, steps = 13, 25
+    mp.spawn(_worker, args=(world, _free_port(), nz, steps, str(tmp_path)), nprocs=world, join=True)
+    ex, ey, th = _global_state(nz)
+    ref = _StandInEM(ex, ey, th)
+    ref.em_step(steps)
+    parts = [np.load(os.path.join(str(tmp_path), "r%d.npz" % r)) for r in range(world)]
+    assert np.array_equal(np.concatenate([p["ex"] for p in parts]), ref.ex)
+    assert np.array_equal(np.concatenate([p["ey"] for p in parts]), ref.ey)
+    assert np.array_equal(np.concatenate([p["th"] for p in parts]), ref.th)
+    # the all-reduced total of the owned layers is the single-domain total on every rank
+    for p in parts:
+        assert abs(float(p["total"]) - ref.th.sum()) <= 1e-12 * abs(ref.th).sum()
+    assert np.abs(ref.ex - ex).max() > 1e-3                      # the recurrence did something
