@@ -43,6 +43,8 @@ def parse():
     ap.add_argument("--force-joule-output", action="store_true",
                     help="one Joule-map output at the end of every timed repetition even when K is below the config's "
                          "cadence (default: outputs fall where the cadence puts them; their count is stated in config)")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="gloo lets several ranks share one GPU (testing the N > 1 path on a one-GPU box; peer halo only)")
     ap.add_argument("--reps", type=int, default=3, help="timed repetitions of the K steps (each after em_reset); the median is reported")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -204,14 +206,22 @@ def run_b200(args):
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     dist = None
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    n_dev = torch.cuda.device_count()
+    if local >= n_dev and args.dist_backend == "nccl":
+        raise RuntimeError("rank %d has no GPU of its own (%d visible): one process per GPU" % (local, n_dev))
+    local_dev = local % n_dev                                  # (--dist-backend gloo: ranks may share a GPU, for testing the N > 1 path)
     if world > 1:
         import torch.distributed as dist_
         dist = dist_
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback for the product path")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
+        if args.dist_backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_dev))
+        else:
+            dist.init_process_group(args.dist_backend)
+    torch.cuda.set_device(local_dev)
+    dev = torch.device("cuda", local_dev)
+    red_dev = dev if args.dist_backend == "nccl" else None     # where the timing scalars are reduced
 
     p = make_problem(args)
     precision = args.precision or p.precision
@@ -230,7 +240,17 @@ def run_b200(args):
     if args.decomp == "slabs" and world > 1:
         slab = slabs.SlabRank(em, meta)
         if args.halo == "peer" and not args.thermal and form == P.EM_FORM_LEAPFROG and kernel != P.EM_KERNEL_SPLIT:
-            slabs.connect_peers_dist(slab, dist)
+            try:
+                slabs.connect_peers_dist(slab, dist)
+            except Exception as exc:                             # no peer mapping between these GPUs: NCCL send/recv instead
+                print("peer halo unavailable (%s): falling back to --halo p2p" % exc, file=sys.stderr)
+                slab.mode = "p2p"
+            modes = [None] * world                               # every rank must use the same transport
+            dist.all_gather_object(modes, slab.mode)
+            if any(m != "peer" for m in modes):
+                if slab.mode == "peer":
+                    em.em_set_peer_halo(0, 0, None); em.em_set_peer_halo(1, 0, None)
+                slab.mode = "p2p"
         args.no_e2e = True                                       # the end-to-end leg is defined for whole problems
     cells = p.n_cells
     je = p.joule_every if p.joule_every else 0
@@ -268,7 +288,7 @@ def run_b200(args):
     # is reported.  Every repetition contains at least one Joule-map output when the config has them.
     run_steps(Wm, 0)
     em.em_timing_enable(True)
-    sampler = ClockSampler(local); sampler.start()
+    sampler = ClockSampler(local_dev); sampler.start()
     l0 = em.launch_count
     rep_ms = []
     for _ in range(max(args.reps, 1)):
@@ -279,7 +299,7 @@ def run_b200(args):
         run_steps(K, 0, force_output=args.force_joule_output)
         ev1.record()
         barrier()
-        rep_ms.append(max_over_ranks(ev0.elapsed_time(ev1), dist, dev))
+        rep_ms.append(max_over_ranks(ev0.elapsed_time(ev1), dist, red_dev))
     sampler.stop_flag = True
     out_ms = None
     if je:                               # one Joule-map output (energy + power maps to device buffers), timed on its own
@@ -332,7 +352,7 @@ def run_b200(args):
         tot = em.em_joule(None, None, total=True); d2h += 8
         torch.cuda.synchronize(dev)
         el = time.perf_counter() - t0
-        el = max_over_ranks(el, dist, dev)
+        el = max_over_ranks(el, dist, red_dev)
         e2e = {"value": aggregate_throughput(cells * K, el, world), "unit": "cell-updates/s", "h2d_bytes_per_step": h2d / K,
                "d2h_bytes_per_step": d2h / K,
                "what": "em_set_field x6 from pinned host, %d x em_step with em_probe reads%s, em_get_field x6 + Joule total to host"

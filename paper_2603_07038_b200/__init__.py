@@ -6,7 +6,7 @@ for device memory and streams.  There is no CPU fallback: importing the binding 
 library raises.
 """
 from .binding import (  # noqa: F401
-    EM, EMError, lib_path, load,
+    EM, EMError, lib_path, load, load_fuzz,
     EM_LOSS_CD, EM_LOSS_EXP, EM_KERNEL_AUTO, EM_KERNEL_SPLIT, EM_KERNEL_TMA, EM_FORM_LEAPFROG, EM_FORM_EONLY,
     EM_ABI_VERSION,
     em_workspace_bytes, em_cfl_dt,

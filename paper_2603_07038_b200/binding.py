@@ -79,6 +79,20 @@ def load():
         build_lib()
     elif not os.path.exists(path):
         raise RuntimeError("libem.so is missing and there is no nvcc to build it (python -m paper_2603_07038_b200.build)")
+    _lib = _open(path)
+    return _lib
+
+
+def load_fuzz():
+    """TEST build of the library with schedule fuzzing in the sweep (build.py fuzz=True; tests/test_gpu_fuzz.py).
+    Pass it to EM(..., lib=...); em_fuzz_seed(seed) switches the random delays on (0: off)."""
+    from .build import build_lib
+    L = _open(build_lib(fuzz=True))
+    L.em_fuzz_seed.argtypes = [C.c_uint32]
+    return L
+
+
+def _open(path: str):
     L = C.CDLL(path)
     try:
         abi = int(L.em_abi_version())
@@ -115,7 +129,6 @@ def load():
     L.em_launch_count.argtypes = [vp, C.POINTER(i64)]
     L.em_timing_enable.argtypes = [vp, i32]
     L.em_timing_read.argtypes = [vp, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(C.c_double)]
-    _lib = L
     return L
 
 
@@ -182,10 +195,10 @@ class EM:
                  stream=None, bc: Optional[Sequence[int]] = None, load_sources: bool = True, load_init: bool = True,
                  max_ports: Optional[int] = None, max_source_edges: Optional[int] = None,
                  max_wave_samples: Optional[int] = None, formulation: int = EM_FORM_LEAPFROG, z_chunks: int = 0,
-                 e_prev=None):
+                 e_prev=None, lib=None):
         import torch
         self._torch = torch
-        self._L = load()
+        self._L = lib if lib is not None else load()
         self.nx, self.ny, self.nz = int(p.nx), int(p.ny), int(p.nz)
         self.precision = int(precision if precision is not None else p.precision)
         self.dtype = torch.float32 if self.precision == 32 else torch.float64

@@ -1061,6 +1061,13 @@ int32_t em_create(const em_grid *gr, const uint8_t *mat_id, const em_material *t
 
 int32_t em_abi_version(void) { return EM_ABI_VERSION; }
 
+#ifdef EM_SWEEP_FUZZ
+// test builds only (libem_fuzz.so; em_sweep.cuh "schedule fuzzing"): 0 switches the random delays off
+int32_t em_fuzz_seed(uint32_t seed) {
+    return cudaMemcpyToSymbol(em::g_em_fuzz_seed, &seed, sizeof(seed)) == cudaSuccess ? EM_OK : EM_ERR_CUDA;
+}
+#endif
+
 int32_t em_destroy(em_ctx *ctx) {
     if (!ctx) return EM_OK;
     DeviceGuard guard(ctx->device);

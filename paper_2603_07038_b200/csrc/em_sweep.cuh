@@ -70,12 +70,32 @@ inline size_t sweep_smem_bytes(int sizeof_real, int n_table, bool thermal = fals
     return tab + (size_t)n_table * 4 * sizeof_real * (thermal ? 2 : 1);
 }
 
+// ---- schedule fuzzing (test builds only: -DEM_SWEEP_FUZZ, libem_fuzz.so) ---------------------------------------------
+// The plane loop orders its shared-memory hazards with mbarriers and named barriers instead of CTA barriers.  compute-
+// sanitizer is closed on this GPU pool, so the evidence that no ordering edge is missing is a stress test: with a
+// non-zero seed every synchronisation point (and every phase boundary) delays its warp by a pseudo-random 0-8 us -- a
+// few plane-times -- and the results must stay bit-identical to the normal build (tests/test_gpu_fuzz.py).
+#ifdef EM_SWEEP_FUZZ
+__device__ unsigned g_em_fuzz_seed = 0;
+__device__ __forceinline__ void em_fuzz() {
+    const unsigned seed = g_em_fuzz_seed;
+    if (seed == 0) return;
+    unsigned x = ((unsigned)(clock64() >> 7) * 2654435761u) ^ seed ^ (blockIdx.x * 97u + (threadIdx.x >> 5) * 131u);
+    x ^= x >> 15; x *= 2246822519u; x ^= x >> 13;
+    if ((x & 3u) == 0u) __nanosleep((x >> 8) & 8191u);
+}
+#define EM_FUZZ() em_fuzz()
+#else
+#define EM_FUZZ() ((void)0)
+#endif
+
 // ---- mbarrier / TMA PTX wrappers ---------------------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(unsigned bar) {
+    EM_FUZZ();
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
@@ -89,6 +109,7 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
         "@!p bra W_%=;\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
+    EM_FUZZ();
 }
 // 1-D bulk copy global -> shared counted on an mbarrier (bytes: multiple of 16)
 __device__ __forceinline__ void bulk_load(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
@@ -96,13 +117,14 @@ __device__ __forceinline__ void bulk_load(unsigned dst, const void *src, unsigne
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 // producer / consumer named barrier of two warps (ids 1..15; id 0 is __syncthreads)
-__device__ __forceinline__ void pair_arrive(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
-__device__ __forceinline__ void pair_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void pair_arrive(int id) { EM_FUZZ(); asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void pair_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); EM_FUZZ(); }
 // Every staged plane is loaded with the L2 evict_last policy (the output planes are written evict-first): the halo
 // rows and columns of a box are re-read by the neighbouring tiles a few planes earlier or later, so input lines should
 // outlive output lines in L2 (measured: -1 % step time on config 4; splitting each plane into halo boxes with evict_last
 // and an interior box with evict_first was 3 % SLOWER).
 __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map, unsigned bar, int x, int y, int z) {
+    EM_FUZZ();
     unsigned long long pol;
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
     asm volatile(
@@ -261,6 +283,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         const bool st = own && k >= kz0 && k < kz1;          // this chunk stores H'(k), E'(k)
 
         // ---- phase A: H' = H - nbar * curl E  (inner factor of S = curl mu^-1 curl) ----------
+        EM_FUZZ();
         mbar_wait(bar_fullE(it & 1), (unsigned)(it >> 1) & 1u);   // E group of plane k has landed
         const R fz = s_z[par * 4 + 0], rdz = s_z[par * 4 + 1], rtz = s_z[par * 4 + 2];
         const unsigned idw = ld_ids(par, w + 1), idj = ld_ids(par, w);
@@ -328,6 +351,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             EM_ST(p.Hn[1] + o, hyn);
             EM_ST(p.Hn[2] + o, hzn);
         }
+        EM_FUZZ();
         smHx[r][lane] = hxn; smHz[r][lane] = hzn;
         // No CTA barrier in the plane loop.  Row j+1 waits only for THIS row's H' (mbarrier rowH), and the producer
         // thread refills the staged slots once every warp has pulled plane k into registers (mbarrier empty).
@@ -409,6 +433,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         cp_async_wait<0>();                       // q(k-1) has landed (private slot: no barrier needed)
 
         // ---- phase C: q(k-1) += dt sigma/16 (pend + Sxy(k)); pend = Sxy(k) + Sz(k) ---------------------------
+        EM_FUZZ();
         if (w != 0 && !is_top) {
             const VecR bxn = smBx[r + 1][lane], bzn = smBz[r + 1][lane];
             const R by_r = shfl_down1(by.v[0]), bz_r = shfl_down1(bz.v[0]), bzn_r = shfl_down1(bzn.v[0]);
