@@ -94,7 +94,7 @@ struct Carved {
     long long *src_off; int *src_comp; R *src_r; int *src_cbeg; int *src_flags;
     int *con_port; R *con_scale; long long *port_woff, *port_wlen; R *wave;
     // fused-sweep tile source index
-    int *tile_sbeg; int4 *tile_ent;
+    int *tile_sbeg; int4 *tile_ent; int *order;
     // thermal coupling (only when em_grid.thermal != 0): theta ping-pong, sigma(T) per cell, thermal table
     R *theta[2]; R *sig, *sig2; em::ThEntry<R> *ttable;
 };
@@ -124,6 +124,7 @@ size_t carve(const Geometry &g, const em_grid &gr, void *base, Carved<R> *c, int
     o.port_woff = w.take<long long>(mp); o.port_wlen = w.take<long long>(mp);
     o.wave = w.take<R>((size_t)std::max<int64_t>(gr.max_wave_samples, 1));
     o.tile_sbeg = w.take<int>((size_t)n_items + 1);
+    o.order = w.take<int>((size_t)n_items);
     o.tile_ent = w.take<int4>(4 * me);
     o.theta[0] = o.theta[1] = o.sig = o.sig2 = nullptr; o.ttable = nullptr;
     if (gr.thermal) {
@@ -443,6 +444,12 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     src = em::DevSources<R>{};
     src.n_unique = 0;
     CU(cudaMemsetAsync(c.tile_sbeg, 0, sizeof(int) * (plan.n_tiles * plan.nzs + 1), stream));
+    {
+        std::vector<int> ord((size_t)plan.n_tiles * plan.nzs);
+        em::launch_order(plan, ord.data());
+        CU(cudaMemcpyAsync(c.order, ord.data(), sizeof(int) * ord.size(), cudaMemcpyHostToDevice, stream));
+        CU(cudaStreamSynchronize(stream));              // ord is a local
+    }
     int32_t rc = zero_state();
     if (rc) return rc;
     if (kernel == EM_KERNEL_TMA) {
@@ -473,7 +480,10 @@ int32_t Ctx<R>::make_maps() {
     EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(fn);
     const int V = 16 / (int)sizeof(R);
     const cuuint32_t ones[3] = {1, 1, 1};
-    const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
+#ifndef EM_SWEEP_PROMO
+#define EM_SWEEP_PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+#endif
+    const CUtensorMapL2promotion promo = (CUtensorMapL2promotion)EM_SWEEP_PROMO;
     auto encode = [&](CUtensorMap *m, CUtensorMapDataType dt, size_t esz, void *base, int bx, int by) -> int32_t {
         const cuuint64_t dims[3] = {(cuuint64_t)g.PX, (cuuint64_t)g.PY, (cuuint64_t)g.PZ};
         const cuuint64_t strides[2] = {(cuuint64_t)g.PX * esz, (cuuint64_t)g.PXY * esz};
@@ -874,7 +884,7 @@ int32_t Ctx<R>::step_thermal_sweep() {
     }
     launches += 1;
     int32_t rc = record_begin(); if (rc) return rc;
-    em::SweepSources fsrc{c.tile_sbeg, c.tile_ent};
+    em::SweepSources fsrc{c.tile_sbeg, c.tile_ent, c.order};
     em::SweepMaps maps;
     for (int a = 0; a < 3; ++a) { maps.E[a] = map_field[e_cur * 3 + a]; maps.H[a] = map_field[6 + h_cur * 3 + a]; }
     maps.q = map_q; maps.mat = map_mat; maps.sig = map_sig[sg_cur];
@@ -890,7 +900,7 @@ int32_t Ctx<R>::step_thermal_sweep() {
 template <typename R>
 int32_t Ctx<R>::step_tma() {
     int32_t rc = record_begin(); if (rc) return rc;
-    em::SweepSources fsrc{c.tile_sbeg, c.tile_ent};
+    em::SweepSources fsrc{c.tile_sbeg, c.tile_ent, c.order};
     em::SweepMaps maps;
     for (int a = 0; a < 3; ++a) {
         if (eonly) { maps.E[a] = map_field[lvl * 3 + a]; maps.H[a] = map_prev[((lvl + 2) % 3) * 3 + a]; }

@@ -123,13 +123,40 @@ __device__ __forceinline__ void pair_sync(int id) { asm volatile("bar.sync %0, 6
 // rows and columns of a box are re-read by the neighbouring tiles a few planes earlier or later, so input lines should
 // outlive output lines in L2 (measured: -1 % step time on config 4; splitting each plane into halo boxes with evict_last
 // and an interior box with evict_first was 3 % SLOWER).
+#ifndef EM_SWEEP_LOADPOL
+#define EM_SWEEP_LOADPOL 1
+#endif
+#ifndef EM_SWEEP_PFPOL
+#define EM_SWEEP_PFPOL 0
+#endif
+template <int POL> __device__ __forceinline__ unsigned long long l2_policy() {
+    unsigned long long pol;
+    if (POL == 1) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    else if (POL == 2) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
 __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map, unsigned bar, int x, int y, int z) {
     EM_FUZZ();
-    unsigned long long pol;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    const unsigned long long pol = l2_policy<EM_SWEEP_LOADPOL>();
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;"
         ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar), "l"(pol) : "memory");
+}
+
+// TMA prefetch of a box into L2 only (no shared memory, no barrier): the boxes of plane k + 2 + kSwL2Ahead can be requested
+// from DRAM when the loads of plane k + 2 are issued.  OFF (0) by default: measured on config 4 it made the step SLOWER
+// (2.30 -> 2.36 / 2.49 / 2.85 ms for 1 / 2 / 4 planes ahead, whatever the L2 policies): the later loads do hit L2 (read
+// misses -37 %) but DRAM reads grow by 0.6 GB (prefetched lines are evicted before use) -- the waits for staged planes
+// are bandwidth, not latency (profiles/r2_experiments.md).
+#ifndef EM_SWEEP_L2AHEAD
+#define EM_SWEEP_L2AHEAD 0
+#endif
+constexpr int kSwL2Ahead = EM_SWEEP_L2AHEAD;
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap *map, int x, int y, int z) {
+    const unsigned long long pol = l2_policy<EM_SWEEP_PFPOL>();
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile.L2::cache_hint [%0, {%1, %2, %3}], %4;"
+                 ::"l"(map), "r"(x), "r"(y), "r"(z), "l"(pol) : "memory");
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------------
@@ -138,7 +165,7 @@ __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map
 // gather; phase C adds the Joule heat of the step to theta (already advanced by the conduction kernel k_diffuse) and
 // writes sigma(T^{n+1}) to the other sigma buffer.  The one-material path is taken only for materials with alpha = 0.
 template <typename R, int LOSS, bool UMU, bool TH = false, bool EO = false>
-__global__ void __launch_bounds__(Tile<sizeof(R), TH>::threads, 1)
+__global__ void __launch_bounds__(Tile<sizeof(R), TH>::threads, kSweepOcc)
 k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R> src, SweepSources fs,
             SweepChunks zc, int ntx, long long step, ThermalSweep<R> th) {
     constexpr int V = 16 / sizeof(R);
@@ -155,7 +182,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     // work item = (tile, z chunk), as in k_fused_sweep: the chunk stores planes kz0 <= k < kz1, starts one
     // plane lower (warm-up, nothing stored) and ends on plane ke (E'(ke) closes the Joule sum of layer ke-1)
-    const int item = blockIdx.x, tile = item / zc.nzs, chunk = item - tile * zc.nzs;
+    const int item = fs.order[blockIdx.x], tile = item / zc.nzs, chunk = item - tile * zc.nzs;     // launch order: em_tile.cuh
     const int tx = tile % ntx, ty = tile / ntx;
     const int kz0 = zc.kb[chunk], kz1 = zc.kb[chunk + 1];
     const int ks = (kz0 > 0 || p.warm_lo) ? kz0 - 1 : 0, ke = kz1 <= p.nz ? kz1 : p.nz;   // PMC at -z: plane -1 warms up too
@@ -235,6 +262,12 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         tma_load_3d(sb + L::ez + (kk & 1) * L::ez_slot, &maps.E[2], bar, cx, cyy, kk + 1);
         tma_load_3d(sb + L::ids + (kk & 1) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, kk + 1);
         if (TH) tma_load_3d(sb + L::sig + (kk & 1) * L::sig_slot, &maps.sig, bar, cx, cyy - 1, kk + 1);   // rows -2 .. TY
+        if (kSwL2Ahead > 0 && kk + kSwL2Ahead <= ke) {          // the same boxes of plane kk + kSwL2Ahead, into L2 only
+            const int kp = kk + kSwL2Ahead;
+            tma_prefetch_3d(&maps.E[0], cx, cyy, kp + 2); tma_prefetch_3d(&maps.E[1], cx, cyy, kp + 2);
+            tma_prefetch_3d(&maps.E[2], cx, cyy, kp + 1); tma_prefetch_3d(&maps.mat, id_x, cyy - 1, kp + 1);
+            if (TH) tma_prefetch_3d(&maps.sig, cx, cyy - 1, kp + 1);
+        }
     };
     // H group of plane kk -> parity kk&1 (two planes in flight)
     auto issue_H = [&](int kk) {
@@ -243,6 +276,11 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         tma_load_3d(sb + L::h + ((kk & 1) * 3 + 0) * L::h_slot, &maps.H[0], bar, cx, cyy, kk + 1);
         tma_load_3d(sb + L::h + ((kk & 1) * 3 + 1) * L::h_slot, &maps.H[1], bar, cx, cyy, kk + 1);
         tma_load_3d(sb + L::h + ((kk & 1) * 3 + 2) * L::h_slot, &maps.H[2], bar, cx, cyy, kk + 1);
+        if (kSwL2Ahead > 0 && kk + kSwL2Ahead <= ke) {
+            const int kp = kk + kSwL2Ahead;
+            tma_prefetch_3d(&maps.H[0], cx, cyy, kp + 1); tma_prefetch_3d(&maps.H[1], cx, cyy, kp + 1);
+            tma_prefetch_3d(&maps.H[2], cx, cyy, kp + 1);
+        }
     };
     if (tid == 0) {
         issue_E(ks, true);

@@ -125,7 +125,31 @@ template <typename R> __device__ __forceinline__ R shfl_down1(R v) { return __sh
 struct SweepSources {
     const int *tile_sbeg;     // indexed by work item = tile * nzs + chunk (entries of a tile are sorted by k)
     const int4 *tile_ent;
+    const int *order;         // work item of CTA blockIdx.x (launch_order below)
 };
+
+// Launch order of the work items.  CTAs are handed to the SMs in blockIdx order, roughly one every (item time / n_sm),
+// and a tile re-reads the halo rows / columns of its neighbours: those re-reads hit L2 only if the neighbour passes the
+// same plane within a few plane-times, i.e. if it was launched within a few items (L2 holds ~9 plane-steps of the whole
+// chip's traffic).  So: chunk-major (the chunks of one tile column share nothing), and inside a chunk the tiles in
+// blocks of kOrderBY x kOrderBX tiles, y fastest -- x neighbours and most y neighbours are then a few items apart.
+#ifndef EM_SWEEP_ORDER_BY
+#define EM_SWEEP_ORDER_BY 1
+#endif
+#ifndef EM_SWEEP_ORDER_BX
+#define EM_SWEEP_ORDER_BX (1 << 20)
+#endif
+inline void launch_order(const SweepPlan &f, int *order /* n_tiles * nzs */) {
+    const int BY = EM_SWEEP_ORDER_BY, BX = EM_SWEEP_ORDER_BX;
+    int n = 0;
+    if (BY <= 0) {                                   // tile-major (the round-1 order)
+        for (int t = 0; t < f.n_tiles; ++t) for (int c = 0; c < f.nzs; ++c) order[n++] = t * f.nzs + c;
+    } else for (int c = 0; c < f.nzs; ++c)
+        for (int by = 0; by < f.nty; by += BY)
+            for (int bx = 0; bx < f.ntx; bx += BX)
+                for (int x = bx; x < std::min(bx + BX, f.ntx); ++x)
+                    for (int y = by; y < std::min(by + BY, f.nty); ++y) order[n++] = (y * f.ntx + x) * f.nzs + c;
+}
 
 // z chunks of the sweep (SweepPlan::kb), passed by value
 struct SweepChunks {
