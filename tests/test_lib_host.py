@@ -55,6 +55,16 @@ def test_cfl_dt_matches_oracle_and_generator(seed):
     assert abs(0.9 * a5 - p5.dt) <= 1e-14 * p5.dt
 
 
+def test_cfl_dt_hand_computed_2x2x2():
+    """the library's em_cfl_dt against the hand-computed bound of tests/golden/cfl_2x2x2.txt"""
+    from workloads.problem import EPS0, MU0
+    want = float([l.split()[1] for l in open(os.path.join(ROOT, "tests", "golden", "cfl_2x2x2.txt")) if l.startswith("dt_max ")][0])
+    dx, dy, dz = np.asarray([1e-3, 2e-3]), np.asarray([1e-3, 3e-3]), np.asarray([2e-3, 1e-3])
+    table = np.asarray([[EPS0, MU0, 0.0], [4.0 * EPS0, MU0, 0.0]])
+    mat = np.zeros((2, 2, 2), np.uint8); mat[1, 0, 0] = 1
+    assert abs(P.em_cfl_dt(2, 2, 2, dx, dy, dz, mat, table) - want) <= 1e-13 * want
+
+
 def test_create_validates_before_touching_the_device():
     L = P.load()
     p = W.random_problem(4, 4, 4, seed=3, n_ports=0)

@@ -323,6 +323,21 @@ def test_p9_cfl_rule_vs_power_iteration():
     assert dt1 > 0.5 * dt_true
 
 
+def test_p9b_cfl_rule_hand_computed_2x2x2():
+    """absolute anchor of emo_cfl_dt on a non-uniform two-material grid: the hand-computed minimum of
+    tests/golden/cfl_2x2x2.txt (the material decides which cell wins, so a wrong min/max, exponent or index order fails)"""
+    kv, _ = _read_kv(os.path.join(GOLD, "cfl_2x2x2.txt"))
+    dx, dy, dz = np.asarray([1e-3, 2e-3]), np.asarray([1e-3, 3e-3]), np.asarray([2e-3, 1e-3])
+    table = np.asarray([[EPS0, MU0, 0.0], [4.0 * EPS0, MU0, 0.0]])
+    mat = np.zeros((2, 2, 2), np.uint8); mat[1, 0, 0] = 1                 # [k][j][i]: cell (i, j, k) = (0, 0, 1)
+    got = emo.cfl_dt(2, 2, 2, dx, dy, dz, mat, table)
+    assert abs(got - float(kv["dt_max"])) <= 1e-13 * got
+    assert abs(W.cfl_dt(dx, dy, dz, mat, table, 1.0) - float(kv["dt_max"])) <= 1e-13 * got
+    mat[:] = 0
+    got = emo.cfl_dt(2, 2, 2, dx, dy, dz, mat, table)
+    assert abs(got - float(kv["dt_max_if_cell_001_were_vacuum"])) <= 1e-13 * got
+
+
 # --------------------------------------------------------------------------- API / edge cases
 def test_oracle_rejects_bad_arguments():
     p = W.random_problem(4, 4, 4, seed=71, n_ports=0)
