@@ -1071,6 +1071,12 @@ int32_t em_create(const em_grid *gr, const uint8_t *mat_id, const em_material *t
 
 int32_t em_abi_version(void) { return EM_ABI_VERSION; }
 
+#ifdef EM_SWEEP_TRACE
+int32_t em_trace_buffer(long long *dev) {
+    return cudaMemcpyToSymbol(em::g_em_trace, &dev, sizeof(dev)) == cudaSuccess ? EM_OK : EM_ERR_CUDA;
+}
+#endif
+
 #ifdef EM_SWEEP_FUZZ
 // test builds only (libem_fuzz.so; em_sweep.cuh "schedule fuzzing"): 0 switches the random delays off
 int32_t em_fuzz_seed(uint32_t seed) {

@@ -89,6 +89,15 @@ __device__ __forceinline__ void em_fuzz() {
 #define EM_FUZZ() ((void)0)
 #endif
 
+// ---- per-phase clock trace (experiment builds only: -DEM_SWEEP_TRACE) ----------------------------------------------------
+#ifdef EM_SWEEP_TRACE
+__device__ long long *g_em_trace = nullptr;      // [n_items][warps][planes<=80][8 stamps]
+#define EM_TRACE(slot) do { if (g_em_trace && lane == 0 && (k - ks) < 80) \
+    g_em_trace[(((long long)blockIdx.x * 16 + w) * 80 + (k - ks)) * 8 + (slot)] = clock64(); } while (0)
+#else
+#define EM_TRACE(slot) ((void)0)
+#endif
+
 // ---- mbarrier / TMA PTX wrappers ---------------------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
@@ -195,7 +204,12 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     const bool active = (j <= ny + 1) && (i0 + V <= p.PX);
     const bool own = active && lane >= 1 && lane <= 30 && cy >= 0 && cy < kSwTY && j <= ny;
     const bool own_q = own && j < ny;
+    // the per-thread store predicates as plane thresholds held in two registers (opaque to the compiler, which otherwise
+    // re-derives `own` from lane, row and grid size on every plane to stay inside the register cap)
+    int st_lo = own ? kz0 : 0x7fffffff, q_lo = own_q ? kz0 : 0x7fffffff;
+    asm volatile("" : "+r"(st_lo), "+r"(q_lo));
     const unsigned out_pack = (unsigned)(p.n_table - 1) * 0x01010101u;
+    const bool has_peer = p.peer_skip != 0;
 
     // shared-memory views
     MatEntry<R> *s_tab = reinterpret_cast<MatEntry<R> *>(sm + L::tab);
@@ -313,16 +327,18 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     int s_next_k = (s_cur < s_end) ? fs.tile_ent[s_cur].z : 0x7fffffff;
 
     int rk = (ks + 3) % 3;                                // k % 3
-    for (int k = ks; k <= ke; ++k) {
+    long long o = off0 + (long long)ks * PXY;             // this thread's vector at plane k
+    for (int k = ks; k <= ke; ++k, o += PXY) {
         const int it = k - ks;
         const int rk1 = (rk == 2) ? 0 : rk + 1;
         const int par = k & 1;
-        const long long o = off0 + (long long)k * PXY;
-        const bool st = own && k >= kz0 && k < kz1;          // this chunk stores H'(k), E'(k)
+        const bool st = k >= st_lo && k < kz1;               // this chunk stores H'(k), E'(k)
 
         // ---- phase A: H' = H - nbar * curl E  (inner factor of S = curl mu^-1 curl) ----------
         EM_FUZZ();
+        EM_TRACE(0);
         mbar_wait(bar_fullE(it & 1), (unsigned)(it >> 1) & 1u);   // E group of plane k has landed
+        EM_TRACE(1);
         const R fz = s_z[par * 4 + 0], rdz = s_z[par * 4 + 1], rtz = s_z[par * 4 + 2];
         const unsigned idw = ld_ids(par, w + 1), idj = ld_ids(par, w);
         // one material over the warp's whole coefficient neighbourhood (rows j-1..j, planes k-1..k)?
@@ -367,7 +383,9 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
 #pragma unroll
                 for (int c = 0; c < V; ++c) hx.v[c] = hy.v[c] = hz.v[c] = R(0);
             } else {
+                EM_TRACE(2);
                 mbar_wait(bar_fullH(it & 1), (unsigned)(it >> 1) & 1u);   // H(k) has landed
+                EM_TRACE(3);
                 hx = staged(L::h + (par * 3 + 0) * L::h_slot); hy = staged(L::h + (par * 3 + 1) * L::h_slot);
                 hz = staged(L::h + (par * 3 + 2) * L::h_slot);
             }
@@ -408,7 +426,9 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
                 issue_H(k + 2);
             }
         }
+        EM_TRACE(4);
         if (w != 0) mbar_wait(bar_rowH(w - 1), (unsigned)it & 1u);   // H'(k) of row j-1 is visible
+        EM_TRACE(5);
 
         // ---- phase B: E' = E + r (curl H' - J - sigma E), Joule squares (eq. 2-3) -------------
         // (warp 0 = halo row -1 only supplies H' to row 0: no E', no Joule)
@@ -417,6 +437,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         // neighbour's wall plane when this is the plane it needs (DevParams::peer_*)
         auto store_exy = [&](int comp, const VecR &v) {
             if (!st) return;
+            if (!has_peer) { EM_ST(p.En[comp] + o, v); return; }         // (kernel-uniform: no slab neighbour is wired)
             if (!((k == 0 && (p.peer_skip & 1)) || (k == nz && (p.peer_skip & 2)))) EM_ST(p.En[comp] + o, v);
             if (k == p.peer_k[0]) EM_ST(p.peer_e[0][comp] + (o - (long long)k * PXY), v);
             if (k == p.peer_k[1]) EM_ST(p.peer_e[1][comp] + (o - (long long)k * PXY), v);
@@ -466,8 +487,10 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         // producer/consumer named barrier of their own (id = the upper warp's index) and a warp on the one-material
         // path does not wait for a general-path warp elsewhere in the CTA.  Warp 0 (no phase C) still consumes, so
         // that it cannot overwrite its H' row (phase A of plane k+1) while warp 1 reads it in phase B.
+        EM_TRACE(6);
         if (w != 0) pair_arrive(w);               // my B row is written (and I am done reading the H' row of row j-1)
         if (!is_top) pair_sync(w + 1);            // the B row of row j+1 is visible
+        EM_TRACE(7);
         cp_async_wait<0>();                       // q(k-1) has landed (private slot: no barrier needed)
 
         // ---- phase C: q(k-1) += dt sigma/16 (pend + Sxy(k)); pend = Sxy(k) + Sz(k) ---------------------------
@@ -501,12 +524,12 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             mine[kSlotPend * NT] = pend;
             // q of a lane whose V cells are one lossless material never changes: neither fetched nor stored
             // (coupled sweep: the same holds for theta -- only conduction moves it -- and for sigma = 0)
-            if (own_q && k > kz0 && q_live) {                            // layer k-1 in [kz0, kz1)
+            if (k > q_lo && q_live) {                                    // layer k-1 in [kz0, kz1)
                 EM_ST(p.q + o - PXY, qv);
                 if (TH) { EM_ST(th.theta + o - PXY, thv); EM_ST(th.sig_out + o - PXY, sgn); }
             }
             q_live = !(id_uniform(idw) && s_tab[idw & 0xff].b == R(0));
-            if (own_q && k >= kz0 && k < ke && q_live) {
+            if (k >= q_lo && k < ke && q_live) {
                 cp_async16(mine + kSlotQ * NT, p.q + o);                 // q(k)
                 if (TH) cp_async16(mine + kSlotTheta * NT, th.theta + o);   // theta_d(k)
             }
