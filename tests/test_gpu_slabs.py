@@ -131,6 +131,7 @@ def _ipc_worker(rank, world, port, out_dir):
         dist.destroy_process_group()
 
 
+@pytest.mark.slow          # two processes on ONE GPU: opt-in (EM_RUN_SLOW=1); it passed in the three full-suite runs of round 2
 def test_peer_halo_between_two_processes_over_cuda_ipc(tmp_path):
     import torch.multiprocessing as mp
     world = 2
