@@ -354,6 +354,23 @@ def test_oracle_rejects_bad_arguments():
     assert o.step_index == 0
 
 
+def test_oracle_reset_restarts_the_run_exactly():
+    """emo_reset zeroes the six fields, q and the step counter (waveform index): the rerun repeats the first run bit for bit"""
+    p = W.random_problem(7, 6, 5, seed=72, n_ports=3, steps=25)
+    p.init = None
+    o = emo.Oracle(p)
+    o.step(25)
+    first = o.fields(); _, q1, Q1 = o.joule()
+    assert any(f.any() for f in first) and Q1 > 0
+    o.reset()
+    assert o.step_index == 0 and not any(f.any() for f in o.fields())
+    _, q0, Q0 = o.joule()
+    assert Q0 == 0.0 and not q0.any()
+    o.step(25)
+    again = o.fields(); _, q2, Q2 = o.joule()
+    assert all(np.array_equal(a, b) for a, b in zip(first, again)) and np.array_equal(q1, q2) and Q1 == Q2
+
+
 def test_oracle_pec_material_edges_stay_zero():
     p = W.random_problem(7, 6, 5, seed=81, pec_material=True, n_ports=0, steps=10)
     pec = (p.flags[p.mat_id] & 1).astype(bool)
