@@ -26,16 +26,19 @@ def _stale(lib: str = LIB) -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_lib(force: bool = False, verbose: bool = False, fuzz: bool = False) -> str:
+def build_lib(force: bool = False, verbose: bool = False, fuzz: bool = False, defines=()) -> str:
     """libem.so; fuzz=True builds libem_fuzz.so, the TEST variant with random delays at every synchronisation point of
-    the sweep (csrc/em_sweep.cuh "schedule fuzzing") and the extra entry em_fuzz_seed"""
+    the sweep (csrc/em_sweep.cuh "schedule fuzzing") and the extra entry em_fuzz_seed.  defines: extra -D switches for
+    the experiment knobs of the sweep (profiles/r2_experiments.md); such a build is always forced and the next plain
+    build (any source newer, or --force) replaces it."""
     lib = LIB_FUZZ if fuzz else LIB
-    if force or _stale(lib):
+    if force or defines or _stale(lib):
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         cmd = [nvcc, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
                "-Xcompiler", "-fPIC", "-shared", "-o", lib] + [os.path.join(CSRC, s) for s in SOURCES]
         if fuzz:
             cmd += ["-DEM_SWEEP_FUZZ"]
+        cmd += list(defines)
         if verbose:
             cmd += ["-Xptxas", "-v"]
         subprocess.check_call(cmd)
@@ -43,4 +46,5 @@ def build_lib(force: bool = False, verbose: bool = False, fuzz: bool = False) ->
 
 
 if __name__ == "__main__":
-    print(build_lib(force="--force" in sys.argv, verbose="-v" in sys.argv, fuzz="--fuzz" in sys.argv))
+    print(build_lib(force="--force" in sys.argv, verbose="-v" in sys.argv, fuzz="--fuzz" in sys.argv,
+                    defines=[a for a in sys.argv[1:] if a.startswith("-D")]))
