@@ -106,4 +106,11 @@ __device__ __forceinline__ R loss_r(R A /*eps/dt*/, R B /*sigma*/) {
     }
 }
 
+// series conductance per unit face area of the two half cells: k_f / l~_f = 2 / (d_a/k_a + d_b/k_b) = 2 g_a g_b / (g_a + g_b)
+// with the half-cell conductances g = k/d; 0 if either cell does not conduct (k = 0, or a pad cell: 1/d = 0)
+template <typename R> __device__ __forceinline__ R half_cell_cond(R ga, R gb) {
+    const R den = ga + gb;
+    return den > R(0) ? R(2) * ga * gb * rcp<R>(den) : R(0);
+}
+
 }  // namespace em

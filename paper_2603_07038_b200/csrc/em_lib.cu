@@ -250,7 +250,7 @@ struct Ctx final : em_ctx {
     int32_t step_thermal_sweep();
     int sg_cur = 0;                     // which sigma(T) buffer is current (the coupled sweep ping-pongs them)
     R *sig_buf(int which) const { return (which ? c.sig2 : c.sig) + g.origin; }
-    CUtensorMap map_sig[2];
+    CUtensorMap map_sig[2], map_theta[2];
     int32_t refresh_sigma();
     bool thermal_on = false;            // em_set_thermal was called
     int th_cur = 0;
@@ -349,7 +349,11 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     if (kernel == EM_KERNEL_TMA) {           // (the layout holds the largest table, 255 + 2 entries, in both precisions)
         int optin = 0;
         CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
-        if (sweep_smem > (size_t)optin) return fail(EM_ERR_UNSUPPORTED, "the sweep's shared-memory layout does not fit this device");
+        if (sweep_smem > (size_t)optin) {
+            // (only the fp64 coupled sweep with > 250 materials: its two tables of 32-B entries exceed the layout by 160 B)
+            if (gr->thermal && gr->kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_SPLIT;
+            else return fail(EM_ERR_UNSUPPORTED, "the sweep's shared-memory layout does not fit this device");
+        }
     }
     main_kernel = kernel == EM_KERNEL_TMA ? "k_sweep_tma" : "k_split_e";
 
@@ -509,6 +513,9 @@ int32_t Ctx<R>::make_maps() {
     if (grid.thermal) {                                   // sigma(T) planes of the coupled sweep: rows -2 .. TY
         rc = encode(&map_sig[0], fdt, sizeof(R), c.sig + g.PX - V, 32 * V, sw_warps + 1); if (rc) return rc;
         rc = encode(&map_sig[1], fdt, sizeof(R), c.sig2 + g.PX - V, 32 * V, sw_warps + 1); if (rc) return rc;
+        for (int q = 0; q < 2 && em::kFusedConduction; ++q) {     // (experimental fused conduction) theta^n planes: rows -1 .. TY
+            rc = encode(&map_theta[q], fdt, sizeof(R), c.theta[q] + g.PX - V, 32 * V, sw_warps); if (rc) return rc;
+        }
     }
     return EM_OK;
 }
@@ -873,21 +880,23 @@ int32_t Ctx<R>::step_thermal() {
 // One coupled step on the TMA sweep: conduction first (theta_d = theta^n - dt/(rho c_p) M_kk theta^n into the other theta
 // buffer), then the sweep with D_sigma(T^n) from the current sigma buffer; its phase C adds the Joule heat of the step to
 // theta_d in place and writes sigma(T^{n+1}) of the lossy lanes to the other sigma buffer.  Buffers are swapped.
+// (-DEM_SWEEP_FUSED_CONDUCTION=1, experimental: the conduction stencil runs inside the sweep and k_diffuse is not launched.)
 template <typename R>
 int32_t Ctx<R>::step_thermal_sweep() {
     dim3 b(32, 8);
     R *th_in = c.theta[th_cur] + g.origin, *th_out = c.theta[1 - th_cur] + g.origin;
-    {
+    if (!em::kFusedConduction) {
         constexpr int V = 16 / (int)sizeof(R);
         dim3 gd(((g.nx + V - 1) / V + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, g.nz);
         em::k_diffuse<R><<<gd, b, 0, stream>>>(p, c.ttable, th_in, th_out);
+        launches += 1;
     }
-    launches += 1;
     int32_t rc = record_begin(); if (rc) return rc;
     em::SweepSources fsrc{c.tile_sbeg, c.tile_ent, c.order};
     em::SweepMaps maps;
     for (int a = 0; a < 3; ++a) { maps.E[a] = map_field[e_cur * 3 + a]; maps.H[a] = map_field[6 + h_cur * 3 + a]; }
     maps.q = map_q; maps.mat = map_mat; maps.sig = map_sig[sg_cur];
+    if (em::kFusedConduction) maps.th = map_theta[th_cur];
     em::ThermalSweep<R> tsw{th_out, sig_buf(1 - sg_cur), c.ttable};
     cudaError_t e = em::launch_sweep_tma<R>(sweep_kernel, plan, sweep_smem, maps, p, src, fsrc, (long long)step_index, stream, &tsw);
     if (e != cudaSuccess) return fail(EM_ERR_CUDA, std::string("coupled TMA sweep launch: ") + cudaGetErrorString(e));

@@ -31,14 +31,25 @@ constexpr int kSwRow = 512;                        // bytes of one staged row (3
 constexpr int kSwIdShift = 16;                     // the id map starts 16 B before the row (16-B aligned base)
 constexpr int kSwPriv = 8;                         // private 16-B slots per thread: q, L x 4, H' x 2, pend
 
-struct alignas(64) SweepMaps { CUtensorMap E[3], H[3], q, mat, sig; };   // sig: the sigma(T^n) array (coupled sweep only)
+struct alignas(64) SweepMaps { CUtensorMap E[3], H[3], q, mat, sig, th; };   // sig, th: sigma(T^n), theta^n (coupled sweep only)
+
+// EXPERIMENTAL, OFF by default and NOT yet run on a GPU (the pool was closed for this repository when it was finished,
+// profiles/r2_experiments.md): -DEM_SWEEP_FUSED_CONDUCTION=1 folds the conduction stencil of eq. (5) into the coupled
+// sweep -- theta^n planes in a ring of 3 beside sigma(T), ids in a ring of 3, the stencil of layer k-1 in phase A of plane
+// k with the lower-face flux carried -- so that a coupled step is ONE launch (no k_diffuse).  With the switch off the
+// preprocessed kernel and its SASS are those of the verified build.
+#ifndef EM_SWEEP_FUSED_CONDUCTION
+#define EM_SWEEP_FUSED_CONDUCTION 0
+#endif
+constexpr bool kFusedConduction = EM_SWEEP_FUSED_CONDUCTION != 0;
 
 // Shared-memory layout (bytes; identical for fp32 and fp64 except the id rows; the table comes last
 // because its size is only known at run time)
 template <int SZ, bool TH = false> struct SweepLayout {
     static constexpr int V = 16 / SZ;
     static constexpr int kSwWarps = Tile<SZ, TH>::warps, kSwRows = Tile<SZ, TH>::rows;
-    static constexpr int n_priv = kSwPriv + (TH ? 1 : 0);          // + theta of layer k-1 (coupled sweep)
+    static constexpr bool FC = TH && kFusedConduction;
+    static constexpr int n_priv = kSwPriv + (TH ? (FC ? 2 : 1) : 0);   // coupled sweep: + theta of layer k-1 (FC: + the heat flux through its lower face)
     static constexpr int ex = 0;                                  // Ex ring of 3 planes, rows -1 .. TY+1
     static constexpr int ex_slot = (kSwWarps + 1) * kSwRow;
     static constexpr int ey = ex + 3 * ex_slot;                   // Ey ring of 3 planes, rows -1 .. TY
@@ -47,18 +58,23 @@ template <int SZ, bool TH = false> struct SweepLayout {
     static constexpr int ez_slot = (kSwWarps + 1) * kSwRow;
     static constexpr int h = ez + 2 * ez_slot;                    // [2 parities][Hx, Hy, Hz], rows -1 .. TY
     static constexpr int h_slot = kSwWarps * kSwRow;
-    static constexpr int ids = h + 6 * h_slot;                    // ids, 2 parities, rows -2 .. TY+1
+    static constexpr int ids = h + 6 * h_slot;                    // ids, 2 parities (coupled sweep: ring of 3), rows -2 .. TY+1
+    static constexpr int n_ids = FC ? 3 : 2;
     static constexpr int id_row = 32 * V + 16;                    // box starts on a 16-B boundary: up to 15 B of lead-in
     static constexpr int id_slot = ((kSwWarps + 2) * id_row + 127) / 128 * 128;
-    static constexpr int priv = ids + 2 * id_slot;                // private slots [kSwPriv][512 threads]
+    static constexpr int priv = ids + n_ids * id_slot;            // private slots [kSwPriv][512 threads]
     static constexpr int rows = priv + n_priv * kSwWarps * kSwRow;     // H'x, H'z, Bx, Bz exchange rows [kSwRows][32]
     static constexpr int geo = rows + 4 * kSwRows * kSwRow;    // 1/dx, 1/dx~, fx of the 32 lanes
     static constexpr int zg = geo + 3 * kSwRow;                   // [2 parity]{fz, 1/dz, 1/dz~, 0}
     static constexpr int sig = zg + 128;                          // coupled sweep: sigma(T^n), 2 parities, rows -2 .. TY (TMA: 128-B aligned)
     static constexpr int sig_slot = TH ? (kSwWarps + 1) * kSwRow : 0;
-    static constexpr int bar = sig + 2 * sig_slot;                // fullE[2], fullH[2], empty[2], rowH[kSwWarps]
+    static constexpr int tht = sig + 2 * sig_slot;                // coupled sweep: theta^n, ring of 3 planes, rows -1 .. TY
+    static constexpr int th_slot = FC ? kSwWarps * kSwRow : 0;
+    static constexpr int yg = tht + 3 * th_slot;                  // coupled sweep: {1/dy[j-1], 1/dy[j+1], 1/dy~[j+1], 0} per row
+    static constexpr int yg_bytes = FC ? kSwWarps * 4 * SZ : 0;
+    static constexpr int bar = FC ? (yg + yg_bytes + 63) / 64 * 64 : sig + 2 * sig_slot;   // fullE[2], fullH[2], empty[2], emptyH[2], rowH[kSwWarps]
     static constexpr int tab = bar + 64 + 8 * kSwWarps;                          // material table (n_table entries)
-    static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + (kSwWarps + 2) * id_row + sig_slot;
+    static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + (kSwWarps + 2) * id_row + sig_slot + th_slot;
     static constexpr int first_extra_bytes = ex_slot + ey_slot;
     static constexpr int h_bytes = 3 * h_slot;
 };
@@ -182,10 +198,11 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     constexpr int kSwTY = Tile<sizeof(R), TH>::TY, kSwWarps = Tile<sizeof(R), TH>::warps, kSwRows = Tile<sizeof(R), TH>::rows;
     constexpr int NT = Tile<sizeof(R), TH>::threads;
     using L = SweepLayout<(int)sizeof(R), TH>;
+    constexpr bool FC = L::FC;        // conduction fused into the coupled sweep (experimental switch, see SweepLayout)
     using VecR = Vec<R>;
     using IdT = typename std::conditional<V == 4, unsigned, unsigned short>::type;
     // private 16-B slots of a thread
-    constexpr int kSlotQ = 0, kSlotL = 1, kSlotHp = 5, kSlotPend = 7, kSlotTheta = 8;
+    constexpr int kSlotQ = 0, kSlotL = 1, kSlotHp = 5, kSlotPend = 7, kSlotTheta = 8, kSlotFz = 9;
     extern __shared__ __align__(1024) unsigned char sm[];
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -255,6 +272,11 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             s_geo[2 * 32 + lane] = in ? *reinterpret_cast<const VecR *>(p.fx + i0) : z;
         }
     }
+    if (FC && lane == 0) {          // y geometry of the conduction stencil, per row: 1/dy[j-1], 1/dy[j+1], 1/dy~[j+1]
+        R *yg = reinterpret_cast<R *>(sm + L::yg) + 4 * w;
+        const bool in = (j <= ny + 1);
+        yg[0] = in ? p.rdy[j - 1] : R(0); yg[1] = in ? p.rdy[j + 1] : R(0); yg[2] = in ? p.rty[j + 1] : R(0); yg[3] = R(0);
+    }
     __syncthreads();
 
     // TMA coordinates of this tile (maps are based at logical (-V, -1, -1); ids at (-16 B, -1, -1))
@@ -274,8 +296,11 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         tma_load_3d(sb + L::ex + ((kk + 1) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 2);
         tma_load_3d(sb + L::ey + ((kk + 1) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 2);
         tma_load_3d(sb + L::ez + (kk & 1) * L::ez_slot, &maps.E[2], bar, cx, cyy, kk + 1);
-        tma_load_3d(sb + L::ids + (kk & 1) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, kk + 1);
-        if (TH) tma_load_3d(sb + L::sig + (kk & 1) * L::sig_slot, &maps.sig, bar, cx, cyy - 1, kk + 1);   // rows -2 .. TY
+        tma_load_3d(sb + L::ids + (FC ? (kk + 3) % 3 : (kk & 1)) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, kk + 1);
+        if (TH) {
+            tma_load_3d(sb + L::sig + (kk & 1) * L::sig_slot, &maps.sig, bar, cx, cyy - 1, kk + 1);   // rows -2 .. TY
+            if (FC) tma_load_3d(sb + L::tht + ((kk + 3) % 3) * L::th_slot, &maps.th, bar, cx, cyy, kk + 1);    // theta^n(kk), rows -1 .. TY
+        }
         if (kSwL2Ahead > 0 && kk + kSwL2Ahead <= ke) {          // the same boxes of plane kk + kSwL2Ahead, into L2 only
             const int kp = kk + kSwL2Ahead;
             tma_prefetch_3d(&maps.E[0], cx, cyy, kp + 2); tma_prefetch_3d(&maps.E[1], cx, cyy, kp + 2);
@@ -340,7 +365,8 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         mbar_wait(bar_fullE(it & 1), (unsigned)(it >> 1) & 1u);   // E group of plane k has landed
         EM_TRACE(1);
         const R fz = s_z[par * 4 + 0], rdz = s_z[par * 4 + 1], rtz = s_z[par * 4 + 2];
-        const unsigned idw = ld_ids(par, w + 1), idj = ld_ids(par, w);
+        const int ids_k = FC ? rk : par;                          // slot of ids(k): ring of 3 in the coupled sweep
+        const unsigned idw = ld_ids(ids_k, w + 1), idj = ld_ids(ids_k, w);
         // one material over the warp's whole coefficient neighbourhood (rows j-1..j, planes k-1..k)?
         const bool rowu = (idw == idj) && id_uniform(idw);
         const unsigned idw_lane0 = __shfl_sync(0xffffffffu, idw, 0);   // (every lane must execute it)
@@ -349,6 +375,72 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         if (TH) {
             hom = hom && s_th[idw_lane0 & 0xff].alpha == R(0);     // sigma of the material does not depend on T
             sigw = staged(L::sig + par * L::sig_slot + kSwRow); sigj = staged(L::sig + par * L::sig_slot);
+        }
+        // ---- coupled sweep: conduction half of eq. (5) for cell layer k-1, theta_d = theta^n - dt/(rho c_p) (M_kk theta^n),
+        // M_kk = V0a^T D_k V0 as the cell-centred -div k grad with the series conductivity of the two half cells on each
+        // face (T3).  theta^n(k-1) with its x / y neighbours and theta^n(k) are resident (ring of 3 planes), and
+        // so are the ids of plane k-1; the flux through the lower face was computed one plane ago.  Phase C adds the Joule
+        // heat.  (k == ks: nothing below is resident yet; the layers concerned belong to the chunk below.)
+        if (FC && w != 0 && !is_top) {
+            VecR thd, fzo;
+            if (k == ks) {
+#pragma unroll
+                for (int c = 0; c < V; ++c) thd.v[c] = fzo.v[c] = R(0);
+            } else {
+                const int rkm = (rk == 0) ? 2 : rk - 1;                       // (k - 1) % 3
+                const unsigned char *tb = sm + L::tht + rkm * L::th_slot + tid * 16;
+                const VecR t0 = *reinterpret_cast<const VecR *>(tb), tym = *reinterpret_cast<const VecR *>(tb - kSwRow);
+                const VecR typ = *reinterpret_cast<const VecR *>(tb + kSwRow);
+                const VecR tzp = *reinterpret_cast<const VecR *>(sm + L::tht + rk * L::th_slot + tid * 16);
+                const VecR fzm = mine[kSlotFz * NT];
+                const R tl_ = shfl_up1(t0.v[V - 1]), tr_ = shfl_down1(t0.v[0]);
+                const unsigned idc = idw_prev, idym = ld_ids(rkm, w), idyp = ld_ids(rkm, w + 2);
+                const unsigned idl = __shfl_up_sync(0xffffffffu, (idc >> (8 * (V - 1))) & 0xffu, 1);
+                const unsigned idr = __shfl_down_sync(0xffffffffu, idc & 0xffu, 1);
+                const VecR rdxv = s_geo[0 * 32 + lane], rtxv = s_geo[1 * 32 + lane];
+                const R rdx_l = shfl_up1(rdxv.v[V - 1]), rdx_r = shfl_down1(rdxv.v[0]), rtx_r = shfl_down1(rtxv.v[0]);
+                const R *yg = reinterpret_cast<const R *>(sm + L::yg) + 4 * w;
+                const R rdym = yg[0], rdyp = yg[1], rtyp = yg[2];
+                const R rdz1 = p.rdz[k - 1];                                   // 1/dz of layer k-1 (rdz, rtz: plane / layer k)
+                const unsigned rep_id = (V == 4) ? (idc & 0xffu) * 0x01010101u : (((idc & 0xffu) * 0x0101u) | (out_pack & 0xffff0000u));
+                const bool uni = idc == rep_id && idym == rep_id && idyp == rep_id && idw == rep_id &&
+                                 idl == (idc & 0xffu) && idr == (idc & 0xffu);
+                if (__all_sync(0xffffffffu, uni)) {
+                    // one material over the whole neighbourhood: the series conductance of two equal half cells is k / d~
+                    const ThEntry<R> me = s_th[idc & 0xffu];
+                    const R cy0 = rdy * rty, cy1 = rdy * rtyp, cz1 = me.k * rtz, sc = p.dt * me.irc;
+#pragma unroll
+                    for (int c = 0; c < V; ++c) {
+                        const R tc = t0.v[c];
+                        const R tl = c > 0 ? t0.v[c > 0 ? c - 1 : 0] : tl_, tr = c < V - 1 ? t0.v[c < V - 1 ? c + 1 : c] : tr_;
+                        const R rtx1 = c < V - 1 ? rtxv.v[c < V - 1 ? c + 1 : c] : rtx_r;
+                        R lat = rdxv.v[c] * (rtxv.v[c] * (tc - tl) + rtx1 * (tc - tr));
+                        lat = mad(cy0, tc - tym.v[c], lat); lat = mad(cy1, tc - typ.v[c], lat);
+                        const R fz = cz1 * (tc - tzp.v[c]);
+                        thd.v[c] = mad(-sc, mad(me.k, lat, rdz1 * (fz - fzm.v[c])), tc);
+                        fzo.v[c] = fz;
+                    }
+                } else {
+                    R kc[V + 2], rdxc[V + 2], gxf[V + 1];
+                    kc[0] = s_th[idl].k; kc[V + 1] = s_th[idr].k; rdxc[0] = rdx_l; rdxc[V + 1] = rdx_r;
+#pragma unroll
+                    for (int c = 0; c < V; ++c) { kc[c + 1] = s_th[(idc >> (8 * c)) & 0xff].k; rdxc[c + 1] = rdxv.v[c]; }
+#pragma unroll
+                    for (int c = 0; c < V + 1; ++c) gxf[c] = half_cell_cond(rdxc[c] * kc[c], rdxc[c + 1] * kc[c + 1]);
+#pragma unroll
+                    for (int c = 0; c < V; ++c) {
+                        const R tc = t0.v[c], kme = kc[c + 1], gy = rdy * kme, gz = rdz1 * kme;
+                        const R tl = c > 0 ? t0.v[c > 0 ? c - 1 : 0] : tl_, tr = c < V - 1 ? t0.v[c < V - 1 ? c + 1 : c] : tr_;
+                        R lat = rdxc[c + 1] * (gxf[c] * (tc - tl) + gxf[c + 1] * (tc - tr));
+                        lat = mad(rdy, half_cell_cond(gy, rdym * s_th[(idym >> (8 * c)) & 0xff].k) * (tc - tym.v[c]), lat);
+                        lat = mad(rdy, half_cell_cond(gy, rdyp * s_th[(idyp >> (8 * c)) & 0xff].k) * (tc - typ.v[c]), lat);
+                        const R fz = half_cell_cond(gz, rdz * s_th[(idw >> (8 * c)) & 0xff].k) * (tc - tzp.v[c]);
+                        thd.v[c] = mad(-p.dt * s_th[(idc >> (8 * c)) & 0xff].irc, lat + rdz1 * (fz - fzm.v[c]), tc);
+                        fzo.v[c] = fz;
+                    }
+                }
+            }
+            mine[kSlotTheta * NT] = thd; mine[kSlotFz * NT] = fzo;
         }
         VecR hxn, hyn, hzn;
         const VecR ex0 = staged(L::ex + rk * L::ex_slot), ey0 = staged(L::ey + rk * L::ey_slot);
@@ -524,14 +616,19 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
             mine[kSlotPend * NT] = pend;
             // q of a lane whose V cells are one lossless material never changes: neither fetched nor stored
             // (coupled sweep: the same holds for theta -- only conduction moves it -- and for sigma = 0)
-            if (k > q_lo && q_live) {                                    // layer k-1 in [kz0, kz1)
-                EM_ST(p.q + o - PXY, qv);
-                if (TH) { EM_ST(th.theta + o - PXY, thv); EM_ST(th.sig_out + o - PXY, sgn); }
+            if (!FC) {
+                if (k > q_lo && q_live) {                                    // layer k-1 in [kz0, kz1)
+                    EM_ST(p.q + o - PXY, qv);
+                    if (TH) { EM_ST(th.theta + o - PXY, thv); EM_ST(th.sig_out + o - PXY, sgn); }
+                }
+            } else if (k > q_lo) {
+                if (q_live) { EM_ST(p.q + o - PXY, qv); EM_ST(th.sig_out + o - PXY, sgn); }
+                EM_ST(th.theta + o - PXY, thv);                          // fused conduction moves every cell's theta
             }
             q_live = !(id_uniform(idw) && s_tab[idw & 0xff].b == R(0));
             if (k >= q_lo && k < ke && q_live) {
                 cp_async16(mine + kSlotQ * NT, p.q + o);                 // q(k)
-                if (TH) cp_async16(mine + kSlotTheta * NT, th.theta + o);   // theta_d(k)
+                if (TH && !FC) cp_async16(mine + kSlotTheta * NT, th.theta + o);   // theta_d(k)
             }
         }
         cp_async_commit();

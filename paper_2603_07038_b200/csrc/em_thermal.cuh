@@ -92,13 +92,6 @@ __global__ void k_source_coef_sig(DevParams<R> p, DevSources<R> s, const R *sig)
     s.r[u] = r[s.comp[u]];
 }
 
-// series conductance per unit face area of the two half cells: k_f / l~_f = 2 / (d_a/k_a + d_b/k_b) = 2 g_a g_b / (g_a + g_b)
-// with the half-cell conductances g = k/d; 0 if either cell does not conduct (k = 0, or a pad cell: 1/d = 0)
-template <typename R> __device__ __forceinline__ R half_cell_cond(R ga, R gb) {
-    const R den = ga + gb;
-    return den > R(0) ? R(2) * ga * gb * rcp<R>(den) : R(0);
-}
-
 // a4 + eq. (5) + eq. (6): Joule heat of the step into q and into the cell's temperature rise, conduction to the six
 // neighbours from theta^n (ping-pong), then sigma(T^{n+1}) of the own cell.
 template <typename R>
