@@ -141,3 +141,42 @@ def test_exchange_dist_gloo_reproduces_the_single_domain_recurrence(world, tmp_p
     for p in parts:
         assert abs(float(p["total"]) - ref.th.sum()) <= 1e-12 * abs(ref.th).sum()
     assert np.abs(ref.ex - ex).max() > 1e-3                      # the recurrence did something
+
+
+class _WiringEM:
+    """records what the peer wiring hands to em_set_peer_halo (no CUDA involved)"""
+    def __init__(self, rank):
+        self.workspace_ptr = 0x10000000 * (rank + 1)
+        self.rank = rank
+        self.calls = []
+
+    def wall_offsets(self, side):               # [parity * 2 + comp], distinct per rank and side
+        return [1000 * self.rank + 100 * side + 10 * q + c for q in (0, 1) for c in (0, 1)]
+
+    def em_set_peer_halo(self, side, k_send, addresses):
+        self.calls.append((side, k_send, list(addresses)))
+
+
+def test_peer_wiring_hands_each_sweep_its_neighbours_wall_planes():
+    """in-process peer wiring (slabs.connect_peers_inprocess): rank r stores its plane b-1 into the -z wall of rank r+1 and
+    its plane a+1 into the +z wall of rank r-1; the addresses are the neighbour's workspace base + ITS wall offsets"""
+    nz, world = 13, 3
+    ranks = [slabs.SlabRank(_WiringEM(r), slabs.slab_meta(nz, r, world)) for r in range(world)]
+    slabs.connect_peers_inprocess(ranks)
+    for r, sr in enumerate(ranks):
+        m = sr.meta
+        want = []
+        if m.has_above:
+            nb = ranks[r + 1].em
+            want.append((1, m.b - 1 - m.lo, [nb.workspace_ptr + o for o in nb.wall_offsets(0)]))
+        if m.has_below:
+            nb = ranks[r - 1].em
+            want.append((0, m.a + 1 - m.lo, [nb.workspace_ptr + o for o in nb.wall_offsets(1)]))
+        assert sr.em.calls == want and sr.mode == "peer"
+    # the plane a slab sends up is the plane its upper neighbour holds as wall plane 0, and vice versa (global indices)
+    for r in range(world - 1):
+        lo, hi = ranks[r], ranks[r + 1]
+        assert lo.meta.lo + lo.k_send_up == hi.meta.lo + hi.k_wall_lo
+        assert hi.meta.lo + hi.k_send_down == lo.meta.lo + lo.k_wall_hi
+        assert lo.meta.lo + lo.layer_send_up == hi.meta.lo + 0                       # theta: my top owned layer = its ghost layer 0
+        assert hi.meta.lo + hi.layer_send_down == lo.meta.lo + lo.nz_local - 1       # my bottom owned layer = its last ghost layer
