@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libem.so")
 LIB_FUZZ = os.path.join(HERE, "libem_fuzz.so")
 SOURCES = ["em_lib.cu"]
-HEADERS = ["em_common.cuh", "em_split.cuh", "em_aux.cuh", "em_tile.cuh", "em_sweep.cuh", "em_sweep_phaseb.inc", "em_sweep_phaseb_hom.inc", "em_thermal.cuh", os.path.join("..", "..", "include", "em.h")]
+HEADERS = ["em_ptx.cuh", "em_common.cuh", "em_split.cuh", "em_aux.cuh", "em_tile.cuh", "em_sweep.cuh", "em_sweep_phaseb.inc", "em_sweep_phaseb_hom.inc", "em_thermal.cuh", os.path.join("..", "..", "include", "em.h")]
 
 
 

@@ -11,7 +11,7 @@
 // the extra table entry n_mat = "outside/PEC" whose mask is 0.
 #pragma once
 #include <cstdint>
-#include <cuda_runtime.h>
+#include "em_ptx.cuh"
 
 namespace em {
 
@@ -74,18 +74,12 @@ __device__ __forceinline__ float  mad(float a, float b, float c)    { return ::f
 __device__ __forceinline__ double mad(double a, double b, double c) { return ::fma(a, b, c); }
 template <typename R> __device__ __forceinline__ R lerp(R lo, R hi, R f) { return mad(f, hi - lo, lo); }
 
-// 16-byte store with the streaming (evict-first) L2 policy: output planes are never re-read within a step,
-// so they should not displace the halo rows the neighbouring tiles are about to re-read
-template <typename T> __device__ __forceinline__ void st_stream16(void *dst, const T &v) {
-    static_assert(sizeof(T) == 16, "16-byte vectors only");
-    __stcs(reinterpret_cast<float4 *>(dst), *reinterpret_cast<const float4 *>(&v));
-}
+// (st_stream16, the 16-byte streaming store of the output planes: em_ptx.cuh)
 
 template <typename R> __device__ __forceinline__ R rcp(R x);
 template <> __device__ __forceinline__ float  rcp<float>(float x) {
     // MUFU.RCP (<= 1 ulp) + one Newton step: no slow-path branch; x is a positive normal number here
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    const float r = rcp_approx(x);
     return fmaf(r, fmaf(-x, r, 1.0f), r);
 }
 template <> __device__ __forceinline__ double rcp<double>(double x) { return 1.0 / x; }

@@ -412,7 +412,7 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
         int pmc_mask = 0;
         for (int b = 0; b < 6; ++b) if (gr->bc[b] == EM_BC_PMC) pmc_mask |= 1 << b;
         const long long n = g.vol;
-        em::k_pad_pmc<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(c.mat + g.origin - g.PXY - g.PX - 1, g.nx, g.ny, g.nz,
+        EM_LAUNCH(em::k_pad_pmc, (unsigned)((n + 255) / 256), 256, 0, stream)(c.mat + g.origin - g.PXY - g.PX - 1, g.nx, g.ny, g.nz,
                                                                         g.PX, g.PY, n, pmc_mask, (uint8_t)n_mat);
         CU(cudaGetLastError());
     }
@@ -618,8 +618,8 @@ int32_t Ctx<R>::set_source(int32_t np, const em_port *ports, const em_edge *edge
     n_unique = nu; n_ports = np;
     if (nu) {
         const int bs = 128, gs = (nu + bs - 1) / bs;
-        if (loss == EM_LOSS_CD) em::k_source_coef<R, 0><<<gs, bs, 0, stream>>>(p, src, c.src_flags);
-        else                    em::k_source_coef<R, 1><<<gs, bs, 0, stream>>>(p, src, c.src_flags);
+        if (loss == EM_LOSS_CD) EM_LAUNCH((em::k_source_coef<R, 0>), gs, bs, 0, stream)(p, src, c.src_flags);
+        else                    EM_LAUNCH((em::k_source_coef<R, 1>), gs, bs, 0, stream)(p, src, c.src_flags);
         CU(cudaGetLastError());
         std::vector<int> flags(nu);
         CU(cudaMemcpyAsync(flags.data(), c.src_flags, sizeof(int) * nu, cudaMemcpyDeviceToHost, stream));
@@ -648,7 +648,7 @@ int32_t Ctx<R>::set_field(int32_t comp, const void *srcp, int32_t is_dev) {
     CU(cudaMemcpy3DAsync(&m, stream));
     if (comp < 3 || comp >= 6) {
         dim3 b(32, 8);
-        em::k_mask_fixed<R><<<node_grid(b, 1), b, 0, stream>>>(p, comp_ptr(comp), comp % 3, 0);
+        EM_LAUNCH(em::k_mask_fixed<R>, node_grid(b, 1), b, 0, stream)(p, comp_ptr(comp), comp % 3, 0);
         CU(cudaGetLastError());
     }
     if (!is_dev) CU(cudaStreamSynchronize(stream));
@@ -672,7 +672,7 @@ int32_t Ctx<R>::plane(int32_t comp, int32_t k, void *dst, const void *srcp, int3
         if (comp < 3 || comp >= 6) {                      // PEC-fixed edges of this plane stay 0
             dim3 b(32, 8);
             dim3 gr((g.nx + 1 + b.x - 1) / b.x, (g.ny + 1 + b.y - 1) / b.y, 1);
-            em::k_mask_fixed<R><<<gr, b, 0, stream>>>(p, comp_ptr(comp), comp % 3, k);
+            EM_LAUNCH(em::k_mask_fixed<R>, gr, b, 0, stream)(p, comp_ptr(comp), comp % 3, k);
             CU(cudaGetLastError());
         }
     }
@@ -706,8 +706,8 @@ int32_t Ctx<R>::halo(int32_t kp, int32_t kl, void *dst, const void *srcp, void *
     int64_t n = 0; halo_elems(&n);
     const unsigned blocks = (unsigned)((n + 255) / 256);
     R *th = thermal_on ? c.theta[th_cur] + g.origin : nullptr;
-    if (dst) em::k_pack_halo<R><<<blocks, 256, 0, s>>>(p, p.E[0], p.E[1], th, kp, kl, static_cast<R *>(dst));
-    else     em::k_unpack_halo<R><<<blocks, 256, 0, s>>>(p, p.E[0], p.E[1], th, thermal_on ? sig_buf(0) : nullptr,
+    if (dst) EM_LAUNCH(em::k_pack_halo<R>, blocks, 256, 0, s)(p, p.E[0], p.E[1], th, kp, kl, static_cast<R *>(dst));
+    else     EM_LAUNCH(em::k_unpack_halo<R>, blocks, 256, 0, s)(p, p.E[0], p.E[1], th, thermal_on ? sig_buf(0) : nullptr,
                                                           thermal_on ? sig_buf(1) : nullptr, c.ttable, kp, kl, static_cast<const R *>(srcp));
     CU(cudaGetLastError());
     launches += 1;
@@ -717,8 +717,8 @@ int32_t Ctx<R>::halo(int32_t kp, int32_t kl, void *dst, const void *srcp, void *
 template <typename R>
 int32_t Ctx<R>::joule_layers(int32_t k0, int32_t k1, double *total) {
     if (k0 < 0 || k1 < k0 || k1 > g.nz || !total) return fail(EM_ERR_INVALID_ARG, "joule_layers: need 0 <= k0 <= k1 <= nz");
-    em::k_energy_partial<R><<<kReduceBlocks, 256, 0, stream>>>(p, c.vx, c.vy, c.vz, k0, k1, c.partial);
-    em::k_energy_final<<<1, 256, 0, stream>>>(c.partial, kReduceBlocks, c.scalar);
+    EM_LAUNCH(em::k_energy_partial<R>, kReduceBlocks, 256, 0, stream)(p, c.vx, c.vy, c.vz, k0, k1, c.partial);
+    EM_LAUNCH(em::k_energy_final, 1, 256, 0, stream)(c.partial, kReduceBlocks, c.scalar);
     CU(cudaGetLastError()); launches += 2;
     CU(cudaMemcpyAsync(total, c.scalar, sizeof(double), cudaMemcpyDeviceToHost, stream));
     CU(cudaStreamSynchronize(stream));
@@ -775,17 +775,17 @@ int32_t Ctx<R>::record_end() {
 template <typename R>
 int32_t Ctx<R>::step_split() {
     dim3 b(32, 8);
-    em::k_split_h<R><<<node_grid(b, 1), b, 0, stream>>>(p);
+    EM_LAUNCH(em::k_split_h<R>, node_grid(b, 1), b, 0, stream)(p);
     int32_t rc = record_begin(); if (rc) return rc;
-    if (loss == EM_LOSS_CD) em::k_split_e<R, 0><<<node_grid(b, 1), b, 0, stream>>>(p);
-    else                    em::k_split_e<R, 1><<<node_grid(b, 1), b, 0, stream>>>(p);
+    if (loss == EM_LOSS_CD) EM_LAUNCH((em::k_split_e<R, 0>), node_grid(b, 1), b, 0, stream)(p);
+    else                    EM_LAUNCH((em::k_split_e<R, 1>), node_grid(b, 1), b, 0, stream)(p);
     rc = record_end(); if (rc) return rc;
     launches += 2;
     if (n_unique) {
-        em::k_apply_source<R><<<(n_unique + 127) / 128, 128, 0, stream>>>(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
+        EM_LAUNCH(em::k_apply_source<R>, (n_unique + 127) / 128, 128, 0, stream)(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
         launches += 1;
     }
-    em::k_split_joule<R><<<node_grid(b, 0), b, 0, stream>>>(p);
+    EM_LAUNCH(em::k_split_joule<R>, node_grid(b, 0), b, 0, stream)(p);
     launches += 1;
     CU(cudaGetLastError());
     e_cur ^= 1; bind();
@@ -797,9 +797,9 @@ template <typename R>
 int32_t Ctx<R>::refresh_sigma() {
     dim3 b(32, 8);
     em::ThermalParams<R> t = tp();
-    em::k_sigma_refresh<R><<<node_grid(b, 0), b, 0, stream>>>(p, t);
+    EM_LAUNCH(em::k_sigma_refresh<R>, node_grid(b, 0), b, 0, stream)(p, t);
     t.sig = sig_buf(1 - sg_cur);                        // both buffers: the coupled sweep rewrites only the lossy lanes
-    em::k_sigma_refresh<R><<<node_grid(b, 0), b, 0, stream>>>(p, t);
+    EM_LAUNCH(em::k_sigma_refresh<R>, node_grid(b, 0), b, 0, stream)(p, t);
     CU(cudaGetLastError());
     return EM_OK;
 }
@@ -857,20 +857,20 @@ template <typename R>
 int32_t Ctx<R>::step_thermal() {
     dim3 b(32, 8);
     const R *sig = sig_buf(sg_cur);
-    em::k_split_h<R><<<node_grid(b, 1), b, 0, stream>>>(p);
+    EM_LAUNCH(em::k_split_h<R>, node_grid(b, 1), b, 0, stream)(p);
     int32_t rc = record_begin(); if (rc) return rc;
-    if (loss == EM_LOSS_CD) em::k_split_e_sig<R, 0><<<node_grid(b, 1), b, 0, stream>>>(p, sig);
-    else                    em::k_split_e_sig<R, 1><<<node_grid(b, 1), b, 0, stream>>>(p, sig);
+    if (loss == EM_LOSS_CD) EM_LAUNCH((em::k_split_e_sig<R, 0>), node_grid(b, 1), b, 0, stream)(p, sig);
+    else                    EM_LAUNCH((em::k_split_e_sig<R, 1>), node_grid(b, 1), b, 0, stream)(p, sig);
     rc = record_end(); if (rc) return rc;
     launches += 2;
     if (n_unique) {
         const int gs = (n_unique + 127) / 128;
-        if (loss == EM_LOSS_CD) em::k_source_coef_sig<R, 0><<<gs, 128, 0, stream>>>(p, src, sig);
-        else                    em::k_source_coef_sig<R, 1><<<gs, 128, 0, stream>>>(p, src, sig);
-        em::k_apply_source<R><<<gs, 128, 0, stream>>>(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
+        if (loss == EM_LOSS_CD) EM_LAUNCH((em::k_source_coef_sig<R, 0>), gs, 128, 0, stream)(p, src, sig);
+        else                    EM_LAUNCH((em::k_source_coef_sig<R, 1>), gs, 128, 0, stream)(p, src, sig);
+        EM_LAUNCH(em::k_apply_source<R>, gs, 128, 0, stream)(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
         launches += 2;
     }
-    em::k_joule_thermal<R><<<node_grid(b, 0), b, 0, stream>>>(p, tp());
+    EM_LAUNCH(em::k_joule_thermal<R>, node_grid(b, 0), b, 0, stream)(p, tp());
     launches += 1;
     CU(cudaGetLastError());
     e_cur ^= 1; th_cur ^= 1; bind();
@@ -888,7 +888,7 @@ int32_t Ctx<R>::step_thermal_sweep() {
     if (!em::kFusedConduction) {
         constexpr int V = 16 / (int)sizeof(R);
         dim3 gd(((g.nx + V - 1) / V + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, g.nz);
-        em::k_diffuse<R><<<gd, b, 0, stream>>>(p, c.ttable, th_in, th_out);
+        EM_LAUNCH(em::k_diffuse<R>, gd, b, 0, stream)(p, c.ttable, th_in, th_out);
         launches += 1;
     }
     int32_t rc = record_begin(); if (rc) return rc;
@@ -943,8 +943,8 @@ template <typename R>
 int32_t Ctx<R>::joule(void *power, void *energy, double *total, int32_t do_reset) {
     dim3 b(32, 8);
     if (power) {
-        if (thermal_on) em::k_power_sig<R><<<node_grid(b, 0), b, 0, stream>>>(p, sig_buf(sg_cur), static_cast<R *>(power));
-        else            em::k_power<R><<<node_grid(b, 0), b, 0, stream>>>(p, static_cast<R *>(power));
+        if (thermal_on) EM_LAUNCH(em::k_power_sig<R>, node_grid(b, 0), b, 0, stream)(p, sig_buf(sg_cur), static_cast<R *>(power));
+        else            EM_LAUNCH(em::k_power<R>, node_grid(b, 0), b, 0, stream)(p, static_cast<R *>(power));
         CU(cudaGetLastError()); launches += 1;
     }
     if (energy) {
@@ -956,8 +956,8 @@ int32_t Ctx<R>::joule(void *power, void *energy, double *total, int32_t do_reset
         CU(cudaMemcpy3DAsync(&m, stream));
     }
     if (total) {
-        em::k_energy_partial<R><<<kReduceBlocks, 256, 0, stream>>>(p, c.vx, c.vy, c.vz, 0, g.nz, c.partial);
-        em::k_energy_final<<<1, 256, 0, stream>>>(c.partial, kReduceBlocks, c.scalar);
+        EM_LAUNCH(em::k_energy_partial<R>, kReduceBlocks, 256, 0, stream)(p, c.vx, c.vy, c.vz, 0, g.nz, c.partial);
+        EM_LAUNCH(em::k_energy_final, 1, 256, 0, stream)(c.partial, kReduceBlocks, c.scalar);
         CU(cudaGetLastError()); launches += 2;
         CU(cudaMemcpyAsync(total, c.scalar, sizeof(double), cudaMemcpyDeviceToHost, stream));
         CU(cudaStreamSynchronize(stream));
@@ -986,7 +986,7 @@ int32_t Ctx<R>::probe(int32_t n, const em_probe_pt *pts, double *out) {
         }
         CU(cudaMemcpyAsync(c.probe_off, off.data(), sizeof(long long) * m, cudaMemcpyHostToDevice, stream));
         CU(cudaMemcpyAsync(c.probe_comp, comp.data(), sizeof(int) * m, cudaMemcpyHostToDevice, stream));
-        em::k_probe<R><<<(m + 127) / 128, 128, 0, stream>>>(pa, c.probe_off, c.probe_comp, m, c.probe_out);
+        EM_LAUNCH(em::k_probe<R>, (m + 127) / 128, 128, 0, stream)(pa, c.probe_off, c.probe_comp, m, c.probe_out);
         CU(cudaGetLastError()); launches += 1;
         CU(cudaMemcpyAsync(out + base, c.probe_out, sizeof(double) * m, cudaMemcpyDeviceToHost, stream));
         CU(cudaStreamSynchronize(stream));

@@ -19,8 +19,6 @@
 // M (N - M - K = -dt^2 S).  The planes of e^{n-1} ride in the staging slots of H.  9 words + 1 B + 2 words per
 // cell-update = 45 B (fp32) / 89 B (fp64) instead of 57 / 113.
 #pragma once
-#include <cuda.h>
-
 #include "em_tile.cuh"
 
 namespace em {
@@ -86,25 +84,6 @@ inline size_t sweep_smem_bytes(int sizeof_real, int n_table, bool thermal = fals
     return tab + (size_t)n_table * 4 * sizeof_real * (thermal ? 2 : 1);
 }
 
-// ---- schedule fuzzing (test builds only: -DEM_SWEEP_FUZZ, libem_fuzz.so) ---------------------------------------------
-// The plane loop orders its shared-memory hazards with mbarriers and named barriers instead of CTA barriers.  compute-
-// sanitizer is closed on this GPU pool, so the evidence that no ordering edge is missing is a stress test: with a
-// non-zero seed every synchronisation point (and every phase boundary) delays its warp by a pseudo-random 0-8 us -- a
-// few plane-times -- and the results must stay bit-identical to the normal build (tests/test_gpu_fuzz.py).
-#ifdef EM_SWEEP_FUZZ
-__device__ unsigned g_em_fuzz_seed = 0;
-__device__ __forceinline__ void em_fuzz() {
-    const unsigned seed = g_em_fuzz_seed;
-    if (seed == 0) return;
-    unsigned x = ((unsigned)(clock64() >> 7) * 2654435761u) ^ seed ^ (blockIdx.x * 97u + (threadIdx.x >> 5) * 131u);
-    x ^= x >> 15; x *= 2246822519u; x ^= x >> 13;
-    if ((x & 3u) == 0u) __nanosleep((x >> 8) & 8191u);
-}
-#define EM_FUZZ() em_fuzz()
-#else
-#define EM_FUZZ() ((void)0)
-#endif
-
 // ---- per-phase clock trace (experiment builds only: -DEM_SWEEP_TRACE) ----------------------------------------------------
 #ifdef EM_SWEEP_TRACE
 __device__ long long *g_em_trace = nullptr;      // [n_items][warps][planes<=80][8 stamps]
@@ -114,36 +93,7 @@ __device__ long long *g_em_trace = nullptr;      // [n_items][warps][planes<=80]
 #define EM_TRACE(slot) ((void)0)
 #endif
 
-// ---- mbarrier / TMA PTX wrappers ---------------------------------------------------------------------
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(unsigned bar) {
-    EM_FUZZ();
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "W_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@!p bra W_%=;\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-    EM_FUZZ();
-}
-// 1-D bulk copy global -> shared counted on an mbarrier (bytes: multiple of 16)
-__device__ __forceinline__ void bulk_load(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-// producer / consumer named barrier of two warps (ids 1..15; id 0 is __syncthreads)
-__device__ __forceinline__ void pair_arrive(int id) { EM_FUZZ(); asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
-__device__ __forceinline__ void pair_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); EM_FUZZ(); }
+// (mbarrier / TMA / named-barrier wrappers and the schedule-fuzzing hook EM_FUZZ: em_ptx.cuh)
 // Every staged plane is loaded with the L2 evict_last policy (the output planes are written evict-first): the halo
 // rows and columns of a box are re-read by the neighbouring tiles a few planes earlier or later, so input lines should
 // outlive output lines in L2 (measured: -1 % step time on config 4; splitting each plane into halo boxes with evict_last
@@ -154,21 +104,6 @@ __device__ __forceinline__ void pair_sync(int id) { asm volatile("bar.sync %0, 6
 #ifndef EM_SWEEP_PFPOL
 #define EM_SWEEP_PFPOL 0
 #endif
-template <int POL> __device__ __forceinline__ unsigned long long l2_policy() {
-    unsigned long long pol;
-    if (POL == 1) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-    else if (POL == 2) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map, unsigned bar, int x, int y, int z) {
-    EM_FUZZ();
-    const unsigned long long pol = l2_policy<EM_SWEEP_LOADPOL>();
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;"
-        ::"r"(dst), "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar), "l"(pol) : "memory");
-}
-
 // TMA prefetch of a box into L2 only (no shared memory, no barrier): the boxes of plane k + 2 + kSwL2Ahead can be requested
 // from DRAM when the loads of plane k + 2 are issued.  OFF (0) by default: measured on config 4 it made the step SLOWER
 // (2.30 -> 2.36 / 2.49 / 2.85 ms for 1 / 2 / 4 planes ahead, whatever the L2 policies): the later loads do hit L2 (read
@@ -178,11 +113,6 @@ __device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap *map
 #define EM_SWEEP_L2AHEAD 0
 #endif
 constexpr int kSwL2Ahead = EM_SWEEP_L2AHEAD;
-__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap *map, int x, int y, int z) {
-    const unsigned long long pol = l2_policy<EM_SWEEP_PFPOL>();
-    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile.L2::cache_hint [%0, {%1, %2, %3}], %4;"
-                 ::"l"(map), "r"(x), "r"(y), "r"(z), "l"(pol) : "memory");
-}
 
 // ---- the kernel ------------------------------------------------------------------------------------------
 // TH = true: the thermally coupled sweep (eq. (4)-(6); DESIGN.md section 9 NEXT-1).  The per-cell sigma(T^n)
@@ -203,7 +133,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     using IdT = typename std::conditional<V == 4, unsigned, unsigned short>::type;
     // private 16-B slots of a thread
     constexpr int kSlotQ = 0, kSlotL = 1, kSlotHp = 5, kSlotPend = 7, kSlotTheta = 8, kSlotFz = 9;
-    extern __shared__ __align__(1024) unsigned char sm[];
+    EM_DYN_SMEM(sm);
 
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     // work item = (tile, z chunk), as in k_fused_sweep: the chunk stores planes kz0 <= k < kz1, starts one
@@ -224,7 +154,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
     // the per-thread store predicates as plane thresholds held in two registers (opaque to the compiler, which otherwise
     // re-derives `own` from lane, row and grid size on every plane to stay inside the register cap)
     int st_lo = own ? kz0 : 0x7fffffff, q_lo = own_q ? kz0 : 0x7fffffff;
-    asm volatile("" : "+r"(st_lo), "+r"(q_lo));
+    opaque2(st_lo, q_lo);
     const unsigned out_pack = (unsigned)(p.n_table - 1) * 0x01010101u;
     const bool has_peer = p.peer_skip != 0;
 
@@ -253,7 +183,7 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         mbar_init(bar_empty(0), kSwWarps); mbar_init(bar_empty(1), kSwWarps);
         mbar_init(bar_emptyH(0), kSwWarps); mbar_init(bar_emptyH(1), kSwWarps);
         for (int ww = 0; ww < kSwWarps; ++ww) mbar_init(bar_rowH(ww), 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
     }
     for (int t = tid; t < p.n_table; t += NT) s_tab[t] = p.table[t];
     ThEntry<R> *s_th = reinterpret_cast<ThEntry<R> *>(s_tab + p.n_table);     // coupled sweep only
@@ -290,35 +220,35 @@ k_sweep_tma(const __grid_constant__ SweepMaps maps, DevParams<R> p, DevSources<R
         mbar_expect_tx(bar, (unsigned)(L::e_bytes + (first ? L::first_extra_bytes : 0) + 4 * sizeof(R)));
         bulk_load(smem_u32(&s_z[(kk & 1) * 4]), p.zgeo + 4 * (long long)kk, 4 * (unsigned)sizeof(R), bar);   // {fz, 1/dz, 1/dz~, 0}
         if (first) {
-            tma_load_3d(sb + L::ex + ((kk + 3) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 1);
-            tma_load_3d(sb + L::ey + ((kk + 3) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 1);
+            tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::ex + ((kk + 3) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 1);
+            tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::ey + ((kk + 3) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 1);
         }
-        tma_load_3d(sb + L::ex + ((kk + 1) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 2);
-        tma_load_3d(sb + L::ey + ((kk + 1) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 2);
-        tma_load_3d(sb + L::ez + (kk & 1) * L::ez_slot, &maps.E[2], bar, cx, cyy, kk + 1);
-        tma_load_3d(sb + L::ids + (FC ? (kk + 3) % 3 : (kk & 1)) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, kk + 1);
+        tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::ex + ((kk + 1) % 3) * L::ex_slot, &maps.E[0], bar, cx, cyy, kk + 2);
+        tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::ey + ((kk + 1) % 3) * L::ey_slot, &maps.E[1], bar, cx, cyy, kk + 2);
+        tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::ez + (kk & 1) * L::ez_slot, &maps.E[2], bar, cx, cyy, kk + 1);
+        tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::ids + (FC ? (kk + 3) % 3 : (kk & 1)) * L::id_slot, &maps.mat, bar, id_x, cyy - 1, kk + 1);
         if (TH) {
-            tma_load_3d(sb + L::sig + (kk & 1) * L::sig_slot, &maps.sig, bar, cx, cyy - 1, kk + 1);   // rows -2 .. TY
-            if (FC) tma_load_3d(sb + L::tht + ((kk + 3) % 3) * L::th_slot, &maps.th, bar, cx, cyy, kk + 1);    // theta^n(kk), rows -1 .. TY
+            tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::sig + (kk & 1) * L::sig_slot, &maps.sig, bar, cx, cyy - 1, kk + 1);   // rows -2 .. TY
+            if (FC) tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::tht + ((kk + 3) % 3) * L::th_slot, &maps.th, bar, cx, cyy, kk + 1);    // theta^n(kk), rows -1 .. TY
         }
         if (kSwL2Ahead > 0 && kk + kSwL2Ahead <= ke) {          // the same boxes of plane kk + kSwL2Ahead, into L2 only
             const int kp = kk + kSwL2Ahead;
-            tma_prefetch_3d(&maps.E[0], cx, cyy, kp + 2); tma_prefetch_3d(&maps.E[1], cx, cyy, kp + 2);
-            tma_prefetch_3d(&maps.E[2], cx, cyy, kp + 1); tma_prefetch_3d(&maps.mat, id_x, cyy - 1, kp + 1);
-            if (TH) tma_prefetch_3d(&maps.sig, cx, cyy - 1, kp + 1);
+            tma_prefetch_3d<EM_SWEEP_PFPOL>(&maps.E[0], cx, cyy, kp + 2); tma_prefetch_3d<EM_SWEEP_PFPOL>(&maps.E[1], cx, cyy, kp + 2);
+            tma_prefetch_3d<EM_SWEEP_PFPOL>(&maps.E[2], cx, cyy, kp + 1); tma_prefetch_3d<EM_SWEEP_PFPOL>(&maps.mat, id_x, cyy - 1, kp + 1);
+            if (TH) tma_prefetch_3d<EM_SWEEP_PFPOL>(&maps.sig, cx, cyy - 1, kp + 1);
         }
     };
     // H group of plane kk -> parity kk&1 (two planes in flight)
     auto issue_H = [&](int kk) {
         const unsigned sb = smem_u32(sm), bar = bar_fullH((kk - ks) & 1);
         mbar_expect_tx(bar, (unsigned)L::h_bytes);
-        tma_load_3d(sb + L::h + ((kk & 1) * 3 + 0) * L::h_slot, &maps.H[0], bar, cx, cyy, kk + 1);
-        tma_load_3d(sb + L::h + ((kk & 1) * 3 + 1) * L::h_slot, &maps.H[1], bar, cx, cyy, kk + 1);
-        tma_load_3d(sb + L::h + ((kk & 1) * 3 + 2) * L::h_slot, &maps.H[2], bar, cx, cyy, kk + 1);
+        tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::h + ((kk & 1) * 3 + 0) * L::h_slot, &maps.H[0], bar, cx, cyy, kk + 1);
+        tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::h + ((kk & 1) * 3 + 1) * L::h_slot, &maps.H[1], bar, cx, cyy, kk + 1);
+        tma_load_3d<EM_SWEEP_LOADPOL>(sb + L::h + ((kk & 1) * 3 + 2) * L::h_slot, &maps.H[2], bar, cx, cyy, kk + 1);
         if (kSwL2Ahead > 0 && kk + kSwL2Ahead <= ke) {
             const int kp = kk + kSwL2Ahead;
-            tma_prefetch_3d(&maps.H[0], cx, cyy, kp + 1); tma_prefetch_3d(&maps.H[1], cx, cyy, kp + 1);
-            tma_prefetch_3d(&maps.H[2], cx, cyy, kp + 1);
+            tma_prefetch_3d<EM_SWEEP_PFPOL>(&maps.H[0], cx, cyy, kp + 1); tma_prefetch_3d<EM_SWEEP_PFPOL>(&maps.H[1], cx, cyy, kp + 1);
+            tma_prefetch_3d<EM_SWEEP_PFPOL>(&maps.H[2], cx, cyy, kp + 1);
         }
     };
     if (tid == 0) {
@@ -672,7 +602,7 @@ cudaError_t launch_sweep_tma(SweepKernel<R> kern, const SweepPlan &plan, size_t 
     ThermalSweep<R> th{};
     if (thermal) th = *thermal;
     const int threads = thermal ? Tile<sizeof(R), true>::threads : Tile<sizeof(R)>::threads;
-    kern<<<plan.n_tiles * plan.nzs, threads, smem_bytes, stream>>>(maps, p, src, fs, zc, plan.ntx, step, th);
+    EM_LAUNCH(kern, plan.n_tiles * plan.nzs, threads, smem_bytes, stream)(maps, p, src, fs, zc, plan.ntx, step, th);
     return cudaGetLastError();
 }
 
