@@ -132,9 +132,10 @@ def _open(path: str):
     return L
 
 
-def _check(rc: int):
+def _check(rc: int, L=None):
+    """L: the library the call went to (EM(..., lib=...)); default: the product library"""
     if rc != EM_OK:
-        raise EMError(rc, load().em_last_error().decode())
+        raise EMError(rc, (L if L is not None else load()).em_last_error().decode())
 
 
 def _dp(a: np.ndarray):
@@ -221,7 +222,7 @@ class EM:
                               1 if getattr(p, "thermal", None) is not None else 0, formulation, z_chunks)
         self.formulation = int(formulation)
         nbytes = C.c_size_t()
-        _check(self._L.em_workspace_bytes(C.byref(self._grid), C.byref(nbytes)))
+        _check(self._L.em_workspace_bytes(C.byref(self._grid), C.byref(nbytes)), self._L)
         self.workspace_bytes = int(nbytes.value)
         with torch.cuda.device(self.device):
             self._ws = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
@@ -235,7 +236,7 @@ class EM:
         with torch.cuda.device(self.device):
             _check(self._L.em_create(C.byref(self._grid), mat.ctypes.data_as(C.c_void_p), tab, len(tab),
                                      C.c_double(float(p.dt)), C.c_void_p(self._ws_ptr), self.workspace_bytes,
-                                     C.c_void_p(self._stream.cuda_stream), C.byref(self._h)))
+                                     C.c_void_p(self._stream.cuda_stream), C.byref(self._h)), self._L)
         if load_sources and n_ports > 0:
             self.em_set_source(p)
         if load_init and getattr(p, "init", None):
@@ -277,28 +278,28 @@ class EM:
             edges[e].comp = int(ec[e]); edges[e].i = int(ei[e, 0]); edges[e].j = int(ei[e, 1]); edges[e].k = int(ei[e, 2])
             edges[e].weight = float(ew[e])
         wave = np.ascontiguousarray(p.wave, np.float64)
-        _check(self._L.em_set_source(self._h, n_ports, ports, edges, ne, _dp(wave), int(wave.shape[0])))
+        _check(self._L.em_set_source(self._h, n_ports, ports, edges, ne, _dp(wave), int(wave.shape[0])), self._L)
 
     def em_set_field(self, comp: int, arr):
         torch = self._torch
         if isinstance(arr, torch.Tensor):
             t = arr.to(device=self.device, dtype=self.dtype).contiguous()
             assert tuple(t.shape) == self.shapes[comp]
-            _check(self._L.em_set_field(self._h, comp, C.c_void_p(t.data_ptr()), 1))
+            _check(self._L.em_set_field(self._h, comp, C.c_void_p(t.data_ptr()), 1), self._L)
             self._torch.cuda.current_stream(self.device).synchronize()
         else:
             a = np.ascontiguousarray(arr, self.np_dtype)
             assert a.shape == self.shapes[comp], (a.shape, self.shapes[comp])
-            _check(self._L.em_set_field(self._h, comp, a.ctypes.data_as(C.c_void_p), 0))
+            _check(self._L.em_set_field(self._h, comp, a.ctypes.data_as(C.c_void_p), 0), self._L)
 
     def em_get_field(self, comp: int, out=None, device: bool = False):
         """host ndarray by default; device=True returns a torch tensor on the GPU"""
         if device:
             t = out if out is not None else self._torch.empty(self.shapes[comp], dtype=self.dtype, device=self.device)
-            _check(self._L.em_get_field(self._h, comp, C.c_void_p(t.data_ptr()), 1))
+            _check(self._L.em_get_field(self._h, comp, C.c_void_p(t.data_ptr()), 1), self._L)
             return t
         a = out if out is not None else np.empty(self.shapes[comp], self.np_dtype)
-        _check(self._L.em_get_field(self._h, comp, a.ctypes.data_as(C.c_void_p), 0))
+        _check(self._L.em_get_field(self._h, comp, a.ctypes.data_as(C.c_void_p), 0), self._L)
         return a
 
     def fields(self):
@@ -310,34 +311,34 @@ class EM:
         """device tensor [sy][sx] holding plane k of component comp"""
         sh = self.shapes[comp][1:]
         t = out if out is not None else self._torch.empty(sh, dtype=self.dtype, device=self.device)
-        _check(self._L.em_get_plane(self._h, comp, int(k), C.c_void_p(t.data_ptr()), 1))
+        _check(self._L.em_get_plane(self._h, comp, int(k), C.c_void_p(t.data_ptr()), 1), self._L)
         return t
 
     def em_set_plane(self, comp: int, k: int, t):
         assert tuple(t.shape) == tuple(self.shapes[comp][1:]) and t.dtype == self.dtype and t.is_contiguous()
-        _check(self._L.em_set_plane(self._h, comp, int(k), C.c_void_p(t.data_ptr()), 1 if t.is_cuda else 0))
+        _check(self._L.em_set_plane(self._h, comp, int(k), C.c_void_p(t.data_ptr()), 1 if t.is_cuda else 0), self._L)
 
     # z-slab halo (include/em.h): packed [Ex | Ey (| theta)] of one node plane (and the cell layer behind it)
     @property
     def halo_elems(self) -> int:
         n = C.c_int64()
-        _check(self._L.em_halo_elems(self._h, C.byref(n)))
+        _check(self._L.em_halo_elems(self._h, C.byref(n)), self._L)
         return int(n.value)
 
     def em_get_halo(self, k_plane: int, k_layer: int, out, stream=None):
         assert out.is_cuda and out.dtype == self.dtype and out.is_contiguous() and out.numel() >= self.halo_elems
         _check(self._L.em_get_halo(self._h, int(k_plane), int(k_layer), C.c_void_p(out.data_ptr()),
-                                   C.c_void_p(stream.cuda_stream) if stream is not None else None))
+                                   C.c_void_p(stream.cuda_stream) if stream is not None else None), self._L)
         return out
 
     def em_set_halo(self, k_plane: int, k_layer: int, src, stream=None):
         assert src.is_cuda and src.dtype == self.dtype and src.is_contiguous() and src.numel() >= self.halo_elems
         _check(self._L.em_set_halo(self._h, int(k_plane), int(k_layer), C.c_void_p(src.data_ptr()),
-                                   C.c_void_p(stream.cuda_stream) if stream is not None else None))
+                                   C.c_void_p(stream.cuda_stream) if stream is not None else None), self._L)
 
     def em_joule_layers(self, k0: int, k1: int) -> float:
         tot = C.c_double()
-        _check(self._L.em_joule_layers(self._h, int(k0), int(k1), C.byref(tot)))
+        _check(self._L.em_joule_layers(self._h, int(k0), int(k1), C.byref(tot)), self._L)
         return tot.value
 
     def new_halo_buffer(self):
@@ -349,7 +350,7 @@ class EM:
 
     def em_wall_offset(self, side: int, parity: int, comp: int) -> int:
         off = C.c_size_t()
-        _check(self._L.em_wall_offset(self._h, int(side), int(parity), int(comp), C.byref(off)))
+        _check(self._L.em_wall_offset(self._h, int(side), int(parity), int(comp), C.byref(off)), self._L)
         return int(off.value)
 
     def wall_offsets(self, side: int):
@@ -359,10 +360,10 @@ class EM:
     def em_set_peer_halo(self, side: int, k_send: int, addresses):
         """addresses: four device addresses [parity * 2 + comp] valid in this process, or None to switch the side off"""
         if addresses is None:
-            _check(self._L.em_set_peer_halo(self._h, int(side), 0, None))
+            _check(self._L.em_set_peer_halo(self._h, int(side), 0, None), self._L)
             return
         arr = (C.c_void_p * 4)(*[C.c_void_p(int(a)) for a in addresses])
-        _check(self._L.em_set_peer_halo(self._h, int(side), int(k_send), arr))
+        _check(self._L.em_set_peer_halo(self._h, int(side), int(k_send), arr), self._L)
 
     # thermal coupling (PAPER.md eq. (4)-(6)); the context must come from a problem with p.thermal set
     def em_set_thermal(self, thermal):
@@ -370,29 +371,29 @@ class EM:
         arr = (em_thermal_material * t.shape[0])()
         for m in range(t.shape[0]):
             arr[m].rho_cp, arr[m].k, arr[m].alpha = float(t[m, 0]), float(t[m, 1]), float(t[m, 2])
-        _check(self._L.em_set_thermal(self._h, arr, int(t.shape[0])))
+        _check(self._L.em_set_thermal(self._h, arr, int(t.shape[0])), self._L)
 
     def em_get_temperature_rise(self, out=None, device: bool = False):
         shape = (self.nz, self.ny, self.nx)
         if device:
             t = out if out is not None else self._torch.empty(shape, dtype=self.dtype, device=self.device)
-            _check(self._L.em_get_temperature_rise(self._h, C.c_void_p(t.data_ptr()), 1))
+            _check(self._L.em_get_temperature_rise(self._h, C.c_void_p(t.data_ptr()), 1), self._L)
             return t
         a = out if out is not None else np.empty(shape, self.np_dtype)
-        _check(self._L.em_get_temperature_rise(self._h, a.ctypes.data_as(C.c_void_p), 0))
+        _check(self._L.em_get_temperature_rise(self._h, a.ctypes.data_as(C.c_void_p), 0), self._L)
         return a
 
     def em_set_temperature_rise(self, theta):
         if self._torch.is_tensor(theta):
             t = theta.to(device=self.device, dtype=self.dtype).contiguous()
-            _check(self._L.em_set_temperature_rise(self._h, C.c_void_p(t.data_ptr()), 1))
+            _check(self._L.em_set_temperature_rise(self._h, C.c_void_p(t.data_ptr()), 1), self._L)
             return
         a = np.ascontiguousarray(theta, self.np_dtype)
         assert a.shape == (self.nz, self.ny, self.nx)
-        _check(self._L.em_set_temperature_rise(self._h, a.ctypes.data_as(C.c_void_p), 0))
+        _check(self._L.em_set_temperature_rise(self._h, a.ctypes.data_as(C.c_void_p), 0), self._L)
 
     def em_step(self, n: int = 1):
-        _check(self._L.em_step(self._h, int(n)))
+        _check(self._L.em_step(self._h, int(n)), self._L)
 
     def em_joule(self, power=None, energy=None, total: bool = False, reset: bool = False):
         """power / energy: torch device tensors (nz, ny, nx) of the working dtype, or None."""
@@ -400,7 +401,7 @@ class EM:
         _check(self._L.em_joule(self._h,
                                 C.c_void_p(power.data_ptr()) if power is not None else None,
                                 C.c_void_p(energy.data_ptr()) if energy is not None else None,
-                                C.byref(tot) if total else None, int(reset)))
+                                C.byref(tot) if total else None, int(reset)), self._L)
         return tot.value if total else None
 
     def joule_maps(self, reset: bool = False):
@@ -417,28 +418,28 @@ class EM:
         for n, (c, i, j, k) in enumerate(pts):
             arr[n].comp, arr[n].i, arr[n].j, arr[n].k = int(c), int(i), int(j), int(k)
         out = np.empty(len(pts), np.float64)
-        _check(self._L.em_probe(self._h, len(pts), arr, _dp(out)))
+        _check(self._L.em_probe(self._h, len(pts), arr, _dp(out)), self._L)
         return out
 
     def em_reset(self):
-        _check(self._L.em_reset(self._h))
+        _check(self._L.em_reset(self._h), self._L)
 
     @property
     def step_index(self) -> int:
         n = C.c_int64()
-        _check(self._L.em_step_index(self._h, C.byref(n)))
+        _check(self._L.em_step_index(self._h, C.byref(n)), self._L)
         return int(n.value)
 
     @property
     def launch_count(self) -> int:
         n = C.c_int64()
-        _check(self._L.em_launch_count(self._h, C.byref(n)))
+        _check(self._L.em_launch_count(self._h, C.byref(n)), self._L)
         return int(n.value)
 
     def em_timing_enable(self, enable: bool = True):
-        _check(self._L.em_timing_enable(self._h, int(enable)))
+        _check(self._L.em_timing_enable(self._h, int(enable)), self._L)
 
     def em_timing_read(self):
         name = C.c_char_p(); n = C.c_int64(); ms = C.c_double()
-        _check(self._L.em_timing_read(self._h, C.byref(name), C.byref(n), C.byref(ms)))
+        _check(self._L.em_timing_read(self._h, C.byref(name), C.byref(n), C.byref(ms)), self._L)
         return (name.value or b"").decode(), int(n.value), float(ms.value)

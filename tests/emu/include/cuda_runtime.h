@@ -1,0 +1,3 @@
+// tests/emu: stands in for the CUDA runtime header in the emulated TEST build (emu_cuda.h)
+#pragma once
+#include "../emu_cuda.h"
