@@ -21,7 +21,7 @@ def _stale(lib: str) -> bool:
         return True
     t = os.path.getmtime(lib)
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    deps += [os.path.join(HERE, f) for f in os.listdir(HERE) if f.endswith((".h", ".cpp", ".py"))]
+    deps += [os.path.join(HERE, f) for f in ("emu_cuda.h", "em_ptx_emu.h", "emu_exports.cpp", "build_emu.py")]
     deps += [os.path.join(ROOT, "include", "em.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 

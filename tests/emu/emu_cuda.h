@@ -17,6 +17,7 @@
 #pragma once
 
 #include <atomic>
+#include <condition_variable>
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
@@ -83,7 +84,10 @@ struct WarpState { uint64_t buf[2][32]; uint32_t gen = 0; int arrived = 0, alive
 struct BarState { uint32_t gen = 0; int arrived = 0; };
 struct AsyncOp { int delay; std::function<void()> fire; };
 
+struct Region { uintptr_t lo, hi; };
+
 struct Cta {
+    const std::vector<Region> *regions = nullptr;       // emu_alloc'ed global memory at launch time
     dim3 bidx, bdim, gdim;
     int nthreads = 0, alive = 0;
     unsigned char *smem = nullptr;
@@ -168,14 +172,13 @@ inline void cta_barrier_arrive(Cta *c, BarState &B, int expected, bool wait, con
 }
 
 // ---- global-memory registry (emu_alloc: guard pages on both sides) ----------------------------------------------
-struct Region { uintptr_t lo, hi; };
 inline std::vector<Region> &regions() { static std::vector<Region> r; return r; }
 inline std::mutex &regions_mutex() { static std::mutex m; return m; }
-inline bool in_registered(const void *p, size_t n) {
-    std::lock_guard<std::mutex> lk(regions_mutex());
-    if (regions().empty()) return true;                     // nothing registered: no range check
+inline bool in_registered(const void *p, size_t n) {       // against the snapshot taken when the kernel was launched
+    const std::vector<Region> &rs = *t_cur->cta->regions;
+    if (rs.empty()) return true;                            // nothing registered: no range check
     const uintptr_t a = (uintptr_t)p;
-    for (const Region &r : regions()) if (a >= r.lo && a + n <= r.hi) return true;
+    for (const Region &r : rs) if (a >= r.lo && a + n <= r.hi) return true;
     return false;
 }
 inline void check_global(const void *p, size_t n, size_t align, const char *what) {
@@ -291,6 +294,72 @@ inline std::map<const void *, size_t> &func_smem() { static std::map<const void 
 constexpr size_t kSmemOptin = 232448;                       // 227 KB: sm_100 per-block opt-in limit
 constexpr size_t kSmemDefault = 48 * 1024;
 
+// fiber stacks and the shared-memory buffer of a worker, reused across launches (fresh mappings would be page-faulted in
+// again on every launch)
+struct Arena { char *stacks = nullptr; size_t stack_bytes = 0; unsigned char *smem_raw = nullptr; size_t smem_alloc = 0; };
+inline std::vector<Arena> &arena_pool() { static std::vector<Arena> p; return p; }
+inline std::mutex &arena_mutex() { static std::mutex m; return m; }
+inline Arena acquire_arena(size_t stack_bytes, size_t smem_alloc) {
+    Arena a;
+    {
+        std::lock_guard<std::mutex> lk(arena_mutex());
+        auto &p = arena_pool();
+        for (size_t q = 0; q < p.size(); ++q)
+            if (p[q].stack_bytes >= stack_bytes && p[q].smem_alloc >= smem_alloc) { a = p[q]; p.erase(p.begin() + q); return a; }
+        if (!p.empty()) { a = p.back(); p.pop_back(); }
+    }
+    if (a.stack_bytes < stack_bytes) {
+        if (a.stacks) munmap(a.stacks, a.stack_bytes);
+        void *m = mmap(nullptr, stack_bytes, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS | MAP_NORESERVE, -1, 0);
+        a.stacks = m == MAP_FAILED ? nullptr : static_cast<char *>(m); a.stack_bytes = stack_bytes;
+    }
+    if (a.smem_alloc < smem_alloc) {
+        free(a.smem_raw);
+        a.smem_raw = static_cast<unsigned char *>(malloc(smem_alloc)); a.smem_alloc = smem_alloc;
+    }
+    return a;
+}
+inline void release_arena(const Arena &a) { std::lock_guard<std::mutex> lk(arena_mutex()); arena_pool().push_back(a); }
+
+// persistent worker threads (a fresh std::thread per launch costs a stack mapping and a malloc arena every time)
+struct WorkerPool {
+    std::mutex m;
+    std::condition_variable cv_job, cv_done;
+    std::vector<std::thread> threads;
+    const std::function<void()> *job = nullptr;
+    long generation = 0;
+    int wanted = 0, started = 0, running = 0;
+    void loop() {
+        long seen = 0;
+        for (;;) {
+            const std::function<void()> *j = nullptr;
+            {
+                std::unique_lock<std::mutex> lk(m);
+                cv_job.wait(lk, [&] { return generation != seen && started < wanted; });
+                if (generation != seen && started < wanted) { started += 1; j = job; }
+                seen = generation;
+            }
+            if (j) {
+                (*j)();
+                std::lock_guard<std::mutex> lk(m);
+                if (--running == 0) cv_done.notify_all();
+            }
+        }
+    }
+    // runs `fn` on n pool threads at once and returns when all n calls have returned; one launch at a time
+    void run(int n, const std::function<void()> &fn) {
+        static std::mutex one_launch;
+        std::lock_guard<std::mutex> serial(one_launch);
+        std::unique_lock<std::mutex> lk(m);
+        while ((int)threads.size() < n) { threads.emplace_back([this] { loop(); }); threads.back().detach(); }
+        job = &fn; wanted = n; started = 0; running = n; generation += 1;
+        cv_job.notify_all();
+        cv_done.wait(lk, [&] { return running == 0; });
+        job = nullptr; wanted = 0;
+    }
+};
+inline WorkerPool &worker_pool() { static WorkerPool *p = new WorkerPool(); return *p; }     // never destroyed
+
 // the grid: CTAs are handed out in blockIdx order (x fastest) to EMU_THREADS workers
 inline int launch(dim3 grid, dim3 block, size_t smem_bytes, const void *func, const char *name, const std::function<void()> &body) {
     const int nthreads = (int)(block.x * block.y * block.z);
@@ -314,13 +383,15 @@ inline int launch(dim3 grid, dim3 block, size_t smem_bytes, const void *func, co
     n_workers = (int)std::max<size_t>(1, std::min<size_t>((size_t)std::max(n_workers, 1), n_cta));
     std::atomic<size_t> next{0};
     std::atomic<bool> failed{false};
+    std::vector<Region> regions_now;
+    { std::lock_guard<std::mutex> lk(regions_mutex()); regions_now = regions(); }
     auto worker = [&]() {
         const size_t stack_bytes = (size_t)nthreads * kStackBytes;
-        char *stacks = static_cast<char *>(mmap(nullptr, stack_bytes, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS | MAP_NORESERVE, -1, 0));
-        const size_t canary = 1024, smem_alloc = (smem_bytes + canary + 1023) / 1024 * 1024 + 1024;
-        unsigned char *smem_raw = static_cast<unsigned char *>(malloc(smem_alloc + 1024));
-        unsigned char *smem = reinterpret_cast<unsigned char *>(((uintptr_t)smem_raw + 1023) / 1024 * 1024);
-        if (stacks == MAP_FAILED || !smem_raw) { failed = true; return; }
+        const size_t canary = 1024, smem_alloc = (smem_bytes + canary + 1023) / 1024 * 1024 + 2048;
+        Arena ar = acquire_arena(stack_bytes, smem_alloc);
+        char *stacks = ar.stacks;
+        if (!stacks || !ar.smem_raw) { failed = true; return; }
+        unsigned char *smem = reinterpret_cast<unsigned char *>(((uintptr_t)ar.smem_raw + 1023) / 1024 * 1024);
         for (;;) {
             const size_t b = next.fetch_add(1);
             if (b >= n_cta || failed.load()) break;
@@ -338,7 +409,7 @@ inline int launch(dim3 grid, dim3 block, size_t smem_bytes, const void *func, co
                 f.tidx = uint3{(unsigned)(t % block.x), (unsigned)((t / block.x) % block.y), (unsigned)(t / (block.x * block.y))};
             }
             if (nthreads % 32) c.warps.back().alive = nthreads % 32;
-            c.body = &body; c.kernel_name = name;
+            c.body = &body; c.kernel_name = name; c.regions = &regions_now;
             c.random = seed != 0;
             c.rng = (uint64_t)seed * 0x2545f4914f6cdd1dull + (uint64_t)launch_no * 1315423911ull + b * 2654435761ull;
             run_cta(c, stacks);
@@ -360,15 +431,10 @@ inline int launch(dim3 grid, dim3 block, size_t smem_bytes, const void *func, co
                 failed = true;
             }
         }
-        munmap(stacks, stack_bytes);
-        free(smem_raw);
+        release_arena(ar);
     };
     if (n_workers == 1) worker();
-    else {
-        std::vector<std::thread> th;
-        for (int w = 0; w < n_workers; ++w) th.emplace_back(worker);
-        for (auto &t : th) t.join();
-    }
+    else worker_pool().run(n_workers, worker);
     return failed.load() ? 1 : 0;
 }
 

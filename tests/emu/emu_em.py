@@ -81,6 +81,16 @@ class EmuEM(B.EM):
     def _check(self, rc):
         B._check(rc, self._L)
 
+    # the z-slab halo calls: as in binding.EM, the packed message lives in host memory here
+    def em_get_halo(self, k_plane: int, k_layer: int, out, stream=None):
+        assert out.dtype == self.dtype and out.is_contiguous() and out.numel() >= self.halo_elems
+        B._check(self._L.em_get_halo(self._h, int(k_plane), int(k_layer), C.c_void_p(out.data_ptr()), None), self._L)
+        return out
+
+    def em_set_halo(self, k_plane: int, k_layer: int, src, stream=None):
+        assert src.dtype == self.dtype and src.is_contiguous() and src.numel() >= self.halo_elems
+        B._check(self._L.em_set_halo(self._h, int(k_plane), int(k_layer), C.c_void_p(src.data_ptr()), None), self._L)
+
     def close(self):
         if getattr(self, "_h", None) and self._h.value:
             self._L.em_destroy(self._h)

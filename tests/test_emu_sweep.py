@@ -1,0 +1,224 @@
+"""The product's CUDA sources under CPU emulation (tests/emu) -- memcheck / synccheck / racecheck stand-in, NO GPU needed.
+
+compute-sanitizer is closed on this GPU pool (profiles/r2_sanitizer.md) and, for most of round 2, so was the pool.  These
+tests compile paper_2603_07038_b200/csrc/em_lib.cu and its headers, UNMODIFIED, with g++ against an emulation of the CUDA
+primitives they use (tests/emu/emu_cuda.h: one fiber per CUDA thread; mbarrier, named-barrier, shuffle and vote
+semantics of the PTX ISA; asynchronous TMA / bulk / cp.async copies that complete late and in random order; deadlock
+detection; range and alignment checks on every address handed to a copy engine; poisoned shared memory with a canary;
+guard pages round the workspace) and then run the SAME parity cases as the `-m gpu` suite -- the test functions of
+tests/test_gpu_parity.py, test_gpu_thermal.py and test_gpu_eonly.py are called as they are, with the binding's EM class
+swapped for tests/emu/emu_em.EmuEM -- element by element against the oracle.  tests/test_emu_selftest.py shows that
+the emulation reports the bugs it is there to catch.
+
+What a green run means: index arithmetic, shared-memory layout, barrier protocol (no CTA barrier in the plane loop),
+staging ring reuse, chunk seams, PMC warm-up plane, source cursor and the coupled / E-only / fused-conduction variants
+are correct on these grids for every thread schedule tried.  What it does not mean: anything about PTX encodings,
+hardware timing or performance -- the C-ABI product has no CPU path and libem.so is never involved here."""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+sys.path.insert(0, os.path.join(os.path.dirname(os.path.abspath(__file__)), "emu"))
+
+import workloads as W
+from workloads.problem import LOSS_CD, LOSS_EXP
+import paper_2603_07038_b200 as P
+from oracle import emo
+from parity import TOL, compare_state, rel_l2
+import emu_em
+
+import test_gpu_parity as TP
+import test_gpu_thermal as TT
+import test_gpu_eonly as TE
+import test_gpu_slabs as TS
+import paper_2603_07038_b200.binding as PB
+
+FC = dict(tag="fc", defines=["-DEM_SWEEP_FUSED_CONDUCTION=1"])      # the coupled sweep with the conduction stencil fused in
+
+
+def _factory(**fixed):
+    def make(p, precision=None, kernel=P.EM_KERNEL_AUTO, device=None, stream=None, lib=None, **kw):
+        kw.update(fixed)
+        return emu_em.EmuEM(p, precision=precision, kernel=kernel, **kw)
+    return make
+
+
+@pytest.fixture
+def emulated(monkeypatch):
+    """P.EM -> EmuEM for the duration of a test; returns a function that switches the library variant"""
+    monkeypatch.setenv("EMU_SEED", "0")
+    monkeypatch.setattr(P, "EM", _factory())
+    monkeypatch.setattr(PB, "EM", _factory())           # (slabs.make_ranks_inprocess takes it from the binding module)
+
+    def variant(**fixed):
+        monkeypatch.setattr(P, "EM", _factory(**fixed))
+        monkeypatch.setattr(PB, "EM", _factory(**fixed))
+    return variant
+
+
+# ------------------------------------------------------------------------------------------- leapfrog sweep + split
+@pytest.mark.parametrize("kernel", [P.EM_KERNEL_SPLIT, P.EM_KERNEL_TMA], ids=["split", "tma"])
+@pytest.mark.parametrize("precision", [64, 32])
+def test_impulse_example(emulated, kernel, precision):
+    TP.test_impulse_example(kernel, precision)
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("dims", TP.SMALL)
+def test_random_grids_cd(emulated, dims, precision):
+    TP.test_random_grids_cd(dims, precision, P.EM_KERNEL_TMA)
+
+
+def test_random_grids_cd_split(emulated):
+    TP.test_random_grids_cd((37, 29, 23), 64, P.EM_KERNEL_SPLIT)
+
+
+@pytest.mark.parametrize("zsplit", [1, 2, 3, 5, 8])
+@pytest.mark.parametrize("bc", [(0,) * 6, (0, 0, 1, 0, 1, 1)])
+def test_z_chunks(emulated, zsplit, bc):
+    TP.test_tma_sweep_z_chunks(zsplit, bc)
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("dims", [(37, 29, 23), (9, 4, 70)])
+def test_random_grids_exp(emulated, dims, precision):
+    TP.test_random_grids_exp(dims, precision, P.EM_KERNEL_TMA)
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("bc", TP.PMC_BC)
+@pytest.mark.parametrize("dims", [(37, 29, 23), (130, 3, 2), (5, 9, 2), (33, 65, 4)])
+def test_random_grids_pmc_walls(emulated, dims, bc, precision):
+    TP.test_random_grids_pmc_walls(dims, bc, precision, P.EM_KERNEL_TMA)
+
+
+def test_pmc_exp_loss_and_z_chunks(emulated):
+    TP.test_pmc_exp_loss_and_z_chunks(P.EM_KERNEL_TMA)
+
+
+def test_percell_ids_pec_material_overlapping_ports(emulated):
+    TP.test_random_grid_percell_ids_and_pec_material(P.EM_KERNEL_TMA)
+    TP.test_overlapping_ports_add(P.EM_KERNEL_TMA)
+
+
+def test_api_contract_and_probe(emulated):
+    TP.test_probe_matches_fields()
+
+
+def test_package_slice_several_tiles_and_chunks(emulated):
+    """config 4 at 1/8 of the x, y and 1/4 of the z cell counts: 128 x 128 x 48 cells = 2 x 10 tiles, sources, fp32"""
+    p = W.make_config(4, scale=8, zscale=4, steps=12)
+    TP.run_pair(p, 12, 32, P.EM_KERNEL_TMA, checkpoints=(3,), z_chunks=3)
+
+
+# -------------------------------------------------------------------------------------------- E-only (eq. (2)) sweep
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("dims", [(37, 29, 23), (130, 3, 2), (1, 1, 1), (33, 65, 4)])
+def test_eonly_random_grids_cd(emulated, dims, precision):
+    TE.test_random_grids_cd(dims, precision)
+
+
+def test_eonly_exp_pmc_chunks(emulated):
+    TE.test_random_grids_exp((37, 29, 23), 64)
+    TE.test_random_grids_pmc_walls((37, 29, 23), (1, 0, 0, 1, 0, 1), 64)
+    TE.test_random_grids_pmc_walls((33, 65, 4), (1, 1, 1, 1, 1, 1), 32)
+    TE.test_z_chunks_and_many_ports(3)
+    TE.test_percell_ids_pec_material_and_uniform_mu()
+
+
+def test_eonly_equals_the_leapfrog_kernel(emulated):
+    TE.test_equals_the_leapfrog_kernel()
+
+
+# --------------------------------------------------- coupled sweep (eq. (4)-(6)): conduction kernel + sweep, and fused
+VARIANTS = [pytest.param({}, id="k_diffuse+sweep"), pytest.param(FC, id="fused-conduction")]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("dims,mode", TT.CASES)
+def test_coupled_random_grids(emulated, dims, mode, precision, variant):
+    emulated(**variant)
+    TT.test_coupled_random_grids(dims, mode, precision, P.EM_KERNEL_AUTO)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_coupled_pmc_walls_chunks_diffusion(emulated, variant):
+    emulated(**variant)
+    TT.test_coupled_with_pmc_walls_and_wall_port(P.EM_KERNEL_AUTO)
+    for zsplit in (1, 3, 8):
+        TT.test_coupled_sweep_z_chunks(zsplit)
+    TT.test_pure_diffusion_and_set_get_temperature()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_coupled_package_slice(emulated, variant):
+    """the package layout (64 x 64 x 48 cells) with the handbook-order thermal table as it stands, fp32"""
+    emulated(**variant)
+    p = W.make_config(4, scale=16, zscale=4, steps=16)
+    p.thermal = W.thermal_table()
+    TT._run(p, 16, 32)
+
+
+def test_coupled_split_kernels(emulated):
+    TT.test_coupled_random_grids((37, 29, 23), LOSS_CD, 64, P.EM_KERNEL_SPLIT)
+
+
+# ------------------------------------------------------------------ z slabs: pack / unpack kernels and fused peer stores
+@pytest.mark.parametrize("n_ranks", [2, 3])
+@pytest.mark.parametrize("mode", ["p2p", "peer"])
+@pytest.mark.parametrize("precision", [64, 32])
+def test_slabs_equal_single_domain(emulated, n_ranks, mode, precision):
+    """peer mode: the sweep of one slab context stores E'x, E'y straight into the wall plane of the neighbouring
+    context's workspace (em_set_peer_halo) -- under the emulation's range checks"""
+    TS.test_slabs_equal_single_domain(n_ranks, P.EM_KERNEL_TMA, mode, precision)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_thermally_coupled_slabs(emulated, variant):
+    emulated(**variant)
+    TS.test_thermally_coupled_slabs(P.EM_KERNEL_AUTO, 64)
+
+
+def test_peer_halo_argument_errors(emulated):
+    TS.test_peer_halo_argument_errors()
+
+
+# ---------------------------------------------------------------------------- schedules: every one gives the same bits
+def _state(g, thermal):
+    out = [g.em_get_field(c) for c in ((0, 1, 2, 3, 4, 5) if g.formulation == P.EM_FORM_LEAPFROG else (0, 1, 2, 6, 7, 8))]
+    out.append(g.joule_maps()[1])
+    if thermal:
+        out.append(g.em_get_temperature_rise())
+    return out
+
+
+SCHEDULE_CASES = [pytest.param(dict(), False, id="leapfrog"), pytest.param(dict(formulation=P.EM_FORM_EONLY), False, id="e-only"),
+                  pytest.param(dict(), True, id="coupled"), pytest.param(dict(FC), True, id="coupled-fused-conduction")]
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("kw,thermal", SCHEDULE_CASES)
+def test_random_schedules_do_not_change_a_bit(monkeypatch, kw, thermal, precision):
+    """The counterpart of tests/test_gpu_fuzz.py: with EMU_SEED != 0 the fibers run in a random order, whole warps lose
+    turns, every synchronisation point may yield and the asynchronous copies complete after random delays and in
+    random order.  3 x 4 tiles (fp32) / 5 x 5 (fp64), 3 z chunks, PMC wall at -z (warm-up plane), 40 ports."""
+    p = W.random_problem(250, 45, 17, seed=4242, steps=6, n_ports=40, bc=(0, 0, 0, 0, 1, 0), init_scale=4.0e6 if thermal else 1.0)
+    if thermal:
+        th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
+        p.thermal = th
+    ref = None
+    for seed in (0, 1, 2, 3):
+        monkeypatch.setenv("EMU_SEED", str(seed))
+        g = emu_em.EmuEM(p, precision=precision, z_chunks=3, **kw)
+        g.em_step(6)
+        out = _state(g, thermal)
+        g.close()
+        if ref is None:
+            ref = out
+            assert all(np.isfinite(a).all() for a in out) and np.abs(out[0]).max() > 0
+        else:
+            for a, b in zip(out, ref):
+                assert np.array_equal(a, b), seed
