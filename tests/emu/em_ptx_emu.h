@@ -53,22 +53,29 @@ inline MBar *mbar_at(unsigned bar, const char *what, bool must_be_init = true) {
     if (must_be_init && !emu::t_cur->cta->mbar_init.count(bar)) emu::fail_here(std::string(what) + ": mbarrier was never initialised");
     return b;
 }
-inline void mbar_complete_if_done(MBar *b) {
+inline emu::SyncClock &mbar_clock(emu::Cta *c, const MBar *b) {
+    return c->mbar_init[(unsigned)(reinterpret_cast<const unsigned char *>(b) - c->smem) + emu::kSmemBase];
+}
+inline void mbar_complete_if_done(emu::Cta *c, MBar *b) {
     const uint32_t pending = (b->state >> 1) & 0x7fffu, expected = (b->state >> 16) & 0x7fffu;
-    if (pending == 0 && b->tx == 0) b->state = (expected << 16) | (expected << 1) | ((b->state & 1u) ^ 1u);
+    if (pending == 0 && b->tx == 0) {
+        b->state = (expected << 16) | (expected << 1) | ((b->state & 1u) ^ 1u);
+        emu::race_complete(c, mbar_clock(c, b));
+    }
 }
 inline void mbar_init(unsigned bar, unsigned count) {
     MBar *b = mbar_at(bar, "mbarrier.init", false);
     if (count < 1 || count > 0x7fffu) emu::fail_here("mbarrier.init: bad count");
     b->state = (count << 16) | (count << 1); b->tx = 0;
-    emu::t_cur->cta->mbar_init[bar] = true;
+    emu::t_cur->cta->mbar_init[bar] = emu::SyncClock();
 }
 inline void mbar_fence_init() {}
 inline void mbar_arrive_n(MBar *b, const char *what) {
     const uint32_t pending = (b->state >> 1) & 0x7fffu;
     if (pending == 0) emu::fail_here(std::string(what) + ": more arrivals than the barrier expects in this phase");
+    emu::race_release(mbar_clock(emu::t_cur->cta, b));
     b->state -= 2u;
-    mbar_complete_if_done(b);
+    mbar_complete_if_done(emu::t_cur->cta, b);
 }
 inline void mbar_arrive(unsigned bar) { emu::sync_point(); mbar_arrive_n(mbar_at(bar, "mbarrier.arrive"), "mbarrier.arrive"); }
 inline void mbar_expect_tx(unsigned bar, unsigned bytes) {
@@ -79,6 +86,7 @@ inline void mbar_expect_tx(unsigned bar, unsigned bytes) {
 inline void mbar_wait(unsigned bar, unsigned parity) {
     MBar *b = mbar_at(bar, "mbarrier.try_wait");
     emu::block_while(&b->state, 1u, parity & 1u, "mbarrier.try_wait.parity, smem offset", (long)(bar - emu::kSmemBase));
+    emu::race_acquire(mbar_clock(emu::t_cur->cta, b));
     emu::sync_point();
 }
 
@@ -99,10 +107,10 @@ inline void pair_sync(int id) {
 // ---- bulk / tensor copies: queued, completed by the scheduler after a delay --------------------------------------------
 template <int POL> inline unsigned long long l2_policy() { return 0; }
 inline int async_delay(emu::Cta *c) { return c->random ? (int)(emu::next_rand(c->rng) % 7) : 1; }
-inline void async_complete_tx(emu::Cta *c, MBar *b, unsigned bytes, const char *what) {
+inline void async_complete_tx(emu::Cta *c, MBar *b, unsigned bytes, const std::shared_ptr<emu::RaceAsync> &ra) {
+    emu::race_async_complete(c, mbar_clock(c, b), ra);
     b->tx -= (int32_t)bytes;
-    mbar_complete_if_done(b);
-    (void)c; (void)what;
+    mbar_complete_if_done(c, b);
 }
 inline void bulk_load(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
     emu::Cta *c = emu::t_cur->cta;
@@ -110,7 +118,13 @@ inline void bulk_load(unsigned dst, const void *src, unsigned bytes, unsigned ba
     unsigned char *d = emu::u32_to_smem(dst, bytes, 16, "cp.async.bulk (destination)");
     emu::check_global(src, bytes, 16, "cp.async.bulk (source)");
     MBar *b = mbar_at(bar, "cp.async.bulk (mbarrier)");
-    c->async.push_back(emu::AsyncOp{async_delay(c), [=]() { memcpy(d, src, bytes); async_complete_tx(c, b, bytes, "cp.async.bulk"); }});
+    const std::shared_ptr<emu::RaceAsync> ra = emu::race_async_issue();
+    const void *pc = __builtin_return_address(0);
+    c->async.push_back(emu::AsyncOp{async_delay(c), [=]() {
+        memcpy(d, src, bytes);
+        emu::race_async_write(c, ra, d, bytes, pc);
+        async_complete_tx(c, b, bytes, ra);
+    }});
 }
 template <int POL>
 inline void tma_load_3d(unsigned dst, const CUtensorMap *map, unsigned bar, int x, int y, int z) {
@@ -136,6 +150,8 @@ inline void tma_load_3d(unsigned dst, const CUtensorMap *map, unsigned bar, int 
             emu::check_global(last, m.esz, 1, "cp.async.bulk.tensor (source, last element)");
         }
     }
+    const std::shared_ptr<emu::RaceAsync> ra = emu::race_async_issue();
+    const void *pc = __builtin_return_address(0);
     c->async.push_back(emu::AsyncOp{async_delay(c), [=]() {
         const int co[3] = {x, y, z};
         unsigned char *out = d;
@@ -150,7 +166,8 @@ inline void tma_load_3d(unsigned dst, const CUtensorMap *map, unsigned bar, int 
                     else memset(out, 0, m.esz);
                 }
             }
-        async_complete_tx(c, b, (unsigned)bytes, "cp.async.bulk.tensor");
+        emu::race_async_write(c, ra, d, bytes, pc);
+        async_complete_tx(c, b, (unsigned)bytes, ra);
     }});
 }
 template <int POL> inline void tma_prefetch_3d(const CUtensorMap *map, int, int, int) {

@@ -13,6 +13,12 @@
 //   * dynamic shared memory is poisoned (0xFF = NaN) per CTA, has a canary behind it, and every address handed to an
 //     mbarrier / TMA / cp.async / streaming-store wrapper is checked for range and alignment (a misaligned or
 //     out-of-range address is what faults a GPU); global allocations made through emu_alloc sit between guard pages.
+//   * RACECHECK (EMU_RACECHECK=1 on a build made with -fsanitize=thread, whose load / store hooks __tsan_read* /
+//     __tsan_write* are implemented HERE, emu_exports.cpp, not by libtsan): a happens-before race detector for the dynamic
+//     shared memory.  Every thread and the asynchronous copy engine carry vector clocks; __syncthreads, __syncwarp,
+//     bar.sync / bar.arrive and mbarrier arrive / complete_tx -> try_wait are the only ordering edges (shuffles and votes
+//     are NOT); two accesses to the same 4 bytes by different agents, one of them a write, with no ordering path between
+//     them are reported as a race with both code addresses -- whether or not the schedule at hand made them collide.
 // What it does not emulate: timing, caches, the memory model between CTAs, PTX itself (em_ptx.cuh is replaced as a whole).
 #pragma once
 
@@ -25,6 +31,7 @@
 #include <cstring>
 #include <functional>
 #include <map>
+#include <memory>
 #include <mutex>
 #include <string>
 #include <thread>
@@ -80,9 +87,13 @@ struct Fiber {
     int open_group = 0;
 };
 
-struct WarpState { uint64_t buf[2][32]; uint32_t gen = 0; int arrived = 0, alive = 32; };
-struct BarState { uint32_t gen = 0; int arrived = 0; };
+// racecheck: the clocks of a synchronisation object -- what its arrivals of the running phase have released (pending) and
+// what a thread that saw a phase complete acquires (completed)
+struct SyncClock { std::vector<uint32_t> pending, completed; };
+struct WarpState { uint64_t buf[2][32]; uint32_t gen = 0; int arrived = 0, alive = 32; SyncClock clk; };
+struct BarState { uint32_t gen = 0; int arrived = 0; SyncClock clk; };
 struct AsyncOp { int delay; std::function<void()> fire; };
+struct RaceState;
 
 struct Region { uintptr_t lo, hi; };
 
@@ -96,7 +107,8 @@ struct Cta {
     std::vector<WarpState> warps;
     BarState bars[16];
     std::vector<AsyncOp> async;
-    std::map<unsigned, bool> mbar_init;         // smem offsets of initialised mbarriers
+    std::map<unsigned, SyncClock> mbar_init;    // smem offsets of initialised mbarriers (+ their racecheck clocks)
+    RaceState *race = nullptr;                  // racecheck state (EMU_RACECHECK=1), else null
     const std::function<void()> *body = nullptr;
     void *sched_sp = nullptr;
     uint64_t rng = 0;
@@ -143,6 +155,116 @@ inline void block_while(volatile uint32_t *addr, uint32_t mask, uint32_t val, co
     f->wait_addr = nullptr;
 }
 
+// ---- racecheck ----------------------------------------------------------------------------------------------------------
+// Agents: the CTA's threads 0 .. n-1 and the asynchronous copy engine (index n).  clock[t][u] = the latest epoch of agent u
+// that happens-before agent t's present; an access is stamped (agent, own epoch); a release bumps the own epoch.
+struct RaceState {
+    int n = 0;                                   // agents = threads + 1
+    std::vector<uint32_t> clocks;                // [n][n]
+    struct Shadow {                              // per 4-byte granule of the dynamic shared memory
+        uint32_t w_agent = 0xffffffffu, w_clk = 0;
+        uint32_t r_agent[4], r_clk[4];
+        uint8_t nr = 0;
+        const void *w_pc = nullptr, *r_pc[4];
+    };
+    std::vector<Shadow> shadow;
+    uint32_t agent_epoch = 0;
+    uint32_t *clk(int t) { return clocks.data() + (size_t)t * n; }
+};
+inline void race_join(std::vector<uint32_t> &dst, const uint32_t *src, int n) {
+    if ((int)dst.size() != n) dst.assign(n, 0);
+    for (int q = 0; q < n; ++q) dst[q] = std::max(dst[q], src[q]);
+}
+// the running thread publishes everything it did so far to the object's running phase
+inline void race_release(SyncClock &s) {
+    Fiber *f = t_cur; RaceState *r = f->cta->race;
+    if (!r) return;
+    race_join(s.pending, r->clk(f->tid), r->n);
+    r->clk(f->tid)[f->tid] += 1;
+}
+// a phase of the object completed: what was released into it becomes visible to those who wait for it
+inline void race_complete(Cta *c, SyncClock &s) {
+    RaceState *r = c->race;
+    if (!r || s.pending.empty()) return;
+    race_join(s.completed, s.pending.data(), r->n);
+}
+inline void race_acquire(SyncClock &s) {
+    Fiber *f = t_cur; RaceState *r = f->cta->race;
+    if (!r || s.completed.empty()) return;
+    uint32_t *c = r->clk(f->tid);
+    for (int q = 0; q < r->n; ++q) c[q] = std::max(c[q], s.completed[q]);
+}
+inline std::string race_pc(const void *pc) { char b[32]; snprintf(b, sizeof(b), "%p", pc); return b; }
+inline void race_report(Cta *c, size_t off, const char *what, uint32_t a0, const void *pc0, uint32_t a1, const void *pc1) {
+    if (c->failed) return;
+    RaceState *r = c->race;
+    auto who = [&](uint32_t a) { return (int)a == r->n - 1 ? std::string("the async copy engine") : "thread " + std::to_string(a) + " (warp " + std::to_string(a / 32) + " lane " + std::to_string(a % 32) + ")"; };
+    c->failed = true;
+    c->error = std::string("emu: RACE in kernel ") + c->kernel_name + ", block (" + std::to_string(c->bidx.x) + "," + std::to_string(c->bidx.y) + "," +
+               std::to_string(c->bidx.z) + "), dynamic shared memory offset " + std::to_string(off) + ": " + what + " -- " + who(a0) + " at pc " + race_pc(pc0) +
+               " and " + who(a1) + " at pc " + race_pc(pc1) + " are not ordered by any barrier";
+}
+// one access of `agent` (clock row vc) to [p, p + n): is_write or read; returns false after reporting a race
+inline bool race_check(Cta *c, const uint32_t *vc, uint32_t agent, uint32_t epoch, const unsigned char *p, size_t n, bool is_write, const void *pc) {
+    RaceState *r = c->race;
+    const size_t off0 = (size_t)(p - c->smem);
+    for (size_t g = off0 / 4; g <= (off0 + n - 1) / 4; ++g) {
+        if (c->mbar_init.count((unsigned)(g * 4 / 8 * 8) + 0x10000u)) continue;         // the mbarrier objects themselves
+        RaceState::Shadow &sh = r->shadow[g];
+        const bool engine = (int)agent == r->n - 1;          // two copies of the engine are NOT ordered by being the engine's
+        if (sh.w_agent != 0xffffffffu && (sh.w_agent != agent || engine) && sh.w_clk > vc[sh.w_agent]) {
+            race_report(c, g * 4, is_write ? "write after write" : "read after write", sh.w_agent, sh.w_pc, agent, pc); return false;
+        }
+        if (is_write) {
+            for (int q = 0; q < sh.nr; ++q)
+                if (sh.r_agent[q] != agent && sh.r_clk[q] > vc[sh.r_agent[q]]) {
+                    race_report(c, g * 4, "write after read", sh.r_agent[q], sh.r_pc[q], agent, pc); return false;
+                }
+            sh.w_agent = agent; sh.w_clk = epoch; sh.w_pc = pc; sh.nr = 0;
+        } else {
+            int slot = -1;
+            for (int q = 0; q < sh.nr; ++q)
+                if (sh.r_agent[q] == agent || sh.r_clk[q] <= vc[sh.r_agent[q]]) { slot = q; break; }      // mine, or subsumed by me
+            if (slot < 0) slot = sh.nr < 4 ? sh.nr++ : (int)(epoch & 3);                                    // (full: one reader is forgotten)
+            sh.r_agent[slot] = agent; sh.r_clk[slot] = epoch; sh.r_pc[slot] = pc;
+        }
+    }
+    return true;
+}
+// the load / store hooks of a -fsanitize=thread build land here (emu_exports.cpp)
+inline void race_access(const void *addr, size_t n, bool is_write, const void *pc) {
+    Fiber *f = t_cur;
+    if (!f) return;
+    Cta *c = f->cta;
+    if (!c->race || c->failed) return;
+    const unsigned char *p = static_cast<const unsigned char *>(addr);
+    if (p < c->smem || p + n > c->smem + c->smem_bytes) return;
+    const uint32_t *vc = c->race->clk(f->tid);
+    race_check(c, vc, (uint32_t)f->tid, vc[f->tid], p, n, is_write, pc);
+}
+// An asynchronous copy is ordered after everything its issuer had seen when it issued it (vc: the issuer's clock then,
+// including the latest copy-engine epoch it had learnt of through a barrier) and before whoever waits for the mbarrier
+// it completes on; two copies are ordered only through such a wait.
+struct RaceAsync { std::vector<uint32_t> vc; uint32_t epoch = 0; };
+inline std::shared_ptr<RaceAsync> race_async_issue() {
+    Fiber *f = t_cur; RaceState *r = f->cta->race;
+    if (!r) return nullptr;
+    auto a = std::make_shared<RaceAsync>();
+    a->vc.assign(r->clk(f->tid), r->clk(f->tid) + r->n);
+    a->epoch = ++r->agent_epoch;
+    r->clk(f->tid)[f->tid] += 1;                       // what the issuer does next is NOT ordered before the copy
+    return a;
+}
+inline void race_async_write(Cta *c, const std::shared_ptr<RaceAsync> &a, const unsigned char *dst, size_t n, const void *pc) {
+    if (!a || !c->race || c->failed) return;
+    race_check(c, a->vc.data(), (uint32_t)c->race->n - 1, a->epoch, dst, n, true, pc);
+}
+inline void race_async_complete(Cta *c, SyncClock &s, const std::shared_ptr<RaceAsync> &a) {
+    if (!a || !c->race) return;
+    race_join(s.pending, a->vc.data(), c->race->n);
+    s.pending[c->race->n - 1] = std::max(s.pending[c->race->n - 1], a->epoch);
+}
+
 // extra yield at a synchronisation point when the schedule is randomised (the counterpart of EM_SWEEP_FUZZ's delays)
 inline void sync_point() {
     Fiber *f = t_cur;
@@ -150,15 +272,18 @@ inline void sync_point() {
 }
 
 // ---- warp collectives -------------------------------------------------------------------------------------------
-inline const uint64_t *warp_xchg(uint64_t v, unsigned mask) {
+// orders = true (__syncwarp): the collective is also a memory barrier among the lanes; shuffles and votes are not
+inline const uint64_t *warp_xchg(uint64_t v, unsigned mask, bool orders = false) {
     Fiber *f = t_cur;
     if (mask != 0xffffffffu) fail_here("warp collective with a partial mask (not emulated)");
     WarpState &W = f->cta->warps[f->warp];
     const uint32_t g = W.gen;
     uint64_t *b = W.buf[g & 1];
     b[f->lane] = v;
-    if (++W.arrived >= W.alive) { W.arrived = 0; W.gen = g + 1; }
+    if (orders) race_release(W.clk);
+    if (++W.arrived >= W.alive) { W.arrived = 0; W.gen = g + 1; if (orders) race_complete(f->cta, W.clk); }
     else block_while(&W.gen, 0xffffffffu, g, "warp collective (shuffle / vote / __syncwarp)");
+    if (orders) race_acquire(W.clk);
     return b;
 }
 template <typename T> inline uint64_t to_bits(T v) { uint64_t u = 0; static_assert(sizeof(T) <= 8, ""); memcpy(&u, &v, sizeof(T)); return u; }
@@ -166,9 +291,10 @@ template <typename T> inline T from_bits(uint64_t u) { T v; memcpy(&v, &u, sizeo
 
 inline void cta_barrier_arrive(Cta *c, BarState &B, int expected, bool wait, const char *what, long arg) {
     const uint32_t g = B.gen;
-    if (++B.arrived >= expected) { B.arrived = 0; B.gen = g + 1; }
+    race_release(B.clk);
+    if (++B.arrived >= expected) { B.arrived = 0; B.gen = g + 1; race_complete(c, B.clk); }
     else if (wait) block_while(&B.gen, 0xffffffffu, g, what, arg);
-    (void)c;
+    if (wait) race_acquire(B.clk);
 }
 
 // ---- global-memory registry (emu_alloc: guard pages on both sides) ----------------------------------------------
@@ -213,7 +339,7 @@ inline void fiber_entry() {
     WarpState &W = c->warps[f->warp];
     W.alive -= 1;
     if (W.arrived > 0 && W.arrived >= W.alive) { W.arrived = 0; W.gen += 1; }           // exited lanes do not hold a collective up
-    if (c->bars[0].arrived > 0 && c->bars[0].arrived >= c->alive) { c->bars[0].arrived = 0; c->bars[0].gen += 1; }
+    if (c->bars[0].arrived > 0 && c->bars[0].arrived >= c->alive) { c->bars[0].arrived = 0; c->bars[0].gen += 1; race_complete(c, c->bars[0].clk); }
     if (!f->copies.empty()) { /* cp.async still in flight at exit: the data would land after the thread is gone */ }
     emu_switch(&f->sp, c->sched_sp);
     abort();
@@ -283,6 +409,14 @@ inline void run_cta(Cta &c, char *stacks) {
             if (!c.async.empty()) { c.async[next_rand(c.rng) % c.async.size()].delay = 0; continue; }
             describe_deadlock(c);
         }
+    }
+    // copies still in flight when the last thread exited: completed now (so that the racecheck sees their writes), and
+    // reported -- on a GPU they would land in shared memory that may already belong to the next CTA
+    if (!c.failed && !c.async.empty()) {
+        std::vector<AsyncOp> rest;
+        rest.swap(c.async);
+        for (AsyncOp &op : rest) if (!c.failed) op.fire();
+        if (!c.failed) { c.failed = true; c.error = std::string("emu: kernel ") + c.kernel_name + ": the CTA exited with TMA / bulk copies in flight"; }
     }
 }
 
@@ -377,6 +511,7 @@ inline int launch(dim3 grid, dim3 block, size_t smem_bytes, const void *func, co
         }
     }
     const long seed = env_long("EMU_SEED", 0);
+    const bool racecheck = env_long("EMU_RACECHECK", 0) != 0;
     const long launch_no = launch_counter()++;
     const size_t n_cta = (size_t)grid.x * grid.y * grid.z;
     int n_workers = (int)env_long("EMU_THREADS", (long)std::thread::hardware_concurrency());
@@ -410,6 +545,14 @@ inline int launch(dim3 grid, dim3 block, size_t smem_bytes, const void *func, co
             }
             if (nthreads % 32) c.warps.back().alive = nthreads % 32;
             c.body = &body; c.kernel_name = name; c.regions = &regions_now;
+            RaceState race;
+            if (racecheck && smem_bytes > 0) {
+                race.n = nthreads + 1;
+                race.clocks.assign((size_t)race.n * race.n, 0);
+                for (int t = 0; t < race.n; ++t) race.clk(t)[t] = 1;
+                race.shadow.assign((smem_bytes + 3) / 4, RaceState::Shadow());
+                c.race = &race;
+            }
             c.random = seed != 0;
             c.rng = (uint64_t)seed * 0x2545f4914f6cdd1dull + (uint64_t)launch_no * 1315423911ull + b * 2654435761ull;
             run_cta(c, stacks);
@@ -424,7 +567,6 @@ inline int launch(dim3 grid, dim3 block, size_t smem_bytes, const void *func, co
             if (!c.failed)
                 for (const Fiber &f : c.fibers)
                     if (!f.copies.empty()) { c.failed = true; c.error = std::string("emu: kernel ") + name + ": a thread exited with cp.async copies never waited for"; break; }
-            if (!c.failed && !c.async.empty()) { c.failed = true; c.error = std::string("emu: kernel ") + name + ": the CTA exited with TMA / bulk copies in flight"; }
             if (c.failed) {
                 std::lock_guard<std::mutex> lk(launch_error().m);
                 if (launch_error().msg.empty()) launch_error().msg = c.error;
@@ -471,7 +613,7 @@ inline void __syncthreads() {
     emu::sync_point();
     emu::cta_barrier_arrive(c, c->bars[0], c->alive, true, "__syncthreads", 0);
 }
-inline void __syncwarp(unsigned mask = 0xffffffffu) { emu::warp_xchg(0, mask); }
+inline void __syncwarp(unsigned mask = 0xffffffffu) { emu::warp_xchg(0, mask, true); }
 template <typename T> inline T __shfl_sync(unsigned mask, T v, int src, int width = 32) {
     (void)width; return emu::from_bits<T>(emu::warp_xchg(emu::to_bits(v), mask)[src & 31]);
 }

@@ -63,4 +63,50 @@ void emu_free(void *ptr, size_t bytes) {
 
 long emu_launch_count(void) { return emu::launch_counter().load(); }
 
+// ---- the hooks a -fsanitize=thread build of the kernels calls on every load and store (libtsan is NOT linked: this is
+// the emulation's own happens-before race detector for the dynamic shared memory, emu_cuda.h "racecheck") -------------
+#define EMU_PC __builtin_return_address(0)
+void __tsan_init(void) {}
+void __tsan_func_entry(void *) {}
+void __tsan_func_exit(void) {}
+void __tsan_vptr_update(void **, void *) {}
+void __tsan_vptr_read(void **) {}
+void __tsan_read1(void *a) { emu::race_access(a, 1, false, EMU_PC); }
+void __tsan_read2(void *a) { emu::race_access(a, 2, false, EMU_PC); }
+void __tsan_read4(void *a) { emu::race_access(a, 4, false, EMU_PC); }
+void __tsan_read8(void *a) { emu::race_access(a, 8, false, EMU_PC); }
+void __tsan_read16(void *a) { emu::race_access(a, 16, false, EMU_PC); }
+void __tsan_write1(void *a) { emu::race_access(a, 1, true, EMU_PC); }
+void __tsan_write2(void *a) { emu::race_access(a, 2, true, EMU_PC); }
+void __tsan_write4(void *a) { emu::race_access(a, 4, true, EMU_PC); }
+void __tsan_write8(void *a) { emu::race_access(a, 8, true, EMU_PC); }
+void __tsan_write16(void *a) { emu::race_access(a, 16, true, EMU_PC); }
+void __tsan_unaligned_read2(void *a) { emu::race_access(a, 2, false, EMU_PC); }
+void __tsan_unaligned_read4(void *a) { emu::race_access(a, 4, false, EMU_PC); }
+void __tsan_unaligned_read8(void *a) { emu::race_access(a, 8, false, EMU_PC); }
+void __tsan_unaligned_read16(void *a) { emu::race_access(a, 16, false, EMU_PC); }
+void __tsan_unaligned_write2(void *a) { emu::race_access(a, 2, true, EMU_PC); }
+void __tsan_unaligned_write4(void *a) { emu::race_access(a, 4, true, EMU_PC); }
+void __tsan_unaligned_write8(void *a) { emu::race_access(a, 8, true, EMU_PC); }
+void __tsan_unaligned_write16(void *a) { emu::race_access(a, 16, true, EMU_PC); }
+void __tsan_read_range(void *a, unsigned long n) { if (n) emu::race_access(a, n, false, EMU_PC); }
+void __tsan_write_range(void *a, unsigned long n) { if (n) emu::race_access(a, n, true, EMU_PC); }
+// atomics of the emulation's own host code (std::atomic in launch()): plain builtins
+#define EMU_ATOMIC(bits, T)                                                                                              \
+    T __tsan_atomic##bits##_load(const volatile T *a, int) { return __atomic_load_n(a, __ATOMIC_SEQ_CST); }              \
+    void __tsan_atomic##bits##_store(volatile T *a, T v, int) { __atomic_store_n(a, v, __ATOMIC_SEQ_CST); }              \
+    T __tsan_atomic##bits##_exchange(volatile T *a, T v, int) { return __atomic_exchange_n(a, v, __ATOMIC_SEQ_CST); }    \
+    T __tsan_atomic##bits##_fetch_add(volatile T *a, T v, int) { return __atomic_fetch_add(a, v, __ATOMIC_SEQ_CST); }    \
+    T __tsan_atomic##bits##_fetch_sub(volatile T *a, T v, int) { return __atomic_fetch_sub(a, v, __ATOMIC_SEQ_CST); }    \
+    int __tsan_atomic##bits##_compare_exchange_strong(volatile T *a, T *e, T v, int, int) {                              \
+        return __atomic_compare_exchange_n(a, e, v, 0, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST); }                            \
+    int __tsan_atomic##bits##_compare_exchange_weak(volatile T *a, T *e, T v, int, int) {                                \
+        return __atomic_compare_exchange_n(a, e, v, 1, __ATOMIC_SEQ_CST, __ATOMIC_SEQ_CST); }
+EMU_ATOMIC(8, unsigned char)
+EMU_ATOMIC(16, unsigned short)
+EMU_ATOMIC(32, unsigned int)
+EMU_ATOMIC(64, unsigned long)
+void __tsan_atomic_thread_fence(int) { __atomic_thread_fence(__ATOMIC_SEQ_CST); }
+void __tsan_atomic_signal_fence(int) { __atomic_signal_fence(__ATOMIC_SEQ_CST); }
+
 }  // extern "C"

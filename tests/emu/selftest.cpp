@@ -94,6 +94,42 @@ __global__ void k_deadlock(float *out) {
     out[threadIdx.x] = 1.f;
 }
 
+// racecheck: lane l writes its slot, a neighbour lane reads it -- ordered by __syncwarp (sync = 1), by a shuffle only
+// (sync = 0: NOT an ordering edge) or by nothing (sync = 2)
+__global__ void k_warp_order(float *out, int sync) {
+    EM_DYN_SMEM(sm);
+    float *slot = reinterpret_cast<float *>(sm);
+    const int lane = threadIdx.x & 31;
+    slot[lane] = (float)lane;
+    float carried = 0.f;
+    if (sync == 1) __syncwarp();
+    else if (sync == 0) carried = __shfl_down_sync(0xffffffffu, (float)lane, 1);
+    out[lane] = slot[(lane + 1) & 31] + 0.f * carried;
+}
+
+// racecheck: a two-slot staging ring refilled by TMA.  The producer (thread 0) may refill a slot only when every warp has
+// arrived on its "empty" mbarrier; early = 1 refills without that wait (WAR on the slot, whatever the schedule).
+__global__ void k_ring(const __grid_constant__ Args a, int early) {
+    EM_DYN_SMEM(sm);
+    const int tid = threadIdx.x, lane = tid & 31;
+    const unsigned full = smem_u32(sm + 2048), empty = smem_u32(sm + 2056);
+    if (tid == 0) { mbar_init(full, 1); mbar_init(empty, 4); mbar_fence_init(); }
+    __syncthreads();
+    float acc = 0.f;
+    for (int it = 0; it < 4; ++it) {
+        if (tid == 0) {
+            if (it > 0 && !early) mbar_wait(empty, (unsigned)(it - 1) & 1u);
+            mbar_expect_tx(full, 32 * 4 * 4);
+            tma_load_3d<0>(smem_u32(sm), &a.map, full, 0, 0, it);
+        }
+        mbar_wait(full, (unsigned)it & 1u);
+        acc += reinterpret_cast<const float *>(sm)[tid];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty);
+    }
+    a.out[tid] = acc;
+}
+
 std::string take_error() {
     std::string s = cudaGetLastError() == cudaSuccess ? "" : cudaGetErrorString(cudaErrorLaunchFailure);
     return s;
@@ -186,6 +222,39 @@ extern "C" int selftest_run(int which, char *msg, int msg_len) {
         EM_LAUNCH(k_deadlock, 1, 64, 1024, 0)(out);
         const std::string e = take_error();
         rc = e.find("DEADLOCK") != std::string::npos && e.find("mbarrier.try_wait") != std::string::npos ? 0 : 1; say(e.empty() ? "(nothing reported)" : e);
+        break;
+    }
+    case 20: case 21: case 22: {   // racecheck: __syncwarp orders (20), a shuffle does not (21), nothing (22)
+        EM_LAUNCH(k_warp_order, 1, 32, 1024, 0)(out, which == 20 ? 1 : which == 21 ? 0 : 2);
+        const std::string e = take_error();
+        if (which == 20) { rc = e.empty() ? 0 : 1; say(e.empty() ? "ok" : e); }
+        else { rc = e.find("RACE") != std::string::npos ? 0 : 1; say(e.empty() ? "(nothing reported)" : e); }
+        break;
+    }
+    case 23: case 24: {   // racecheck: staging ring, refilled after the empty barrier (23) / too early (24)
+        a.bug = 0;
+        EM_LAUNCH(k_ring, 1, 128, 4096, 0)(a, which == 24 ? 1 : 0);
+        const std::string e = take_error();
+        if (which == 23) {
+            bool good = e.empty();
+            for (int tid = 0; tid < 128 && good; ++tid) {
+                float want = 0.f;
+                for (int it = 0; it < 4; ++it) want += tma_expected(tid, 0, 0, it);
+                if (out[tid] != want) good = false;
+            }
+            rc = good ? 0 : 1; say(good ? "ok" : (e.empty() ? "wrong sums" : e));
+        } else { rc = e.find("RACE") != std::string::npos && e.find("async copy engine") != std::string::npos ? 0 : 1; say(e.empty() ? "(nothing reported)" : e); }
+        break;
+    }
+    case 25: {   // racecheck: the hand-off with a skipped bar.sync is a race even if the values happen to come out right
+        EM_LAUNCH(k_pair, 1, 64, 1024, 0)(out, 1);
+        const std::string e = take_error();
+        rc = e.find("RACE") != std::string::npos ? 0 : 1; say(e.empty() ? "(nothing reported)" : e);
+        break;
+    }
+    case 26: {   // racecheck: the consumer that does not wait for the staged box
+        const std::string e = run_tma(2, 16, 2, 1);
+        rc = e.find("RACE") != std::string::npos ? 0 : 1; say(e.empty() ? "(nothing reported)" : e);
         break;
     }
     default: say("unknown case");
