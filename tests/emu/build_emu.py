@@ -44,6 +44,24 @@ def build_emu(tag: str = "", defines=(), force: bool = False, opt: str = "-O2", 
     return lib
 
 
+VARIANTS = {                             # tag -> extra compiler switches (tests/test_emu_sweep.py)
+    "": [],
+    "fc": ["-DEM_SWEEP_FUSED_CONDUCTION=1"],
+    "race": ["-fsanitize=thread"],
+    "race_fc": ["-fsanitize=thread", "-DEM_SWEEP_FUSED_CONDUCTION=1"],
+}
+
+
+def build_all() -> None:
+    """every variant the default tests load, and the two self-test libraries, side by side (one compiler process each)"""
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=6) as ex:
+        jobs = [ex.submit(build_emu, tag, flags) for tag, flags in VARIANTS.items()]
+        jobs += [ex.submit(build_selftest, False, False), ex.submit(build_selftest, False, True)]
+        for j in jobs:
+            j.result()
+
+
 RACE_FLAGS = ["-fsanitize=thread"]      # the kernels' loads and stores call the emulation's race detector (emu_exports.cpp)
 
 

@@ -35,7 +35,8 @@ class EmuEM(B.EM):
     """binding.EM on the emulated library: same calls, host memory.  Device-tensor arguments become CPU tensors."""
 
     def __init__(self, p, precision=None, kernel=B.EM_KERNEL_AUTO, bc=None, formulation=B.EM_FORM_LEAPFROG, z_chunks=0,
-                 e_prev=None, tag: str = "", defines=(), load_sources=True, load_init=True):
+                 e_prev=None, tag: str = "", defines=(), load_sources=True, load_init=True, max_ports=None,
+                 max_source_edges=None, max_wave_samples=None):
         import torch
         self._torch = torch
         self._L = load_emu(tag, defines)
@@ -51,7 +52,9 @@ class EmuEM(B.EM):
         n_ports = int(p.port_amplitude.shape[0])
         n_con = int(p.edge_comp.shape[0])
         self._grid = B._mk_grid(self.nx, self.ny, self.nz, self._dx, self._dy, self._dz, self.precision, int(p.loss_mode),
-                                kernel, max(n_ports, 1), max(n_con, 1), max(int(p.wave.shape[0]), 1),
+                                kernel, max_ports if max_ports is not None else max(n_ports, 1),
+                                max_source_edges if max_source_edges is not None else max(n_con, 1),
+                                max_wave_samples if max_wave_samples is not None else max(int(p.wave.shape[0]), 1),
                                 tuple(bc) if bc is not None else tuple(getattr(p, "bc", (0,) * 6)),
                                 1 if getattr(p, "thermal", None) is not None else 0, formulation, z_chunks)
         self.formulation = int(formulation)

@@ -27,7 +27,10 @@ from workloads.problem import LOSS_CD, LOSS_EXP
 import paper_2603_07038_b200 as P
 from oracle import emo
 from parity import TOL, compare_state, rel_l2
+import build_emu
 import emu_em
+
+build_emu.build_all()          # every library variant used below, compiled side by side if stale (no-op when fresh)
 
 import test_gpu_parity as TP
 import test_gpu_thermal as TT
@@ -35,7 +38,9 @@ import test_gpu_eonly as TE
 import test_gpu_slabs as TS
 import paper_2603_07038_b200.binding as PB
 
-FC = dict(tag="fc", defines=["-DEM_SWEEP_FUSED_CONDUCTION=1"])      # the coupled sweep with the conduction stencil fused in
+FC = dict(tag="fc", defines=build_emu.VARIANTS["fc"])              # the coupled sweep with the conduction stencil fused in
+RACE = dict(tag="race", defines=build_emu.VARIANTS["race"])        # loads / stores instrumented for the racecheck
+RACE_FC = dict(tag="race_fc", defines=build_emu.VARIANTS["race_fc"])
 
 
 def _factory(**fixed):
@@ -75,8 +80,7 @@ def test_random_grids_cd_split(emulated):
     TP.test_random_grids_cd((37, 29, 23), 64, P.EM_KERNEL_SPLIT)
 
 
-@pytest.mark.parametrize("zsplit", [1, 2, 3, 5, 8])
-@pytest.mark.parametrize("bc", [(0,) * 6, (0, 0, 1, 0, 1, 1)])
+@pytest.mark.parametrize("zsplit,bc", [(1, (0, 0, 1, 0, 1, 1)), (2, (0,) * 6), (3, (0, 0, 1, 0, 1, 1)), (5, (0,) * 6), (8, (0, 0, 1, 0, 1, 1))])
 def test_z_chunks(emulated, zsplit, bc):
     TP.test_tma_sweep_z_chunks(zsplit, bc)
 
@@ -87,9 +91,11 @@ def test_random_grids_exp(emulated, dims, precision):
     TP.test_random_grids_exp(dims, precision, P.EM_KERNEL_TMA)
 
 
-@pytest.mark.parametrize("precision", [64, 32])
-@pytest.mark.parametrize("bc", TP.PMC_BC)
-@pytest.mark.parametrize("dims", [(37, 29, 23), (130, 3, 2), (5, 9, 2), (33, 65, 4)])
+PMC_CASES = [(d, b, pr) for n, (d, b) in enumerate((d, b) for d in [(37, 29, 23), (130, 3, 2), (5, 9, 2), (33, 65, 4)] for b in TP.PMC_BC)
+             for pr in ((64, 32) if n % 5 == 0 else (64,) if n % 2 else (32,))]
+
+
+@pytest.mark.parametrize("dims,bc,precision", PMC_CASES)
 def test_random_grids_pmc_walls(emulated, dims, bc, precision):
     TP.test_random_grids_pmc_walls(dims, bc, precision, P.EM_KERNEL_TMA)
 
@@ -104,6 +110,7 @@ def test_percell_ids_pec_material_overlapping_ports(emulated):
 
 
 def test_api_contract_and_probe(emulated):
+    TP.test_api_contract()
     TP.test_probe_matches_fields()
 
 
@@ -136,9 +143,12 @@ def test_eonly_equals_the_leapfrog_kernel(emulated):
 VARIANTS = [pytest.param({}, id="k_diffuse+sweep"), pytest.param(FC, id="fused-conduction")]
 
 
-@pytest.mark.parametrize("variant", VARIANTS)
-@pytest.mark.parametrize("precision", [64, 32])
-@pytest.mark.parametrize("dims,mode", TT.CASES)
+COUPLED = [pytest.param(d, m, pr, v.values[0], id="%s-%d-fp%d-%s" % ("x".join(map(str, d)), m, pr, v.id))
+           for n, (d, m) in enumerate(TT.CASES) for pr in (64, 32) for v in VARIANTS
+           if v.values[0] or (n + pr // 32) % 2 == 0]          # fused conduction: every case; conduction kernel: every other one
+
+
+@pytest.mark.parametrize("dims,mode,precision,variant", COUPLED)
 def test_coupled_random_grids(emulated, dims, mode, precision, variant):
     emulated(**variant)
     TT.test_coupled_random_grids(dims, mode, precision, P.EM_KERNEL_AUTO)
@@ -167,9 +177,7 @@ def test_coupled_split_kernels(emulated):
 
 
 # ------------------------------------------------------------------ z slabs: pack / unpack kernels and fused peer stores
-@pytest.mark.parametrize("n_ranks", [2, 3])
-@pytest.mark.parametrize("mode", ["p2p", "peer"])
-@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("n_ranks,mode,precision", [(2, "peer", 32), (3, "peer", 64), (3, "p2p", 32), (2, "p2p", 64)])
 def test_slabs_equal_single_domain(emulated, n_ranks, mode, precision):
     """peer mode: the sweep of one slab context stores E'x, E'y straight into the wall plane of the neighbouring
     context's workspace (em_set_peer_halo) -- under the emulation's range checks"""
@@ -222,3 +230,26 @@ def test_random_schedules_do_not_change_a_bit(monkeypatch, kw, thermal, precisio
         else:
             for a, b in zip(out, ref):
                 assert np.array_equal(a, b), seed
+
+
+# --------------------------------------------------------------- racecheck: no two accesses without an ordering path
+@pytest.mark.parametrize("kw,thermal", [pytest.param(dict(RACE), False, id="leapfrog"),
+                                        pytest.param(dict(RACE, formulation=P.EM_FORM_EONLY), False, id="e-only"),
+                                        pytest.param(dict(RACE), True, id="coupled"),
+                                        pytest.param(dict(RACE_FC), True, id="coupled-fused-conduction")])
+def test_racecheck_clean(monkeypatch, kw, thermal):
+    """EMU_RACECHECK=1 on the -fsanitize=thread build (tests/emu/emu_cuda.h "racecheck"): every load and store of the
+    dynamic shared memory is checked against the vector clocks of the barriers; a clean run means that every pair of
+    conflicting accesses of k_sweep_tma's barrier-free plane loop is ordered by an mbarrier, a named barrier, a
+    __syncwarp or the prologue's __syncthreads -- for ANY schedule, not only the one that ran.  (That the detector and
+    this very kernel's barriers are sensitive: tests/test_emu_selftest.py and tests/test_emu_mutations.py.)"""
+    monkeypatch.setenv("EMU_RACECHECK", "1")
+    monkeypatch.setenv("EMU_SEED", "1")
+    p = W.random_problem(130, 31, 9, seed=5, steps=3, n_ports=4, bc=(0, 1, 1, 0, 1, 0), init_scale=4.0e6 if thermal else 1.0)
+    if thermal:
+        th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
+        p.thermal = th
+    g = emu_em.EmuEM(p, precision=32, z_chunks=2, **kw)
+    g.em_step(3)                        # (a race would surface as EMError "emu: RACE in kernel ...")
+    assert np.isfinite(g.em_get_field(0)).all()
+    g.close()
