@@ -30,7 +30,6 @@ from parity import TOL, compare_state, rel_l2
 import build_emu
 import emu_em
 
-build_emu.build_all()          # every library variant used below, compiled side by side if stale (no-op when fresh)
 
 import test_gpu_parity as TP
 import test_gpu_thermal as TT
@@ -48,6 +47,13 @@ def _factory(**fixed):
         kw.update(fixed)
         return emu_em.EmuEM(p, precision=precision, kernel=kernel, **kw)
     return make
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _libraries():
+    """every library variant used below, compiled side by side if stale (no-op when fresh); only when a test of this
+    module actually runs -- collecting the module (e.g. under -m gpu) builds nothing"""
+    build_emu.build_all()
 
 
 @pytest.fixture
