@@ -76,7 +76,7 @@ extern "C" {
 #define EM_FORM_LEAPFROG 0
 #define EM_FORM_EONLY 1
 
-#define EM_ABI_VERSION 3 /* bumped whenever em_grid or a signature changes; em_abi_version() returns it */
+#define EM_ABI_VERSION 4 /* bumped whenever em_grid or a signature changes; em_abi_version() returns it */
 
 typedef struct em_ctx em_ctx; /* opaque, host-side */
 
@@ -234,6 +234,23 @@ int32_t em_set_temperature_rise(em_ctx *ctx, const void *src, int32_t src_is_dev
 
 /* Absolute step index n (host bookkeeping). */
 int32_t em_step_index(em_ctx *ctx, int64_t *n);
+
+/* ---- checkpoint / resume and failure detection -----------------------------------------------
+ * The state of a run is: the six field arrays (E-only contexts: e^n and e^{n-1}), the Joule accumulator q, the step
+ * index n (it selects the waveform samples J((n + 1/2) dt), C3) and, in a coupled context, theta.  A checkpoint is
+ * em_get_field x 6, em_joule(energy_density), em_step_index (, em_get_temperature_rise); a resume on a context created
+ * with the same grid, materials, dt and sources is em_set_field x 6, em_set_joule_energy, em_set_step_index
+ * (, em_set_temperature_rise) -- after which em_step continues BIT FOR BIT as the uninterrupted run would.
+ *
+ * em_set_joule_energy: q [J/m^3], dense [nz][ny][nx] in the working precision, device or host pointer (host copies
+ * synchronise).  em_set_step_index: n >= 0.  Errors: INVALID_ARG, CUDA. */
+int32_t em_set_joule_energy(em_ctx *ctx, const void *energy_density, int32_t src_is_device);
+int32_t em_set_step_index(em_ctx *ctx, int64_t n);
+
+/* *all_finite (HOST) = 1 if every value of the field arrays, q and (coupled contexts) theta is finite, else 0: an
+ * unstable dt or a corrupted input shows as Inf / NaN within a few hundred steps.  One small kernel per array;
+ * synchronises the stream.  Errors: INVALID_ARG, CUDA. */
+int32_t em_check_finite(em_ctx *ctx, int32_t *all_finite);
 
 /* Number of kernel launches enqueued by this context so far (for bench accounting). */
 int32_t em_launch_count(em_ctx *ctx, int64_t *n);

@@ -16,7 +16,7 @@ EM_OK = 0
 EM_LOSS_CD, EM_LOSS_EXP = 0, 1
 EM_KERNEL_AUTO, EM_KERNEL_SPLIT, EM_KERNEL_TMA = 0, 1, 2
 EM_FORM_LEAPFROG, EM_FORM_EONLY = 0, 1
-EM_ABI_VERSION = 3            # include/em.h: this binding's em_grid layout and signatures
+EM_ABI_VERSION = 4            # include/em.h: this binding's em_grid layout and signatures
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -126,6 +126,9 @@ def _open(path: str):
     L.em_get_temperature_rise.argtypes = [vp, vp, i32]
     L.em_set_temperature_rise.argtypes = [vp, vp, i32]
     L.em_step_index.argtypes = [vp, C.POINTER(i64)]
+    L.em_set_step_index.argtypes = [vp, i64]
+    L.em_set_joule_energy.argtypes = [vp, vp, i32]
+    L.em_check_finite.argtypes = [vp, C.POINTER(i32)]
     L.em_launch_count.argtypes = [vp, C.POINTER(i64)]
     L.em_timing_enable.argtypes = [vp, i32]
     L.em_timing_read.argtypes = [vp, C.POINTER(C.c_char_p), C.POINTER(i64), C.POINTER(C.c_double)]
@@ -420,6 +423,42 @@ class EM:
         out = np.empty(len(pts), np.float64)
         _check(self._L.em_probe(self._h, len(pts), arr, _dp(out)), self._L)
         return out
+
+    # checkpoint / resume and failure detection (include/em.h)
+    def em_set_joule_energy(self, q):
+        if self._torch.is_tensor(q):
+            t = q.to(device=self.device, dtype=self.dtype).contiguous()
+            assert tuple(t.shape) == (self.nz, self.ny, self.nx)
+            _check(self._L.em_set_joule_energy(self._h, C.c_void_p(t.data_ptr()), 1 if t.is_cuda else 0), self._L)
+            return
+        a = np.ascontiguousarray(q, self.np_dtype)
+        assert a.shape == (self.nz, self.ny, self.nx)
+        _check(self._L.em_set_joule_energy(self._h, a.ctypes.data_as(C.c_void_p), 0), self._L)
+
+    def em_set_step_index(self, n: int):
+        _check(self._L.em_set_step_index(self._h, int(n)), self._L)
+
+    def em_check_finite(self) -> bool:
+        ok = C.c_int32()
+        _check(self._L.em_check_finite(self._h, C.byref(ok)), self._L)
+        return bool(ok.value)
+
+    def checkpoint(self) -> dict:
+        """the whole state of the run as host arrays (include/em.h "checkpoint / resume")"""
+        comps = range(6) if self.formulation == EM_FORM_LEAPFROG else (0, 1, 2, 6, 7, 8)
+        ck = {"fields": {c: self.em_get_field(c) for c in comps}, "q": self.joule_maps()[1], "step": self.step_index}
+        if (self._grid.thermal):
+            ck["theta"] = self.em_get_temperature_rise()
+        return ck
+
+    def resume(self, ck: dict):
+        """restore a checkpoint into a context created with the same grid, materials, dt and sources"""
+        for c, f in ck["fields"].items():
+            self.em_set_field(c, f)
+        self.em_set_joule_energy(ck["q"])
+        if "theta" in ck:
+            self.em_set_temperature_rise(ck["theta"])
+        self.em_set_step_index(ck["step"])
 
     def em_reset(self):
         _check(self._L.em_reset(self._h), self._L)

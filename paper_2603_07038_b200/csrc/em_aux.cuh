@@ -197,6 +197,16 @@ __global__ void __launch_bounds__(256) k_energy_final(const double *partial, int
     if (threadIdx.x == 0) *out = sh[0];
 }
 
+// em_check_finite: *flag = 1 if any of the n values is Inf or NaN (every thread that finds one stores the same 1)
+template <typename R>
+__global__ void __launch_bounds__(256) k_check_finite(const R *a, long long n, int *flag) {
+    const R big = sizeof(R) == 4 ? (R)3.402823466e+38F : (R)1.7976931348623157e+308;
+    bool bad = false;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x)
+        bad = bad || !(::fabs(a[t]) <= big);
+    if (bad) *flag = 1;
+}
+
 template <typename R>
 struct ProbeArrays { const R *f[9]; };
 

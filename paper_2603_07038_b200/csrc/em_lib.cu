@@ -162,6 +162,8 @@ struct em_ctx {
     virtual int32_t joule_layers(int32_t k0, int32_t k1, double *total) = 0;
     virtual int32_t wall_offset(int32_t side, int32_t parity, int32_t comp, size_t *off) = 0;
     virtual int32_t set_peer_halo(int32_t side, int32_t k_send, void *const dst[4]) = 0;
+    virtual int32_t set_joule_energy(const void *src, int32_t is_dev) = 0;
+    virtual int32_t check_finite(int32_t *all_finite) = 0;
     int64_t step_index = 0, launches = 0;
     Timing timing;
     const char *main_kernel = "";
@@ -244,6 +246,8 @@ struct Ctx final : em_ctx {
     int32_t joule_layers(int32_t k0, int32_t k1, double *total) override;
     int32_t wall_offset(int32_t side, int32_t parity, int32_t comp, size_t *off) override;
     int32_t set_peer_halo(int32_t side, int32_t k_send, void *const dst[4]) override;
+    int32_t set_joule_energy(const void *src, int32_t is_dev) override;
+    int32_t check_finite(int32_t *all_finite) override;
     void *ws_base = nullptr;
     R *peer_dst[2][2][2] = {};          // [side][parity of the neighbour's E array][comp]
     int32_t step_thermal();
@@ -966,6 +970,38 @@ int32_t Ctx<R>::joule(void *power, void *energy, double *total, int32_t do_reset
     return EM_OK;
 }
 
+// ---- checkpoint / resume, failure detection (em.h) ------------------------------------------------------------------
+template <typename R>
+int32_t Ctx<R>::set_joule_energy(const void *srcp, int32_t is_dev) {
+    if (!srcp) return fail(EM_ERR_INVALID_ARG, "set_joule_energy: null");
+    cudaMemcpy3DParms m = {};
+    m.srcPtr = make_cudaPitchedPtr(const_cast<void *>(srcp), sizeof(R) * g.nx, g.nx, g.ny);
+    m.dstPtr = make_cudaPitchedPtr(p.q, sizeof(R) * g.PX, g.PX, g.PY);
+    m.extent = make_cudaExtent(sizeof(R) * g.nx, g.ny, g.nz);
+    m.kind = is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CU(cudaMemcpy3DAsync(&m, stream));
+    if (!is_dev) CU(cudaStreamSynchronize(stream));
+    return EM_OK;
+}
+
+template <typename R>
+int32_t Ctx<R>::check_finite(int32_t *all_finite) {
+    if (!all_finite) return fail(EM_ERR_INVALID_ARG, "check_finite: null");
+    int *flag = reinterpret_cast<int *>(c.partial);                      // (scratch of the Joule reduction)
+    CU(cudaMemsetAsync(flag, 0, sizeof(int), stream));
+    const long long n = g.alloc_elems;                                   // whole allocations: the pads hold zeros
+    const unsigned blocks = (unsigned)std::min<long long>((n + 255) / 256, 4096);
+    for (int a = 0; a < n_field; ++a) { EM_LAUNCH(em::k_check_finite<R>, blocks, 256, 0, stream)(c.field[a], n, flag); launches += 1; }
+    EM_LAUNCH(em::k_check_finite<R>, blocks, 256, 0, stream)(c.q, n, flag); launches += 1;
+    if (thermal_on) { EM_LAUNCH(em::k_check_finite<R>, blocks, 256, 0, stream)(c.theta[th_cur], n, flag); launches += 1; }
+    CU(cudaGetLastError());
+    int host_flag = 0;
+    CU(cudaMemcpyAsync(&host_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    *all_finite = host_flag ? 0 : 1;
+    return EM_OK;
+}
+
 template <typename R>
 int32_t Ctx<R>::probe(int32_t n, const em_probe_pt *pts, double *out) {
     if (n < 0 || (n && (!pts || !out))) return fail(EM_ERR_INVALID_ARG, "probe arguments");
@@ -1139,6 +1175,11 @@ int32_t em_joule_layers(em_ctx *ctx, int32_t k0, int32_t k1, double *total) { EM
 int32_t em_wall_offset(em_ctx *ctx, int32_t side, int32_t parity, int32_t comp, size_t *off) { EM_CHECK_CTX; return ctx->wall_offset(side, parity, comp, off); }
 int32_t em_set_peer_halo(em_ctx *ctx, int32_t side, int32_t k_send, void *const dst[4]) { EM_CHECK_CTX; return ctx->set_peer_halo(side, k_send, dst); }
 
+int32_t em_set_joule_energy(em_ctx *ctx, const void *src, int32_t is_dev) { EM_CHECK_CTX; return ctx->set_joule_energy(src, is_dev); }
+int32_t em_set_step_index(em_ctx *ctx, int64_t n) {
+    EM_CHECK_CTX; if (n < 0) return fail(EM_ERR_INVALID_ARG, "step index must be >= 0"); ctx->step_index = n; return EM_OK;
+}
+int32_t em_check_finite(em_ctx *ctx, int32_t *all_finite) { EM_CHECK_CTX; return ctx->check_finite(all_finite); }
 int32_t em_step_index(em_ctx *ctx, int64_t *n) { EM_CHECK_CTX; if (!n) return fail(EM_ERR_INVALID_ARG, "null"); *n = ctx->step_index; return EM_OK; }
 int32_t em_launch_count(em_ctx *ctx, int64_t *n) { EM_CHECK_CTX; if (!n) return fail(EM_ERR_INVALID_ARG, "null"); *n = ctx->launches; return EM_OK; }
 

@@ -71,10 +71,20 @@ template <int SZ, bool TH = false> struct SweepLayout {
     static constexpr int yg = tht + 3 * th_slot;                  // coupled sweep: {1/dy[j-1], 1/dy[j+1], 1/dy~[j+1], 0} per row
     static constexpr int yg_bytes = FC ? kSwWarps * 4 * SZ : 0;
     static constexpr int bar = FC ? (yg + yg_bytes + 63) / 64 * 64 : sig + 2 * sig_slot;   // fullE[2], fullH[2], empty[2], emptyH[2], rowH[kSwWarps]
-    static constexpr int tab = bar + 64 + 8 * kSwWarps;                          // material table (n_table entries)
+    static constexpr int tab = (bar + 64 + 8 * kSwWarps + 31) / 32 * 32;         // material table (n_table entries of 4 reals)
     static constexpr int e_bytes = ex_slot + ey_slot + ez_slot + (kSwWarps + 2) * id_row + sig_slot + th_slot;
     static constexpr int first_extra_bytes = ex_slot + ey_slot;
     static constexpr int h_bytes = 3 * h_slot;
+    // what the hardware requires of these offsets (the base is 1024-byte aligned): TMA box destinations 128 B, bulk-copy
+    // destinations and 16-byte vector slots 16 B, mbarriers 8 B, table entries their own size -- for EVERY tile shape the
+    // experiment switches can produce (a 5-row variant once faulted on a GPU with "misaligned address": its table sat
+    // at 8 mod 16; tests/emu reproduces that on the host)
+    static_assert(ex % 128 == 0 && ex_slot % 128 == 0 && ey % 128 == 0 && ey_slot % 128 == 0 && ez % 128 == 0 && ez_slot % 128 == 0,
+                  "E plane slots: TMA destinations");
+    static_assert(h % 128 == 0 && h_slot % 128 == 0 && ids % 128 == 0 && id_slot % 128 == 0, "H and id slots: TMA destinations");
+    static_assert(sig % 128 == 0 && sig_slot % 128 == 0 && tht % 128 == 0 && th_slot % 128 == 0, "sigma(T) and theta slots: TMA destinations");
+    static_assert(priv % 16 == 0 && rows % 16 == 0 && geo % 16 == 0 && zg % 16 == 0 && yg % 16 == 0, "16-byte vector regions");
+    static_assert(bar % 8 == 0 && tab % (4 * SZ) == 0, "mbarriers and table entries");
 };
 
 // the material table, and for the coupled sweep the thermal table (ThEntry, same size) behind it

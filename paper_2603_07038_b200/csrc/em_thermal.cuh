@@ -223,7 +223,9 @@ __global__ void __launch_bounds__(256) k_sigma_refresh(DevParams<R> p, ThermalPa
     if (i >= p.nx || j >= p.ny) return;
     const long long o = ((long long)k * p.PY + j) * p.PX + i;
     const ThEntry<R> me = t.ttable[p.mat[o]];
-    t.sig[o] = me.sigma0 / thermal_den(me.alpha, t.theta[o]);
+    // the expression of the stepping kernels, so that sigma(T) restored from theta (em_set_temperature_rise: resume of a
+    // checkpoint, slab halos) has the bits the uninterrupted run holds
+    t.sig[o] = me.sigma0 * rcp<R>(thermal_den(me.alpha, t.theta[o]));
 }
 
 // p_c = sigma_c(T) * 1/4 sum_12 (E_e)^2 with the CURRENT conductivity (PAPER.md L86 with eq. (6))

@@ -121,6 +121,8 @@ struct Cta {
 inline thread_local Fiber *t_cur = nullptr;
 
 extern "C" void emu_switch(void **save_sp, void *load_sp);
+extern "C" void emu_install_fault_handler(void);      // emu_exports.cpp: SIGSEGV / SIGBUS inside a kernel -> who, where
+extern "C" void emu_thread_altstack(void);
 // (defined once, in emu_exports.cpp: saves the callee-saved registers, swaps the stack pointer)
 
 inline uint64_t next_rand(uint64_t &s) {       // splitmix64
@@ -520,7 +522,9 @@ inline int launch(dim3 grid, dim3 block, size_t smem_bytes, const void *func, co
     std::atomic<bool> failed{false};
     std::vector<Region> regions_now;
     { std::lock_guard<std::mutex> lk(regions_mutex()); regions_now = regions(); }
+    if (env_long("EMU_FAULT_HANDLER", 1)) emu_install_fault_handler();
     auto worker = [&]() {
+        emu_thread_altstack();
         const size_t stack_bytes = (size_t)nthreads * kStackBytes;
         const size_t canary = 1024, smem_alloc = (smem_bytes + canary + 1023) / 1024 * 1024 + 2048;
         Arena ar = acquire_arena(stack_bytes, smem_alloc);

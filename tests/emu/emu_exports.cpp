@@ -2,6 +2,7 @@
 // build; linked with csrc/em_lib.cu into libem_emu*.so.
 #include "emu_cuda.h"
 
+#include <signal.h>
 #include <unistd.h>
 
 #if defined(__x86_64__)
@@ -32,7 +33,60 @@ emu_switch:
 #error "tests/emu: the fiber switch is written for x86-64"
 #endif
 
+// ---- a fault inside an emulated kernel (guard page of the workspace, wild pointer, misaligned SSE access): say where ----
+namespace {
+void fault_handler(int sig, siginfo_t *si, void *) {
+    char buf[1024];
+    const emu::Fiber *f = emu::t_cur;
+    const uintptr_t a = (uintptr_t)si->si_addr;
+    int n;
+    if (f && f->cta) {
+        const emu::Cta *c = f->cta;
+        long smem_off = (a >= (uintptr_t)c->smem && a < (uintptr_t)c->smem + c->smem_bytes + 4096) ? (long)(a - (uintptr_t)c->smem) : -1;
+        long best = 0; int where = 0;                                  // distance to the nearest registered region
+        if (c->regions)
+            for (const emu::Region &r : *c->regions) {
+                if (a < r.lo && (where == 0 || (long)(r.lo - a) < best)) { best = (long)(r.lo - a); where = -1; }
+                if (a >= r.hi && (where == 0 || (long)(a - r.hi) < best)) { best = (long)(a - r.hi); where = 1; }
+            }
+        n = snprintf(buf, sizeof(buf), "\nemu: FAULT (signal %d) in kernel %s, block (%u,%u,%u), thread %d (warp %d lane %d): address %p%s",
+                     sig, c->kernel_name, c->bidx.x, c->bidx.y, c->bidx.z, f->tid, f->warp, f->lane, si->si_addr,
+                     smem_off >= 0 ? " = dynamic shared memory offset " : "");
+        if (!si->si_addr) n += snprintf(buf + n, sizeof(buf) - n, " -- no address: a general-protection fault, i.e. almost certainly a MISALIGNED 16-byte "
+                                "vector access (what a GPU reports as 'misaligned address'); rebuild with the UBSan traps to get the line");
+        else if (smem_off >= 0) n += snprintf(buf + n, sizeof(buf) - n, "%ld (of %zu bytes)", smem_off, c->smem_bytes);
+        else if (where && si->si_addr) n += snprintf(buf + n, sizeof(buf) - n, ", %ld bytes %s an emu_alloc'ed region (out-of-bounds global access)", best, where < 0 ? "BEFORE" : "BEHIND");
+        n += snprintf(buf + n, sizeof(buf) - n, "\n");
+    } else {
+        n = snprintf(buf, sizeof(buf), "\nemu: FAULT (signal %d) at address %p outside any emulated kernel\n", sig, si->si_addr);
+    }
+    if (write(2, buf, (size_t)n) < 0) {}
+    _exit(128 + sig);
+}
+}  // namespace
+
 extern "C" {
+
+// installs the handler (idempotent); every worker thread also gets an alternate signal stack (emu_cuda.h)
+void emu_install_fault_handler(void) {
+    static bool done = false;
+    if (done) return;
+    done = true;
+    struct sigaction sa;
+    memset(&sa, 0, sizeof(sa));
+    sa.sa_sigaction = fault_handler;
+    sa.sa_flags = SA_SIGINFO | SA_ONSTACK;
+    sigemptyset(&sa.sa_mask);
+    sigaction(SIGSEGV, &sa, nullptr);
+    sigaction(SIGBUS, &sa, nullptr);
+}
+void emu_thread_altstack(void) {
+    static thread_local char *stk = nullptr;
+    if (stk) return;
+    stk = static_cast<char *>(malloc(64 * 1024));
+    stack_t ss; ss.ss_sp = stk; ss.ss_size = 64 * 1024; ss.ss_flags = 0;
+    sigaltstack(&ss, nullptr);
+}
 
 // bytes of "device memory" between two PROT_NONE guard pages, registered for the range checks of the emulated
 // wrappers; the returned pointer is 256-byte aligned and its end is within 255 bytes of the trailing guard page

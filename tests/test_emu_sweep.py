@@ -120,6 +120,11 @@ def test_api_contract_and_probe(emulated):
     TP.test_probe_matches_fields()
 
 
+@pytest.mark.parametrize("what", ["leapfrog-fp32", "e-only-fp64", "coupled-fp32", "split-fp64"])
+def test_checkpoint_resume_and_check_finite(emulated, what):
+    TP.test_checkpoint_resume_is_bit_exact_and_check_finite(what)
+
+
 def test_package_slice_several_tiles_and_chunks(emulated):
     """config 4 at 1/8 of the x, y and 1/4 of the z cell counts: 128 x 128 x 48 cells = 2 x 10 tiles, sources, fp32"""
     p = W.make_config(4, scale=8, zscale=4, steps=12)
@@ -259,3 +264,29 @@ def test_racecheck_clean(monkeypatch, kw, thermal):
     g.em_step(3)                        # (a race would surface as EMError "emu: RACE in kernel ...")
     assert np.isfinite(g.em_get_field(0)).all()
     g.close()
+
+
+# ------------------------------------------------------------------------------------------- the largest material table
+@pytest.mark.parametrize("precision,thermal", [(32, False), (64, False), (32, True), (64, True)])
+def test_largest_material_table(emulated, precision, thermal):
+    """254 materials + the 'outside / PMC' and 'outside / PEC' entries = the 256-entry table the shared-memory layout must
+    hold (em_lib.cu init: the fp64 coupled sweep with its two tables of 32-byte entries does not fit and takes the split
+    kernels); ids spread over the whole table"""
+    p = W.random_problem(70, 25, 11, seed=77, steps=6, n_ports=3, bc=(1, 0, 0, 1, 0, 1), init_scale=4.0e6 if thermal else 1.0)
+    rng = np.random.default_rng(78)
+    n = 254
+    rep = (n + 15) // 16
+    scale = 1.0 + 0.05 * rng.random((rep * 16, 1))
+    p.table = (np.tile(np.asarray(p.table, np.float64), (rep, 1)) * scale)[:n]
+    p.table[:, 1] = np.tile(np.asarray(p.table[:16, 1]), rep)[:n]                  # (mu unchanged: keeps dt inside the CFL bound)
+    p.table[:, 0] = np.maximum(p.table[:, 0], np.tile(np.asarray(p.table[:16, 0]), rep)[:n])
+    if getattr(p, "flags", None) is not None:
+        p.flags = np.tile(np.asarray(p.flags), rep)[:n]
+    p.mat_id = (p.mat_id.astype(np.int64) + 16 * rng.integers(0, rep, size=p.mat_id.shape)).clip(max=n - 1).astype(np.uint8)
+    if thermal:
+        th = np.tile(W.thermal_table(), (rep, 1))[:n]
+        th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
+        p.thermal = th
+        TT._run(p, 6, precision)
+    else:
+        TP.run_pair(p, 6, precision, P.EM_KERNEL_TMA, z_chunks=2)

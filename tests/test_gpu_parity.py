@@ -335,3 +335,52 @@ def test_configs_4_and_5_at_their_stated_1000_steps():
         p = W.make_config(cfg, steps=1000, **kw)
         res = run_pair(p, 1000, 32, P.EM_KERNEL_AUTO)
         assert res["E"] < 5e-6 and res["H"] < 1e-5, res
+
+
+# ------------------------------------------------------- checkpoint / resume, failure detection (include/em.h)
+def _full_state(g):
+    ck = g.checkpoint()
+    return [ck["fields"][c] for c in sorted(ck["fields"])] + [ck["q"]] + ([ck["theta"]] if "theta" in ck else [])
+
+
+@pytest.mark.parametrize("what", ["leapfrog-fp32", "e-only-fp64", "coupled-fp32", "split-fp64"])
+def test_checkpoint_resume_is_bit_exact_and_check_finite(what):
+    """state = fields + q + step index (+ theta): a run interrupted after 5 of 12 steps and resumed in a NEW context
+    continues bit for bit (the step index selects the waveform samples; q and theta are accumulators)"""
+    precision = 32 if what.endswith("32") else 64
+    kw = {}
+    p = W.random_problem(37, 29, 23, seed=6100, steps=12, n_ports=5, bc=(0, 1, 0, 0, 1, 0), init_scale=4.0e6 if "coupled" in what else 1.0)
+    if what.startswith("e-only"):
+        kw["formulation"] = P.EM_FORM_EONLY
+    if what.startswith("split"):
+        kw["kernel"] = P.EM_KERNEL_SPLIT
+    if what.startswith("coupled"):
+        th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
+        p.thermal = th
+    ref = P.EM(p, precision=precision, **kw)
+    ref.em_step(12)
+    a = P.EM(p, precision=precision, **kw)
+    a.em_step(5)
+    assert a.em_check_finite()
+    ck = a.checkpoint()
+    assert ck["step"] == 5
+    a.close()
+    b = P.EM(p, precision=precision, load_init=False, **kw)
+    b.resume(ck)
+    assert b.step_index == 5
+    b.em_step(7)
+    for x, y in zip(_full_state(b), _full_state(ref)):
+        assert np.array_equal(x, y)
+    assert np.abs(_full_state(ref)[-1]).max() > 0
+    # failure detection: one NaN in a field, one Inf in q
+    bad = ck["fields"][1].copy(); bad[2, 3, 4] = np.nan
+    b.em_set_field(1, bad)
+    assert not b.em_check_finite()
+    b.em_set_field(1, ck["fields"][1])
+    assert b.em_check_finite()
+    q = ck["q"].copy(); q[0, 0, 0] = np.inf
+    b.em_set_joule_energy(q)
+    assert not b.em_check_finite()
+    with pytest.raises(P.EMError):
+        b.em_set_step_index(-1)
+    ref.close(); b.close()
