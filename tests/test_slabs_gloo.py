@@ -180,3 +180,57 @@ def test_peer_wiring_hands_each_sweep_its_neighbours_wall_planes():
         assert hi.meta.lo + hi.k_send_down == lo.meta.lo + lo.k_wall_hi
         assert lo.meta.lo + lo.layer_send_up == hi.meta.lo + 0                       # theta: my top owned layer = its ghost layer 0
         assert hi.meta.lo + hi.layer_send_down == lo.meta.lo + lo.nz_local - 1       # my bottom owned layer = its last ghost layer
+
+
+# ---- the REAL kernels under the exchange, one process per slab, gloo: the product's sweep sources on the emulated build ----
+# (tests/emu: em_lib.cu compiled against the CPU emulation of the CUDA primitives; no GPU.  This is the N > 1 path of
+# bench.py --gpus N --decomp slabs with transport p2p -- sub_problem, SlabRank.step, exchange_dist with the pack / unpack
+# kernels, the all-reduced Joule total -- with every arithmetic step in the kernels' own code.)
+def _problem_for_slabs(thermal):
+    p = W.random_problem(21, 18, 13, seed=9400, steps=12, n_ports=25, bc=(0, 1, 0, 0, 0, 1), init_scale=4.0e6 if thermal else 1.0)
+    if thermal:
+        th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
+        p.thermal = th
+    return p
+
+
+def _emu_worker(rank, world, port, thermal, steps, out):
+    sys.path.insert(0, os.path.join(ROOT, "tests", "emu"))
+    import emu_em
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), EMU_THREADS="2")
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        s, meta = slabs.sub_problem(_problem_for_slabs(thermal), rank, world)
+        sr = slabs.SlabRank(emu_em.EmuEM(s, precision=64), meta, mode="p2p")
+        sr.step(steps, dist)
+        total = sr.joule_total(dist)
+        fields = sr.owned_fields()
+        extra = {"theta": sr.owned_theta()} if thermal else {}
+        np.savez(os.path.join(out, "r%d.npz" % rank), total=total, q=sr.owned_joule()[1], **{"f%d" % c: f for c, f in enumerate(fields)}, **extra)
+        dist.barrier()
+        sr.em.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,thermal", [(2, False), (3, True)])
+def test_real_kernels_under_the_gloo_exchange_equal_the_single_domain_run(world, thermal, tmp_path):
+    sys.path.insert(0, os.path.join(ROOT, "tests", "emu"))
+    import build_emu
+    import emu_em
+    build_emu.build_emu()                      # (before the workers start: they must not race to build it)
+    steps = 12
+    mp.spawn(_emu_worker, args=(world, _free_port(), thermal, steps, str(tmp_path)), nprocs=world, join=True)
+    p = _problem_for_slabs(thermal)
+    single = emu_em.EmuEM(p, precision=64)
+    single.em_step(steps)
+    fs = single.fields(); _, qs, Qs = single.joule_maps()
+    parts = [np.load(os.path.join(str(tmp_path), "r%d.npz" % r)) for r in range(world)]
+    for c in range(6):
+        assert np.array_equal(np.concatenate([pt["f%d" % c] for pt in parts], axis=0), fs[c]), c      # bit for bit
+    assert np.array_equal(np.concatenate([pt["q"] for pt in parts], axis=0), qs)
+    if thermal:
+        assert np.array_equal(np.concatenate([pt["theta"] for pt in parts], axis=0), single.em_get_temperature_rise())
+    for pt in parts:                                                                                     # all-reduced on every rank
+        assert abs(float(pt["total"]) - Qs) <= 1e-12 * abs(Qs) and Qs > 0
+    single.close()
