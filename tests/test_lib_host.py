@@ -135,3 +135,18 @@ def test_sweep_kernels_do_not_spill():
     # leapfrog: {float, double} x {CD, EXP} x {uniform mu, general} = 8; fp32 coupled x {CD, EXP} = 2;
     # fp64 coupled x {CD, EXP} = 2; E-only: double x {CD, EXP} x {umu, general} + float x CD x {umu, general} = 6
     assert seen == 18
+
+
+def test_product_library_has_no_emulation_in_it():
+    """tests/emu compiles the kernel sources against a CPU emulation of the CUDA primitives for checking; none of that may
+    leak into the product: libem.so exports no emu_* entry point, its build never defines EM_EMULATE, and nothing in the
+    package, bench.py or __graft_entry__.smoke() loads an emulated library."""
+    L = P.load()
+    for name in ("emu_alloc", "emu_free", "emu_launch_count", "emu_install_fault_handler"):
+        assert not hasattr(L, name)
+    build_py = open(os.path.join(ROOT, "paper_2603_07038_b200", "build.py")).read()
+    assert "EM_EMULATE" not in build_py
+    for rel in ("bench.py", os.path.join("paper_2603_07038_b200", "binding.py"), os.path.join("paper_2603_07038_b200", "slabs.py"),
+                os.path.join("paper_2603_07038_b200", "__init__.py"), os.path.join("paper_2603_07038_b200", "replicas.py")):
+        src = open(os.path.join(ROOT, rel)).read()
+        assert "emu_em" not in src and "libem_emu" not in src and "build_emu" not in src, rel
