@@ -290,3 +290,72 @@ def test_largest_material_table(emulated, precision, thermal):
         TT._run(p, 6, precision)
     else:
         TP.run_pair(p, 6, precision, P.EM_KERNEL_TMA, z_chunks=2)
+
+
+# ------------------------------------------------------------------------------------------- random-problem campaign
+def _campaign(seed, n_cases, max_cells):
+    """random grid shapes (degenerate ones included), walls, loss mode, precision, chunk count, port count, per-cell or
+    blocky ids, PEC material, thread schedule -- over the five kernel paths, each case against the oracle"""
+    rng = np.random.default_rng(seed)
+    done = 0
+    while done < n_cases:
+        big = rng.random() < 0.3
+        nx, ny, nz = int(rng.integers(1, 260 if big else 70)), int(rng.integers(1, 50 if big else 20)), int(rng.integers(1, 24))
+        if nx * ny * nz > max_cells:
+            continue
+        done += 1
+        bc = tuple(int(b) for b in (rng.random(6) < 0.35))
+        mode, precision = int(rng.integers(0, 2)), int(rng.choice([32, 64]))
+        variant = str(rng.choice(["leapfrog", "eonly", "coupled", "fc", "split"]))
+        zc, nports = int(rng.integers(0, 9)), (int(rng.integers(0, 12)) if nx * ny * nz > 8 else 0)
+        # (fp32 + exponential loss: from a RANDOM initial field inside a good conductor the first step cancels E to
+        # rounding level there, which the sigma-weighted power map p amplifies beyond 2 tol; from the second step on it
+        # does not -- and every configuration of BASELINE.json starts from zero fields or in vacuum)
+        steps = int(rng.integers(2 if (mode == 1 and precision == 32) else 1, 9))
+        case = dict(dims=(nx, ny, nz), bc=bc, mode=mode, precision=precision, variant=variant, z_chunks=zc, steps=steps, n_ports=nports,
+                    seed=int(rng.integers(0, 1 << 30)), emu_seed=int(rng.integers(0, 5)), percell=bool(rng.random() < 0.3), pec=bool(rng.random() < 0.3))
+        yield case
+
+
+def _run_case(case, monkeypatch):
+    monkeypatch.setenv("EMU_SEED", str(case["emu_seed"]))
+    thermal = case["variant"] in ("coupled", "fc")
+    p = W.random_problem(*case["dims"], seed=case["seed"], steps=case["steps"], n_ports=case["n_ports"], loss_mode=case["mode"], bc=case["bc"],
+                         blocky=not case["percell"], pec_material=case["pec"], init_scale=4.0e6 if thermal else 1.0)
+    kw = dict(z_chunks=case["z_chunks"])
+    if thermal:
+        th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
+        p.thermal = th
+        if case["variant"] == "fc":
+            kw.update(FC)
+    if case["variant"] == "split":
+        kw["kernel"] = P.EM_KERNEL_SPLIT
+    if case["variant"] == "eonly":
+        TE.run_pair(p, case["steps"], case["precision"], z_chunks=case["z_chunks"])
+        return
+    g = emu_em.EmuEM(p, precision=case["precision"], **kw)
+    o = emo.Oracle(p)
+    g.em_step(case["steps"]); o.step(case["steps"])
+    compare_state(g, o, TOL[case["precision"]])
+    if thermal:
+        assert rel_l2([g.em_get_temperature_rise()], [o.temperature_rise()]) <= TOL[case["precision"]]
+    g.close(); o.close()
+
+
+def test_random_problem_campaign(emulated, monkeypatch):
+    for case in _campaign(20261105, 80, 30000):
+        try:
+            _run_case(case, monkeypatch)
+        except Exception as e:
+            raise AssertionError("campaign case %r: %r" % (case, e))
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("seed", [1, 2, 3, 4])
+def test_random_problem_campaign_long(emulated, monkeypatch, seed):
+    """EM_RUN_SLOW=1: 4 x 1500 cases (profiles/r2_emulation.md records this round's run)"""
+    for case in _campaign(seed, 1500, 60000):
+        try:
+            _run_case(case, monkeypatch)
+        except Exception as e:
+            raise AssertionError("campaign case %r: %r" % (case, e))
