@@ -9,7 +9,9 @@
 
 namespace em {
 
-#define EM_LAUNCH(kernel, grid, block, smem, stream) ((void)(stream), emu::make_launcher(kernel, dim3(grid), dim3(block), (size_t)(smem), #kernel))
+// (launch_sweep_tma launches through a function pointer called `kern`: the instantiation selected at em_create)
+inline const char *kernel_label(const char *s) { return strcmp(s, "kern") == 0 ? "k_sweep_tma" : s; }
+#define EM_LAUNCH(kernel, grid, block, smem, stream) ((void)(stream), emu::make_launcher(kernel, dim3(grid), dim3(block), (size_t)(smem), em::kernel_label(#kernel)))
 #define EM_DYN_SMEM(name) unsigned char *name = emu::t_cur->cta->smem
 #define EM_FUZZ() emu::sync_point()
 
