@@ -75,8 +75,8 @@ typedef struct emo_ctx {
     double *eps_c;                 /* per-cell eps (from the table) */
     uint8_t *pec_c;                /* per-cell PEC-material flag */
     /* thermal coupling (eq. (4)-(6), L84-L96; NEXT-1 of SURVEY.md 8(f)); off unless emo_set_thermal */
-    int32_t thermal;
-    double *theta, *theta_n;       /* temperature rise T - T0 per cell, and the next level */
+    int32_t thermal;               /* 0 off, 1 theta per CELL (readings T1-T5), 2 theta per NODE (the paper's placement, N1-N4) */
+    double *theta, *theta_n;       /* temperature rise T - T0 per cell (thermal = 1) or per node (2), and the next level */
     double *dq;                    /* Joule energy density deposited in the current step [J/m^3] */
     double *sigma0_c, *rho_cp_c, *kth_c, *alpha_c;
     double *E[3], *H[3];           /* fields */
@@ -385,6 +385,73 @@ static void thermal_step(emo_ctx *c) {
     edge_coefficients(c);                               /* D_sigma(T^{n+1}) for the next step */
 }
 
+/* ---- the NODAL thermal stage: the paper's placement of T (7 092 878 thermal unknowns = the nodes of its
+ * 376 x 408 x 45 mesh) -- readings N1-N4 of DESIGN.md section 9, emo_set_thermal_nodal ----------------------------------
+ *   N1  theta on the (nx+1)(ny+1)(nz+1) mesh nodes.
+ *   N2  M_kk = V0a^T D_k V0 literally: V0 = node-to-edge difference over the edge length l_e (the negative
+ *       gradient), D_k = diag(k_e A~_e) with k_e A~_e = sum over the <= 4 cells round the edge of k_c A_{c,e} / 4 (the
+ *       area-weighted mean of C5 times the dual face, halved / quartered at the walls), V0a^T = the transposed
+ *       incidence over the node's dual volume.  In heat units: C_n dtheta_n/dt = -sum_{e at n} (k_e A~_e / l_e)
+ *       (theta_n - theta_m) + ..., C_n = sum over the <= 8 cells round the node of rho c_p V_c / 8.  No flux leaves
+ *       the mesh (adiabatic, L142).
+ *   N3  P_total = D_sigma e^2 (L86) is an EDGE vector: the energy the step dissipates on edge e,
+ *       dQ_e = dt Ebar_e^2 l_e sum_{c round e} sigma_c(T^n) A_{c,e} / 4  (time-centred Ebar = (E^{n+1} + E^n)/2; summed
+ *       over the edges this is exactly the dissipation of the discrete Poynting theorem and equals sum_c dq_c V_c of
+ *       a4), goes half to each end node.
+ *   N4  eq. (6) per cell with the mean of the cell's 8 node temperatures; everything else as T4. */
+static double edge_cells_sum(const emo_ctx *c, int comp, int i, int j, int k, const double *val) {
+    /* sum over the existing cells round edge (comp, i, j, k) of val_c * (cross-section of c normal to the edge) / 4 */
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    double s = 0.0;
+    for (int b = -1; b <= 0; ++b) for (int a = -1; a <= 0; ++a) {
+        int ci = i, cj = j, ck = k; double area;
+        if (comp == 0) { cj = j + a; ck = k + b; if (cj < 0 || cj >= ny || ck < 0 || ck >= nz) continue; area = c->dy[cj] * c->dz[ck]; }
+        else if (comp == 1) { ci = i + a; ck = k + b; if (ci < 0 || ci >= nx || ck < 0 || ck >= nz) continue; area = c->dx[ci] * c->dz[ck]; }
+        else { ci = i + a; cj = j + b; if (ci < 0 || ci >= nx || cj < 0 || cj >= ny) continue; area = c->dx[ci] * c->dy[cj]; }
+        s += val[CELL(ci, cj, ck)] * area / 4.0;
+    }
+    return s;
+}
+
+static void thermal_step_nodal(emo_ctx *c) {
+    const int nx = c->nx, ny = c->ny, nz = c->nz;
+    const double dt = c->dt;
+    const double *th = c->theta;
+    /* after one_step swapped them, E holds E^{n+1} and En holds E^n */
+#define NODE(i, j, k) IX(nx + 1, ny + 1, i, j, k)
+    int k;
+#pragma omp parallel for schedule(static)
+    for (k = 0; k <= nz; ++k) for (int j = 0; j <= ny; ++j) for (int i = 0; i <= nx; ++i) {
+        double out = 0.0, heat = 0.0, cap = 0.0;
+        /* the <= 6 edges at the node: (component, edge index, the node at its other end) */
+        for (int comp = 0; comp < 3; ++comp) for (int side = -1; side <= 0; ++side) {
+            int ei = i, ej = j, ek = k, mi = i, mj = j, mk = k; double len;
+            if (comp == 0) { ei = i + side; mi = i + (side ? -1 : 1); if (ei < 0 || ei >= nx) continue; len = c->dx[ei]; }
+            else if (comp == 1) { ej = j + side; mj = j + (side ? -1 : 1); if (ej < 0 || ej >= ny) continue; len = c->dy[ej]; }
+            else { ek = k + side; mk = k + (side ? -1 : 1); if (ek < 0 || ek >= nz) continue; len = c->dz[ek]; }
+            int sx, sy, sz; dims_of(c, comp, &sx, &sy, &sz);
+            const int64_t e = IX(sx, sy, ei, ej, ek);
+            out += edge_cells_sum(c, comp, ei, ej, ek, c->kth_c) / len * (th[NODE(i, j, k)] - th[NODE(mi, mj, mk)]);
+            const double eb = 0.5 * (c->E[comp][e] + c->En[comp][e]);
+            heat += 0.5 * dt * eb * eb * len * edge_cells_sum(c, comp, ei, ej, ek, c->sigma_c);
+        }
+        for (int dk = -1; dk <= 0; ++dk) for (int dj = -1; dj <= 0; ++dj) for (int di = -1; di <= 0; ++di) {
+            const int ci = i + di, cj = j + dj, ck = k + dk;
+            if (ci < 0 || ci >= nx || cj < 0 || cj >= ny || ck < 0 || ck >= nz) continue;
+            cap += c->rho_cp_c[CELL(ci, cj, ck)] * c->dx[ci] * c->dy[cj] * c->dz[ck] / 8.0;
+        }
+        c->theta_n[NODE(i, j, k)] = th[NODE(i, j, k)] - dt * out / cap + heat / cap;
+    }
+    { double *t = c->theta; c->theta = c->theta_n; c->theta_n = t; }
+    for (k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+        double m = 0.0;
+        for (int dk = 0; dk <= 1; ++dk) for (int dj = 0; dj <= 1; ++dj) for (int di = 0; di <= 1; ++di) m += c->theta[NODE(i + di, j + dj, k + dk)];
+        c->sigma_c[CELL(i, j, k)] = c->sigma0_c[CELL(i, j, k)] / (1.0 + c->alpha_c[CELL(i, j, k)] * (m / 8.0));      /* eq. (6) */
+    }
+#undef NODE
+    edge_coefficients(c);
+}
+
 /* One step n -> n+1 (SURVEY.md 8(c) "One step"): a1 H update, a3 source, a2 E update, a4 Joule. */
 static void one_step(emo_ctx *c) {
     const int nx = c->nx, ny = c->ny, nz = c->nz;
@@ -476,7 +543,8 @@ static void one_step(emo_ctx *c) {
             c->J[ed->comp][IX(sx, sy, ed->i, ed->j, ed->k)] = 0.0;
         }
     }
-    if (c->thermal) thermal_step(c);
+    if (c->thermal == 1) thermal_step(c);
+    if (c->thermal == 2) thermal_step_nodal(c);
     c->step += 1;
 }
 
@@ -539,7 +607,7 @@ int32_t emo_reset(emo_ctx *c) {
     memset(c->q, 0, sizeof(double) * (int64_t)c->nx * c->ny * c->nz);
     if (c->thermal) {
         const int64_t ncell = (int64_t)c->nx * c->ny * c->nz;
-        memset(c->theta, 0, sizeof(double) * ncell);
+        memset(c->theta, 0, sizeof(double) * (c->thermal == 2 ? (int64_t)(c->nx + 1) * (c->ny + 1) * (c->nz + 1) : ncell));
         memcpy(c->sigma_c, c->sigma0_c, sizeof(double) * ncell);
         edge_coefficients(c);
     }
@@ -554,30 +622,41 @@ typedef struct { double rho_cp, k, alpha; } emo_thermal_material;   /* J/(m^3 K)
 
 /* Switches the coupling on: per-material volumetric heat capacity, thermal conductivity and temperature coefficient
  * of resistance; theta = 0, sigma = sigma_0 (the table's).  rho_cp > 0, k >= 0 (0 = no conduction through the cell). */
-int32_t emo_set_thermal(emo_ctx *c, const emo_thermal_material *tt, int32_t n_mat) {
+static int32_t set_thermal_placed(emo_ctx *c, const emo_thermal_material *tt, int32_t n_mat, int32_t placement) {
     if (!c || !tt || n_mat < 1) return EMO_ERR_INVALID_ARG;
+    if (c->thermal && c->thermal != placement) return EMO_ERR_INVALID_ARG;      /* one placement per context */
     const int64_t ncell = (int64_t)c->nx * c->ny * c->nz;
+    const int64_t nth = placement == 2 ? (int64_t)(c->nx + 1) * (c->ny + 1) * (c->nz + 1) : ncell;
     for (int64_t q = 0; q < ncell; ++q) if (c->mat[q] >= n_mat) return EMO_ERR_INVALID_ARG;
     for (int m = 0; m < n_mat; ++m) if (!(tt[m].rho_cp > 0.0) || !(tt[m].k >= 0.0)) return EMO_ERR_INVALID_ARG;
     if (!c->thermal) {
-        c->theta = (double *)calloc(ncell, sizeof(double)); c->theta_n = (double *)calloc(ncell, sizeof(double));
+        c->theta = (double *)calloc(nth, sizeof(double)); c->theta_n = (double *)calloc(nth, sizeof(double));
         c->dq = (double *)calloc(ncell, sizeof(double));
         c->sigma0_c = (double *)malloc(sizeof(double) * ncell); c->rho_cp_c = (double *)malloc(sizeof(double) * ncell);
         c->kth_c = (double *)malloc(sizeof(double) * ncell); c->alpha_c = (double *)malloc(sizeof(double) * ncell);
         memcpy(c->sigma0_c, c->sigma_c, sizeof(double) * ncell);
-        c->thermal = 1;
+        c->thermal = placement;
     }
     for (int64_t q = 0; q < ncell; ++q) {
         c->rho_cp_c[q] = tt[c->mat[q]].rho_cp; c->kth_c[q] = tt[c->mat[q]].k; c->alpha_c[q] = tt[c->mat[q]].alpha;
-        c->theta[q] = 0.0; c->sigma_c[q] = c->sigma0_c[q];
+        c->sigma_c[q] = c->sigma0_c[q];
     }
+    memset(c->theta, 0, sizeof(double) * nth);
     edge_coefficients(c);
     return EMO_OK;
+}
+int32_t emo_set_thermal(emo_ctx *c, const emo_thermal_material *tt, int32_t n_mat) { return set_thermal_placed(c, tt, n_mat, 1); }
+/* the same with theta on the mesh NODES (the paper's placement; thermal_step_nodal above) */
+int32_t emo_set_thermal_nodal(emo_ctx *c, const emo_thermal_material *tt, int32_t n_mat) { return set_thermal_placed(c, tt, n_mat, 2); }
+/* number of temperature unknowns: cells (placement 1) or nodes (2); 0 if the coupling is off */
+int64_t emo_thermal_unknowns(const emo_ctx *c) {
+    if (!c || !c->thermal) return 0;
+    return c->thermal == 2 ? (int64_t)(c->nx + 1) * (c->ny + 1) * (c->nz + 1) : (int64_t)c->nx * c->ny * c->nz;
 }
 
 int32_t emo_get_temperature_rise(emo_ctx *c, double *dst) {
     if (!c || !dst || !c->thermal) return EMO_ERR_INVALID_ARG;
-    memcpy(dst, c->theta, sizeof(double) * (int64_t)c->nx * c->ny * c->nz);
+    memcpy(dst, c->theta, sizeof(double) * emo_thermal_unknowns(c));
     return EMO_OK;
 }
 
@@ -585,6 +664,19 @@ int32_t emo_get_temperature_rise(emo_ctx *c, double *dst) {
 int32_t emo_set_temperature_rise(emo_ctx *c, const double *src) {
     if (!c || !src || !c->thermal) return EMO_ERR_INVALID_ARG;
     const int64_t ncell = (int64_t)c->nx * c->ny * c->nz;
+    if (c->thermal == 2) {                    /* nodal: sigma(T) from the mean of the cell's 8 node temperatures (N4) */
+        const int nx = c->nx, ny = c->ny, nz = c->nz;
+        memcpy(c->theta, src, sizeof(double) * emo_thermal_unknowns(c));
+        for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+            double m = 0.0;
+            for (int dk = 0; dk <= 1; ++dk) for (int dj = 0; dj <= 1; ++dj) for (int di = 0; di <= 1; ++di)
+                m += c->theta[IX(nx + 1, ny + 1, i + di, j + dj, k + dk)];
+            if (!(1.0 + c->alpha_c[CELL(i, j, k)] * (m / 8.0) > 0.0)) return EMO_ERR_INVALID_ARG;
+            c->sigma_c[CELL(i, j, k)] = c->sigma0_c[CELL(i, j, k)] / (1.0 + c->alpha_c[CELL(i, j, k)] * (m / 8.0));
+        }
+        edge_coefficients(c);
+        return EMO_OK;
+    }
     for (int64_t q = 0; q < ncell; ++q) if (!(1.0 + c->alpha_c[q] * src[q] > 0.0)) return EMO_ERR_INVALID_ARG;
     memcpy(c->theta, src, sizeof(double) * ncell);
     for (int64_t q = 0; q < ncell; ++q) c->sigma_c[q] = c->sigma0_c[q] / (1.0 + c->alpha_c[q] * c->theta[q]);

@@ -146,8 +146,9 @@ class Oracle:
         if load_init and p.init:
             for comp, arr in p.init.items():
                 self.set_field(comp, arr)
+        self.nodal = False
         if getattr(p, "thermal", None) is not None:
-            self.set_thermal(p.thermal)
+            self.set_thermal(p.thermal, nodal=getattr(p, "thermal_placement", "cell") == "node")
 
     def close(self):
         if self._h:
@@ -226,15 +227,22 @@ class Oracle:
         lib().emo_reset(self._h)
 
     # ---- thermal coupling (NEXT-1; eq. (4)-(6)) --------------------------------------
-    def set_thermal(self, thermal):
-        """thermal: (n_mat, 3) float64 rows (rho_cp [J/m^3/K], k [W/m/K], alpha [1/K])"""
+    def set_thermal(self, thermal, nodal: bool = False):
+        """thermal: (n_mat, 3) float64 rows (rho_cp [J/m^3/K], k [W/m/K], alpha [1/K]); nodal: theta on the mesh nodes
+        (the paper's placement, readings N1-N4) instead of per cell (T1-T5)"""
         t = np.ascontiguousarray(thermal, np.float64)
-        rc = lib().emo_set_thermal(self._h, _dp(t), int(t.shape[0]))
+        fn = lib().emo_set_thermal_nodal if nodal else lib().emo_set_thermal
+        rc = fn(self._h, _dp(t), int(t.shape[0]))
         if rc:
             raise RuntimeError("emo_set_thermal rc=%d" % rc)
+        self.nodal = bool(nodal)
+
+    @property
+    def theta_shape(self):
+        return (self.nz + 1, self.ny + 1, self.nx + 1) if self.nodal else (self.nz, self.ny, self.nx)
 
     def temperature_rise(self) -> np.ndarray:
-        out = np.empty((self.nz, self.ny, self.nx), np.float64)
+        out = np.empty(self.theta_shape, np.float64)
         rc = lib().emo_get_temperature_rise(self._h, _dp(out))
         if rc:
             raise RuntimeError("emo_get_temperature_rise rc=%d" % rc)
@@ -242,7 +250,7 @@ class Oracle:
 
     def set_temperature_rise(self, theta):
         a = np.ascontiguousarray(theta, np.float64)
-        assert a.shape == (self.nz, self.ny, self.nx)
+        assert a.shape == self.theta_shape
         rc = lib().emo_set_temperature_rise(self._h, _dp(a))
         if rc:
             raise RuntimeError("emo_set_temperature_rise rc=%d" % rc)
