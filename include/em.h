@@ -90,8 +90,9 @@ typedef struct em_grid {
     int32_t max_ports;           /* capacity reserved in the workspace for em_set_source            */
     int64_t max_source_edges;
     int64_t max_wave_samples;
-    int32_t thermal;             /* 1: reserve workspace for the thermal stage (em_set_thermal): AUTO / TMA run */
-                                 /*    the coupled TMA sweep, SPLIT the split kernels                            */
+    int32_t thermal;             /* EM_THERMAL_CELL (1): reserve workspace for the thermal stage (em_set_thermal),  */
+                                 /*    theta per cell: AUTO / TMA run the coupled TMA sweep, SPLIT the split kernels; */
+                                 /* EM_THERMAL_NODE (2): theta on the mesh nodes, the paper's placement (split kernels) */
     int32_t formulation;         /* EM_FORM_LEAPFROG or EM_FORM_EONLY                                            */
     int32_t z_chunks;            /* 0: the library chooses how many z chunks a tile column is cut into (work     */
                                  /* items = tiles x chunks, from the SM count); 1..8 forces it (tests, tuning)   */
@@ -222,12 +223,23 @@ int32_t em_reset(em_ctx *ctx);
  * M_kk theta) and the coupled TMA sweep (sigma(T^n) staged as one more plane per step plane, Joule heat added to theta
  * and sigma(T^{n+1}) written in its Joule phase); kernel = SPLIT runs the same step on the split kernels.  Until
  * em_set_thermal is called such a context steps EM-only on the split kernels. */
+/* em_grid.thermal = EM_THERMAL_NODE -- the paper's OWN placement: theta on the (nx+1)(ny+1)(nz+1) mesh nodes (7 092 878
+ * on its mesh), dense [nz+1][ny+1][nx+1] maps in em_get / em_set_temperature_rise.  Readings N1-N4
+ * (DESIGN.md section 9): M_kk = V0a^T D_k V0 literally -- per edge the conductance k_e A~_e / l_e with k_e A~_e = the sum over the
+ * <= 4 cells round the edge of k_c A_{c,e} / 4 (the area-weighted mean of C5 times the dual face), nodal heat capacities C_n =
+ * sum over the <= 8 cells of rho c_p V_c / 8, adiabatic walls; the EDGE vector P = D_sigma e^2 (L86), as energy of the step
+ * dQ_e = dt Ebar_e^2 l_e sum_c sigma_c(T^n) A_{c,e} / 4, goes half to each end node (its total is the Joule map's, so EM
+ * loss == heat gained exactly); eq. (6) per cell with the mean of its 8 node temperatures.  Runs on the split kernels
+ * (kernel = AUTO or SPLIT; TMA: UNSUPPORTED); the z-slab halo calls cover the per-cell stage only. */
+#define EM_THERMAL_CELL 1
+#define EM_THERMAL_NODE 2
 typedef struct em_thermal_material { double rho_cp /* J/(m^3 K) > 0 */, k /* W/(m K) >= 0 */, alpha /* 1/K */; } em_thermal_material;
 
 /* Switches the coupling on (theta = 0).  table: HOST, n_mat entries (the n_mat of em_create).
  * Errors: STATE (ctx created with em_grid.thermal = 0), INVALID_ARG, CUDA. */
 int32_t em_set_thermal(em_ctx *ctx, const em_thermal_material *table, int32_t n_mat);
-/* theta out / in (in: also refreshes sigma(T)); device or host pointer; host copies synchronise.
+/* theta out / in (in: also refreshes sigma(T)); device or host pointer; host copies synchronise.  Dense [nz][ny][nx]
+ * (EM_THERMAL_CELL) or [nz+1][ny+1][nx+1] (EM_THERMAL_NODE) in the working precision.
  * Errors: STATE (coupling not switched on), INVALID_ARG, CUDA. */
 int32_t em_get_temperature_rise(em_ctx *ctx, void *dst, int32_t dst_is_device);
 int32_t em_set_temperature_rise(em_ctx *ctx, const void *src, int32_t src_is_device);

@@ -192,6 +192,16 @@ def _shapes(nx, ny, nz):
     return e + [(nz, ny, nx + 1), (nz, ny + 1, nx), (nz + 1, ny, nx)] + e     # 6..8: e^{n-1} (E-only contexts)
 
 
+EM_THERMAL_CELL, EM_THERMAL_NODE = 1, 2
+
+
+def _thermal_flag(p) -> int:
+    """em_grid.thermal of a problem: 0, per cell (p.thermal set), per node (p.thermal_placement == "node")"""
+    if getattr(p, "thermal", None) is None:
+        return 0
+    return EM_THERMAL_NODE if getattr(p, "thermal_placement", "cell") == "node" else EM_THERMAL_CELL
+
+
 class EM:
     """One em_ctx.  ``p`` is any object with the attributes of workloads.Problem (plain arrays)."""
 
@@ -222,7 +232,7 @@ class EM:
                               max_source_edges if max_source_edges is not None else max(n_con, 1),
                               max_wave_samples if max_wave_samples is not None else max(int(p.wave.shape[0]), 1),
                               tuple(bc) if bc is not None else tuple(getattr(p, "bc", (0,) * 6)),
-                              1 if getattr(p, "thermal", None) is not None else 0, formulation, z_chunks)
+                              _thermal_flag(p), formulation, z_chunks)
         self.formulation = int(formulation)
         nbytes = C.c_size_t()
         _check(self._L.em_workspace_bytes(C.byref(self._grid), C.byref(nbytes)), self._L)
@@ -376,8 +386,12 @@ class EM:
             arr[m].rho_cp, arr[m].k, arr[m].alpha = float(t[m, 0]), float(t[m, 1]), float(t[m, 2])
         _check(self._L.em_set_thermal(self._h, arr, int(t.shape[0])), self._L)
 
+    @property
+    def theta_shape(self):
+        return (self.nz + 1, self.ny + 1, self.nx + 1) if self._grid.thermal == EM_THERMAL_NODE else (self.nz, self.ny, self.nx)
+
     def em_get_temperature_rise(self, out=None, device: bool = False):
-        shape = (self.nz, self.ny, self.nx)
+        shape = self.theta_shape
         if device:
             t = out if out is not None else self._torch.empty(shape, dtype=self.dtype, device=self.device)
             _check(self._L.em_get_temperature_rise(self._h, C.c_void_p(t.data_ptr()), 1), self._L)
@@ -392,7 +406,7 @@ class EM:
             _check(self._L.em_set_temperature_rise(self._h, C.c_void_p(t.data_ptr()), 1), self._L)
             return
         a = np.ascontiguousarray(theta, self.np_dtype)
-        assert a.shape == (self.nz, self.ny, self.nx)
+        assert a.shape == self.theta_shape
         _check(self._L.em_set_temperature_rise(self._h, a.ctypes.data_as(C.c_void_p), 0), self._L)
 
     def em_step(self, n: int = 1):

@@ -251,6 +251,8 @@ struct Ctx final : em_ctx {
     void *ws_base = nullptr;
     R *peer_dst[2][2][2] = {};          // [side][parity of the neighbour's E array][comp]
     int32_t step_thermal();
+    int32_t step_thermal_nodal();
+    bool nodal = false;                 // em_grid.thermal = EM_THERMAL_NODE: theta on the mesh nodes (split kernels)
     int32_t step_thermal_sweep();
     int sg_cur = 0;                     // which sigma(T) buffer is current (the coupled sweep ping-pongs them)
     R *sig_buf(int which) const { return (which ? c.sig2 : c.sig) + g.origin; }
@@ -297,7 +299,9 @@ int32_t validate_grid(const em_grid *g) {
     if (g->precision != 32 && g->precision != 64) return fail(EM_ERR_INVALID_ARG, "precision must be 32 or 64");
     if (g->loss_mode != EM_LOSS_CD && g->loss_mode != EM_LOSS_EXP) return fail(EM_ERR_INVALID_ARG, "bad loss_mode");
     if (g->kernel < EM_KERNEL_AUTO || g->kernel > EM_KERNEL_TMA) return fail(EM_ERR_INVALID_ARG, "bad kernel strategy");
-    if (g->thermal != 0 && g->thermal != 1) return fail(EM_ERR_INVALID_ARG, "thermal must be 0 or 1");
+    if (g->thermal < 0 || g->thermal > EM_THERMAL_NODE) return fail(EM_ERR_INVALID_ARG, "thermal must be 0, 1 (per cell) or 2 (per node)");
+    if (g->thermal == EM_THERMAL_NODE && g->kernel == EM_KERNEL_TMA)
+        return fail(EM_ERR_UNSUPPORTED, "the nodal thermal stage runs on the split kernels");
     if (g->formulation != EM_FORM_LEAPFROG && g->formulation != EM_FORM_EONLY) return fail(EM_ERR_INVALID_ARG, "bad formulation");
     if (g->formulation == EM_FORM_EONLY && (g->thermal || g->kernel == EM_KERNEL_SPLIT))
         return fail(EM_ERR_UNSUPPORTED, "the E-only recurrence runs on the TMA sweep, without thermal coupling");
@@ -345,7 +349,9 @@ int32_t Ctx<R>::init(const em_grid *gr, const uint8_t *mat_id, const em_material
     n_mat_ = n_mat;
     // thermal coupling: the coupled TMA sweep (sigma(T) planes staged beside the ids) or, if its shared-memory layout
     // does not fit / on request, the split kernels (em_thermal.cuh)
-    if (gr->thermal) {
+    nodal = gr->thermal == EM_THERMAL_NODE;
+    if (nodal) kernel = EM_KERNEL_SPLIT;                 // (theta on the mesh nodes: em_thermal.cuh k_thermal_nodal)
+    if (gr->thermal && !nodal) {
         sweep_smem = em::sweep_smem_bytes((int)sizeof(R), n_mat + 2, true);
         if (kernel == EM_KERNEL_AUTO) kernel = EM_KERNEL_TMA;
     }
@@ -704,6 +710,7 @@ int32_t Ctx<R>::get_field(int32_t comp, void *dst, int32_t is_dev) {
 template <typename R>
 int32_t Ctx<R>::halo(int32_t kp, int32_t kl, void *dst, const void *srcp, void *st) {
     if (eonly) return fail(EM_ERR_UNSUPPORTED, "the halo calls cover the leapfrog formulation");
+    if (nodal) return fail(EM_ERR_UNSUPPORTED, "the halo calls cover the per-cell thermal stage");
     if (kp < 0 || kp > g.nz) return fail(EM_ERR_INVALID_ARG, "halo: node plane out of range");
     if (thermal_on && (kl < 0 || kl >= g.nz)) return fail(EM_ERR_INVALID_ARG, "halo: cell layer out of range");
     cudaStream_t s = st ? static_cast<cudaStream_t>(st) : stream;
@@ -801,6 +808,13 @@ template <typename R>
 int32_t Ctx<R>::refresh_sigma() {
     dim3 b(32, 8);
     em::ThermalParams<R> t = tp();
+    if (nodal) {
+        EM_LAUNCH(em::k_sigma_nodal<R>, node_grid(b, 0), b, 0, stream)(p, t);
+        t.sig = sig_buf(1 - sg_cur);
+        EM_LAUNCH(em::k_sigma_nodal<R>, node_grid(b, 0), b, 0, stream)(p, t);
+        CU(cudaGetLastError());
+        return EM_OK;
+    }
     EM_LAUNCH(em::k_sigma_refresh<R>, node_grid(b, 0), b, 0, stream)(p, t);
     t.sig = sig_buf(1 - sg_cur);                        // both buffers: the coupled sweep rewrites only the lossy lanes
     EM_LAUNCH(em::k_sigma_refresh<R>, node_grid(b, 0), b, 0, stream)(p, t);
@@ -839,14 +853,16 @@ int32_t Ctx<R>::temperature_rise(void *dst, const void *srcp, int32_t is_dev) {
     if (!thermal_on) return fail(EM_ERR_STATE, "thermal coupling is not switched on (em_set_thermal)");
     R *th = c.theta[th_cur] + g.origin;
     cudaMemcpy3DParms m = {};
-    m.extent = make_cudaExtent(sizeof(R) * g.nx, g.ny, g.nz);
+    const int ex = nodal ? 1 : 0;                         // nodal: dense [nz+1][ny+1][nx+1] maps
+    const size_t tx = (size_t)g.nx + ex, ty = (size_t)g.ny + ex, tz = (size_t)g.nz + ex;
+    m.extent = make_cudaExtent(sizeof(R) * tx, ty, tz);
     if (dst) {
         m.srcPtr = make_cudaPitchedPtr(th, sizeof(R) * g.PX, g.PX, g.PY);
-        m.dstPtr = make_cudaPitchedPtr(dst, sizeof(R) * g.nx, g.nx, g.ny);
+        m.dstPtr = make_cudaPitchedPtr(dst, sizeof(R) * tx, tx, ty);
         m.kind = is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
         CU(cudaMemcpy3DAsync(&m, stream));
     } else {
-        m.srcPtr = make_cudaPitchedPtr(const_cast<void *>(srcp), sizeof(R) * g.nx, g.nx, g.ny);
+        m.srcPtr = make_cudaPitchedPtr(const_cast<void *>(srcp), sizeof(R) * tx, tx, ty);
         m.dstPtr = make_cudaPitchedPtr(th, sizeof(R) * g.PX, g.PX, g.PY);
         m.kind = is_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
         CU(cudaMemcpy3DAsync(&m, stream));
@@ -878,6 +894,36 @@ int32_t Ctx<R>::step_thermal() {
     launches += 1;
     CU(cudaGetLastError());
     e_cur ^= 1; th_cur ^= 1; bind();
+    return EM_OK;
+}
+
+// One coupled step with theta on the mesh NODES (em_grid.thermal = EM_THERMAL_NODE; readings N1-N4): a1, a2 with
+// D_sigma(T^n), a3, a4 into the per-cell Joule map, then eq. (5) on the nodes (edge heat split between the end nodes, edge
+// conductances, nodal capacities) and eq. (6) per cell from the mean of its 8 node temperatures.
+template <typename R>
+int32_t Ctx<R>::step_thermal_nodal() {
+    dim3 b(32, 8);
+    const R *sig = sig_buf(sg_cur);
+    EM_LAUNCH(em::k_split_h<R>, node_grid(b, 1), b, 0, stream)(p);
+    int32_t rc = record_begin(); if (rc) return rc;
+    if (loss == EM_LOSS_CD) EM_LAUNCH((em::k_split_e_sig<R, 0>), node_grid(b, 1), b, 0, stream)(p, sig);
+    else                    EM_LAUNCH((em::k_split_e_sig<R, 1>), node_grid(b, 1), b, 0, stream)(p, sig);
+    rc = record_end(); if (rc) return rc;
+    launches += 2;
+    if (n_unique) {
+        const int gs = (n_unique + 127) / 128;
+        if (loss == EM_LOSS_CD) EM_LAUNCH((em::k_source_coef_sig<R, 0>), gs, 128, 0, stream)(p, src, sig);
+        else                    EM_LAUNCH((em::k_source_coef_sig<R, 1>), gs, 128, 0, stream)(p, src, sig);
+        EM_LAUNCH(em::k_apply_source<R>, gs, 128, 0, stream)(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
+        launches += 2;
+    }
+    EM_LAUNCH(em::k_joule_sig<R>, node_grid(b, 0), b, 0, stream)(p, sig);
+    EM_LAUNCH(em::k_thermal_nodal<R>, node_grid(b, 1), b, 0, stream)(p, tp(), c.vx, c.vy, c.vz);
+    th_cur ^= 1;
+    EM_LAUNCH(em::k_sigma_nodal<R>, node_grid(b, 0), b, 0, stream)(p, tp());          // sigma(T^{n+1}) from the new theta
+    launches += 3;
+    CU(cudaGetLastError());
+    e_cur ^= 1; bind();
     return EM_OK;
 }
 
@@ -933,7 +979,7 @@ template <typename R>
 int32_t Ctx<R>::step(int64_t n) {
     if (n < 0) return fail(EM_ERR_INVALID_ARG, "n < 0");
     for (int64_t s = 0; s < n; ++s) {
-        int32_t rc = thermal_on ? (kernel == EM_KERNEL_TMA ? step_thermal_sweep() : step_thermal())
+        int32_t rc = thermal_on ? (nodal ? step_thermal_nodal() : kernel == EM_KERNEL_TMA ? step_thermal_sweep() : step_thermal())
                    : grid.thermal ? step_split()            // (tile geometry of the coupled sweep: EM-only steps run split)
                    : kernel == EM_KERNEL_TMA ? step_tma() : step_split();
         if (rc) return rc;

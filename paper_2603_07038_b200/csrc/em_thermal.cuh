@@ -214,6 +214,113 @@ __global__ void __launch_bounds__(256) k_diffuse(DevParams<R> p, const ThEntry<R
     }
 }
 
+// ---- NODAL thermal stage: the paper's placement of T (7 092 878 thermal unknowns = the mesh nodes; eq.
+// (4)-(6) L84-L96, M_kk = V0a^T D_k V0 L86; readings N1-N4 of DESIGN.md section 9; em_grid.thermal = 2, split kernels) ------
+// a4 with the per-cell sigma(T^n): q_c += dt sigma_c / 16 sum_12 (E' + E)^2 (the Joule map stays per cell, C7)
+template <typename R>
+__global__ void __launch_bounds__(256) k_joule_sig(DevParams<R> p, const R *sig) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= p.nx || j >= p.ny) return;
+    const long long PX = p.PX, PXY = p.PXY;
+    const long long o = ((long long)k * p.PY + j) * PX + i;
+    const R sg = sig[o];
+    if (sg == R(0)) return;
+    R s = 0;
+#define EM_ACC(c, off) { const R t_ = p.En[c][o + (off)] + p.E[c][o + (off)]; s = mad(t_, t_, s); }
+    EM_ACC(0, 0) EM_ACC(0, PX) EM_ACC(0, PXY) EM_ACC(0, PXY + PX)
+    EM_ACC(1, 0) EM_ACC(1, 1)  EM_ACC(1, PXY) EM_ACC(1, PXY + 1)
+    EM_ACC(2, 0) EM_ACC(2, 1)  EM_ACC(2, PX)  EM_ACC(2, PX + 1)
+#undef EM_ACC
+    p.q[o] = mad(p.dt * sg * R(0.0625), s, p.q[o]);
+}
+
+// eq. (5) on the nodes.  One thread per node n = (i, j, k):
+//   C_n theta_n' = C_n theta_n - dt sum_{e at n} (k_e A~_e / l_e) (theta_n - theta_m) + 1/2 sum_{e at n} dQ_e
+//   k_e A~_e = sum over the <= 4 cells round e of k_c A_{c,e} / 4,   dQ_e = dt Ebar_e^2 l_e sum_c sigma_c(T^n) A_{c,e} / 4,
+//   C_n = sum over the <= 8 cells round n of rho c_p V_c / 8.
+// Cells outside the grid contribute nothing by themselves: their table entries hold k = 0 and 1/(rho c_p) = 0, their
+// sigma(T) is 0 and their sizes read as 0 (vx, vy, vz are the cell sizes in fp64, length nx, ny, nz).
+template <typename R>
+__global__ void __launch_bounds__(256) k_thermal_nodal(DevParams<R> p, ThermalParams<R> t, const double *vx, const double *vy, const double *vz) {
+    __shared__ ThEntry<R> s_th[kMaxTable];
+    {
+        const int tid = threadIdx.y * blockDim.x + threadIdx.x, nth = blockDim.x * blockDim.y;
+        for (int m = tid; m < p.n_table; m += nth) s_th[m] = t.ttable[m];
+        __syncthreads();
+    }
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i > p.nx || j > p.ny) return;
+    const long long PX = p.PX, PXY = p.PXY;
+    const long long o = ((long long)k * p.PY + j) * PX + i;
+    const long long stride[3] = {1, PX, PXY};
+    const int node[3] = {i, j, k}, n[3] = {p.nx, p.ny, p.nz};
+    const double *vv[3] = {vx, vy, vz};
+    auto size = [&](int a, int c) -> R { return (c >= 0 && c < n[a]) ? (R)vv[a][c] : R(0); };
+    // sizes of the two cell layers below (index 0) and above (1) the node along every axis
+    R d[3][2];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { d[a][0] = size(a, node[a] - 1); d[a][1] = size(a, node[a]); }
+    const R th0 = t.theta[o];
+    R out = R(0), heat = R(0), cap = R(0);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {                        // edges along axis a; b, c: the two transverse axes
+        const int b = (a + 1) % 3, c = (a + 2) % 3;
+#pragma unroll
+        for (int side = 0; side < 2; ++side) {           // the edge below (0) / above (1) the node
+            const R len = d[a][side];
+            if (len == R(0)) continue;
+            const long long oe = side ? o : o - stride[a];                       // the edge is indexed by its lower node
+            const long long om = side ? o + stride[a] : o - stride[a];           // the node at its other end
+            R ka = R(0), sa = R(0);                                               // sum k_c A / 4, sum sigma_c A / 4
+#pragma unroll
+            for (int sb = 0; sb < 2; ++sb)
+#pragma unroll
+                for (int sc = 0; sc < 2; ++sc) {
+                    const R area = d[b][sb] * d[c][sc] * R(0.25);
+                    if (area == R(0)) continue;
+                    const long long oc = oe - (sb ? 0 : stride[b]) - (sc ? 0 : stride[c]);   // cell (edge cell along a, b - 1 + sb, c - 1 + sc)
+                    ka = mad(s_th[p.mat[oc]].k, area, ka);
+                    sa = mad(t.sig[oc], area, sa);
+                }
+            out = mad(ka * rcp<R>(len), th0 - t.theta[om], out);
+            const R eb = R(0.5) * (p.E[a][oe] + p.En[a][oe]);
+            heat = mad(R(0.5) * p.dt * eb * eb * len, sa, heat);
+        }
+    }
+#pragma unroll
+    for (int sa_ = 0; sa_ < 2; ++sa_)
+#pragma unroll
+        for (int sb = 0; sb < 2; ++sb)
+#pragma unroll
+            for (int sc = 0; sc < 2; ++sc) {
+                const R vol = d[0][sa_] * d[1][sb] * d[2][sc] * R(0.125);
+                if (vol == R(0)) continue;
+                const long long oc = o - (sa_ ? 0 : 1) - (sb ? 0 : PX) - (sc ? 0 : PXY);
+                const R irc = s_th[p.mat[oc]].irc;
+                if (irc > R(0)) cap = mad(rcp<R>(irc), vol, cap);
+            }
+    t.theta_n[o] = cap > R(0) ? th0 + (heat - p.dt * out) * rcp<R>(cap) : th0;
+}
+
+// eq. (6) per cell with the mean of the cell's 8 node temperatures (N4)
+template <typename R>
+__global__ void __launch_bounds__(256) k_sigma_nodal(DevParams<R> p, ThermalParams<R> t) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= p.nx || j >= p.ny) return;
+    const long long PX = p.PX, PXY = p.PXY;
+    const long long o = ((long long)k * p.PY + j) * PX + i;
+    const ThEntry<R> me = t.ttable[p.mat[o]];
+    const R m = ((t.theta[o] + t.theta[o + 1]) + (t.theta[o + PX] + t.theta[o + PX + 1])) +
+                ((t.theta[o + PXY] + t.theta[o + PXY + 1]) + (t.theta[o + PXY + PX] + t.theta[o + PXY + PX + 1]));
+    t.sig[o] = me.sigma0 * rcp<R>(thermal_den(me.alpha, R(0.125) * m));
+}
+
 // sigma = sigma_0 / (1 + alpha theta) on every cell (after em_set_thermal / em_set_temperature_rise / em_reset)
 template <typename R>
 __global__ void __launch_bounds__(256) k_sigma_refresh(DevParams<R> p, ThermalParams<R> t) {

@@ -56,7 +56,7 @@ class EmuEM(B.EM):
                                 max_source_edges if max_source_edges is not None else max(n_con, 1),
                                 max_wave_samples if max_wave_samples is not None else max(int(p.wave.shape[0]), 1),
                                 tuple(bc) if bc is not None else tuple(getattr(p, "bc", (0,) * 6)),
-                                1 if getattr(p, "thermal", None) is not None else 0, formulation, z_chunks)
+                                B._thermal_flag(p), formulation, z_chunks)
         self.formulation = int(formulation)
         nbytes = C.c_size_t()
         self._check(self._L.em_workspace_bytes(C.byref(self._grid), C.byref(nbytes)))

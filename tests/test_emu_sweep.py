@@ -120,7 +120,7 @@ def test_api_contract_and_probe(emulated):
     TP.test_probe_matches_fields()
 
 
-@pytest.mark.parametrize("what", ["leapfrog-fp32", "e-only-fp64", "coupled-fp32", "split-fp64"])
+@pytest.mark.parametrize("what", ["leapfrog-fp32", "e-only-fp64", "coupled-fp32", "split-fp64", "coupled-nodal-fp64"])
 def test_checkpoint_resume_and_check_finite(emulated, what):
     TP.test_checkpoint_resume_is_bit_exact_and_check_finite(what)
 
@@ -181,6 +181,17 @@ def test_coupled_package_slice(emulated, variant):
     p = W.make_config(4, scale=16, zscale=4, steps=16)
     p.thermal = W.thermal_table()
     TT._run(p, 16, 32)
+
+
+# ------------------------------------------------ nodal thermal stage (theta on the mesh nodes, the paper's placement)
+@pytest.mark.parametrize("dims,mode,precision", TT.NODAL_CASES)
+def test_nodal_coupled_random_grids(emulated, dims, mode, precision):
+    TT.test_nodal_coupled_random_grids(dims, mode, precision)
+
+
+def test_nodal_pmc_walls_diffusion_api_and_paper_mesh(emulated):
+    TT.test_nodal_with_pmc_walls_diffusion_and_api()
+    TT.test_nodal_paper_mesh_unknown_count_and_package_slice()
 
 
 def test_coupled_split_kernels(emulated):
@@ -306,7 +317,7 @@ def _campaign(seed, n_cases, max_cells):
         done += 1
         bc = tuple(int(b) for b in (rng.random(6) < 0.35))
         mode, precision = int(rng.integers(0, 2)), int(rng.choice([32, 64]))
-        variant = str(rng.choice(["leapfrog", "eonly", "coupled", "fc", "split"]))
+        variant = str(rng.choice(["leapfrog", "eonly", "coupled", "fc", "split", "nodal"]))
         zc, nports = int(rng.integers(0, 9)), (int(rng.integers(0, 12)) if nx * ny * nz > 8 else 0)
         # (fp32 + exponential loss: from a RANDOM initial field inside a good conductor the first step cancels E to
         # rounding level there, which the sigma-weighted power map p amplifies beyond 2 tol; from the second step on it
@@ -319,7 +330,9 @@ def _campaign(seed, n_cases, max_cells):
 
 def _run_case(case, monkeypatch):
     monkeypatch.setenv("EMU_SEED", str(case["emu_seed"]))
-    thermal = case["variant"] in ("coupled", "fc")
+    thermal = case["variant"] in ("coupled", "fc", "nodal")
+    if case["variant"] == "nodal" and case["precision"] == 32 and min(case["dims"]) < 3:
+        case = dict(case, precision=64)          # (split-kernel Joule sum in fp32 on degenerate grids: tests/test_gpu_thermal.py NODAL_CASES)
     p = W.random_problem(*case["dims"], seed=case["seed"], steps=case["steps"], n_ports=case["n_ports"], loss_mode=case["mode"], bc=case["bc"],
                          blocky=not case["percell"], pec_material=case["pec"], init_scale=4.0e6 if thermal else 1.0)
     kw = dict(z_chunks=case["z_chunks"])
@@ -328,6 +341,8 @@ def _run_case(case, monkeypatch):
         p.thermal = th
         if case["variant"] == "fc":
             kw.update(FC)
+        if case["variant"] == "nodal":
+            p.thermal_placement = "node"
     if case["variant"] == "split":
         kw["kernel"] = P.EM_KERNEL_SPLIT
     if case["variant"] == "eonly":

@@ -343,7 +343,7 @@ def _full_state(g):
     return [ck["fields"][c] for c in sorted(ck["fields"])] + [ck["q"]] + ([ck["theta"]] if "theta" in ck else [])
 
 
-@pytest.mark.parametrize("what", ["leapfrog-fp32", "e-only-fp64", "coupled-fp32", "split-fp64"])
+@pytest.mark.parametrize("what", ["leapfrog-fp32", "e-only-fp64", "coupled-fp32", "split-fp64", "coupled-nodal-fp64"])
 def test_checkpoint_resume_is_bit_exact_and_check_finite(what):
     """state = fields + q + step index (+ theta): a run interrupted after 5 of 12 steps and resumed in a NEW context
     continues bit for bit (the step index selects the waveform samples; q and theta are accumulators)"""
@@ -357,6 +357,8 @@ def test_checkpoint_resume_is_bit_exact_and_check_finite(what):
     if what.startswith("coupled"):
         th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
         p.thermal = th
+        if "nodal" in what:
+            p.thermal_placement = "node"
     ref = P.EM(p, precision=precision, **kw)
     ref.em_step(12)
     a = P.EM(p, precision=precision, **kw)

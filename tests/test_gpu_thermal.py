@@ -110,3 +110,56 @@ def test_thermal_needs_flag_and_a_coupled_strategy():
     p.thermal = bad
     with pytest.raises(P.EMError):
         P.EM(p)                                               # alpha must be finite
+
+
+# ---- the NODAL thermal stage: theta on the mesh nodes, the paper's placement (em_grid.thermal = EM_THERMAL_NODE; N1-N4) ----
+def _nodal(p):
+    p.thermal_placement = "node"
+    return p
+
+
+# fp32 on the non-degenerate grids only: the nodal stage runs on the SPLIT kernels, whose Joule sum adds the stored E' and E
+# (the sweep forms E' + E without cancellation); from a random initial field inside a good conductor, where the CD update
+# gives E' = -E + small, that costs fp32 a factor ~40 in q on the first steps (1 x 5 x 7: 8 of 20 seeds beyond 2e-5, for the
+# per-cell split path exactly as for the nodal one).  fp64 covers every shape.
+NODAL_CASES = [((37, 29, 23), LOSS_CD, 64), ((37, 29, 23), LOSS_CD, 32), ((9, 7, 6), LOSS_EXP, 64), ((9, 7, 6), LOSS_EXP, 32),
+               ((130, 3, 2), LOSS_CD, 64), ((1, 5, 7), LOSS_CD, 64), ((2, 2, 2), LOSS_CD, 64), ((33, 65, 4), LOSS_CD, 32)]
+
+
+@pytest.mark.parametrize("dims,mode,precision", NODAL_CASES)
+def test_nodal_coupled_random_grids(dims, mode, precision):
+    p = _nodal(_coupled(dims, 8600 + sum(dims), loss_mode=mode, steps=60, n_ports=3 if min(dims) > 1 else 0, init_scale=4.0e6))
+    res, theta = _run(p, 60, precision, checkpoints=(1, 10))
+    assert theta.shape == (dims[2] + 1, dims[1] + 1, dims[0] + 1)
+    if min(dims) > 2:
+        assert np.abs(p.thermal[:, 2]).max() * np.abs(theta).max() > 1e-3        # the feedback is not below the tolerance
+
+
+def test_nodal_with_pmc_walls_diffusion_and_api():
+    p = _nodal(_coupled((21, 18, 12), 8601, steps=40, n_ports=4, init_scale=4.0e6, bc=(1, 1, 0, 1, 1, 1)))
+    _run(p, 40, 64, checkpoints=(1,))
+    # pure diffusion from a random nodal temperature, set / get / reset
+    p = _nodal(_coupled((12, 9, 8), 8602, steps=30, n_ports=0, lossless=True))
+    p.init = None
+    th0 = np.random.default_rng(9).uniform(0.0, 1.0, size=(p.nz + 1, p.ny + 1, p.nx + 1))
+    for precision in (64, 32):
+        g = P.EM(p, precision=precision); o = emo.Oracle(p)
+        g.em_set_temperature_rise(th0); o.set_temperature_rise(th0)
+        g.em_step(30); o.step(30)
+        to = o.temperature_rise()
+        assert np.linalg.norm(to - th0) > 1e-3 * np.linalg.norm(th0)
+        assert rel_l2([g.em_get_temperature_rise()], [to]) <= TOL[precision]
+        g.em_reset()
+        assert not np.any(g.em_get_temperature_rise())
+        g.close(); o.close()
+    with pytest.raises(P.EMError) as e:
+        P.EM(p, kernel=P.EM_KERNEL_TMA)                       # the nodal stage runs on the split kernels
+    assert e.value.code == 5
+
+
+def test_nodal_paper_mesh_unknown_count_and_package_slice():
+    """config 6 scaled: (nx+1)(ny+1)(nz+1) temperature unknowns (full size: 377 x 409 x 46 = 7 092 878)"""
+    p = _nodal(W.make_config(6, scale=8, steps=40))
+    p.thermal = W.thermal_table()
+    res, theta = _run(p, 40, 32)
+    assert theta.size == (p.nx + 1) * (p.ny + 1) * (p.nz + 1) and 377 * 409 * 46 == 7092878
