@@ -217,7 +217,8 @@ int32_t em_reset(em_ctx *ctx);
  * adiabatic walls (L142).  NOTE -- a deviation from the paper's placement: the paper solves T on the mesh NODES
  * (7 092 878 unknowns on its 376x408x45 mesh) and does not print its edge-to-node map of D_sigma e^2;
  * here theta lives per CELL (6 903 360 unknowns on that mesh), where the Joule heat is defined (T1, T3), so
- * the coupled numbers quoted for this library are for that cell-centred variant of eq. (4)-(5).
+ * the coupled numbers quoted for this library are for that cell-centred variant of eq. (4)-(5); em_grid.thermal =
+ * EM_THERMAL_NODE (below) selects the paper's nodal placement instead.
  * Valid range: 1 + alpha theta > 0 (copper: theta > -256 K); below it sigma(T) is clamped at sigma_0 / 1e-6.  sigma_0 = the em_material.sigma given to em_create.  em_joule's power density then uses
  * the current sigma(T).  em_reset also zeroes theta.  Per step: one conduction kernel (theta^n -> theta - dt/(rho c_p)
  * M_kk theta) and the coupled TMA sweep (sigma(T^n) staged as one more plane per step plane, Joule heat added to theta
