@@ -122,16 +122,17 @@ __global__ void k_source_coef(DevParams<R> p, DevSources<R> s, int *fixed_flags)
     const long long PX = p.PX, PXY = p.PXY;
     const long long kk = o / PXY, rem = o - kk * PXY;   // o >= 0 for in-range edges
     const int j = (int)(rem / PX), i = (int)(rem - (long long)j * PX), k = (int)kk;
-    R r[3], sg[3];
-    edge_coeffs<R, LOSS>(p.table, p.mat, o, PX, PXY, p.fx[i], p.fy[j], p.fz[k], r, sg);
+    R r[3], sg[3], h2[3];
+    edge_coeffs<R, LOSS>(p.table, p.mat, o, PX, PXY, p.fx[i], p.fy[j], p.fz[k], r, sg, h2);
     const R re = r[s.comp[u]];
     s.r[u] = re;
     fixed_flags[u] = (re == R(0)) ? 1 : 0;
 }
 
 // a3 -- E^{n+1} -= r_e * J_e^{n+1/2}   ("-dt^2 (dJ/dt)^n")
+// (t0..t2: the E' + E arrays of the split strategy, which carry the same -r_e J)
 template <typename R>
-__global__ void k_apply_source(R *e0, R *e1, R *e2, DevSources<R> s, long long step) {
+__global__ void k_apply_source(R *e0, R *e1, R *e2, R *t0, R *t1, R *t2, DevSources<R> s, long long step) {
     const int u = blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= s.n_unique) return;
     R J = 0;
@@ -141,6 +142,8 @@ __global__ void k_apply_source(R *e0, R *e1, R *e2, DevSources<R> s, long long s
     }
     R *e = s.comp[u] == 0 ? e0 : (s.comp[u] == 1 ? e1 : e2);
     e[s.off[u]] = mad(-s.r[u], J, e[s.off[u]]);
+    R *t = s.comp[u] == 0 ? t0 : (s.comp[u] == 1 ? t1 : t2);
+    t[s.off[u]] = mad(-s.r[u], J, t[s.off[u]]);
 }
 
 // p_c = sigma_c * 1/4 sum_12 (E_e)^2 into a dense [nz][ny][nx] map

@@ -31,7 +31,7 @@ struct DevParams {
     int PX, PY;              // pitches (elements)
     long long PXY;           // plane stride
     R *E[3], *En[3];         // E^n and E^{n+1} (ping-pong)
-    R *H[3], *Hn[3];         // H^{n-1/2} and H^{n+1/2} (ping-pong, fused sweep only; split: Hn == H)
+    R *H[3], *Hn[3];         // H^{n-1/2} and H^{n+1/2} (ping-pong in the sweep; split: H in place, Hn carries E' + E to the Joule kernels)
     R *q;                    // Joule energy density accumulator
     const uint8_t *mat;      // material ids, same geometry
     const MatEntry<R> *table;// n_table entries in global memory

@@ -793,7 +793,7 @@ int32_t Ctx<R>::step_split() {
     rc = record_end(); if (rc) return rc;
     launches += 2;
     if (n_unique) {
-        EM_LAUNCH(em::k_apply_source<R>, (n_unique + 127) / 128, 128, 0, stream)(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
+        EM_LAUNCH(em::k_apply_source<R>, (n_unique + 127) / 128, 128, 0, stream)(p.En[0], p.En[1], p.En[2], p.Hn[0], p.Hn[1], p.Hn[2], src, (long long)step_index);
         launches += 1;
     }
     EM_LAUNCH(em::k_split_joule<R>, node_grid(b, 0), b, 0, stream)(p);
@@ -887,7 +887,7 @@ int32_t Ctx<R>::step_thermal() {
         const int gs = (n_unique + 127) / 128;
         if (loss == EM_LOSS_CD) EM_LAUNCH((em::k_source_coef_sig<R, 0>), gs, 128, 0, stream)(p, src, sig);
         else                    EM_LAUNCH((em::k_source_coef_sig<R, 1>), gs, 128, 0, stream)(p, src, sig);
-        EM_LAUNCH(em::k_apply_source<R>, gs, 128, 0, stream)(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
+        EM_LAUNCH(em::k_apply_source<R>, gs, 128, 0, stream)(p.En[0], p.En[1], p.En[2], p.Hn[0], p.Hn[1], p.Hn[2], src, (long long)step_index);
         launches += 2;
     }
     EM_LAUNCH(em::k_joule_thermal<R>, node_grid(b, 0), b, 0, stream)(p, tp());
@@ -914,7 +914,7 @@ int32_t Ctx<R>::step_thermal_nodal() {
         const int gs = (n_unique + 127) / 128;
         if (loss == EM_LOSS_CD) EM_LAUNCH((em::k_source_coef_sig<R, 0>), gs, 128, 0, stream)(p, src, sig);
         else                    EM_LAUNCH((em::k_source_coef_sig<R, 1>), gs, 128, 0, stream)(p, src, sig);
-        EM_LAUNCH(em::k_apply_source<R>, gs, 128, 0, stream)(p.En[0], p.En[1], p.En[2], src, (long long)step_index);
+        EM_LAUNCH(em::k_apply_source<R>, gs, 128, 0, stream)(p.En[0], p.En[1], p.En[2], p.Hn[0], p.Hn[1], p.Hn[2], src, (long long)step_index);
         launches += 2;
     }
     EM_LAUNCH(em::k_joule_sig<R>, node_grid(b, 0), b, 0, stream)(p, sig);

@@ -45,11 +45,13 @@ __global__ void __launch_bounds__(256) k_split_h(DevParams<R> p) {
     p.H[2][o] -= nbz * ((eyi - ey) * rdx - (exj - ex) * rdy);
 }
 
-// Edge coefficients (r, sigma_bar) of the three edges at node (i,j,k) from the 7 surrounding cells.
+// Edge coefficients (r, sigma_bar) of the three edges at node (i,j,k) from the 7 surrounding cells, and h2 = 2 - r sigma_bar
+// formed WITHOUT cancellation (CD: 2 (eps/dt) r): E' + E = r (C_h H' - J) + h2 E is what the Joule sum needs, and in a good
+// conductor (CD: E' = -E + small) adding the stored E' and E instead loses the digits in fp32.
 template <typename R, int LOSS>
 __device__ __forceinline__ void edge_coeffs(const MatEntry<R> *tab, const uint8_t *mat, long long o,
                                             long long PX, long long PXY, R fx, R fy, R fz,
-                                            R r[3], R sg[3]) {
+                                            R r[3], R sg[3], R h2[3]) {
     const MatEntry<R> c000 = tab[mat[o]], c100 = tab[mat[o - 1]], c010 = tab[mat[o - PX]];
     const MatEntry<R> c110 = tab[mat[o - PX - 1]], c001 = tab[mat[o - PXY]];
     const MatEntry<R> c101 = tab[mat[o - PXY - 1]], c011 = tab[mat[o - PXY - PX]];
@@ -58,21 +60,24 @@ __device__ __forceinline__ void edge_coeffs(const MatEntry<R> *tab, const uint8_
         const R A = lerp(lerp(c011.a, c001.a, fy), lerp(c010.a, c000.a, fy), fz);
         const R B = lerp(lerp(c011.b, c001.b, fy), lerp(c010.b, c000.b, fy), fz);
         const R m = (c011.m * c001.m) * (c010.m * c000.m);
-        r[0] = m * loss_r<R, LOSS>(A, B); sg[0] = B;
+        const R rr = loss_r<R, LOSS>(A, B);
+        r[0] = m * rr; sg[0] = B; h2[0] = (LOSS == 0) ? R(2) * A * rr : R(2) - rr * B;
     }
     // Ey: cells (i-1..i, j, k-1..k)
     {
         const R A = lerp(lerp(c101.a, c001.a, fx), lerp(c100.a, c000.a, fx), fz);
         const R B = lerp(lerp(c101.b, c001.b, fx), lerp(c100.b, c000.b, fx), fz);
         const R m = (c101.m * c001.m) * (c100.m * c000.m);
-        r[1] = m * loss_r<R, LOSS>(A, B); sg[1] = B;
+        const R rr = loss_r<R, LOSS>(A, B);
+        r[1] = m * rr; sg[1] = B; h2[1] = (LOSS == 0) ? R(2) * A * rr : R(2) - rr * B;
     }
     // Ez: cells (i-1..i, j-1..j, k)
     {
         const R A = lerp(lerp(c110.a, c010.a, fx), lerp(c100.a, c000.a, fx), fy);
         const R B = lerp(lerp(c110.b, c010.b, fx), lerp(c100.b, c000.b, fx), fy);
         const R m = (c110.m * c010.m) * (c100.m * c000.m);
-        r[2] = m * loss_r<R, LOSS>(A, B); sg[2] = B;
+        const R rr = loss_r<R, LOSS>(A, B);
+        r[2] = m * rr; sg[2] = B; h2[2] = (LOSS == 0) ? R(2) * A * rr : R(2) - rr * B;
     }
 }
 
@@ -87,8 +92,8 @@ __global__ void __launch_bounds__(256) k_split_e(DevParams<R> p) {
     if (i > p.nx || j > p.ny) return;
     const long long PX = p.PX, PXY = p.PXY;
     const long long o = ((long long)k * p.PY + j) * PX + i;
-    R r[3], sg[3];
-    edge_coeffs<R, LOSS>(s_tab, p.mat, o, PX, PXY, p.fx[i], p.fy[j], p.fz[k], r, sg);
+    R r[3], sg[3], h2[3];
+    edge_coeffs<R, LOSS>(s_tab, p.mat, o, PX, PXY, p.fx[i], p.fy[j], p.fz[k], r, sg, h2);
     const R hx = p.H[0][o], hxj = p.H[0][o - PX], hxk = p.H[0][o - PXY];
     const R hy = p.H[1][o], hyi = p.H[1][o - 1], hyk = p.H[1][o - PXY];
     const R hz = p.H[2][o], hzi = p.H[2][o - 1], hzj = p.H[2][o - PX];
@@ -100,6 +105,10 @@ __global__ void __launch_bounds__(256) k_split_e(DevParams<R> p) {
     p.En[0][o] = mad(r[0], mad(-sg[0], ex, cx), ex);
     p.En[1][o] = mad(r[1], mad(-sg[1], ey, cy), ey);
     p.En[2][o] = mad(r[2], mad(-sg[2], ez, cz), ez);
+    // E' + E for the Joule kernels, in the arrays the split strategy does not use otherwise (H is updated in place)
+    p.Hn[0][o] = mad(r[0], cx, h2[0] * ex);
+    p.Hn[1][o] = mad(r[1], cy, h2[1] * ey);
+    p.Hn[2][o] = mad(r[2], cz, h2[2] * ez);
 }
 
 // a4 -- PAPER.md L86 (P = D_sigma e^2), SURVEY.md 8(c) a4/C7 (time-centred, cell-centred).
@@ -116,7 +125,7 @@ __global__ void __launch_bounds__(256) k_split_joule(DevParams<R> p) {
     const R sig = s_tab[p.mat[o]].b;
     if (sig == R(0)) return;                    // sigma_c = 0: q_c never changes
     R s = 0;
-#define EM_ACC(c, off) { const R t_ = p.En[c][o + (off)] + p.E[c][o + (off)]; s = mad(t_, t_, s); }
+#define EM_ACC(c, off) { const R t_ = p.Hn[c][o + (off)]; s = mad(t_, t_, s); }      /* E' + E as k_split_e formed it */
     EM_ACC(0, 0) EM_ACC(0, PX) EM_ACC(0, PXY) EM_ACC(0, PXY + PX)
     EM_ACC(1, 0) EM_ACC(1, 1)  EM_ACC(1, PXY) EM_ACC(1, PXY + 1)
     EM_ACC(2, 0) EM_ACC(2, 1)  EM_ACC(2, PX)  EM_ACC(2, PX + 1)

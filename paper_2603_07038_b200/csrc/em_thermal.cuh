@@ -26,7 +26,7 @@ struct ThermalParams {
 // Edge coefficients with the per-cell sigma array instead of the table's sigma (same arithmetic as edge_coeffs).
 template <typename R, int LOSS>
 __device__ __forceinline__ void edge_coeffs_sig(const MatEntry<R> *tab, const uint8_t *mat, const R *sig, long long o,
-                                                long long PX, long long PXY, R fx, R fy, R fz, R r[3], R sg[3]) {
+                                                long long PX, long long PXY, R fx, R fy, R fz, R r[3], R sg[3], R h2[3]) {
     const MatEntry<R> c000 = tab[mat[o]], c100 = tab[mat[o - 1]], c010 = tab[mat[o - PX]];
     const MatEntry<R> c110 = tab[mat[o - PX - 1]], c001 = tab[mat[o - PXY]];
     const MatEntry<R> c101 = tab[mat[o - PXY - 1]], c011 = tab[mat[o - PXY - PX]];
@@ -36,19 +36,22 @@ __device__ __forceinline__ void edge_coeffs_sig(const MatEntry<R> *tab, const ui
         const R A = lerp(lerp(c011.a, c001.a, fy), lerp(c010.a, c000.a, fy), fz);
         const R B = lerp(lerp(b011, b001, fy), lerp(b010, b000, fy), fz);
         const R m = (c011.m * c001.m) * (c010.m * c000.m);
-        r[0] = m * loss_r<R, LOSS>(A, B); sg[0] = B;
+        const R rr = loss_r<R, LOSS>(A, B);
+        r[0] = m * rr; sg[0] = B; h2[0] = (LOSS == 0) ? R(2) * A * rr : R(2) - rr * B;
     }
     {   // Ey: cells (i-1..i, j, k-1..k)
         const R A = lerp(lerp(c101.a, c001.a, fx), lerp(c100.a, c000.a, fx), fz);
         const R B = lerp(lerp(b101, b001, fx), lerp(b100, b000, fx), fz);
         const R m = (c101.m * c001.m) * (c100.m * c000.m);
-        r[1] = m * loss_r<R, LOSS>(A, B); sg[1] = B;
+        const R rr = loss_r<R, LOSS>(A, B);
+        r[1] = m * rr; sg[1] = B; h2[1] = (LOSS == 0) ? R(2) * A * rr : R(2) - rr * B;
     }
     {   // Ez: cells (i-1..i, j-1..j, k)
         const R A = lerp(lerp(c110.a, c010.a, fx), lerp(c100.a, c000.a, fx), fy);
         const R B = lerp(lerp(b110, b010, fx), lerp(b100, b000, fx), fy);
         const R m = (c110.m * c010.m) * (c100.m * c000.m);
-        r[2] = m * loss_r<R, LOSS>(A, B); sg[2] = B;
+        const R rr = loss_r<R, LOSS>(A, B);
+        r[2] = m * rr; sg[2] = B; h2[2] = (LOSS == 0) ? R(2) * A * rr : R(2) - rr * B;
     }
 }
 
@@ -63,8 +66,8 @@ __global__ void __launch_bounds__(256) k_split_e_sig(DevParams<R> p, const R *si
     if (i > p.nx || j > p.ny) return;
     const long long PX = p.PX, PXY = p.PXY;
     const long long o = ((long long)k * p.PY + j) * PX + i;
-    R r[3], sg[3];
-    edge_coeffs_sig<R, LOSS>(s_tab, p.mat, sig, o, PX, PXY, p.fx[i], p.fy[j], p.fz[k], r, sg);
+    R r[3], sg[3], h2[3];
+    edge_coeffs_sig<R, LOSS>(s_tab, p.mat, sig, o, PX, PXY, p.fx[i], p.fy[j], p.fz[k], r, sg, h2);
     const R hx = p.H[0][o], hxj = p.H[0][o - PX], hxk = p.H[0][o - PXY];
     const R hy = p.H[1][o], hyi = p.H[1][o - 1], hyk = p.H[1][o - PXY];
     const R hz = p.H[2][o], hzi = p.H[2][o - 1], hzj = p.H[2][o - PX];
@@ -76,6 +79,9 @@ __global__ void __launch_bounds__(256) k_split_e_sig(DevParams<R> p, const R *si
     p.En[0][o] = mad(r[0], mad(-sg[0], ex, cx), ex);
     p.En[1][o] = mad(r[1], mad(-sg[1], ey, cy), ey);
     p.En[2][o] = mad(r[2], mad(-sg[2], ez, cz), ez);
+    p.Hn[0][o] = mad(r[0], cx, h2[0] * ex);               // E' + E without cancellation (em_split.cuh edge_coeffs)
+    p.Hn[1][o] = mad(r[1], cy, h2[1] * ey);
+    p.Hn[2][o] = mad(r[2], cz, h2[2] * ez);
 }
 
 // r_e of every unique source edge with the current sigma(T^n): recomputed every step in the coupled mode.
@@ -87,8 +93,8 @@ __global__ void k_source_coef_sig(DevParams<R> p, DevSources<R> s, const R *sig)
     const long long PX = p.PX, PXY = p.PXY;
     const long long kk = o / PXY, rem = o - kk * PXY;
     const int j = (int)(rem / PX), i = (int)(rem - (long long)j * PX), k = (int)kk;
-    R r[3], sg[3];
-    edge_coeffs_sig<R, LOSS>(p.table, p.mat, sig, o, PX, PXY, p.fx[i], p.fy[j], p.fz[k], r, sg);
+    R r[3], sg[3], h2[3];
+    edge_coeffs_sig<R, LOSS>(p.table, p.mat, sig, o, PX, PXY, p.fx[i], p.fy[j], p.fz[k], r, sg, h2);
     s.r[u] = r[s.comp[u]];
 }
 
@@ -113,7 +119,7 @@ __global__ void __launch_bounds__(256) k_joule_thermal(DevParams<R> p, ThermalPa
     R dq = R(0);
     if (sig != R(0)) {
         R s = 0;
-#define EM_ACC(c, off) { const R t_ = p.En[c][o + (off)] + p.E[c][o + (off)]; s = mad(t_, t_, s); }
+#define EM_ACC(c, off) { const R t_ = p.Hn[c][o + (off)]; s = mad(t_, t_, s); }      /* E' + E as k_split_e_sig formed it */
         EM_ACC(0, 0) EM_ACC(0, PX) EM_ACC(0, PXY) EM_ACC(0, PXY + PX)
         EM_ACC(1, 0) EM_ACC(1, 1)  EM_ACC(1, PXY) EM_ACC(1, PXY + 1)
         EM_ACC(2, 0) EM_ACC(2, 1)  EM_ACC(2, PX)  EM_ACC(2, PX + 1)
@@ -228,7 +234,7 @@ __global__ void __launch_bounds__(256) k_joule_sig(DevParams<R> p, const R *sig)
     const R sg = sig[o];
     if (sg == R(0)) return;
     R s = 0;
-#define EM_ACC(c, off) { const R t_ = p.En[c][o + (off)] + p.E[c][o + (off)]; s = mad(t_, t_, s); }
+#define EM_ACC(c, off) { const R t_ = p.Hn[c][o + (off)]; s = mad(t_, t_, s); }      /* E' + E as k_split_e_sig formed it */
     EM_ACC(0, 0) EM_ACC(0, PX) EM_ACC(0, PXY) EM_ACC(0, PXY + PX)
     EM_ACC(1, 0) EM_ACC(1, 1)  EM_ACC(1, PXY) EM_ACC(1, PXY + 1)
     EM_ACC(2, 0) EM_ACC(2, 1)  EM_ACC(2, PX)  EM_ACC(2, PX + 1)
@@ -287,7 +293,7 @@ __global__ void __launch_bounds__(256) k_thermal_nodal(DevParams<R> p, ThermalPa
                     sa = mad(t.sig[oc], area, sa);
                 }
             out = mad(ka * rcp<R>(len), th0 - t.theta[om], out);
-            const R eb = R(0.5) * (p.E[a][oe] + p.En[a][oe]);
+            const R eb = R(0.5) * p.Hn[a][oe];                                    // (E' + E) / 2 as k_split_e_sig formed it
             heat = mad(R(0.5) * p.dt * eb * eb * len, sa, heat);
         }
     }

@@ -18,6 +18,7 @@ inline const char *kernel_label(const char *s) { return strcmp(s, "kern") == 0 ?
 template <typename T> inline void st_stream16(void *dst, const T &v) {
     static_assert(sizeof(T) == 16, "16-byte vectors only");
     emu::check_global(dst, 16, 16, "st.global.cs.v4");
+    emu::traffic_counters()[3].fetch_add(16, std::memory_order_relaxed);
     memcpy(dst, &v, 16);
 }
 inline float rcp_approx(float x) { return 1.0f / x; }
@@ -28,6 +29,7 @@ inline void cp_async_n(void *smem_dst, const void *gsrc, int n) {
     emu::Fiber *f = emu::t_cur;
     emu::check_smem(smem_dst, n, n, "cp.async");
     emu::check_global(gsrc, n, n, "cp.async");
+    emu::traffic_counters()[2].fetch_add(n, std::memory_order_relaxed);
     f->copies.push_back(emu::Fiber::Copy{smem_dst, gsrc, n, f->open_group});
 }
 inline void cp_async16(void *d, const void *s) { cp_async_n(d, s, 16); }
@@ -120,6 +122,7 @@ inline void bulk_load(unsigned dst, const void *src, unsigned bytes, unsigned ba
     unsigned char *d = emu::u32_to_smem(dst, bytes, 16, "cp.async.bulk (destination)");
     emu::check_global(src, bytes, 16, "cp.async.bulk (source)");
     MBar *b = mbar_at(bar, "cp.async.bulk (mbarrier)");
+    emu::traffic_counters()[1].fetch_add(bytes, std::memory_order_relaxed);
     const std::shared_ptr<emu::RaceAsync> ra = emu::race_async_issue();
     const void *pc = __builtin_return_address(0);
     c->async.push_back(emu::AsyncOp{async_delay(c), [=]() {
@@ -146,6 +149,7 @@ inline void tma_load_3d(unsigned dst, const CUtensorMap *map, unsigned bar, int 
             if (hi[a] < lo[a]) any = false;
         }
         if (any) {
+            emu::traffic_counters()[0].fetch_add((long long)(hi[0] - lo[0] + 1) * (hi[1] - lo[1] + 1) * (hi[2] - lo[2] + 1) * m.esz, std::memory_order_relaxed);
             const char *first = m.base + lo[2] * (long long)m.strides[1] + lo[1] * (long long)m.strides[0] + lo[0] * m.esz;
             const char *last = m.base + hi[2] * (long long)m.strides[1] + hi[1] * (long long)m.strides[0] + hi[0] * m.esz;
             emu::check_global(first, m.esz, 1, "cp.async.bulk.tensor (source, first element)");

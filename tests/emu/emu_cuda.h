@@ -426,6 +426,9 @@ struct LaunchError { std::mutex m; std::string msg; };
 inline LaunchError &launch_error() { static LaunchError e; return e; }
 inline long env_long(const char *name, long dflt) { const char *v = getenv(name); return v && *v ? atol(v) : dflt; }
 inline std::atomic<long> &launch_counter() { static std::atomic<long> n{0}; return n; }
+// bytes the kernels REQUEST from / send to global memory through the copy engines and the streaming stores (what the L2
+// sees before any caching): [0] TMA boxes (the part inside the tensor), [1] bulk copies, [2] cp.async, [3] streaming stores
+inline std::atomic<long long> *traffic_counters() { static std::atomic<long long> c[4]; return c; }
 inline std::map<const void *, size_t> &func_smem() { static std::map<const void *, size_t> m; return m; }
 constexpr size_t kSmemOptin = 232448;                       // 227 KB: sm_100 per-block opt-in limit
 constexpr size_t kSmemDefault = 48 * 1024;

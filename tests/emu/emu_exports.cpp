@@ -116,6 +116,8 @@ void emu_free(void *ptr, size_t bytes) {
 }
 
 long emu_launch_count(void) { return emu::launch_counter().load(); }
+// reads (and clears) the requested-traffic counters of emu_cuda.h: TMA, bulk, cp.async, streaming stores [bytes]
+void emu_traffic(long long out[4]) { for (int q = 0; q < 4; ++q) out[q] = emu::traffic_counters()[q].exchange(0); }
 
 // ---- the hooks a -fsanitize=thread build of the kernels calls on every load and store (libtsan is NOT linked: this is
 // the emulation's own happens-before race detector for the dynamic shared memory, emu_cuda.h "racecheck") -------------

@@ -331,8 +331,6 @@ def _campaign(seed, n_cases, max_cells):
 def _run_case(case, monkeypatch):
     monkeypatch.setenv("EMU_SEED", str(case["emu_seed"]))
     thermal = case["variant"] in ("coupled", "fc", "nodal")
-    if case["variant"] == "nodal" and case["precision"] == 32 and min(case["dims"]) < 3:
-        case = dict(case, precision=64)          # (split-kernel Joule sum in fp32 on degenerate grids: tests/test_gpu_thermal.py NODAL_CASES)
     p = W.random_problem(*case["dims"], seed=case["seed"], steps=case["steps"], n_ports=case["n_ports"], loss_mode=case["mode"], bc=case["bc"],
                          blocky=not case["percell"], pec_material=case["pec"], init_scale=4.0e6 if thermal else 1.0)
     kw = dict(z_chunks=case["z_chunks"])

@@ -118,12 +118,8 @@ def _nodal(p):
     return p
 
 
-# fp32 on the non-degenerate grids only: the nodal stage runs on the SPLIT kernels, whose Joule sum adds the stored E' and E
-# (the sweep forms E' + E without cancellation); from a random initial field inside a good conductor, where the CD update
-# gives E' = -E + small, that costs fp32 a factor ~40 in q on the first steps (1 x 5 x 7: 8 of 20 seeds beyond 2e-5, for the
-# per-cell split path exactly as for the nodal one).  fp64 covers every shape.
-NODAL_CASES = [((37, 29, 23), LOSS_CD, 64), ((37, 29, 23), LOSS_CD, 32), ((9, 7, 6), LOSS_EXP, 64), ((9, 7, 6), LOSS_EXP, 32),
-               ((130, 3, 2), LOSS_CD, 64), ((1, 5, 7), LOSS_CD, 64), ((2, 2, 2), LOSS_CD, 64), ((33, 65, 4), LOSS_CD, 32)]
+NODAL_CASES = [(d, m, pr) for d, m in (((37, 29, 23), LOSS_CD), ((9, 7, 6), LOSS_EXP), ((130, 3, 2), LOSS_CD), ((1, 5, 7), LOSS_CD),
+                                        ((2, 2, 2), LOSS_CD), ((33, 65, 4), LOSS_CD)) for pr in (64, 32)]
 
 
 @pytest.mark.parametrize("dims,mode,precision", NODAL_CASES)
