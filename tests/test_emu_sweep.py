@@ -212,6 +212,11 @@ def test_thermally_coupled_slabs(emulated, variant):
     TS.test_thermally_coupled_slabs(P.EM_KERNEL_AUTO, 64)
 
 
+def test_slabs_split_kernels(emulated):
+    TS.test_slabs_equal_single_domain(3, P.EM_KERNEL_SPLIT, "p2p", 32)
+    TS.test_thermally_coupled_slabs(P.EM_KERNEL_SPLIT, 64)
+
+
 def test_peer_halo_argument_errors(emulated):
     TS.test_peer_halo_argument_errors()
 
