@@ -54,10 +54,15 @@ def parse():
     ap.add_argument("--halo", default="peer", choices=["peer", "p2p"],
                     help="slabs: halo stores fused into the sweep over a CUDA IPC / NVLink peer mapping + one tiny all-reduce "
                          "per step (default), or pack kernel -> NCCL send/recv -> unpack kernel")
+    ap.add_argument("--thermal-nodal", action="store_true",
+                    help="--thermal with theta on the mesh NODES (the paper's placement, em_grid.thermal = EM_THERMAL_NODE; split kernels)")
     ap.add_argument("--thermal", action="store_true",
                     help="two-way EM-thermal coupling (PAPER.md eq. (4)-(6)) with the handbook-order thermal table")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
-    return ap.parse_args()
+    args = ap.parse_args()
+    if args.thermal_nodal:
+        args.thermal = True
+    return args
 
 
 # ------------------------------------------------------------------------------------------------
@@ -129,6 +134,8 @@ def make_problem(args):
     p = W.make_config(1) if args.config == 1 else W.make_config(args.config, scale=args.scale, **kw)
     if getattr(args, "thermal", False):
         p.thermal = W.thermal_table(p.table.shape[0])
+        if getattr(args, "thermal_nodal", False):
+            p.thermal_placement = "node"
     return p
 
 
@@ -143,6 +150,8 @@ def cpu_oracle_rate(args, seconds: float):
     p = W.make_config(args.config, scale=scale, **kw) if args.config != 1 else W.make_config(1)
     if getattr(args, "thermal", False):
         p.thermal = W.thermal_table(p.table.shape[0])
+        if getattr(args, "thermal_nodal", False):
+            p.thermal_placement = "node"
     o = emo.Oracle(p)
     o.step(1)                                        # warm the pages
     t0 = time.perf_counter(); n = 0
@@ -380,7 +389,8 @@ def run_b200(args):
         avg_ms = step_ms
         if kname.startswith("k_split"):
             kname = "split step: k_split_h + %s + %s" % ("k_split_e_sig" if args.thermal else "k_split_e",
-                                                         "k_joule_thermal" if args.thermal else "k_split_joule")
+                                                         "k_joule_sig + k_thermal_nodal + k_sigma_nodal" if getattr(args, "thermal_nodal", False)
+                                                         else "k_joule_thermal" if args.thermal else "k_split_joule")
         else:
             kname = "coupled step: k_diffuse + k_sweep_tma<TH> (sweep alone %.3f ms)" % (kms / max(klaunch, 1))
     roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -410,7 +420,8 @@ def run_b200(args):
                                + (", E-only three-level recurrence of eq. (2)" if form == P.EM_FORM_EONLY else "")
                                + (", %d Joule-map output(s) inside each timed repetition of %d steps (one output = %.2f ms, "
                                   "i.e. +%.3f ms/step at the config's cadence)" % (outputs[0], K, out_ms, out_ms / je) if je else "")
-                               + (", two-way thermal coupling (%s)" % ("split kernels" if args.kernel == "split" else "coupled TMA sweep + conduction kernel") if args.thermal else ""),
+                               + (", two-way thermal coupling (%s)" % ("theta on the mesh nodes, split kernels" if getattr(args, "thermal_nodal", False) else
+                                                                      "split kernels" if args.kernel == "split" else "coupled TMA sweep + conduction kernel") if args.thermal else ""),
                    "kernel_strategy": args.kernel, "l2": "state %.1f GB >> 126 MB L2 (no flush needed)" % (em.workspace_bytes / 1e9)
                    if em.workspace_bytes > 1e9 else "state fits L2: %.0f MB" % (em.workspace_bytes / 1e6),
                    "parallelism": ("z-slabs x%d, halo per step: %s" % (world, "Ex, Ey wall planes stored by the sweep into the "

@@ -19,7 +19,7 @@ import emu_em                              # noqa: E402
 
 
 def report(config, scale, zscale, steps, precision=32, **kw):
-    p = W.make_config(config, scale=scale, zscale=zscale, steps=steps)
+    p = W.make_config(config, scale=scale, steps=steps, **({"zscale": zscale} if zscale != 1 else {}))
     g = emu_em.EmuEM(p, precision=precision, **kw)
     out = (C.c_longlong * 4)()
     g._L.emu_traffic(out)                  # clear what the set-up moved
