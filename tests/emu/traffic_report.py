@@ -18,8 +18,10 @@ import workloads as W                      # noqa: E402
 import emu_em                              # noqa: E402
 
 
-def report(config, scale, zscale, steps, precision=32, **kw):
+def report(config, scale, zscale, steps, precision=32, thermal=False, **kw):
     p = W.make_config(config, scale=scale, steps=steps, **({"zscale": zscale} if zscale != 1 else {}))
+    if thermal:
+        p.thermal = W.thermal_table(p.table.shape[0])
     g = emu_em.EmuEM(p, precision=precision, **kw)
     out = (C.c_longlong * 4)()
     g._L.emu_traffic(out)                  # clear what the set-up moved
@@ -28,12 +30,18 @@ def report(config, scale, zscale, steps, precision=32, **kw):
     cells = p.nx * p.ny * p.nz * steps
     tma, bulk, cpa, st = (out[q] / cells for q in range(4))
     print("config %d %dx%dx%d fp%d %s: TMA %.2f + bulk %.3f + cp.async %.2f = %.2f B read, %.2f B stored per cell-update; total %.2f B "
-          "(algorithmic %d)" % (config, p.nx, p.ny, p.nz, precision, kw or "", tma, bulk, cpa, tma + bulk + cpa, st, tma + bulk + cpa + st,
+          "(algorithmic %d)" % (config, p.nx, p.ny, p.nz, precision, ("coupled " if thermal else "") + (kw.get("tag", "") or ""), tma, bulk, cpa, tma + bulk + cpa, st, tma + bulk + cpa + st,
                                 57 if precision == 32 else 113))
     g.close()
 
 
 if __name__ == "__main__":
-    args = [int(a) for a in sys.argv[1:]] or [4, 4, 1, 2]
+    flags = [a for a in sys.argv[1:] if a.startswith("--")]
+    args = [int(a) for a in sys.argv[1:] if not a.startswith("--")] or [4, 4, 1, 2]
     for q in range(0, len(args), 4):
-        report(*args[q:q + 4])
+        if "--thermal" in flags:          # the coupled sweep (k_diffuse's plain loads and stores are not counted) and the fused one
+            import build_emu
+            report(*args[q:q + 4], thermal=True)
+            report(*args[q:q + 4], thermal=True, tag="fc", defines=build_emu.VARIANTS["fc"])
+        else:
+            report(*args[q:q + 4])
