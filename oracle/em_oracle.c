@@ -28,7 +28,10 @@
  * doubled domain, quarter-wave closed form, energy and Poynting balance with mixed walls, dense eq. (2)-(3)).
  * Thermal stage (NEXT-1: PAPER.md eq. (4)-(6)) -- emo_set_thermal & co. at the end of this file -- is pinned by
  * tests/test_oracle_thermal.py (adiabatic scalar recurrence + exact energy balance, cosine-mode diffusion closed form,
- * heat conservation == Joule energy, dense V0a^T D_k V0).
+ * heat conservation == Joule energy, dense V0a^T D_k V0); its NODAL variant (the paper's placement of T, emo_set_thermal_nodal,
+ * thermal_step_nodal) by tests/test_oracle_thermal_nodal.py (the paper's printed DOF count, the dense B^T diag(k A~/l) B
+ * assembled cell by cell, the DCT-I cosine-mode decay, the adiabatic scalar recurrence with the wall nodes, heat gained ==
+ * Joule energy per step).
  * No function here is "parity unpinned".
  */
 #include <math.h>
