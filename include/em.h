@@ -181,7 +181,10 @@ int32_t em_set_halo(em_ctx *ctx, int32_t k_plane, int32_t k_layer, const void *s
  * E'x, E'y of its node plane k_send there, and no longer stores its own wall plane on that side (the neighbour feeds it).
  * Both contexts must step in lockstep (same number of steps since em_create / em_reset) with one cross-rank barrier
  * between steps; dst = NULL switches the side off.  Leapfrog TMA sweep only, no thermal coupling (UNSUPPORTED).
- * Errors: INVALID_ARG, STATE (the wall on that side is not an artificial PMC wall), UNSUPPORTED. */
+ * The four addresses must be 16-byte aligned (the sweep writes them with 16-byte vector stores; a workspace base from
+ * cudaMalloc / cudaIpcOpenMemHandle plus em_wall_offset always is).
+ * Errors: INVALID_ARG (side, k_send, a null or misaligned address), STATE (the wall on that side is not an artificial
+ * PMC wall), UNSUPPORTED. */
 int32_t em_wall_offset(em_ctx *ctx, int32_t side, int32_t parity, int32_t comp, size_t *byte_offset);
 int32_t em_set_peer_halo(em_ctx *ctx, int32_t side, int32_t k_send, void *const dst[4]);
 

@@ -761,6 +761,8 @@ int32_t Ctx<R>::set_peer_halo(int32_t side, int32_t k_send, void *const dst[4]) 
     if (grid.bc[4 + side] != EM_BC_PMC) return fail(EM_ERR_STATE, "the wall on that side is not an artificial (PMC) slab wall");
     if (k_send < 0 || k_send > g.nz) return fail(EM_ERR_INVALID_ARG, "k_send out of range");
     for (int q = 0; q < 4; ++q) if (!dst[q]) return fail(EM_ERR_INVALID_ARG, "null peer address");
+    for (int q = 0; q < 4; ++q)                                  // (the sweep writes them with 16-byte vector stores)
+        if (reinterpret_cast<uintptr_t>(dst[q]) % 16) return fail(EM_ERR_INVALID_ARG, "peer addresses must be 16-byte aligned");
     for (int q = 0; q < 2; ++q) for (int cc = 0; cc < 2; ++cc) peer_dst[side][q][cc] = static_cast<R *>(dst[q * 2 + cc]);
     p.peer_k[side] = k_send; p.peer_skip |= 1 << side;
     bind();

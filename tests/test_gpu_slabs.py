@@ -101,6 +101,14 @@ def test_peer_halo_argument_errors():
         eo.em_get_halo(1, 0, eo._torch.empty(1000, dtype=eo.dtype, device=eo.device))
     assert e.value.code == 5
     g.close(); eo.close()
+    s, _ = slabs.sub_problem(W.random_problem(9, 8, 7, seed=9201, n_ports=0), 0, 2)      # a slab with an artificial +z wall
+    gs = P.EM(s, precision=64)
+    with pytest.raises(P.EMError) as e:
+        gs.em_set_peer_halo(1, 2, [gs.workspace_ptr + 8] * 4)      # the sweep stores 16 bytes at a time
+    assert e.value.code == 1
+    gs.em_set_peer_halo(1, 2, [gs.workspace_ptr] * 4)
+    gs.em_set_peer_halo(1, 0, None)
+    gs.close()
 
 
 # ---- two processes sharing the GPU: CUDA IPC peer mapping + gloo for the host-side barrier ----------------------------
