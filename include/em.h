@@ -81,7 +81,7 @@ extern "C" {
 typedef struct em_ctx em_ctx; /* opaque, host-side */
 
 typedef struct em_grid {
-    int32_t nx, ny, nz;          /* cells per axis, each >= 1                                       */
+    int32_t nx, ny, nz;          /* cells per axis, each >= 1; ny <= 524272, nz <= 65534 (launch grid) */
     const double *dx, *dy, *dz;  /* HOST: cell sizes [m], lengths nx, ny, nz, all > 0                */
     int32_t precision;           /* 32 or 64: working precision of fields, maps and arithmetic      */
     int32_t loss_mode;           /* EM_LOSS_CD or EM_LOSS_EXP                                        */

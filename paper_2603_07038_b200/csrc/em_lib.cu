@@ -296,6 +296,8 @@ int32_t validate_grid(const em_grid *g) {
     if (!g) return fail(EM_ERR_INVALID_ARG, "grid is null");
     if (g->nx < 1 || g->ny < 1 || g->nz < 1) return fail(EM_ERR_INVALID_ARG, "grid dims must be >= 1");
     if ((long long)g->nx + 34 > 2147483647LL / 4) return fail(EM_ERR_INVALID_ARG, "nx too large");
+    if (g->ny > 8 * 65535 - 8 || g->nz > 65534)                     // (the light kernels run one 32 x 8 block column per z plane)
+        return fail(EM_ERR_INVALID_ARG, "ny must be <= 524272 and nz <= 65534");
     if (g->precision != 32 && g->precision != 64) return fail(EM_ERR_INVALID_ARG, "precision must be 32 or 64");
     if (g->loss_mode != EM_LOSS_CD && g->loss_mode != EM_LOSS_EXP) return fail(EM_ERR_INVALID_ARG, "bad loss_mode");
     if (g->kernel < EM_KERNEL_AUTO || g->kernel > EM_KERNEL_TMA) return fail(EM_ERR_INVALID_ARG, "bad kernel strategy");

@@ -502,7 +502,8 @@ inline WorkerPool &worker_pool() { static WorkerPool *p = new WorkerPool(); retu
 // the grid: CTAs are handed out in blockIdx order (x fastest) to EMU_THREADS workers
 inline int launch(dim3 grid, dim3 block, size_t smem_bytes, const void *func, const char *name, const std::function<void()> &body) {
     const int nthreads = (int)(block.x * block.y * block.z);
-    if (nthreads < 1 || nthreads > 1024 || grid.x < 1 || grid.y < 1 || grid.z < 1) {
+    if (nthreads < 1 || nthreads > 1024 || block.z > 64 || grid.x < 1 || grid.y < 1 || grid.z < 1 || grid.x > 2147483647u ||
+        grid.y > 65535u || grid.z > 65535u) {                                               // the limits of the CUDA programming guide
         std::lock_guard<std::mutex> lk(launch_error().m);
         launch_error().msg = "emu: invalid launch configuration"; return 1;
     }

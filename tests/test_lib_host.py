@@ -41,6 +41,12 @@ def test_workspace_bytes_and_argument_errors():
     assert e.value.code == 1
     with pytest.raises(P.EMError):
         P.em_workspace_bytes(0, 16, 16)
+    # the light kernels launch one 32 x 8 block column per z plane: grid.y, grid.z <= 65535 (em.h states the limits)
+    assert P.em_workspace_bytes(2, 2, 65534) > 0 and P.em_workspace_bytes(2, 524272, 2) > 0
+    for dims in [(2, 2, 65535), (2, 524273, 2)]:
+        with pytest.raises(P.EMError) as e:
+            P.em_workspace_bytes(*dims)
+        assert e.value.code == 1
 
 
 @pytest.mark.parametrize("seed", [1, 2])
