@@ -167,8 +167,12 @@ int32_t em_set_plane(em_ctx *ctx, int32_t comp, int32_t k, const void *src, int3
  * conduction and edge conductivities).  Packed DEVICE buffer of em_halo_elems values in the working precision:
  * [Ex plane (ny+1) x nx | Ey plane ny x (nx+1) | theta layer ny x nx (coupled contexts only)].
  * em_get_halo packs node plane k_plane (and cell layer k_layer) with one kernel; em_set_halo unpacks with one kernel,
- * keeping PEC-fixed edges at 0 and refreshing sigma(T) of the layer.  stream: cudaStream_t to enqueue on (NULL: the
- * context's stream); ordering between streams is the caller's.  Leapfrog contexts only (UNSUPPORTED otherwise). */
+ * keeping PEC-fixed edges at 0 and refreshing sigma(T) of the layer.  With theta on the NODES (EM_THERMAL_NODE) the
+ * third part is instead the temperature rise of node plane k_plane itself, (ny+1) x (nx+1): the wall plane's nodes are
+ * the only ones a slab cannot update itself; em_set_halo then refreshes sigma(T) of cell layer k_layer (the ghost layer
+ * behind the wall plane) from its 8 node temperatures (two light kernels out, four in).  stream: cudaStream_t to
+ * enqueue on (NULL: the context's stream); ordering between streams is the caller's.  Leapfrog contexts only
+ * (UNSUPPORTED otherwise). */
 int32_t em_halo_elems(em_ctx *ctx, int64_t *n);
 int32_t em_get_halo(em_ctx *ctx, int32_t k_plane, int32_t k_layer, void *dst_device, void *stream);
 int32_t em_set_halo(em_ctx *ctx, int32_t k_plane, int32_t k_layer, const void *src_device, void *stream);

@@ -240,7 +240,8 @@ struct Ctx final : em_ctx {
     int32_t temperature_rise(void *dst, const void *src, int32_t is_dev) override;
     int32_t halo(int32_t kp, int32_t kl, void *dst, const void *src, void *stream) override;
     int32_t halo_elems(int64_t *n) override {
-        *n = (int64_t)(g.ny + 1) * g.nx + (int64_t)g.ny * (g.nx + 1) + (thermal_on ? (int64_t)g.ny * g.nx : 0);
+        *n = (int64_t)(g.ny + 1) * g.nx + (int64_t)g.ny * (g.nx + 1) +
+             (!thermal_on ? 0 : nodal ? (int64_t)(g.ny + 1) * (g.nx + 1) : (int64_t)g.ny * g.nx);
         return EM_OK;
     }
     int32_t joule_layers(int32_t k0, int32_t k1, double *total) override;
@@ -712,10 +713,33 @@ int32_t Ctx<R>::get_field(int32_t comp, void *dst, int32_t is_dev) {
 template <typename R>
 int32_t Ctx<R>::halo(int32_t kp, int32_t kl, void *dst, const void *srcp, void *st) {
     if (eonly) return fail(EM_ERR_UNSUPPORTED, "the halo calls cover the leapfrog formulation");
-    if (nodal) return fail(EM_ERR_UNSUPPORTED, "the halo calls cover the per-cell thermal stage");
     if (kp < 0 || kp > g.nz) return fail(EM_ERR_INVALID_ARG, "halo: node plane out of range");
     if (thermal_on && (kl < 0 || kl >= g.nz)) return fail(EM_ERR_INVALID_ARG, "halo: cell layer out of range");
     cudaStream_t s = st ? static_cast<cudaStream_t>(st) : stream;
+    if (nodal && thermal_on) {
+        // theta lives on the nodes: the message is [Ex | Ey | theta] of node plane kp; on the way in, sigma(T) of cell
+        // layer kl (the ghost layer behind the wall plane, eq. (6) from its 8 node temperatures) is refreshed
+        const long long n_e = (long long)(g.ny + 1) * g.nx + (long long)g.ny * (g.nx + 1), n_t = (long long)(g.ny + 1) * (g.nx + 1);
+        const unsigned be = (unsigned)((n_e + 255) / 256), bt = (unsigned)((n_t + 255) / 256);
+        R *th = c.theta[th_cur] + g.origin;
+        if (dst) {
+            EM_LAUNCH(em::k_pack_halo<R>, be, 256, 0, s)(p, p.E[0], p.E[1], nullptr, kp, kl, static_cast<R *>(dst));
+            EM_LAUNCH(em::k_node_plane<R>, bt, 256, 0, s)(p, th, kp, static_cast<R *>(dst) + n_e, 0);
+            launches += 2;
+        } else {
+            R *src = const_cast<R *>(static_cast<const R *>(srcp));
+            EM_LAUNCH(em::k_unpack_halo<R>, be, 256, 0, s)(p, p.E[0], p.E[1], nullptr, nullptr, nullptr, c.ttable, kp, kl, src);
+            EM_LAUNCH(em::k_node_plane<R>, bt, 256, 0, s)(p, th, kp, src + n_e, 1);
+            dim3 b(32, 8), gr((g.nx + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, 1);
+            em::ThermalParams<R> t = tp();
+            EM_LAUNCH(em::k_sigma_nodal<R>, gr, b, 0, s)(p, t, kl);
+            t.sig = sig_buf(1 - sg_cur);
+            EM_LAUNCH(em::k_sigma_nodal<R>, gr, b, 0, s)(p, t, kl);
+            launches += 4;
+        }
+        CU(cudaGetLastError());
+        return EM_OK;
+    }
     int64_t n = 0; halo_elems(&n);
     const unsigned blocks = (unsigned)((n + 255) / 256);
     R *th = thermal_on ? c.theta[th_cur] + g.origin : nullptr;
@@ -813,9 +837,9 @@ int32_t Ctx<R>::refresh_sigma() {
     dim3 b(32, 8);
     em::ThermalParams<R> t = tp();
     if (nodal) {
-        EM_LAUNCH(em::k_sigma_nodal<R>, node_grid(b, 0), b, 0, stream)(p, t);
+        EM_LAUNCH(em::k_sigma_nodal<R>, node_grid(b, 0), b, 0, stream)(p, t, 0);
         t.sig = sig_buf(1 - sg_cur);
-        EM_LAUNCH(em::k_sigma_nodal<R>, node_grid(b, 0), b, 0, stream)(p, t);
+        EM_LAUNCH(em::k_sigma_nodal<R>, node_grid(b, 0), b, 0, stream)(p, t, 0);
         CU(cudaGetLastError());
         return EM_OK;
     }
@@ -924,7 +948,7 @@ int32_t Ctx<R>::step_thermal_nodal() {
     EM_LAUNCH(em::k_joule_sig<R>, node_grid(b, 0), b, 0, stream)(p, sig);
     EM_LAUNCH(em::k_thermal_nodal<R>, node_grid(b, 1), b, 0, stream)(p, tp(), c.vx, c.vy, c.vz);
     th_cur ^= 1;
-    EM_LAUNCH(em::k_sigma_nodal<R>, node_grid(b, 0), b, 0, stream)(p, tp());          // sigma(T^{n+1}) from the new theta
+    EM_LAUNCH(em::k_sigma_nodal<R>, node_grid(b, 0), b, 0, stream)(p, tp(), 0);       // sigma(T^{n+1}) from the new theta
     launches += 3;
     CU(cudaGetLastError());
     e_cur ^= 1; bind();

@@ -312,12 +312,12 @@ __global__ void __launch_bounds__(256) k_thermal_nodal(DevParams<R> p, ThermalPa
     t.theta_n[o] = cap > R(0) ? th0 + (heat - p.dt * out) * rcp<R>(cap) : th0;
 }
 
-// eq. (6) per cell with the mean of the cell's 8 node temperatures (N4)
+// eq. (6) per cell with the mean of the cell's 8 node temperatures (N4); cell layers k0 .. k0 + gridDim.z - 1
 template <typename R>
-__global__ void __launch_bounds__(256) k_sigma_nodal(DevParams<R> p, ThermalParams<R> t) {
+__global__ void __launch_bounds__(256) k_sigma_nodal(DevParams<R> p, ThermalParams<R> t, int k0) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k = blockIdx.z;
+    const int k = k0 + blockIdx.z;
     if (i >= p.nx || j >= p.ny) return;
     const long long PX = p.PX, PXY = p.PXY;
     const long long o = ((long long)k * p.PY + j) * PX + i;
@@ -325,6 +325,18 @@ __global__ void __launch_bounds__(256) k_sigma_nodal(DevParams<R> p, ThermalPara
     const R m = ((t.theta[o] + t.theta[o + 1]) + (t.theta[o + PX] + t.theta[o + PX + 1])) +
                 ((t.theta[o + PXY] + t.theta[o + PXY + 1]) + (t.theta[o + PXY + PX] + t.theta[o + PXY + PX + 1]));
     t.sig[o] = me.sigma0 * rcp<R>(thermal_den(me.alpha, R(0.125) * m));
+}
+
+// z-slab halo of the nodal stage: the temperature rise of node plane kp, dense [(ny+1) x (nx+1)], out of (unpack = 0) or
+// into (1) the padded array.  (The tangential E of the plane travels in k_pack_halo / k_unpack_halo as for every context.)
+template <typename R>
+__global__ void __launch_bounds__(256) k_node_plane(DevParams<R> p, R *theta, int kp, R *packed, int unpack) {
+    const long long n = (long long)(p.ny + 1) * (p.nx + 1);
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const int j = (int)(t / (p.nx + 1)), i = (int)(t % (p.nx + 1));
+    const long long o = ((long long)kp * p.PY + j) * p.PX + i;
+    if (unpack) theta[o] = packed[t]; else packed[t] = theta[o];
 }
 
 // sigma = sigma_0 / (1 + alpha theta) on every cell (after em_set_thermal / em_set_temperature_rise / em_reset)

@@ -9,7 +9,8 @@ the Joule sum that closes on the plane above) follows from correct inputs.  So t
     to the slab below : my Ex, Ey at global node plane a+1   -> its upper wall plane
 (2 x nx*ny reals per neighbour), point-to-point only; with the two-way thermal coupling the temperature
 rise of the owned boundary layer rides along (-> the neighbour's ghost layer, whose theta and sigma(T) feed the owned
-layer's conduction and edge conductivities).  Two ways to move it, both with every arithmetic step in the CUDA kernels:
+layer's conduction and edge conductivities); with theta on the mesh NODES (the paper's placement) it is the temperature
+rise of the same node plane as Ex, Ey that rides along (-> the neighbour's wall plane, the only nodes it cannot update).  Two ways to move it, both with every arithmetic step in the CUDA kernels:
 
   mode "p2p"  : em_get_halo packs the message with one kernel into a preallocated buffer, torch.distributed moves it
                 (batched isend/irecv: NCCL over NVLink, stream-ordered, no host synchronisation; gloo in the CPU tests),
@@ -201,8 +202,11 @@ class SlabRank:
         return pw[m.a - m.lo:m.b - m.lo], q[m.a - m.lo:m.b - m.lo]
 
     def owned_theta(self):
+        """per-cell stage: the owned cell layers; nodal stage: node planes a .. b-1 (the last slab also owns plane nz)"""
         m = self.meta
-        return self.em.em_get_temperature_rise()[m.a - m.lo:m.b - m.lo]
+        th = self.em.em_get_temperature_rise()
+        nodal = th.shape[0] == self.nz_local + 1
+        return th[m.a - m.lo:m.b - m.lo + (1 if nodal and not m.has_above else 0)]
 
 
 def exchange_dist(rank: SlabRank, dist, group=None):

@@ -217,6 +217,11 @@ def test_slabs_split_kernels(emulated):
     TS.test_thermally_coupled_slabs(P.EM_KERNEL_SPLIT, 64)
 
 
+@pytest.mark.parametrize("n_ranks,precision", [(2, 64), (3, 32), (3, 64)])
+def test_nodal_thermally_coupled_slabs(emulated, n_ranks, precision):
+    TS.test_nodal_thermally_coupled_slabs(n_ranks, precision)
+
+
 def test_peer_halo_argument_errors(emulated):
     TS.test_peer_halo_argument_errors()
 

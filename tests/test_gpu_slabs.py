@@ -88,6 +88,38 @@ def test_thermally_coupled_slabs(kernel, precision):
     single.close(); o.close()
 
 
+@pytest.mark.parametrize("n_ranks", [2, 3])
+@pytest.mark.parametrize("precision", [64, 32])
+def test_nodal_thermally_coupled_slabs(n_ranks, precision):
+    """the paper's placement (theta on the mesh nodes, em_grid.thermal = EM_THERMAL_NODE) shards the same way: the halo
+    carries the temperature rise of the node plane that carries Ex, Ey -- a slab cannot update the nodes of its artificial
+    wall plane (half of their cells, edges and heat lie in the neighbour) -- and sigma(T) of the ghost layer follows"""
+    p = W.random_problem(17, 14, 13, seed=9150 + n_ranks, loss_mode=LOSS_CD if n_ranks == 2 else LOSS_EXP, steps=40, n_ports=12,
+                         init_scale=4.0e6, bc=(0, 1, 0, 0, 1, 0))
+    th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
+    p.thermal = th
+    p.thermal_placement = "node"
+    ranks = slabs.make_ranks_inprocess(p, n_ranks, precision=precision)
+    single = P.EM(p, precision=precision)
+    o = emo.Oracle(p)
+    slabs.step_inprocess(ranks, 40); single.em_step(40); o.step(40)
+    fields, pw, q = slabs.gather_inprocess(ranks)
+    theta = np.concatenate([r.owned_theta() for r in ranks], axis=0)
+    fs = single.fields(); _, qs, Qs = single.joule_maps(); ts = single.em_get_temperature_rise()
+    assert theta.shape == ts.shape == (p.nz + 1, p.ny + 1, p.nx + 1)
+    for c in range(6):
+        assert np.array_equal(fields[c], fs[c]), c
+    assert np.array_equal(q, qs) and np.array_equal(theta, ts)
+    to = o.temperature_rise()
+    assert np.max(np.abs(p.thermal[p.mat_id, 2])) * np.max(to) > 1e-3             # the feedback on sigma matters
+    assert rel_l2([theta], [to]) <= TOL[precision] and rel_l2(fields[:3], o.fields()[:3]) <= TOL[precision]
+    Q = sum(r.joule_total() for r in ranks)
+    assert abs(Q - Qs) <= 1e-12 * Qs and abs(Q - o.joule()[2]) <= TOL[precision] * Qs
+    for r in ranks:
+        r.em.close()
+    single.close(); o.close()
+
+
 def test_peer_halo_argument_errors():
     p = W.random_problem(9, 8, 7, seed=9200, n_ports=0)
     g = P.EM(p, precision=64)

@@ -191,6 +191,8 @@ def _problem_for_slabs(thermal):
     if thermal:
         th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
         p.thermal = th
+        if thermal == "node":
+            p.thermal_placement = "node"                  # theta on the mesh nodes: the halo carries a node plane of it
     return p
 
 
@@ -213,7 +215,7 @@ def _emu_worker(rank, world, port, thermal, steps, out):
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("world,thermal", [(2, False), (3, True)])
+@pytest.mark.parametrize("world,thermal", [(2, False), (3, True), (2, "node")])
 def test_real_kernels_under_the_gloo_exchange_equal_the_single_domain_run(world, thermal, tmp_path):
     sys.path.insert(0, os.path.join(ROOT, "tests", "emu"))
     import build_emu
