@@ -113,6 +113,13 @@ class SlabRank:
         self.em, self.meta, self.mode = em, meta, mode
         self._buf = {}
         self._token = None
+        # False until the wall planes hold the neighbours' values of the CURRENT state.  A slab cannot apply the whole-domain
+        # rules to its wall plane by itself: an initial Ex, Ey there that the single-domain em_set_field would force to 0
+        # because the edge touches a PEC-flagged cell ABOVE the plane -- a cell this slab does not hold -- stays as given.
+        # The neighbour holds that plane as an interior one, correctly masked, so one exchange before the first step
+        # settles it (found by the random slab campaign of tests/test_emu_sweep.py).  Set it to False again after
+        # em_set_field / em_set_temperature_rise on a slab context.
+        self.halo_synced = False
 
     # local indices --------------------------------------------------------------------------------------------
     @property
@@ -163,6 +170,11 @@ class SlabRank:
 
     # stepping with torch.distributed (rank == slab rank) ---------------------------------------------------------
     def step(self, n: int, dist, group=None):
+        if not self.halo_synced:
+            exchange_dist(self, dist, group)              # (pack / unpack kernels, whatever the transport of the steps)
+            self.halo_synced = True
+            if self.mode == "peer":
+                barrier_on_stream(self, dist, group)      # the neighbours' sweeps store into my planes from step 1 on
         for _ in range(n):
             self.em.em_step(1)
             if self.mode == "p2p":
@@ -215,15 +227,27 @@ def exchange_dist(rank: SlabRank, dist, group=None):
     that the two directions overlap.  With nccl everything is stream-ordered (wait() makes the current stream wait)."""
     m = rank.meta
     ops = []
+    # (a backend without device-to-device send / recv -- gloo with CUDA buffers, i.e. the one-GPU IPC test -- goes through
+    # host copies of the packed messages; nccl and the CPU tests move the buffers themselves)
+    staged = []
+    def out(t):
+        return t if (t.device.type == "cpu" or dist.get_backend(group) == "nccl") else t.cpu()
+    def into(t):
+        if t.device.type == "cpu" or dist.get_backend(group) == "nccl":
+            return t
+        staged.append((t, t.cpu()))
+        return staged[-1][1]
     if m.has_above:
-        ops += [dist.P2POp(dist.isend, rank.pack_up(), m.rank + 1, group),
-                dist.P2POp(dist.irecv, rank.buf("recv_hi"), m.rank + 1, group)]
+        ops += [dist.P2POp(dist.isend, out(rank.pack_up()), m.rank + 1, group),
+                dist.P2POp(dist.irecv, into(rank.buf("recv_hi")), m.rank + 1, group)]
     if m.has_below:
-        ops += [dist.P2POp(dist.isend, rank.pack_down(), m.rank - 1, group),
-                dist.P2POp(dist.irecv, rank.buf("recv_lo"), m.rank - 1, group)]
+        ops += [dist.P2POp(dist.isend, out(rank.pack_down()), m.rank - 1, group),
+                dist.P2POp(dist.irecv, into(rank.buf("recv_lo")), m.rank - 1, group)]
     if ops:
         for w in dist.batch_isend_irecv(ops):
             w.wait()
+    for dev, host in staged:
+        dev.copy_(host)
     if m.has_below:
         rank.unpack_lo(rank.buf("recv_lo"))
     if m.has_above:
@@ -312,6 +336,10 @@ def make_ranks_inprocess(p, n_ranks: int, mode: str = "p2p", **em_kw) -> List[Sl
 
 
 def step_inprocess(ranks: Sequence[SlabRank], n: int = 1):
+    if not all(r.halo_synced for r in ranks):
+        exchange_inprocess(ranks)                   # wall planes of the initial state (SlabRank.halo_synced)
+        for r in ranks:
+            r.halo_synced = True
     for _ in range(n):
         for r in ranks:
             r.em.em_step(1)

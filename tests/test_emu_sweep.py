@@ -217,6 +217,11 @@ def test_slabs_split_kernels(emulated):
     TS.test_thermally_coupled_slabs(P.EM_KERNEL_SPLIT, 64)
 
 
+@pytest.mark.parametrize("kernel,mode", TS.CASES)
+def test_slabs_initial_state_with_pec_material_across_the_cut(emulated, kernel, mode):
+    TS.test_slabs_initial_state_with_pec_material_across_the_cut(kernel, mode)
+
+
 @pytest.mark.parametrize("n_ranks,precision", [(2, 64), (3, 32), (3, 64)])
 def test_nodal_thermally_coupled_slabs(emulated, n_ranks, precision):
     TS.test_nodal_thermally_coupled_slabs(n_ranks, precision)
@@ -376,6 +381,75 @@ def test_random_problem_campaign(emulated, monkeypatch):
             _run_case(case, monkeypatch)
         except Exception as e:
             raise AssertionError("campaign case %r: %r" % (case, e))
+
+
+def _slab_campaign(seed, n_cases, max_cells):
+    """random z-slab decompositions -- grid shape, walls, loss mode, precision, slab count, chunk count, ports, thread
+    schedule -- over the transports and the coupled variants; each against the SINGLE-DOMAIN run of the same kernels"""
+    rng = np.random.default_rng(seed)
+    done = 0
+    while done < n_cases:
+        nx, ny, nz = int(rng.integers(1, 90)), int(rng.integers(1, 24)), int(rng.integers(4, 20))
+        n_ranks = int(rng.integers(2, 5))
+        if nx * ny * nz > max_cells or nz < 2 * n_ranks:
+            continue
+        done += 1
+        yield dict(dims=(nx, ny, nz), n_ranks=n_ranks, bc=tuple(int(b) for b in (rng.random(6) < 0.35)), mode=int(rng.integers(0, 2)),
+                   precision=int(rng.choice([32, 64])), variant=str(rng.choice(["tma-p2p", "tma-peer", "split-p2p", "coupled", "coupled-split", "nodal"])),
+                   z_chunks=int(rng.integers(0, 4)), steps=int(rng.integers(2, 10)), n_ports=int(rng.integers(0, 12)) if nx * ny > 4 else 0,
+                   seed=int(rng.integers(0, 1 << 30)), emu_seed=int(rng.integers(0, 5)), percell=bool(rng.random() < 0.3), pec=bool(rng.random() < 0.3))
+
+
+def _run_slab_case(case, monkeypatch):
+    from paper_2603_07038_b200 import slabs
+    monkeypatch.setenv("EMU_SEED", str(case["emu_seed"]))
+    v = case["variant"]
+    thermal = v in ("coupled", "coupled-split", "nodal")
+    p = W.random_problem(*case["dims"], seed=case["seed"], steps=case["steps"], n_ports=case["n_ports"], loss_mode=case["mode"], bc=case["bc"],
+                         blocky=not case["percell"], pec_material=case["pec"], init_scale=4.0e6 if thermal else 1.0)
+    kw = dict(precision=case["precision"])
+    if thermal:
+        th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
+        p.thermal = th
+        if v == "nodal":
+            p.thermal_placement = "node"
+    if v in ("split-p2p", "coupled-split"):
+        kw["kernel"] = P.EM_KERNEL_SPLIT
+    elif v != "nodal":
+        kw["z_chunks"] = case["z_chunks"]
+    ranks = slabs.make_ranks_inprocess(p, case["n_ranks"], mode="peer" if v == "tma-peer" else "p2p", **kw)
+    single = emu_em.EmuEM(p, **kw)
+    slabs.step_inprocess(ranks, case["steps"]); single.em_step(case["steps"])
+    fields, pw, q = slabs.gather_inprocess(ranks)
+    fs = single.fields(); ps, qs, Qs = single.joule_maps()
+    for c in range(6):
+        assert np.array_equal(fields[c], fs[c]), c
+    assert np.array_equal(q, qs) and np.array_equal(pw, ps)
+    if thermal:
+        assert np.array_equal(np.concatenate([r.owned_theta() for r in ranks], axis=0), single.em_get_temperature_rise())
+    assert abs(sum(r.joule_total() for r in ranks) - Qs) <= 1e-12 * abs(Qs)
+    for r in ranks:
+        r.em.close()
+    single.close()
+
+
+def test_random_slab_campaign(emulated, monkeypatch):
+    for case in _slab_campaign(20261106, 36, 12000):
+        try:
+            _run_slab_case(case, monkeypatch)
+        except Exception as e:
+            raise AssertionError("slab campaign case %r: %r" % (case, e))
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("seed", [1, 2])
+def test_random_slab_campaign_long(emulated, monkeypatch, seed):
+    """EM_RUN_SLOW=1: 2 x 600 cases (profiles/r2_emulation.md records this round's run)"""
+    for case in _slab_campaign(seed, 600, 30000):
+        try:
+            _run_slab_case(case, monkeypatch)
+        except Exception as e:
+            raise AssertionError("slab campaign case %r: %r" % (case, e))
 
 
 @pytest.mark.slow

@@ -49,6 +49,26 @@ def test_slabs_equal_single_domain(n_ranks, kernel, mode, precision):
     single.close(); o.close()
 
 
+@pytest.mark.parametrize("kernel,mode", CASES)
+def test_slabs_initial_state_with_pec_material_across_the_cut(kernel, mode):
+    """an initial Ex, Ey on a slab's wall plane whose edge touches a PEC-flagged cell ABOVE the plane (a cell the slab does
+    not hold) is forced to 0 in the single-domain run; the slab learns it from its neighbour in the exchange that precedes
+    the first step (slabs.SlabRank.halo_synced).  The case is the one the random slab campaign of tests/test_emu_sweep.py found."""
+    p = W.random_problem(62, 23, 7, seed=811118369, loss_mode=LOSS_EXP, steps=2, n_ports=8, blocky=False, pec_material=True)
+    ranks = slabs.make_ranks_inprocess(p, 3, mode=mode, precision=32, kernel=kernel)
+    single = P.EM(p, precision=32, kernel=kernel)
+    slabs.step_inprocess(ranks, 2); single.em_step(2)
+    fields, pw, q = slabs.gather_inprocess(ranks)
+    fs = single.fields(); ps, qs, _ = single.joule_maps()
+    assert any(np.any(f != 0) for f in fs)
+    for c in range(6):
+        assert np.array_equal(fields[c], fs[c]), c
+    assert np.array_equal(q, qs) and np.array_equal(pw, ps)
+    for r in ranks:
+        r.em.close()
+    single.close()
+
+
 @pytest.mark.parametrize("mode", ["p2p", "peer"])
 def test_slabs_config4_scaled_ports_everywhere(mode):
     p = W.make_config(4, scale=16, zscale=4, steps=60)            # 64 x 64 x 48, ports in several layers
