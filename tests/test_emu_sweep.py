@@ -383,6 +383,133 @@ def test_random_problem_campaign(emulated, monkeypatch):
             raise AssertionError("campaign case %r: %r" % (case, e))
 
 
+# ---------------------------------------------------------------------------------------- random API-sequence campaign
+def _sequence_campaign(seed, n_cases, max_cells):
+    """random SEQUENCES of calls on one context -- steps, a field overwritten mid-run (odd and even ping-pong parities), the
+    source set replaced, Joule maps read with and without reset, em_reset, the temperature rise overwritten, a checkpoint
+    resumed into a second context -- mirrored on the oracle; compared after the sequence and at one point inside it"""
+    rng = np.random.default_rng(seed)
+    done = 0
+    while done < n_cases:
+        nx, ny, nz = int(rng.integers(1, 80)), int(rng.integers(1, 20)), int(rng.integers(1, 16))
+        if nx * ny * nz > max_cells:
+            continue
+        done += 1
+        variant = str(rng.choice(["leapfrog", "split", "coupled", "fc", "coupled-split", "nodal"]))
+        thermal = variant in ("coupled", "fc", "coupled-split", "nodal")
+        pec = bool(rng.random() < 0.25)
+        kinds = ["step", "step", "step", "set_field", "joule", "joule_reset", "reset", "checkpoint"] + ([] if pec else ["set_source"]) + \
+                (["set_theta"] if thermal else [])
+        ops = [(str(rng.choice(kinds)), int(rng.integers(0, 1 << 30))) for _ in range(int(rng.integers(3, 9)))] + [("step", int(rng.integers(0, 1 << 30)))]
+        yield dict(dims=(nx, ny, nz), bc=tuple(int(b) for b in (rng.random(6) < 0.35)), mode=int(rng.integers(0, 2)), precision=int(rng.choice([32, 64])),
+                   variant=variant, z_chunks=int(rng.integers(0, 5)), n_ports=int(rng.integers(0, 10)) if nx * ny * nz > 8 else 0,
+                   seed=int(rng.integers(0, 1 << 30)), emu_seed=int(rng.integers(0, 5)), percell=bool(rng.random() < 0.3), pec=pec, ops=ops)
+
+
+def _run_sequence_case(case, monkeypatch):
+    monkeypatch.setenv("EMU_SEED", str(case["emu_seed"]))
+    v = case["variant"]
+    thermal = v in ("coupled", "fc", "coupled-split", "nodal")
+    mk = lambda seed, n_ports: W.random_problem(*case["dims"], seed=seed, steps=64, n_ports=n_ports, loss_mode=case["mode"], bc=case["bc"],
+                                                blocky=not case["percell"], pec_material=case["pec"], init_scale=4.0e6 if thermal else 1.0)
+    p = mk(case["seed"], case["n_ports"])
+    kw = dict(precision=case["precision"], max_ports=32, max_source_edges=1 << 14, max_wave_samples=1 << 14)
+    if thermal:
+        th = W.thermal_table(); th[:, 1] *= 2.0e5; th[:, 2] *= 1.0e4
+        p.thermal = th
+        if v == "fc":
+            kw.update(FC)
+        if v == "nodal":
+            p.thermal_placement = "node"
+    if v in ("split", "coupled-split"):
+        kw["kernel"] = P.EM_KERNEL_SPLIT
+    elif v != "nodal":
+        kw["z_chunks"] = case["z_chunks"]
+    tol = TOL[case["precision"]]
+    g = emu_em.EmuEM(p, **kw)
+    o = emo.Oracle(p)
+    # (fp32 + exponential loss: one step from a random field inside a good conductor is the documented rounding corner of the
+    # power map -- DESIGN.md section 9; the sequences take >= 2 steps after every new random field in that combination)
+    min_steps = 2 if (case["mode"] == 1 and case["precision"] == 32) else 1
+    fresh = True
+    src_p = p
+    mid = len(case["ops"]) // 2
+
+    def check():
+        compare_state(g, o, tol)
+        if thermal:
+            assert rel_l2([g.em_get_temperature_rise()], [o.temperature_rise()]) <= tol
+        # probes = the raw samples of the fields; the layer totals add up to the Joule total; no NaN / Inf
+        F = g.fields()
+        rp = np.random.default_rng(case["seed"])
+        pts = []
+        for _ in range(6):
+            c = int(rp.integers(0, 6)); sz, sy, sx = g.shapes[c]
+            pts.append((c, int(rp.integers(0, sx)), int(rp.integers(0, sy)), int(rp.integers(0, sz))))
+        vals, want = g.em_probe(pts), o.probe(pts)
+        for v, w, (c, i, j, k) in zip(vals, want, pts):
+            assert v == F[c][k, j, i] and abs(v - w) <= tol * max(float(np.max(np.abs(o.get_field(c)))), 1e-300), (c, i, j, k)
+        nz = case["dims"][2]; cut = int(rp.integers(0, nz + 1))
+        Q = g.joule_maps()[2]
+        assert abs(g.em_joule_layers(0, cut) + g.em_joule_layers(cut, nz) - Q) <= 1e-12 * abs(Q)
+        assert g.em_check_finite()
+
+    for n, (kind, r) in enumerate(case["ops"]):
+        rr = np.random.default_rng(r)
+        if kind == "step":
+            k = int(rr.integers(min_steps if fresh else 1, 5))
+            g.em_step(k); o.step(k); fresh = False
+        elif kind == "set_field":
+            comp = int(rr.integers(0, 6))
+            a = rr.standard_normal(g.shapes[comp]) * (4.0e6 if thermal else 1.0) * (1.0 if comp < 3 else 1.0 / 376.73)
+            g.em_set_field(comp, a); o.set_field(comp, a.astype(g.np_dtype).astype(np.float64)); fresh = True
+            g.em_step(min_steps); o.step(min_steps); fresh = False
+        elif kind == "set_source":
+            p2 = mk(int(rr.integers(0, 1 << 30)), int(rr.integers(0, 10)) if p.n_cells > 8 else 0)
+            g.em_set_source(p2); o.set_source(p2); src_p = p2
+        elif kind in ("joule", "joule_reset"):
+            if fresh:
+                g.em_step(min_steps); o.step(min_steps); fresh = False
+            pg, qg, Qg = g.joule_maps(reset=kind == "joule_reset"); po, qo, Qo = o.joule(reset=kind == "joule_reset")
+            assert rel_l2([qg], [qo]) <= tol and rel_l2([pg], [po]) <= 2 * tol and abs(Qg - Qo) <= tol * abs(Qo), (n, kind)
+        elif kind == "reset":
+            g.em_reset(); o.reset(); fresh = False
+        elif kind == "set_theta":
+            a = rr.uniform(0.0, 40.0, size=g.theta_shape)
+            g.em_set_temperature_rise(a); o.set_temperature_rise(a.astype(g.np_dtype).astype(np.float64))
+        elif kind == "checkpoint":                          # carry on in a second context: bit-identical state
+            ck = g.checkpoint()
+            g2 = emu_em.EmuEM(p, load_init=False, **kw)
+            g2.em_set_source(src_p)
+            g2.resume(ck)
+            for c in range(6):
+                assert np.array_equal(g2.em_get_field(c), g.em_get_field(c)), (n, c)
+            g.close(); g = g2
+        if n == mid and not fresh:
+            check()
+    check()
+    g.close(); o.close()
+
+
+def test_random_sequence_campaign(emulated, monkeypatch):
+    for case in _sequence_campaign(20261107, 40, 12000):
+        try:
+            _run_sequence_case(case, monkeypatch)
+        except Exception as e:
+            raise AssertionError("sequence campaign case %r: %r" % (case, e))
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("seed", [1, 2])
+def test_random_sequence_campaign_long(emulated, monkeypatch, seed):
+    """EM_RUN_SLOW=1: 2 x 500 sequences (profiles/r2_emulation.md records this round's run)"""
+    for case in _sequence_campaign(seed, 500, 30000):
+        try:
+            _run_sequence_case(case, monkeypatch)
+        except Exception as e:
+            raise AssertionError("sequence campaign case %r: %r" % (case, e))
+
+
 def _slab_campaign(seed, n_cases, max_cells):
     """random z-slab decompositions -- grid shape, walls, loss mode, precision, slab count, chunk count, ports, thread
     schedule -- over the transports and the coupled variants; each against the SINGLE-DOMAIN run of the same kernels"""
