@@ -14,7 +14,22 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "slow: minutes of host-side oracle time per test; runs only with EM_RUN_SLOW=1")
 
 
+# GPU tests written AFTER GPU use was closed for this repository in round 2: green on the emulated
+# build (tests/emu), never run on a B200.  They are collected LAST: the suite runs with `pytest -x`, and a first-contact
+# failure in one of them must not hide the hardware-verified suite behind it.
+HARDWARE_UNSEEN = {
+    "test_checkpoint_resume_is_bit_exact_and_check_finite",
+    "test_slabs_initial_state_with_pec_material_across_the_cut",
+    "test_nodal_thermally_coupled_slabs",
+    "test_peer_halo_argument_errors",
+    "test_nodal_coupled_random_grids",
+    "test_nodal_with_pmc_walls_diffusion_and_api",
+    "test_nodal_paper_mesh_unknown_count_and_package_slice",
+}
+
+
 def pytest_collection_modifyitems(config, items):
+    items.sort(key=lambda it: getattr(it, "originalname", None) in HARDWARE_UNSEEN)      # stable: order kept otherwise
     if os.environ.get("EM_RUN_SLOW", "") != "1":
         slow = pytest.mark.skip(reason="slow: set EM_RUN_SLOW=1")
         for it in items:
