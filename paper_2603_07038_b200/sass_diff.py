@@ -5,11 +5,13 @@ For every kernel present in both libraries: `identical`, `parameter offsets only
 c[0x0][..] kernel-parameter offsets moved because a parameter struct grew) or `changed` (with the instruction counts)."""
 from __future__ import annotations
 
+import functools
 import re
 import subprocess
 import sys
 
 
+@functools.lru_cache(maxsize=4)
 def kernels(lib: str) -> dict[str, list[str]]:
     out = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
     mangled = re.findall(r"Function : (\S+)", out)

@@ -156,3 +156,20 @@ def test_product_library_has_no_emulation_in_it():
                 os.path.join("paper_2603_07038_b200", "__init__.py"), os.path.join("paper_2603_07038_b200", "replicas.py")):
         src = open(os.path.join(ROOT, rel)).read()
         assert "emu_em" not in src and "libem_emu" not in src and "build_emu" not in src, rel
+
+
+def test_sass_diff_reads_the_built_library():
+    """paper_2603_07038_b200/sass_diff.py (profiles/r2_sass_check.md): the built library compared with itself is identical
+    kernel by kernel, and holds the 20 instantiations of the sweep the bench lines are about"""
+    import shutil
+    from paper_2603_07038_b200 import sass_diff
+    if shutil.which("cuobjdump") is None or shutil.which("c++filt") is None:
+        pytest.skip("cuobjdump / c++filt not on PATH")
+    lib = os.path.join(ROOT, "paper_2603_07038_b200", "libem.so")
+    P.load()
+    res = sass_diff.compare(lib, lib)
+    assert res and set(res.values()) == {"identical"}
+    assert sum("k_sweep_tma<" in k for k in res) == 20
+    k = sass_diff.kernels(lib)
+    sweep = next(v for n, v in k.items() if "k_sweep_tma<float, 0, false, false, false>" in n)
+    assert any(i.startswith("UTMALDG") for i in sweep) and any("SYNCS" in i for i in sweep)      # TMA boxes on mbarriers
